@@ -1,0 +1,228 @@
+/* mcx.h -- C ABI of libmcx_b200.so: the data-parallel hot path of McXtrace-style X-ray ray tracing
+ * (arxiv 2410.08747) as hand-written sm_100a CUDA kernels.
+ *
+ * What the library computes.  "Rays are generated at the source component and sequentially propagated through
+ * the list of X-ray components" (section 1); each ray is independent and carries the
+ * particle state of PAPER.md:92-98 (here: position, direction, energy, weight); monitors are histogram arrays
+ * updated atomically.  The paper prints no physics formulas; every formula follows the reading
+ * in DESIGN.md ("Readings", steps 1-15 of SURVEY.md 8(c)).  BASELINE.json:north_star names the three primary
+ * entry points: mcx_instrument_create, mcx_trace, mcx_tally_read.
+ *
+ * Conventions.  Units: metres, keV, 1/m, radians.  A pose maps lab to component coordinates,
+ * r_local = rot * (r_lab - origin), rot row-major, rows = local axes in lab coordinates (the paper's
+ * "AT (...) RELATIVE" placement, given as an absolute rigid transform).  The ray between components
+ * is held in lab coordinates.  Component 0 of a chain must be a source.
+ *
+ * Memory.  Pointers marked HOST are read during mcx_instrument_create only and may be freed afterwards.
+ * Pointers marked DEVICE must stay valid (and, for inputs, unchanged) until mcx_instrument_destroy.  The library
+ * never allocates device memory: everything it keeps on the device lives in the caller's `workspace`.
+ *
+ * Streams.  `cuda_stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  All calls enqueue
+ * work on it and return without synchronising; the caller synchronises before reading outputs.
+ *
+ * Errors.  Every call returns an mcx_status; mcx_last_error() gives a thread-local message for the last failure.
+ * Argument and range errors are found synchronously at create.  A sticky CUDA error is reported by the next call
+ * as MCX_ERR_CUDA.  A handle must be used from one host thread at a time; distinct handles are independent.
+ */
+#ifndef MCX_H_
+#define MCX_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mcx_instrument mcx_instrument; /* opaque, host side */
+
+typedef enum {
+  MCX_OK = 0,
+  MCX_ERR_INVALID_ARG = 1, /* null pointer, bad enum, chain not starting with a source, ... */
+  MCX_ERR_UNSUPPORTED = 2, /* a limit of this build exceeded (see MCX_MAX_*) */
+  MCX_ERR_RANGE = 3,       /* a source energy range not covered by a reflectivity table grid, bad table order */
+  MCX_ERR_WORKSPACE = 4,   /* workspace too small or misaligned (needs 256-byte alignment) */
+  MCX_ERR_CUDA = 5,        /* a CUDA runtime call failed */
+  MCX_ERR_CAPACITY = 6     /* a per-ray scratch capacity (intervals, mesh hits) overflowed during a trace */
+} mcx_status;
+
+enum { MCX_MAX_COMPONENTS = 16, MCX_MAX_DETECTORS = 4, MCX_MAX_MATERIALS = 32, MCX_MAX_SOLIDS = 16 };
+
+typedef enum {
+  MCX_SOURCE = 0,          /* step 3 (point / flat / Gaussian emitters) */
+  MCX_SLIT_RECT = 1,       /* step 6 */
+  MCX_SLIT_CIRC = 2,       /* step 6 */
+  MCX_SOLIDS = 3,          /* steps 8-10: primitives and closed triangle meshes, Beer-Lambert */
+  MCX_VOXELS = 4,          /* step 11: uint8 material-ID volume, exact traversal */
+  MCX_MIRROR_ELLIPTIC = 5, /* step 12 (optics category) */
+  MCX_CRYSTAL_BRAGG = 6,   /* step 13 */
+  MCX_DETECTOR = 7         /* step 14: PSD / E / EPSD monitors */
+} mcx_kind;
+
+typedef enum { MCX_POS_POINT = 0, MCX_POS_DISK = 1, MCX_POS_GAUSS = 2 } mcx_pos_mode;
+typedef enum { MCX_DIR_TARGET = 0, MCX_DIR_GAUSS = 1 } mcx_dir_mode;
+typedef enum { MCX_E_MONO = 0, MCX_E_UNIFORM = 1, MCX_E_SPECTRUM = 2 } mcx_energy_mode;
+typedef enum { MCX_BOX = 0, MCX_CYLINDER = 1, MCX_SPHERE = 2, MCX_MESH = 3 } mcx_shape;
+
+/* Fate of a ray (mcx_ray_fate.fate): >= 0 means "absorbed by the component with that chain index". */
+enum { MCX_FATE_DETECTED = -1, MCX_FATE_MISSED = -2, MCX_FATE_DEGENERATE = -3 };
+
+typedef struct mcx_pose {
+  double rot[9];    /* row-major 3x3, orthonormal */
+  double origin[3]; /* lab position of the component origin */
+} mcx_pose;
+
+/* mu(E) table of one material (step 7: log-log interpolation, end segments extrapolate).
+ * n_points == 0: vacuum (mu = 0).  Otherwise n_points >= 2, energy strictly increasing, mu > 0. */
+typedef struct mcx_material {
+  int64_t n_points;
+  const double* energy_keV; /* HOST [n_points] */
+  const double* mu_per_m;   /* HOST [n_points] */
+} mcx_material;
+
+/* One solid of a MCX_SOLIDS group (step 8).  Its pose is absolute (lab), like a component's. */
+typedef struct mcx_solid {
+  int32_t shape;    /* mcx_shape */
+  int32_t material; /* index into the materials array */
+  int32_t priority; /* the highest priority owns an overlap; equal priorities: the earlier solid wins */
+  int32_t reserved;
+  mcx_pose pose;
+  double dims[3];          /* BOX: half extents x,y,z.  CYLINDER (axis = local y): radius, half height.  SPHERE: radius */
+  int64_t n_vertices;      /* MESH only */
+  int64_t n_triangles;     /* MESH only; closed, outward-wound */
+  const double* vertices;  /* HOST [n_vertices][3], solid-local frame */
+  const int32_t* triangles;/* HOST [n_triangles][3] */
+} mcx_solid;
+
+typedef struct mcx_source_params {
+  int32_t pos_mode, dir_mode, energy_mode, reserved;
+  double radius;             /* POS_DISK */
+  double sigma_x, sigma_y;   /* POS_GAUSS */
+  double target_w, target_h, target_dist; /* DIR_TARGET: uniform in area on a rectangle at z = target_dist */
+  double div_x, div_y;       /* DIR_GAUSS: sigma of the direction tangents */
+  double e0;                 /* E_MONO / E_UNIFORM centre */
+  double de_rel;             /* E_UNIFORM: E = e0 (1 + de_rel (2u - 1)) */
+  double spec_emin, spec_emax; /* E_SPECTRUM: bins of equal width over [emin, emax] */
+  int64_t spec_n;
+  const double* spectrum;    /* HOST [spec_n], non-negative bin weights */
+} mcx_source_params;
+
+typedef struct mcx_slit_params {
+  double xw, yh;  /* SLIT_RECT full widths */
+  double radius;  /* SLIT_CIRC */
+} mcx_slit_params;
+
+typedef struct mcx_solids_params {
+  int64_t n_solids;         /* <= MCX_MAX_SOLIDS */
+  const mcx_solid* solids;  /* HOST [n_solids] */
+} mcx_solids_params;
+
+typedef struct mcx_voxels_params {
+  double h;                 /* voxel edge; the component origin is the outer corner of voxel (0,0,0) */
+  int64_t nx, ny, nz;
+  const uint8_t* ids;       /* DEVICE [nz][ny][nx], x fastest; values index the materials array.
+                               Read once by create (copied into the workspace in the traversal layout). */
+} mcx_voxels_params;
+
+typedef struct mcx_mirror_params {
+  double p, q, theta;       /* source distance, image distance, grazing angle at the pole */
+  double length, width;     /* along the local z (tangential) and x (sagittal) axes; local y = surface normal */
+  double theta_min, theta_max, e_min, e_max; /* uniform reflectivity grid */
+  int64_t n_theta, n_e;
+  const double* reflectivity; /* HOST [n_theta][n_e] */
+} mcx_mirror_params;
+
+typedef struct mcx_crystal_params {
+  double length, width;     /* along local z and x; the reflecting surface is the plane y = 0, normal +y */
+  double d_hkl;             /* Angstrom */
+  double zeta;              /* relative Darwin width: w_D = zeta tan(theta_B) */
+  double delta0;            /* refraction offset of the curve centre, radians */
+} mcx_crystal_params;
+
+typedef struct mcx_detector_params {
+  double xmin, xmax, ymin, ymax, emin, emax; /* half-open bins */
+  int64_t nx, ny, ne;
+} mcx_detector_params;
+
+typedef struct mcx_component {
+  int32_t kind; /* mcx_kind */
+  int32_t reserved;
+  mcx_pose pose;
+  union {
+    mcx_source_params source;
+    mcx_slit_params slit;
+    mcx_solids_params solids;
+    mcx_voxels_params voxels;
+    mcx_mirror_params mirror;
+    mcx_crystal_params crystal;
+    mcx_detector_params detector;
+  } u;
+} mcx_component;
+
+/* Per-ray record written by mcx_trace_dump (per-ray branch parity). */
+typedef struct mcx_ray_fate {
+  int32_t fate;  /* MCX_FATE_* or the chain index of the absorbing component */
+  int32_t reserved;
+  int64_t bin;   /* bin in the last detector if fate == MCX_FATE_DETECTED, else -1 */
+  double p;      /* final weight */
+} mcx_ray_fate;
+
+/* Number of int64 counters mcx_counters_read writes: [0, n_components) absorbed per component, then
+ * detected, missed, degenerate, capacity_overflows. */
+#define MCX_N_COUNTERS(n_components) ((n_components) + 4)
+
+/* Bytes of device workspace mcx_instrument_create needs for this instrument (tables, BVH, re-laid voxel volume,
+ * tally records, counters).  Reads only sizes, never the HOST/DEVICE arrays. */
+mcx_status mcx_instrument_workspace_size(const mcx_component* components, int n_components,
+                                         const mcx_material* materials, int n_materials, size_t* bytes_out);
+
+/* Builds the device image of an instrument in `workspace` (DEVICE, caller-owned, 256-byte aligned, at least
+ * mcx_instrument_workspace_size bytes): ln-tables of mu(E), spectrum CDFs, mirror constants, a BVH per mesh,
+ * the voxel volume in its traversal layout; zeroes tallies and counters.  HOST inputs are consumed before return. */
+mcx_status mcx_instrument_create(const mcx_component* components, int n_components,
+                                 const mcx_material* materials, int n_materials,
+                                 void* workspace, size_t workspace_bytes, void* cuda_stream,
+                                 mcx_instrument** out);
+
+/* Traces rays with indices [0, n_rays) (mcx_trace) or [first_ray, first_ray + n_rays) (mcx_trace_range).
+ * Ray i draws from Philox4x32-10 with key = seed and counter = (i lo, i hi, slot, component index), so a ray is
+ * a pure function of (instrument, seed, i).  Tallies and counters ACCUMULATE over calls; weights are not divided
+ * by n_rays. */
+mcx_status mcx_trace(mcx_instrument* inst, uint64_t n_rays, uint64_t seed, void* cuda_stream);
+mcx_status mcx_trace_range(mcx_instrument* inst, uint64_t first_ray, uint64_t n_rays, uint64_t seed,
+                           void* cuda_stream);
+
+/* Finalises detector `detector` (ordinal among MCX_DETECTOR components): writes N (ray counts), p (sum of
+ * weights) and p2 (sum of squared weights) for all bins, bin = (iy * nx + ix) * ne + ie.
+ * N, p, p2: DEVICE [n_bins]; n_bins must equal nx*ny*ne. */
+mcx_status mcx_tally_read(mcx_instrument* inst, int detector, uint64_t* N, double* p, double* p2, size_t n_bins,
+                          void* cuda_stream);
+
+/* Zeroes all tallies and counters. */
+mcx_status mcx_tally_reset(mcx_instrument* inst, void* cuda_stream);
+
+/* Copies the MCX_N_COUNTERS(n_components) ray-accounting counters to `counters` (DEVICE [n]).  Their sum over
+ * absorbed + detected + missed + degenerate equals the number of rays traced since the last reset. */
+mcx_status mcx_counters_read(mcx_instrument* inst, uint64_t* counters, int n, void* cuda_stream);
+
+/* Traces rays [first_ray, first_ray + n_rays) and writes one record per ray to `out` (DEVICE [n_rays]) instead of
+ * tallying: tallies and counters are left untouched.  For parity tests. */
+mcx_status mcx_trace_dump(mcx_instrument* inst, uint64_t first_ray, uint64_t n_rays, uint64_t seed,
+                          mcx_ray_fate* out, void* cuda_stream);
+
+/* Number of kernel launches this handle has enqueued so far (create, trace, read, reset). */
+uint64_t mcx_launch_count(const mcx_instrument* inst);
+
+/* Sustained-FP64 probe used for the ALU roofline: enqueues a kernel in which every thread of a
+ * (n_blocks x 256) grid runs n_iters x 8 dependent-chain-free DFMAs; `sink` is DEVICE [n_blocks*256] doubles.
+ * Lane-ops performed = n_blocks * 256 * n_iters * 8. */
+mcx_status mcx_probe_dfma(double* sink, int n_blocks, int64_t n_iters, void* cuda_stream);
+
+void mcx_instrument_destroy(mcx_instrument* inst);
+
+const char* mcx_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MCX_H_ */

@@ -1,0 +1,338 @@
+"""ctypes binding of libmcx_b200.so (include/mcx.h).  Argument marshalling only: every step of the hot path runs
+in the CUDA kernels.  PyTorch is used for device memory and streams, nothing else.
+
+The instrument descriptions come from the `workloads` module (plain dicts of numbers and numpy arrays).
+There is no CPU fallback: if the library is missing or no CUDA device is present, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+MCX_OK = 0
+STATUS_NAMES = {0: "MCX_OK", 1: "MCX_ERR_INVALID_ARG", 2: "MCX_ERR_UNSUPPORTED", 3: "MCX_ERR_RANGE", 4: "MCX_ERR_WORKSPACE",
+                5: "MCX_ERR_CUDA", 6: "MCX_ERR_CAPACITY"}
+KIND = {"source": 0, "slit_rect": 1, "slit_circ": 2, "solids": 3, "voxels": 4, "mirror": 5, "crystal": 6, "detector": 7}
+POS_MODE = {"point": 0, "disk": 1, "gauss": 2}
+DIR_MODE = {"target": 0, "gauss": 1}
+ENERGY_MODE = {"mono": 0, "uniform": 1, "spectrum": 2}
+SHAPE = {"box": 0, "cyl": 1, "sphere": 2, "mesh": 3}
+FATE_DETECTED, FATE_MISSED, FATE_DEGENERATE = -1, -2, -3
+
+EXPORTS = ["mcx_instrument_workspace_size", "mcx_instrument_create", "mcx_trace", "mcx_trace_range", "mcx_tally_read",
+           "mcx_tally_reset", "mcx_counters_read", "mcx_trace_dump", "mcx_launch_count", "mcx_probe_dfma",
+           "mcx_instrument_destroy", "mcx_last_error"]
+
+_dp = C.POINTER(C.c_double)
+_u64p = C.POINTER(C.c_uint64)
+
+
+class McxPose(C.Structure):
+    _fields_ = [("rot", C.c_double * 9), ("origin", C.c_double * 3)]
+
+
+class McxMaterial(C.Structure):
+    _fields_ = [("n_points", C.c_int64), ("energy_keV", _dp), ("mu_per_m", _dp)]
+
+
+class McxSolid(C.Structure):
+    _fields_ = [("shape", C.c_int32), ("material", C.c_int32), ("priority", C.c_int32), ("reserved", C.c_int32),
+                ("pose", McxPose), ("dims", C.c_double * 3), ("n_vertices", C.c_int64), ("n_triangles", C.c_int64),
+                ("vertices", _dp), ("triangles", C.POINTER(C.c_int32))]
+
+
+class McxSourceParams(C.Structure):
+    _fields_ = [("pos_mode", C.c_int32), ("dir_mode", C.c_int32), ("energy_mode", C.c_int32), ("reserved", C.c_int32),
+                ("radius", C.c_double), ("sigma_x", C.c_double), ("sigma_y", C.c_double),
+                ("target_w", C.c_double), ("target_h", C.c_double), ("target_dist", C.c_double),
+                ("div_x", C.c_double), ("div_y", C.c_double), ("e0", C.c_double), ("de_rel", C.c_double),
+                ("spec_emin", C.c_double), ("spec_emax", C.c_double), ("spec_n", C.c_int64), ("spectrum", _dp)]
+
+
+class McxSlitParams(C.Structure):
+    _fields_ = [("xw", C.c_double), ("yh", C.c_double), ("radius", C.c_double)]
+
+
+class McxSolidsParams(C.Structure):
+    _fields_ = [("n_solids", C.c_int64), ("solids", C.POINTER(McxSolid))]
+
+
+class McxVoxelsParams(C.Structure):
+    _fields_ = [("h", C.c_double), ("nx", C.c_int64), ("ny", C.c_int64), ("nz", C.c_int64), ("ids", C.c_void_p)]
+
+
+class McxMirrorParams(C.Structure):
+    _fields_ = [("p", C.c_double), ("q", C.c_double), ("theta", C.c_double), ("length", C.c_double), ("width", C.c_double),
+                ("theta_min", C.c_double), ("theta_max", C.c_double), ("e_min", C.c_double), ("e_max", C.c_double),
+                ("n_theta", C.c_int64), ("n_e", C.c_int64), ("reflectivity", _dp)]
+
+
+class McxCrystalParams(C.Structure):
+    _fields_ = [("length", C.c_double), ("width", C.c_double), ("d_hkl", C.c_double), ("zeta", C.c_double),
+                ("delta0", C.c_double)]
+
+
+class McxDetectorParams(C.Structure):
+    _fields_ = [("xmin", C.c_double), ("xmax", C.c_double), ("ymin", C.c_double), ("ymax", C.c_double),
+                ("emin", C.c_double), ("emax", C.c_double), ("nx", C.c_int64), ("ny", C.c_int64), ("ne", C.c_int64)]
+
+
+class McxParamsUnion(C.Union):
+    _fields_ = [("source", McxSourceParams), ("slit", McxSlitParams), ("solids", McxSolidsParams),
+                ("voxels", McxVoxelsParams), ("mirror", McxMirrorParams), ("crystal", McxCrystalParams),
+                ("detector", McxDetectorParams)]
+
+
+class McxComponent(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("reserved", C.c_int32), ("pose", McxPose), ("u", McxParamsUnion)]
+
+
+FATE_DTYPE = np.dtype([("fate", np.int32), ("reserved", np.int32), ("bin", np.int64), ("p", np.float64)])
+
+_libs = {}
+
+
+def lib(strict=False):
+    """Loads (building first if needed) libmcx_b200.so and declares the prototypes of include/mcx.h.
+    strict=True loads the -fmad=false build of the same sources (parity diagnostics, reading R20)."""
+    if strict in _libs:
+        return _libs[strict]
+    path = _build.build(strict=strict)
+    if not os.path.exists(path):
+        raise RuntimeError("libmcx_b200.so is missing and could not be built; there is no CPU fallback")
+    L = C.CDLL(path)
+    cp, vp = C.POINTER(McxComponent), C.c_void_p
+    mp = C.POINTER(McxMaterial)
+    L.mcx_instrument_workspace_size.argtypes = [cp, C.c_int, mp, C.c_int, C.POINTER(C.c_size_t)]
+    L.mcx_instrument_create.argtypes = [cp, C.c_int, mp, C.c_int, vp, C.c_size_t, vp, C.POINTER(vp)]
+    L.mcx_trace.argtypes = [vp, C.c_uint64, C.c_uint64, vp]
+    L.mcx_trace_range.argtypes = [vp, C.c_uint64, C.c_uint64, C.c_uint64, vp]
+    L.mcx_tally_read.argtypes = [vp, C.c_int, vp, vp, vp, C.c_size_t, vp]
+    L.mcx_tally_reset.argtypes = [vp, vp]
+    L.mcx_counters_read.argtypes = [vp, vp, C.c_int, vp]
+    L.mcx_trace_dump.argtypes = [vp, C.c_uint64, C.c_uint64, C.c_uint64, vp, vp]
+    L.mcx_launch_count.argtypes = [vp]
+    L.mcx_launch_count.restype = C.c_uint64
+    L.mcx_probe_dfma.argtypes = [vp, C.c_int, C.c_int64, vp]
+    L.mcx_instrument_destroy.argtypes = [vp]
+    L.mcx_instrument_destroy.restype = None
+    L.mcx_last_error.restype = C.c_char_p
+    for name in ("mcx_instrument_workspace_size", "mcx_instrument_create", "mcx_trace", "mcx_trace_range",
+                 "mcx_tally_read", "mcx_tally_reset", "mcx_counters_read", "mcx_trace_dump", "mcx_probe_dfma"):
+        getattr(L, name).restype = C.c_int
+    _libs[strict] = L
+    return L
+
+
+class McxError(RuntimeError):
+    def __init__(self, status, message):
+        super().__init__(f"{STATUS_NAMES.get(status, status)}: {message}")
+        self.status = status
+
+
+def _check(status, L=None):
+    if status != MCX_OK:
+        raise McxError(status, (L or lib()).mcx_last_error().decode("utf-8", "replace"))
+
+
+def _set_pose(pose, d):
+    R = np.ascontiguousarray(d["R"], dtype=np.float64).reshape(9)
+    T = np.ascontiguousarray(d["T"], dtype=np.float64).reshape(3)
+    pose.rot[:] = R.tolist()
+    pose.origin[:] = T.tolist()
+
+
+def _ptr(a, typ=_dp):
+    return a.ctypes.data_as(typ)
+
+
+def marshal(inst, keep, device_voxels):
+    """workloads dict -> (McxComponent array, McxMaterial array).  `keep` collects the host buffers that must live
+    until create returns; `device_voxels(ids_numpy)` uploads a voxel volume and returns its device pointer."""
+    comps = (McxComponent * len(inst["components"]))()
+    for c, cd in zip(comps, inst["components"]):
+        k = cd["kind"]
+        c.kind = KIND[k]
+        _set_pose(c.pose, cd)
+        if k == "source":
+            s = c.u.source
+            s.pos_mode, s.dir_mode, s.energy_mode = POS_MODE[cd["pos_mode"]], DIR_MODE[cd["dir_mode"]], ENERGY_MODE[cd["e_mode"]]
+            s.radius, s.sigma_x, s.sigma_y = cd["radius"], cd["sigma_x"], cd["sigma_y"]
+            s.target_w, s.target_h, s.target_dist = cd["target_w"], cd["target_h"], cd["target_dist"]
+            s.div_x, s.div_y, s.e0, s.de_rel = cd["div_x"], cd["div_y"], cd["E0"], cd["dE_rel"]
+            s.spec_emin, s.spec_emax = cd["spec_Emin"], cd["spec_Emax"]
+            if cd["spectrum"] is not None:
+                sp = np.ascontiguousarray(cd["spectrum"], dtype=np.float64)
+                keep.append(sp)
+                s.spec_n, s.spectrum = len(sp), _ptr(sp)
+        elif k == "slit_rect":
+            c.u.slit.xw, c.u.slit.yh = cd["xw"], cd["yh"]
+        elif k == "slit_circ":
+            c.u.slit.radius = cd["radius"]
+        elif k == "solids":
+            arr = (McxSolid * max(1, len(cd["solids"])))()
+            for s, sd in zip(arr, cd["solids"]):
+                s.shape, s.material, s.priority = SHAPE[sd["shape"]], sd["material"], sd["priority"]
+                _set_pose(s.pose, sd)
+                if sd["shape"] == "box":
+                    s.dims[:] = list(sd["half"])
+                elif sd["shape"] == "cyl":
+                    s.dims[:] = [sd["radius"], sd["half_height"], 0.0]
+                elif sd["shape"] == "sphere":
+                    s.dims[:] = [sd["radius"], 0.0, 0.0]
+                else:
+                    v = np.ascontiguousarray(sd["verts"], dtype=np.float64)
+                    t = np.ascontiguousarray(sd["tris"], dtype=np.int32)
+                    keep += [v, t]
+                    s.n_vertices, s.n_triangles = len(v), len(t)
+                    s.vertices, s.triangles = _ptr(v), _ptr(t, C.POINTER(C.c_int32))
+            keep.append(arr)
+            c.u.solids.n_solids, c.u.solids.solids = len(cd["solids"]), arr
+        elif k == "voxels":
+            ids = np.ascontiguousarray(cd["ids"], dtype=np.uint8)
+            v = c.u.voxels
+            v.h = cd["h"]
+            v.nz, v.ny, v.nx = ids.shape
+            v.ids = device_voxels(ids)
+        elif k == "mirror":
+            m, t = c.u.mirror, cd["table"]
+            m.p, m.q, m.theta, m.length, m.width = cd["p"], cd["q"], cd["theta"], cd["length"], cd["width"]
+            m.theta_min, m.theta_max, m.e_min, m.e_max = t["theta_min"], t["theta_max"], t["E_min"], t["E_max"]
+            Rt = np.ascontiguousarray(t["R"], dtype=np.float64)
+            keep.append(Rt)
+            m.n_theta, m.n_e, m.reflectivity = t["n_theta"], t["n_E"], _ptr(Rt)
+        elif k == "crystal":
+            x = c.u.crystal
+            x.length, x.width, x.d_hkl, x.zeta, x.delta0 = cd["length"], cd["width"], cd["d_hkl"], cd["zeta"], cd["delta0"]
+        elif k == "detector":
+            d = c.u.detector
+            d.xmin, d.xmax, d.ymin, d.ymax = cd["xmin"], cd["xmax"], cd["ymin"], cd["ymax"]
+            d.emin, d.emax, d.nx, d.ny, d.ne = cd["Emin"], cd["Emax"], cd["nx"], cd["ny"], cd["nE"]
+        else:
+            raise ValueError(f"unknown component kind {k!r}")
+    mats = (McxMaterial * max(1, len(inst["materials"])))()
+    for m, md in zip(mats, inst["materials"]):
+        if md is None:
+            m.n_points = 0
+            continue
+        E = np.ascontiguousarray(md["E"], dtype=np.float64)
+        mu = np.ascontiguousarray(md["mu"], dtype=np.float64)
+        keep += [E, mu]
+        m.n_points, m.energy_keV, m.mu_per_m = len(E), _ptr(E), _ptr(mu)
+    return comps, mats
+
+
+class Instrument:
+    """A device-resident instrument (mcx_instrument handle + the torch buffers it lives in)."""
+
+    def __init__(self, inst, device="cuda:0", strict=False):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("no CUDA device: the mcx hot path has no CPU fallback")
+        self.torch = torch
+        self.device = torch.device(device)
+        self.inst = inst
+        self.n_rays, self.seed = inst["n_rays"], inst["seed"]
+        self.dets = [c for c in inst["components"] if c["kind"] == "detector"]
+        self.n_comps, self.n_mats = len(inst["components"]), len(inst["materials"])
+        self._keep, self._dev = [], []
+        self.handle = None
+        L = self.L = lib(strict)
+
+        def device_voxels(ids):
+            t = torch.from_numpy(ids).to(self.device)
+            self._dev.append(t)
+            return t.data_ptr()
+
+        with torch.cuda.device(self.device):
+            comps, mats = marshal(inst, self._keep, device_voxels)
+            nbytes = C.c_size_t()
+            _check(L.mcx_instrument_workspace_size(comps, self.n_comps, mats, self.n_mats, C.byref(nbytes)), L)
+            self.workspace_bytes = nbytes.value
+            self.workspace = torch.empty(self.workspace_bytes + 256, dtype=torch.uint8, device=self.device)
+            base = (self.workspace.data_ptr() + 255) // 256 * 256
+            h = C.c_void_p()
+            _check(L.mcx_instrument_create(comps, self.n_comps, mats, self.n_mats, base, self.workspace_bytes,
+                                           self._stream(), C.byref(h)), L)
+            self.handle = h
+            torch.cuda.current_stream().synchronize()
+        self._keep.clear()   # HOST inputs are consumed by create
+        self._dev.clear()    # the voxel volume was copied into the workspace
+
+    def _stream(self):
+        return C.c_void_p(self.torch.cuda.current_stream(self.device).cuda_stream)
+
+    def trace(self, n_rays=None, seed=None, first=0):
+        """mcx_trace_range: enqueue rays [first, first+n_rays) on the current stream (asynchronous)."""
+        n = self.n_rays if n_rays is None else int(n_rays)
+        s = self.seed if seed is None else int(seed)
+        _check(self.L.mcx_trace_range(self.handle, int(first), n, s, self._stream()), self.L)
+
+    def tally(self, detector=0, out=None):
+        """mcx_tally_read -> (N uint64-as-int64, p, p2) device tensors of n_bins."""
+        torch = self.torch
+        d = self.dets[detector]
+        nb = d["nx"] * d["ny"] * d["nE"]
+        if out is None:
+            out = (torch.empty(nb, dtype=torch.int64, device=self.device), torch.empty(nb, dtype=torch.float64, device=self.device),
+                   torch.empty(nb, dtype=torch.float64, device=self.device))
+        N, P, P2 = out
+        _check(self.L.mcx_tally_read(self.handle, detector, N.data_ptr(), P.data_ptr(), P2.data_ptr(), nb, self._stream()), self.L)
+        return N, P, P2
+
+    def reset(self):
+        _check(self.L.mcx_tally_reset(self.handle, self._stream()), self.L)
+
+    def counters(self):
+        """mcx_counters_read -> dict(absorbed=[n_comps], detected, missed, degenerate, overflows); synchronises."""
+        torch = self.torch
+        n = self.n_comps + 4
+        buf = torch.empty(n, dtype=torch.int64, device=self.device)
+        _check(self.L.mcx_counters_read(self.handle, buf.data_ptr(), n, self._stream()), self.L)
+        v = buf.cpu().numpy()
+        return {"absorbed": v[:self.n_comps].copy(), "detected": int(v[self.n_comps]), "missed": int(v[self.n_comps + 1]),
+                "degenerate": int(v[self.n_comps + 2]), "overflows": int(v[self.n_comps + 3])}
+
+    def trace_dump(self, first, n_rays, seed=None):
+        """mcx_trace_dump -> numpy structured array (fate, bin, p) per ray; synchronises."""
+        torch = self.torch
+        s = self.seed if seed is None else int(seed)
+        buf = torch.empty(max(1, int(n_rays)) * FATE_DTYPE.itemsize, dtype=torch.uint8, device=self.device)
+        _check(self.L.mcx_trace_dump(self.handle, int(first), int(n_rays), s, buf.data_ptr(), self._stream()), self.L)
+        return buf.cpu().numpy()[:int(n_rays) * FATE_DTYPE.itemsize].view(FATE_DTYPE)
+
+    def launch_count(self):
+        return int(self.L.mcx_launch_count(self.handle))
+
+    def close(self):
+        if self.handle is not None:
+            self.torch.cuda.synchronize(self.device)
+            self.L.mcx_instrument_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def probe_dfma(n_blocks, n_iters, device="cuda:0"):
+    """mcx_probe_dfma: returns the sustained FP64 rate in lane-ops (DFMA) per second, CUDA-event timed."""
+    import torch
+    dev = torch.device(device)
+    with torch.cuda.device(dev):
+        sink = torch.empty(n_blocks * 256, dtype=torch.float64, device=dev)
+        st = C.c_void_p(torch.cuda.current_stream(dev).cuda_stream)
+        _check(lib().mcx_probe_dfma(sink.data_ptr(), n_blocks, n_iters // 4, st))
+        torch.cuda.synchronize(dev)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        _check(lib().mcx_probe_dfma(sink.data_ptr(), n_blocks, n_iters, st))
+        e1.record()
+        torch.cuda.synchronize(dev)
+        return n_blocks * 256 * n_iters * 8 / (e0.elapsed_time(e1) * 1e-3)

@@ -1,0 +1,144 @@
+// mcx_device.h -- device-side image of an instrument (what mcx_instrument_create packs into the workspace) and
+// the host-side launch interface between mcx_host.cu and mcx_kernels.cu.  Product code: shares nothing with
+// oracle/.  Step numbers refer to DESIGN.md "Readings".
+#ifndef MCX_DEVICE_H_
+#define MCX_DEVICE_H_
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/mcx.h"
+
+namespace mcx {
+
+struct DPose {
+  double R[9];
+  double T[3];
+};
+
+// mu(E) of one material as ln-tables (step 7); slope[j] = (lnMu[j+1]-lnMu[j]) / (lnE[j+1]-lnE[j]).
+struct DMaterial {
+  int n;  // 0 = vacuum
+  int pad;
+  const double* E;
+  const double* lnE;
+  const double* lnMu;
+  const double* slope;
+  double inv_dlnE;  // (n-1) / (lnE[n-1]-lnE[0]): first guess of the segment, verified against E[]
+};
+
+struct DSource {
+  int pos_mode, dir_mode, e_mode, spec_n;
+  double radius, sigma_x, sigma_y;
+  double target_w, target_h, target_dist, div_x, div_y;
+  double e0, de_rel, spec_emin, spec_bin_w;
+  const double* cdf;  // [spec_n + 1] running sum of the spectrum
+};
+
+struct DSlit {
+  double half_x, half_y, radius2;
+};
+
+// BVH2 node, 32 bytes.  Boxes are fp32, rounded outward and padded; they only select candidate triangles, the
+// exact fp64 triangle test decides.  Leaf: count > 0, first = first triangle; inner: count == 0, first = index of
+// the left child, right child = first + 1.
+struct BvhNode {
+  float lo[3];
+  int first;
+  float hi[3];
+  int count;
+};
+
+struct DSolid {
+  int shape, material, priority, n_tris;
+  DPose pose;
+  double dims[3];
+  double root_lo[3], root_hi[3];  // fp64 AABB of the mesh (solid-local)
+  const BvhNode* nodes;
+  const double* tris;  // [n_tris][9] vertices in BVH leaf order
+};
+
+struct DSolids {
+  int n_solids, n_mesh;
+  const DSolid* solids;
+};
+
+struct DVoxels {
+  double h;
+  int n[3];       // nx, ny, nz
+  int fast;       // axis stored fastest in the traversal layout
+  int a1, a2;     // the other two axes: address = (i[a2] * n[a1] + i[a1]) * pitch + i[fast]
+  int pitch;      // n[fast] rounded up to a multiple of 16
+  const uint8_t* ids;
+};
+
+struct DMirror {
+  double a, b, inv_a2, inv_b2;
+  double Z0, Y0, nZ, nY, tZ, tY;
+  double half_length, half_width;
+  double theta_min, theta_max, e_min, e_max;
+  int n_theta, n_e;
+  const double* table;
+};
+
+struct DCrystal {
+  double half_length, half_width, d_hkl, zeta, delta0;
+};
+
+struct DDetector {
+  double xmin, xmax, ymin, ymax, emin, emax;
+  int nx, ny, ne, index;
+  uint64_t n_bins;
+};
+
+struct DComponent {
+  int kind;
+  int pad;
+  DPose pose;
+  union {
+    DSource source;
+    DSlit slit;
+    DSolids solids;
+    DVoxels voxels;
+    DMirror mirror;
+    DCrystal crystal;
+    DDetector detector;
+  } u;
+};
+
+// One tally record = one 32-byte sector: a detected ray touches exactly one sector.
+struct TallyBin {
+  unsigned long long N;
+  double P;
+  double P2;
+  unsigned long long pad;
+};
+
+enum { CNT_DETECTED = 0, CNT_MISSED = 1, CNT_DEGENERATE = 2, CNT_OVERFLOW = 3 };
+
+struct alignas(16) DInstrument {
+  int n_comps, n_mats, n_dets, features;
+  DComponent comps[MCX_MAX_COMPONENTS];
+  DMaterial mats[MCX_MAX_MATERIALS];
+  TallyBin* tallies[MCX_MAX_DETECTORS];
+  unsigned long long* counters;  // [n_comps + 4]
+};
+
+static_assert(sizeof(DInstrument) % 16 == 0, "copied to shared memory as int4");
+static_assert(sizeof(TallyBin) == 32, "one tally record per 32-byte sector");
+
+// feature bits: select the kernel instantiation (code for absent component kinds is compiled out)
+enum { F_SOLIDS = 1, F_MESH = 2, F_VOXELS = 4, F_OPTICS = 8, F_ALL = 15 };
+
+// ---- launch interface (defined in mcx_kernels.cu) ----
+cudaError_t launch_trace(const DInstrument* d_inst, int features, int n_mats, uint64_t first, uint64_t n, uint64_t seed,
+                         mcx_ray_fate* dump, cudaStream_t stream);
+cudaError_t launch_tally_read(const TallyBin* bins, uint64_t n_bins, unsigned long long* N, double* p, double* p2,
+                              cudaStream_t stream);
+cudaError_t launch_voxel_relayout(const uint8_t* src, uint8_t* dst, int nx, int ny, int nz, int fast, int a1, int a2,
+                                  int pitch, cudaStream_t stream);
+cudaError_t launch_probe_dfma(double* sink, int n_blocks, long long n_iters, cudaStream_t stream);
+cudaError_t kernels_init();
+
+}  // namespace mcx
+#endif

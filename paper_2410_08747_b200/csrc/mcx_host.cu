@@ -1,0 +1,584 @@
+// mcx_host.cu -- the C ABI of include/mcx.h: validation, host-side precomputation (ln-tables, spectrum CDFs,
+// mirror constants, BVH build), packing of the device image into the caller's workspace, and kernel launches.
+// Product code: shares nothing with oracle/.
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <new>
+#include <vector>
+
+#include "mcx_device.h"
+
+using namespace mcx;
+
+struct mcx_instrument {
+  DInstrument host_image;            // what sits at workspace offset 0
+  std::vector<unsigned char> blob;   // host copy of the table section (kept alive for the async H2D copy)
+  unsigned char* workspace = nullptr;
+  size_t workspace_bytes = 0;
+  size_t zero_begin = 0, zero_end = 0;  // tallies + counters
+  int n_comps = 0, n_mats = 0, n_dets = 0, features = 0;
+  uint64_t det_bins[MCX_MAX_DETECTORS] = {0, 0, 0, 0};
+  uint64_t launches = 0;
+};
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+mcx_status fail(mcx_status s, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+  return s;
+}
+
+mcx_status cuda_fail(cudaError_t e, const char* what) {
+  return fail(MCX_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+constexpr size_t kAlign = 256;
+size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
+
+// Bump allocator over the workspace.  The same sequence of reserve() calls is made by the size query and by
+// create, so both arrive at the same offsets.
+struct Arena {
+  size_t top = 0;
+  size_t reserve(size_t bytes) {
+    const size_t off = top;
+    top = align_up(top + bytes);
+    return off;
+  }
+};
+
+bool pose_ok(const mcx_pose& P) {
+  for (int k = 0; k < 9; ++k) if (!std::isfinite(P.rot[k])) return false;
+  for (int k = 0; k < 3; ++k) if (!std::isfinite(P.origin[k])) return false;
+  return true;
+}
+
+void copy_pose(DPose* d, const mcx_pose& s) {
+  std::memcpy(d->R, s.rot, sizeof(d->R));
+  std::memcpy(d->T, s.origin, sizeof(d->T));
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// BVH over one mesh: top-down, median split of the triangle centroids along the widest axis, <= 4 triangles
+// per leaf.  Node boxes are stored in fp32 rounded outward and padded by 2^-16 of the mesh scale, far above the
+// fp32 rounding of the box walk (<= a few 2^-24 of the scale), so the walk never loses a triangle the exact
+// fp64 test would hit.
+// ---------------------------------------------------------------------------------------------------------
+struct TriRef {
+  double c[3], lo[3], hi[3];
+  int idx;
+};
+
+float round_down(double x) {
+  float f = (float)x;
+  if ((double)f > x) f = std::nextafterf(f, -std::numeric_limits<float>::infinity());
+  return f;
+}
+float round_up(double x) {
+  float f = (float)x;
+  if ((double)f < x) f = std::nextafterf(f, std::numeric_limits<float>::infinity());
+  return f;
+}
+
+struct BvhBuilder {
+  std::vector<TriRef>& refs;
+  std::vector<BvhNode>& nodes;
+  double pad;
+  void build(int node, int begin, int end) {
+    double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+    double clo[3] = {1e300, 1e300, 1e300}, chi[3] = {-1e300, -1e300, -1e300};
+    for (int k = begin; k < end; ++k)
+      for (int a = 0; a < 3; ++a) {
+        lo[a] = std::min(lo[a], refs[k].lo[a]); hi[a] = std::max(hi[a], refs[k].hi[a]);
+        clo[a] = std::min(clo[a], refs[k].c[a]); chi[a] = std::max(chi[a], refs[k].c[a]);
+      }
+    for (int a = 0; a < 3; ++a) {
+      nodes[node].lo[a] = round_down(lo[a] - pad);
+      nodes[node].hi[a] = round_up(hi[a] + pad);
+    }
+    const int count = end - begin;
+    if (count <= 4) {
+      nodes[node].first = begin;
+      nodes[node].count = count;
+      return;
+    }
+    int axis = 0;
+    if (chi[1] - clo[1] > chi[axis] - clo[axis]) axis = 1;
+    if (chi[2] - clo[2] > chi[axis] - clo[axis]) axis = 2;
+    const int mid = begin + count / 2;
+    std::nth_element(refs.begin() + begin, refs.begin() + mid, refs.begin() + end,
+                     [axis](const TriRef& x, const TriRef& y) { return x.c[axis] < y.c[axis]; });
+    const int left = (int)nodes.size();
+    nodes.push_back(BvhNode{});
+    nodes.push_back(BvhNode{});
+    nodes[node].first = left;
+    nodes[node].count = 0;
+    build(left, begin, mid);
+    build(left + 1, mid, end);
+  }
+};
+
+size_t bvh_node_bound(int64_t n_tris) { return (size_t)(2 * n_tris + 2); }
+
+// sizes and offsets of everything in the workspace
+struct Plan {
+  size_t off_inst = 0;
+  size_t blob_begin = 0, blob_end = 0;  // tables, built on the host
+  size_t off_voxels[MCX_MAX_COMPONENTS];
+  size_t off_tally[MCX_MAX_DETECTORS];
+  size_t off_counters = 0;
+  size_t zero_begin = 0, zero_end = 0;
+  size_t total = 0;
+  // blob offsets
+  size_t off_mat[MCX_MAX_MATERIALS];      // 4 arrays of n doubles each
+  size_t off_cdf[MCX_MAX_COMPONENTS];
+  size_t off_table[MCX_MAX_COMPONENTS];
+  size_t off_solids[MCX_MAX_COMPONENTS];  // DSolid array
+  size_t off_nodes[MCX_MAX_COMPONENTS][MCX_MAX_SOLIDS];
+  size_t off_tris[MCX_MAX_COMPONENTS][MCX_MAX_SOLIDS];
+};
+
+int voxel_pitch(int64_t n_fast) { return (int)((n_fast + 15) / 16 * 16); }
+
+// chooses the axis stored fastest: the voxel axis most aligned with the line from the source to the volume centre
+void voxel_axes(const mcx_component& src, const mcx_component& vox, int* fast, int* a1, int* a2) {
+  const mcx_voxels_params& V = vox.u.voxels;
+  const double half[3] = {0.5 * V.nx * V.h, 0.5 * V.ny * V.h, 0.5 * V.nz * V.h};
+  // volume centre in lab coordinates: origin + R^T half
+  double dirl[3];
+  for (int a = 0; a < 3; ++a) {
+    double c = vox.pose.origin[a];
+    for (int k = 0; k < 3; ++k) c += vox.pose.rot[3 * k + a] * half[k];
+    dirl[a] = c - src.pose.origin[a];
+  }
+  double best = -1.0;
+  *fast = 2;
+  for (int k = 0; k < 3; ++k) {
+    const double comp = std::fabs(vox.pose.rot[3 * k] * dirl[0] + vox.pose.rot[3 * k + 1] * dirl[1] + vox.pose.rot[3 * k + 2] * dirl[2]);
+    if (comp > best) { best = comp; *fast = k; }
+  }
+  *a1 = (*fast + 1) % 3;
+  *a2 = (*fast + 2) % 3;
+  if (*a1 > *a2) std::swap(*a1, *a2);
+}
+
+mcx_status make_plan(const mcx_component* comps, int n_comps, const mcx_material* mats, int n_mats, Plan* P) {
+  if (!comps || n_comps < 1) return fail(MCX_ERR_INVALID_ARG, "no components");
+  if (n_comps > MCX_MAX_COMPONENTS) return fail(MCX_ERR_UNSUPPORTED, "more than %d components", MCX_MAX_COMPONENTS);
+  if (n_mats < 0 || n_mats > MCX_MAX_MATERIALS) return fail(MCX_ERR_UNSUPPORTED, "more than %d materials", MCX_MAX_MATERIALS);
+  if (n_mats > 0 && !mats) return fail(MCX_ERR_INVALID_ARG, "materials is null");
+  if (comps[0].kind != MCX_SOURCE) return fail(MCX_ERR_INVALID_ARG, "component 0 must be a source");
+  Arena A;
+  P->off_inst = A.reserve(sizeof(DInstrument));
+  P->blob_begin = A.top;
+  for (int m = 0; m < n_mats; ++m) {
+    if (mats[m].n_points < 0 || mats[m].n_points == 1) return fail(MCX_ERR_INVALID_ARG, "material %d: n_points must be 0 or >= 2", m);
+    P->off_mat[m] = A.reserve((size_t)mats[m].n_points * 4 * sizeof(double));
+  }
+  int n_dets = 0;
+  for (int c = 0; c < n_comps; ++c) {
+    const mcx_component& C = comps[c];
+    if (c > 0 && C.kind == MCX_SOURCE) return fail(MCX_ERR_INVALID_ARG, "component %d: only component 0 may be a source", c);
+    if (!pose_ok(C.pose)) return fail(MCX_ERR_INVALID_ARG, "component %d: pose is not finite", c);
+    switch (C.kind) {
+      case MCX_SOURCE:
+        if (C.u.source.energy_mode == MCX_E_SPECTRUM) {
+          if (C.u.source.spec_n < 1) return fail(MCX_ERR_INVALID_ARG, "source: empty spectrum");
+          P->off_cdf[c] = A.reserve((size_t)(C.u.source.spec_n + 1) * sizeof(double));
+        }
+        break;
+      case MCX_SLIT_RECT: case MCX_SLIT_CIRC: case MCX_CRYSTAL_BRAGG: break;
+      case MCX_SOLIDS: {
+        const mcx_solids_params& G = C.u.solids;
+        if (G.n_solids < 0 || G.n_solids > MCX_MAX_SOLIDS) return fail(MCX_ERR_UNSUPPORTED, "component %d: more than %d solids", c, MCX_MAX_SOLIDS);
+        if (G.n_solids > 0 && !G.solids) return fail(MCX_ERR_INVALID_ARG, "component %d: solids is null", c);
+        P->off_solids[c] = A.reserve((size_t)std::max<int64_t>(G.n_solids, 1) * sizeof(DSolid));
+        for (int64_t s = 0; s < G.n_solids; ++s)
+          if (G.solids[s].shape == MCX_MESH) {
+            if (G.solids[s].n_triangles < 1 || G.solids[s].n_vertices < 3) return fail(MCX_ERR_INVALID_ARG, "component %d solid %d: empty mesh", c, (int)s);
+            P->off_nodes[c][s] = A.reserve(bvh_node_bound(G.solids[s].n_triangles) * sizeof(BvhNode));
+            P->off_tris[c][s] = A.reserve((size_t)G.solids[s].n_triangles * 9 * sizeof(double));
+          }
+        break;
+      }
+      case MCX_VOXELS: break;  // below, outside the blob
+      case MCX_MIRROR_ELLIPTIC:
+        if (C.u.mirror.n_theta < 2 || C.u.mirror.n_e < 2) return fail(MCX_ERR_INVALID_ARG, "component %d: reflectivity grid needs >= 2x2 points", c);
+        P->off_table[c] = A.reserve((size_t)C.u.mirror.n_theta * C.u.mirror.n_e * sizeof(double));
+        break;
+      case MCX_DETECTOR:
+        if (n_dets >= MCX_MAX_DETECTORS) return fail(MCX_ERR_UNSUPPORTED, "more than %d detectors", MCX_MAX_DETECTORS);
+        if (C.u.detector.nx < 1 || C.u.detector.ny < 1 || C.u.detector.ne < 1) return fail(MCX_ERR_INVALID_ARG, "component %d: empty detector", c);
+        ++n_dets;
+        break;
+      default: return fail(MCX_ERR_INVALID_ARG, "component %d: unknown kind %d", c, C.kind);
+    }
+  }
+  P->blob_end = A.top;
+  for (int c = 0; c < n_comps; ++c)
+    if (comps[c].kind == MCX_VOXELS) {
+      const mcx_voxels_params& V = comps[c].u.voxels;
+      if (V.nx < 1 || V.ny < 1 || V.nz < 1 || V.nx > 4096 || V.ny > 4096 || V.nz > 4096 || !(V.h > 0.0))
+        return fail(MCX_ERR_INVALID_ARG, "component %d: bad voxel grid", c);
+      int f, a1, a2;
+      voxel_axes(comps[0], comps[c], &f, &a1, &a2);
+      const int64_t n[3] = {V.nx, V.ny, V.nz};
+      P->off_voxels[c] = A.reserve((size_t)n[a2] * n[a1] * voxel_pitch(n[f]));
+    }
+  P->zero_begin = A.top;
+  int d = 0;
+  for (int c = 0; c < n_comps; ++c)
+    if (comps[c].kind == MCX_DETECTOR) {
+      const mcx_detector_params& D = comps[c].u.detector;
+      P->off_tally[d++] = A.reserve((size_t)D.nx * D.ny * D.ne * sizeof(TallyBin));
+    }
+  P->off_counters = A.reserve((size_t)MCX_N_COUNTERS(n_comps) * sizeof(unsigned long long));
+  P->zero_end = A.top;
+  P->total = A.top;
+  return MCX_OK;
+}
+
+mcx_status check_sticky() {
+  const cudaError_t e = cudaPeekAtLastError();
+  if (e != cudaSuccess) return cuda_fail(e, "earlier CUDA error");
+  return MCX_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* mcx_last_error(void) { return g_err; }
+
+mcx_status mcx_instrument_workspace_size(const mcx_component* components, int n_components, const mcx_material* materials,
+                                         int n_materials, size_t* bytes_out) {
+  if (!bytes_out) return fail(MCX_ERR_INVALID_ARG, "bytes_out is null");
+  Plan P;
+  const mcx_status s = make_plan(components, n_components, materials, n_materials, &P);
+  if (s != MCX_OK) return s;
+  *bytes_out = P.total;
+  return MCX_OK;
+}
+
+mcx_status mcx_instrument_create(const mcx_component* components, int n_components, const mcx_material* materials,
+                                 int n_materials, void* workspace, size_t workspace_bytes, void* cuda_stream,
+                                 mcx_instrument** out) {
+  if (!out) return fail(MCX_ERR_INVALID_ARG, "out is null");
+  *out = nullptr;
+  Plan P;
+  mcx_status st = make_plan(components, n_components, materials, n_materials, &P);
+  if (st != MCX_OK) return st;
+  if (!workspace || ((uintptr_t)workspace % kAlign) != 0) return fail(MCX_ERR_WORKSPACE, "workspace is null or not 256-byte aligned");
+  if (workspace_bytes < P.total) return fail(MCX_ERR_WORKSPACE, "workspace has %zu bytes, %zu needed", workspace_bytes, P.total);
+  if ((st = check_sticky()) != MCX_OK) return st;
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  unsigned char* ws = (unsigned char*)workspace;
+
+  mcx_instrument* H = new (std::nothrow) mcx_instrument();
+  if (!H) return fail(MCX_ERR_INVALID_ARG, "out of host memory");
+  H->workspace = ws;
+  H->workspace_bytes = workspace_bytes;
+  H->n_comps = n_components;
+  H->n_mats = n_materials;
+  H->zero_begin = P.zero_begin;
+  H->zero_end = P.zero_end;
+  H->blob.assign(P.blob_end - P.blob_begin, 0);
+  unsigned char* blob = H->blob.data();
+  auto host_ptr = [&](size_t off) { return blob + (off - P.blob_begin); };
+  auto dev_ptr = [&](size_t off) { return ws + off; };
+  DInstrument& I = H->host_image;
+  std::memset(&I, 0, sizeof(I));
+  I.n_comps = n_components;
+  I.n_mats = n_materials;
+  int features = 0;
+
+#define MCX_BAIL(status, ...) do { const mcx_status s_ = fail(status, __VA_ARGS__); delete H; return s_; } while (0)
+
+  // ---- materials: ln-tables (step 7) ----
+  for (int m = 0; m < n_materials; ++m) {
+    const mcx_material& M = materials[m];
+    DMaterial& D = I.mats[m];
+    D.n = (int)M.n_points;
+    if (M.n_points == 0) continue;
+    if (!M.energy_keV || !M.mu_per_m) MCX_BAIL(MCX_ERR_INVALID_ARG, "material %d: null table", m);
+    const size_t n = (size_t)M.n_points;
+    double* E = (double*)host_ptr(P.off_mat[m]);
+    double* lnE = E + n;
+    double* lnMu = lnE + n;
+    double* slope = lnMu + n;
+    for (size_t j = 0; j < n; ++j) {
+      if (!(M.energy_keV[j] > 0.0) || !(M.mu_per_m[j] > 0.0)) MCX_BAIL(MCX_ERR_RANGE, "material %d: non-positive table entry %zu", m, j);
+      if (j > 0 && !(M.energy_keV[j] > M.energy_keV[j - 1])) MCX_BAIL(MCX_ERR_RANGE, "material %d: energies not increasing at %zu", m, j);
+      E[j] = M.energy_keV[j];
+      lnE[j] = std::log(M.energy_keV[j]);
+      lnMu[j] = std::log(M.mu_per_m[j]);
+    }
+    for (size_t j = 0; j + 1 < n; ++j) slope[j] = (lnMu[j + 1] - lnMu[j]) / (lnE[j + 1] - lnE[j]);
+    slope[n - 1] = 0.0;
+    D.E = (const double*)dev_ptr(P.off_mat[m]);
+    D.lnE = D.E + n;
+    D.lnMu = D.lnE + n;
+    D.slope = D.lnMu + n;
+    D.inv_dlnE = (double)(n - 1) / (lnE[n - 1] - lnE[0]);
+  }
+
+  int n_dets = 0;
+  for (int c = 0; c < n_components; ++c) {
+    const mcx_component& C = components[c];
+    DComponent& D = I.comps[c];
+    D.kind = C.kind;
+    copy_pose(&D.pose, C.pose);
+    switch (C.kind) {
+      case MCX_SOURCE: {
+        const mcx_source_params& S = C.u.source;
+        DSource& d = D.u.source;
+        if (S.pos_mode < 0 || S.pos_mode > 2 || S.dir_mode < 0 || S.dir_mode > 1 || S.energy_mode < 0 || S.energy_mode > 2)
+          MCX_BAIL(MCX_ERR_INVALID_ARG, "source: bad mode");
+        d.pos_mode = S.pos_mode; d.dir_mode = S.dir_mode; d.e_mode = S.energy_mode;
+        d.radius = S.radius; d.sigma_x = S.sigma_x; d.sigma_y = S.sigma_y;
+        d.target_w = S.target_w; d.target_h = S.target_h; d.target_dist = S.target_dist;
+        d.div_x = S.div_x; d.div_y = S.div_y; d.e0 = S.e0; d.de_rel = S.de_rel;
+        if (S.energy_mode == MCX_E_SPECTRUM) {
+          if (!S.spectrum) MCX_BAIL(MCX_ERR_INVALID_ARG, "source: spectrum is null");
+          if (!(S.spec_emax > S.spec_emin)) MCX_BAIL(MCX_ERR_RANGE, "source: empty spectrum range");
+          double* cdf = (double*)host_ptr(P.off_cdf[c]);
+          cdf[0] = 0.0;
+          for (int64_t j = 0; j < S.spec_n; ++j) {  // plain running sum (step 3)
+            if (!(S.spectrum[j] >= 0.0)) MCX_BAIL(MCX_ERR_RANGE, "source: negative spectrum bin %lld", (long long)j);
+            cdf[j + 1] = cdf[j] + S.spectrum[j];
+          }
+          if (!(cdf[S.spec_n] > 0.0)) MCX_BAIL(MCX_ERR_RANGE, "source: spectrum sums to zero");
+          d.spec_n = (int)S.spec_n;
+          d.spec_emin = S.spec_emin;
+          d.spec_bin_w = (S.spec_emax - S.spec_emin) / (double)S.spec_n;
+          d.cdf = (const double*)dev_ptr(P.off_cdf[c]);
+        }
+        break;
+      }
+      case MCX_SLIT_RECT:
+        D.u.slit.half_x = 0.5 * C.u.slit.xw;
+        D.u.slit.half_y = 0.5 * C.u.slit.yh;
+        break;
+      case MCX_SLIT_CIRC:
+        D.u.slit.radius2 = C.u.slit.radius * C.u.slit.radius;
+        break;
+      case MCX_SOLIDS: {
+        features |= F_SOLIDS;
+        const mcx_solids_params& G = C.u.solids;
+        DSolid* hs = (DSolid*)host_ptr(P.off_solids[c]);
+        D.u.solids.n_solids = (int)G.n_solids;
+        D.u.solids.solids = (const DSolid*)dev_ptr(P.off_solids[c]);
+        for (int64_t s = 0; s < G.n_solids; ++s) {
+          const mcx_solid& S = G.solids[s];
+          DSolid& d = hs[s];
+          if (S.shape < 0 || S.shape > 3) MCX_BAIL(MCX_ERR_INVALID_ARG, "component %d solid %d: bad shape", c, (int)s);
+          if (S.material < 0 || S.material >= n_materials) MCX_BAIL(MCX_ERR_INVALID_ARG, "component %d solid %d: material out of range", c, (int)s);
+          if (!pose_ok(S.pose)) MCX_BAIL(MCX_ERR_INVALID_ARG, "component %d solid %d: pose is not finite", c, (int)s);
+          d.shape = S.shape; d.material = S.material; d.priority = S.priority;
+          copy_pose(&d.pose, S.pose);
+          for (int k = 0; k < 3; ++k) d.dims[k] = S.dims[k];
+          if (S.shape != MCX_MESH) continue;
+          features |= F_MESH;
+          D.u.solids.n_mesh++;
+          if (!S.vertices || !S.triangles) MCX_BAIL(MCX_ERR_INVALID_ARG, "component %d solid %d: null mesh arrays", c, (int)s);
+          const int nt = (int)S.n_triangles;
+          std::vector<TriRef> refs((size_t)nt);
+          double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+          for (int t = 0; t < nt; ++t) {
+            TriRef& r = refs[t];
+            r.idx = t;
+            for (int a = 0; a < 3; ++a) { r.lo[a] = 1e300; r.hi[a] = -1e300; r.c[a] = 0.0; }
+            for (int v = 0; v < 3; ++v) {
+              const int32_t vi = S.triangles[3 * (size_t)t + v];
+              if (vi < 0 || vi >= S.n_vertices) MCX_BAIL(MCX_ERR_INVALID_ARG, "component %d solid %d: vertex index out of range", c, (int)s);
+              for (int a = 0; a < 3; ++a) {
+                const double x = S.vertices[3 * (size_t)vi + a];
+                r.lo[a] = std::min(r.lo[a], x); r.hi[a] = std::max(r.hi[a], x); r.c[a] += x / 3.0;
+              }
+            }
+            for (int a = 0; a < 3; ++a) { lo[a] = std::min(lo[a], r.lo[a]); hi[a] = std::max(hi[a], r.hi[a]); }
+          }
+          double scale = 0.0;
+          for (int a = 0; a < 3; ++a) scale = std::max(scale, std::max(std::fabs(lo[a]), std::fabs(hi[a])));
+          const double pad = scale * (1.0 / 65536.0);
+          std::vector<BvhNode> nodes;
+          nodes.reserve(bvh_node_bound(nt));
+          nodes.push_back(BvhNode{});
+          BvhBuilder B{refs, nodes, pad};
+          B.build(0, 0, nt);
+          if (nodes.size() > bvh_node_bound(nt)) MCX_BAIL(MCX_ERR_UNSUPPORTED, "BVH node bound exceeded");
+          std::memcpy(host_ptr(P.off_nodes[c][s]), nodes.data(), nodes.size() * sizeof(BvhNode));
+          double* tri = (double*)host_ptr(P.off_tris[c][s]);
+          for (int t = 0; t < nt; ++t)
+            for (int v = 0; v < 3; ++v)
+              for (int a = 0; a < 3; ++a)
+                tri[9 * (size_t)t + 3 * v + a] = S.vertices[3 * (size_t)S.triangles[3 * (size_t)refs[t].idx + v] + a];
+          for (int a = 0; a < 3; ++a) { d.root_lo[a] = lo[a] - pad; d.root_hi[a] = hi[a] + pad; }
+          d.n_tris = nt;
+          d.nodes = (const BvhNode*)dev_ptr(P.off_nodes[c][s]);
+          d.tris = (const double*)dev_ptr(P.off_tris[c][s]);
+        }
+        break;
+      }
+      case MCX_VOXELS: {
+        features |= F_VOXELS;
+        const mcx_voxels_params& V = C.u.voxels;
+        if (!V.ids) MCX_BAIL(MCX_ERR_INVALID_ARG, "component %d: ids is null", c);
+        DVoxels& d = D.u.voxels;
+        d.h = V.h;
+        d.n[0] = (int)V.nx; d.n[1] = (int)V.ny; d.n[2] = (int)V.nz;
+        voxel_axes(components[0], C, &d.fast, &d.a1, &d.a2);
+        d.pitch = voxel_pitch(d.n[d.fast]);
+        d.ids = (const uint8_t*)dev_ptr(P.off_voxels[c]);
+        const cudaError_t e = launch_voxel_relayout(V.ids, (uint8_t*)dev_ptr(P.off_voxels[c]), d.n[0], d.n[1], d.n[2], d.fast,
+                                                    d.a1, d.a2, d.pitch, stream);
+        if (e != cudaSuccess) { const mcx_status s_ = cuda_fail(e, "voxel relayout"); delete H; return s_; }
+        H->launches++;
+        break;
+      }
+      case MCX_MIRROR_ELLIPTIC: {
+        features |= F_OPTICS;
+        const mcx_mirror_params& M = C.u.mirror;
+        DMirror& d = D.u.mirror;
+        if (!M.reflectivity) MCX_BAIL(MCX_ERR_INVALID_ARG, "component %d: reflectivity is null", c);
+        if (!(M.p > 0.0) || !(M.q > 0.0) || !(M.theta > 0.0)) MCX_BAIL(MCX_ERR_INVALID_ARG, "component %d: p, q, theta must be positive", c);
+        if (!(M.theta_max > M.theta_min) || !(M.e_max > M.e_min)) MCX_BAIL(MCX_ERR_RANGE, "component %d: empty reflectivity grid", c);
+        // step 12: ellipse with foci at the source and image points, pole at distance p from the first focus
+        d.a = 0.5 * (M.p + M.q);
+        d.b = std::sqrt(M.p * M.q) * std::sin(M.theta);
+        d.inv_a2 = 1.0 / (d.a * d.a);
+        d.inv_b2 = 1.0 / (d.b * d.b);
+        const double cfoc = std::sqrt(d.a * d.a - d.b * d.b);
+        d.Z0 = (M.p - d.a) * d.a / cfoc;
+        d.Y0 = -d.b * std::sqrt(1.0 - (d.Z0 * d.Z0) / (d.a * d.a));
+        const double gZ = d.Z0 / (d.a * d.a), gY = d.Y0 / (d.b * d.b);
+        const double gn = std::sqrt(gZ * gZ + gY * gY);
+        d.nZ = -gZ / gn; d.nY = -gY / gn;
+        d.tZ = d.nY; d.tY = -d.nZ;
+        d.half_length = 0.5 * M.length; d.half_width = 0.5 * M.width;
+        d.theta_min = M.theta_min; d.theta_max = M.theta_max; d.e_min = M.e_min; d.e_max = M.e_max;
+        d.n_theta = (int)M.n_theta; d.n_e = (int)M.n_e;
+        std::memcpy(host_ptr(P.off_table[c]), M.reflectivity, (size_t)M.n_theta * M.n_e * sizeof(double));
+        d.table = (const double*)dev_ptr(P.off_table[c]);
+        break;
+      }
+      case MCX_CRYSTAL_BRAGG: {
+        features |= F_OPTICS;
+        const mcx_crystal_params& X = C.u.crystal;
+        if (!(X.d_hkl > 0.0) || !(X.zeta > 0.0)) MCX_BAIL(MCX_ERR_INVALID_ARG, "component %d: d_hkl and zeta must be positive", c);
+        D.u.crystal.half_length = 0.5 * X.length; D.u.crystal.half_width = 0.5 * X.width;
+        D.u.crystal.d_hkl = X.d_hkl; D.u.crystal.zeta = X.zeta; D.u.crystal.delta0 = X.delta0;
+        break;
+      }
+      case MCX_DETECTOR: {
+        const mcx_detector_params& T = C.u.detector;
+        if (!(T.xmax > T.xmin) || !(T.ymax > T.ymin) || !(T.emax > T.emin)) MCX_BAIL(MCX_ERR_RANGE, "component %d: empty detector range", c);
+        DDetector& d = D.u.detector;
+        d.xmin = T.xmin; d.xmax = T.xmax; d.ymin = T.ymin; d.ymax = T.ymax; d.emin = T.emin; d.emax = T.emax;
+        d.nx = (int)T.nx; d.ny = (int)T.ny; d.ne = (int)T.ne; d.index = n_dets;
+        d.n_bins = (uint64_t)T.nx * T.ny * T.ne;
+        H->det_bins[n_dets] = d.n_bins;
+        I.tallies[n_dets] = (TallyBin*)dev_ptr(P.off_tally[n_dets]);
+        ++n_dets;
+        break;
+      }
+    }
+  }
+#undef MCX_BAIL
+  // voxel IDs must index the materials array; the kernel sizes its per-thread mu[] by n_materials
+  I.n_dets = n_dets;
+  I.features = features;
+  I.counters = (unsigned long long*)dev_ptr(P.off_counters);
+  H->n_dets = n_dets;
+  H->features = features;
+
+  cudaError_t e = cudaMemcpyAsync(ws + P.off_inst, &H->host_image, sizeof(DInstrument), cudaMemcpyHostToDevice, stream);
+  if (e == cudaSuccess && !H->blob.empty())
+    e = cudaMemcpyAsync(ws + P.blob_begin, H->blob.data(), H->blob.size(), cudaMemcpyHostToDevice, stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(ws + P.zero_begin, 0, P.zero_end - P.zero_begin, stream);
+  if (e != cudaSuccess) { const mcx_status s_ = cuda_fail(e, "upload of the instrument image"); delete H; return s_; }
+  *out = H;
+  return MCX_OK;
+}
+
+mcx_status mcx_trace_range(mcx_instrument* inst, uint64_t first_ray, uint64_t n_rays, uint64_t seed, void* cuda_stream) {
+  if (!inst) return fail(MCX_ERR_INVALID_ARG, "inst is null");
+  mcx_status st = check_sticky();
+  if (st != MCX_OK) return st;
+  const cudaError_t e = launch_trace((const DInstrument*)inst->workspace, inst->features, inst->n_mats, first_ray, n_rays, seed,
+                                     nullptr, (cudaStream_t)cuda_stream);
+  if (e != cudaSuccess) return cuda_fail(e, "trace launch");
+  if (n_rays) inst->launches++;
+  return MCX_OK;
+}
+
+mcx_status mcx_trace(mcx_instrument* inst, uint64_t n_rays, uint64_t seed, void* cuda_stream) {
+  return mcx_trace_range(inst, 0, n_rays, seed, cuda_stream);
+}
+
+mcx_status mcx_trace_dump(mcx_instrument* inst, uint64_t first_ray, uint64_t n_rays, uint64_t seed, mcx_ray_fate* out,
+                          void* cuda_stream) {
+  if (!inst) return fail(MCX_ERR_INVALID_ARG, "inst is null");
+  if (!out && n_rays) return fail(MCX_ERR_INVALID_ARG, "out is null");
+  mcx_status st = check_sticky();
+  if (st != MCX_OK) return st;
+  const cudaError_t e = launch_trace((const DInstrument*)inst->workspace, inst->features, inst->n_mats, first_ray, n_rays, seed,
+                                     out, (cudaStream_t)cuda_stream);
+  if (e != cudaSuccess) return cuda_fail(e, "trace_dump launch");
+  if (n_rays) inst->launches++;
+  return MCX_OK;
+}
+
+mcx_status mcx_tally_read(mcx_instrument* inst, int detector, uint64_t* N, double* p, double* p2, size_t n_bins,
+                          void* cuda_stream) {
+  if (!inst) return fail(MCX_ERR_INVALID_ARG, "inst is null");
+  if (detector < 0 || detector >= inst->n_dets) return fail(MCX_ERR_INVALID_ARG, "detector %d out of range (%d detectors)", detector, inst->n_dets);
+  if (!N || !p || !p2) return fail(MCX_ERR_INVALID_ARG, "null output array");
+  if ((uint64_t)n_bins != inst->det_bins[detector]) return fail(MCX_ERR_INVALID_ARG, "n_bins is %zu, detector has %llu", n_bins, (unsigned long long)inst->det_bins[detector]);
+  mcx_status st = check_sticky();
+  if (st != MCX_OK) return st;
+  const cudaError_t e = launch_tally_read(inst->host_image.tallies[detector], n_bins, (unsigned long long*)N, p, p2, (cudaStream_t)cuda_stream);
+  if (e != cudaSuccess) return cuda_fail(e, "tally_read launch");
+  inst->launches++;
+  return MCX_OK;
+}
+
+mcx_status mcx_tally_reset(mcx_instrument* inst, void* cuda_stream) {
+  if (!inst) return fail(MCX_ERR_INVALID_ARG, "inst is null");
+  mcx_status st = check_sticky();
+  if (st != MCX_OK) return st;
+  const cudaError_t e = cudaMemsetAsync(inst->workspace + inst->zero_begin, 0, inst->zero_end - inst->zero_begin, (cudaStream_t)cuda_stream);
+  if (e != cudaSuccess) return cuda_fail(e, "tally reset");
+  return MCX_OK;
+}
+
+mcx_status mcx_counters_read(mcx_instrument* inst, uint64_t* counters, int n, void* cuda_stream) {
+  if (!inst) return fail(MCX_ERR_INVALID_ARG, "inst is null");
+  if (!counters || n != MCX_N_COUNTERS(inst->n_comps)) return fail(MCX_ERR_INVALID_ARG, "counters must hold %d values", MCX_N_COUNTERS(inst->n_comps));
+  mcx_status st = check_sticky();
+  if (st != MCX_OK) return st;
+  const cudaError_t e = cudaMemcpyAsync(counters, inst->host_image.counters, (size_t)n * sizeof(uint64_t), cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream);
+  if (e != cudaSuccess) return cuda_fail(e, "counters copy");
+  return MCX_OK;
+}
+
+uint64_t mcx_launch_count(const mcx_instrument* inst) { return inst ? inst->launches : 0; }
+
+mcx_status mcx_probe_dfma(double* sink, int n_blocks, int64_t n_iters, void* cuda_stream) {
+  if (!sink || n_blocks < 1 || n_iters < 0) return fail(MCX_ERR_INVALID_ARG, "bad probe arguments");
+  const cudaError_t e = launch_probe_dfma(sink, n_blocks, (long long)n_iters, (cudaStream_t)cuda_stream);
+  if (e != cudaSuccess) return cuda_fail(e, "probe launch");
+  return MCX_OK;
+}
+
+void mcx_instrument_destroy(mcx_instrument* inst) { delete inst; }
+
+}  // extern "C"

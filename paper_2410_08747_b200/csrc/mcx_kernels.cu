@@ -1,0 +1,841 @@
+// mcx_kernels.cu -- the ray-tracing megakernel and its helper kernels, hand-written for sm_100a.
+//
+// One thread traces one ray at a time through the whole component chain with its state (r, d, E, p) in fp64
+// registers; a grid of 148 x k blocks strides over the ray-index range.  Step numbers are
+// those of DESIGN.md "Readings".  This file shares no code with oracle/.
+#include <math_constants.h>
+
+#include "mcx_device.h"
+
+namespace mcx {
+
+namespace {
+
+constexpr int kBlock = 256;
+constexpr int kMaxIntervals = 32;  // per ray and solids group
+constexpr int kMaxHits = 32;       // per ray and mesh
+constexpr int kBvhStack = 64;
+
+// ------------------------------------------------------------------------------------------------------------
+// Step 1: Philox4x32-10 (Salmon et al., SC'11); key = seed, counter = (i lo, i hi, slot, component).
+// ------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1,
+                                              uint32_t (&out)[4]) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+    const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+    c0 = hi1 ^ c1 ^ k0;
+    c1 = lo1;
+    c2 = hi0 ^ c3 ^ k1;
+    c3 = lo0;
+    k0 += 0x9E3779B9u;
+    k1 += 0xBB67AE85u;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// Step 2: the top 52 bits of (wa:wb), centred in their cell: u = (m + 1/2) 2^-52, exact in fp64.
+// Built as [1 + m 2^-52] - [1 - 2^-53]; both the operand and the difference are exactly representable.
+__device__ __forceinline__ double u01(uint32_t wa, uint32_t wb) {
+  const double one_plus = __hiloint2double(0x3FF00000 | (int)(wa >> 12), (int)((wa << 20) | (wb >> 12)));
+  return one_plus - 0.99999999999999988897769753748434595763683319091796875;  // 1 - 2^-53
+}
+
+__device__ __forceinline__ void draw2(uint64_t seed, uint64_t i, uint32_t slot, uint32_t comp, double& ua, double& ub) {
+  uint32_t w[4];
+  philox4x32_10((uint32_t)i, (uint32_t)(i >> 32), slot, comp, (uint32_t)seed, (uint32_t)(seed >> 32), w);
+  ua = u01(w[0], w[1]);
+  ub = u01(w[2], w[3]);
+}
+
+// Box-Muller, both values used (step 2)
+__device__ __forceinline__ void gauss_pair(double ua, double ub, double& g0, double& g1) {
+  const double rad = sqrt(-2.0 * log(ua));
+  double s, c;
+  sincos(2.0 * CUDART_PI * ub, &s, &c);
+  g0 = rad * c;
+  g1 = rad * s;
+}
+
+struct Vec3 {
+  double x, y, z;
+};
+__device__ __forceinline__ Vec3 operator+(Vec3 a, Vec3 b) { return {a.x + b.x, a.y + b.y, a.z + b.z}; }
+__device__ __forceinline__ Vec3 operator-(Vec3 a, Vec3 b) { return {a.x - b.x, a.y - b.y, a.z - b.z}; }
+__device__ __forceinline__ Vec3 operator*(double s, Vec3 a) { return {s * a.x, s * a.y, s * a.z}; }
+__device__ __forceinline__ double dot(Vec3 a, Vec3 b) { return a.x * b.x + a.y * b.y + a.z * b.z; }
+
+// Step 4: into a component frame and back
+__device__ __forceinline__ Vec3 rotate(const double* R, Vec3 v) {
+  return {R[0] * v.x + R[1] * v.y + R[2] * v.z, R[3] * v.x + R[4] * v.y + R[5] * v.z, R[6] * v.x + R[7] * v.y + R[8] * v.z};
+}
+__device__ __forceinline__ Vec3 rotate_back(const double* R, Vec3 v) {
+  return {R[0] * v.x + R[3] * v.y + R[6] * v.z, R[1] * v.x + R[4] * v.y + R[7] * v.z, R[2] * v.x + R[5] * v.y + R[8] * v.z};
+}
+__device__ __forceinline__ Vec3 to_local(const DPose& P, Vec3 r) { return rotate(P.R, r - Vec3{P.T[0], P.T[1], P.T[2]}); }
+__device__ __forceinline__ Vec3 to_lab(const DPose& P, Vec3 r) { return rotate_back(P.R, r) + Vec3{P.T[0], P.T[1], P.T[2]}; }
+
+struct Ray {
+  Vec3 r, d;
+  double E, p;
+};
+
+// ------------------------------------------------------------------------------------------------------------
+// Step 3: source.  Slot 0 -> position, slot 1 -> direction, slot 2 -> energy.
+// ------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void sample_source(const DComponent& C, uint64_t seed, uint64_t i, Ray& ray) {
+  const DSource& S = C.u.source;
+  Vec3 r{0.0, 0.0, 0.0}, d;
+  double ua, ub;
+  if (S.pos_mode == MCX_POS_DISK) {
+    draw2(seed, i, 0u, 0u, ua, ub);
+    const double rad = S.radius * sqrt(ua);
+    double s, c;
+    sincos(2.0 * CUDART_PI * ub, &s, &c);
+    r = {rad * c, rad * s, 0.0};
+  } else if (S.pos_mode == MCX_POS_GAUSS) {
+    draw2(seed, i, 0u, 0u, ua, ub);
+    double g0, g1;
+    gauss_pair(ua, ub, g0, g1);
+    r = {S.sigma_x * g0, S.sigma_y * g1, 0.0};
+  }
+  draw2(seed, i, 1u, 0u, ua, ub);
+  Vec3 v;
+  if (S.dir_mode == MCX_DIR_TARGET) {  // uniform in area on the target rectangle, no solid-angle weight
+    v = Vec3{(ua - 0.5) * S.target_w, (ub - 0.5) * S.target_h, S.target_dist} - r;
+  } else {  // Gaussian tangents, then normalise
+    double g0, g1;
+    gauss_pair(ua, ub, g0, g1);
+    v = {S.div_x * g0, S.div_y * g1, 1.0};
+  }
+  d = (1.0 / sqrt(dot(v, v))) * v;
+  double E = S.e0;
+  if (S.e_mode == MCX_E_UNIFORM) {
+    draw2(seed, i, 2u, 0u, ua, ub);
+    E = S.e0 * (1.0 + S.de_rel * (2.0 * ua - 1.0));
+  } else if (S.e_mode == MCX_E_SPECTRUM) {  // inverse CDF, weight stays 1
+    draw2(seed, i, 2u, 0u, ua, ub);
+    const double* __restrict__ cdf = S.cdf;
+    const int n = S.spec_n;
+    const double v01 = ua * cdf[n];
+    // largest j in [0, n-1] with cdf[j] <= v01
+    int lo = 0, hi = n;  // invariant: cdf[lo] <= v01 (cdf[0] = 0), answer in [lo, hi)
+    while (hi - lo > 1) {
+      const int mid = (lo + hi) >> 1;
+      if (cdf[mid] <= v01) lo = mid; else hi = mid;
+    }
+    const double c0 = cdf[lo], c1 = cdf[lo + 1];
+    E = S.spec_emin + ((double)lo + (v01 - c0) / (c1 - c0)) * S.spec_bin_w;
+  }
+  ray.r = to_lab(C.pose, r);
+  ray.d = rotate_back(C.pose.R, d);
+  ray.E = E;
+  ray.p = 1.0;
+}
+
+// Step 5: intersection with the plane z' = 0 of a component frame
+__device__ __forceinline__ bool plane_hit(const DPose& P, const Ray& ray, Vec3& hit) {
+  const Vec3 o = to_local(P, ray.r);
+  const Vec3 d = rotate(P.R, ray.d);
+  if (!(d.z > 0.0)) return false;
+  const double t = -o.z / d.z;
+  if (t < 0.0) return false;
+  hit = o + t * d;
+  return true;
+}
+
+// Step 14: bin index or -1
+__device__ __forceinline__ long long detector_bin(const DComponent& C, const Ray& ray) {
+  const DDetector& D = C.u.detector;
+  Vec3 h;
+  if (!plane_hit(C.pose, ray, h)) return -1;
+  const double fx = floor((h.x - D.xmin) / (D.xmax - D.xmin) * (double)D.nx);
+  const double fy = floor((h.y - D.ymin) / (D.ymax - D.ymin) * (double)D.ny);
+  const double fe = floor((ray.E - D.emin) / (D.emax - D.emin) * (double)D.ne);
+  if (!(fx >= 0.0 && fx < (double)D.nx)) return -1;
+  if (!(fy >= 0.0 && fy < (double)D.ny)) return -1;
+  if (!(fe >= 0.0 && fe < (double)D.ne)) return -1;
+  return ((long long)fy * D.nx + (long long)fx) * D.ne + (long long)fe;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Step 7: mu(E) by log-log interpolation.  lnE = log(E) is computed once per ray by the caller.
+// ------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double mu_of(const DMaterial& M, double E, double lnE) {
+  const int n = M.n;
+  if (n == 0) return 0.0;
+  const double* __restrict__ Eg = M.E;
+  // segment j with Eg[j] <= E < Eg[j+1], clamped to [0, n-2]: guess from a uniform-in-lnE grid, then verify
+  int j = (int)((lnE - M.lnE[0]) * M.inv_dlnE);
+  j = max(0, min(j, n - 2));
+  if (Eg[j] <= E && (j == n - 2 || E < Eg[j + 1])) {
+    // guess was right
+  } else if (Eg[j] > E) {
+    if (j >= 2 && Eg[j - 1] <= E) {
+      j = j - 1;
+    } else if (j >= 1) {
+      int lo = 0, hi = j;  // answer in [lo, hi): largest k with Eg[k] <= E, or 0
+      while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (Eg[mid] <= E) lo = mid; else hi = mid;
+      }
+      j = lo;
+    }
+  } else {  // E >= Eg[j+1], j < n-2
+    if (j + 2 <= n - 2 && E < Eg[j + 2]) {
+      j = j + 1;
+    } else {
+      int lo = j + 1, hi = n - 1;  // largest k in [j+1, n-2] with Eg[k] <= E
+      while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (Eg[mid] <= E) lo = mid; else hi = mid;
+      }
+      j = lo;
+    }
+  }
+  return exp(M.lnMu[j] + (lnE - M.lnE[j]) * M.slope[j]);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Step 8: inside-interval of the ray parameter for the convex primitives, in the solid's own frame.
+// ------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ bool clip_axis(double o, double d, double lo, double hi, double& tmin, double& tmax) {
+  if (d == 0.0) return o > lo && o < hi;
+  const double ta = (lo - o) / d, tb = (hi - o) / d;
+  tmin = fmax(tmin, fmin(ta, tb));
+  tmax = fmin(tmax, fmax(ta, tb));
+  return true;
+}
+
+__device__ __forceinline__ bool primitive_interval(const DSolid& S, Vec3 o, Vec3 d, double& tin, double& tout) {
+  double tmin = -CUDART_INF, tmax = CUDART_INF;
+  if (S.shape == MCX_BOX) {
+    if (!clip_axis(o.x, d.x, -S.dims[0], S.dims[0], tmin, tmax)) return false;
+    if (!clip_axis(o.y, d.y, -S.dims[1], S.dims[1], tmin, tmax)) return false;
+    if (!clip_axis(o.z, d.z, -S.dims[2], S.dims[2], tmin, tmax)) return false;
+  } else if (S.shape == MCX_SPHERE) {
+    const double b = dot(o, d);
+    const double c = dot(o, o) - S.dims[0] * S.dims[0];
+    const double disc = b * b - c;
+    if (!(disc > 0.0)) return false;
+    const double s = sqrt(disc);
+    tmin = -b - s;
+    tmax = -b + s;
+  } else {  // finite cylinder, axis = local y
+    const double a = d.x * d.x + d.z * d.z;
+    const double c = o.x * o.x + o.z * o.z - S.dims[0] * S.dims[0];
+    if (a == 0.0) {
+      if (!(c < 0.0)) return false;
+    } else {
+      const double b = o.x * d.x + o.z * d.z;
+      const double disc = b * b - a * c;
+      if (!(disc > 0.0)) return false;
+      const double s = sqrt(disc);
+      tmin = (-b - s) / a;
+      tmax = (-b + s) / a;
+    }
+    if (!clip_axis(o.y, d.y, -S.dims[1], S.dims[1], tmin, tmax)) return false;
+  }
+  if (!(tmin < tmax)) return false;
+  tin = tmin;
+  tout = tmax;
+  return true;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Step 9: watertight ray/triangle test (Woop, Benthin, Wald 2013) in fp64.  The shear constants depend on the ray
+// only.  Every product and difference of the edge functions is rounded separately (__dmul_rn/__dsub_rn are never
+// contracted to FMA), so an edge shared by two triangles gives exactly negated values in both.
+// ------------------------------------------------------------------------------------------------------------
+struct Shear {
+  int kx, ky, kz;
+  double Sx, Sy, Sz;
+};
+
+__device__ __forceinline__ double pick(Vec3 v, int k) { return k == 0 ? v.x : (k == 1 ? v.y : v.z); }
+
+__device__ __forceinline__ Shear make_shear(Vec3 d) {
+  Shear s;
+  s.kz = 0;
+  double m = fabs(d.x);
+  if (fabs(d.y) > m) { s.kz = 1; m = fabs(d.y); }
+  if (fabs(d.z) > m) { s.kz = 2; }
+  s.kx = s.kz == 2 ? 0 : s.kz + 1;
+  s.ky = s.kx == 2 ? 0 : s.kx + 1;
+  const double dz = pick(d, s.kz);
+  if (dz < 0.0) { const int t = s.kx; s.kx = s.ky; s.ky = t; }
+  s.Sx = pick(d, s.kx) / dz;
+  s.Sy = pick(d, s.ky) / dz;
+  s.Sz = 1.0 / dz;
+  return s;
+}
+
+// returns 0 = miss, +1 = entering, -1 = exiting
+__device__ __forceinline__ int ray_triangle(const Shear& s, Vec3 o, const double* __restrict__ tri, double& t_out) {
+  const Vec3 A{tri[0] - o.x, tri[1] - o.y, tri[2] - o.z};
+  const Vec3 B{tri[3] - o.x, tri[4] - o.y, tri[5] - o.z};
+  const Vec3 C{tri[6] - o.x, tri[7] - o.y, tri[8] - o.z};
+  const double Akz = pick(A, s.kz), Bkz = pick(B, s.kz), Ckz = pick(C, s.kz);
+  const double Ax = __dsub_rn(pick(A, s.kx), __dmul_rn(s.Sx, Akz)), Ay = __dsub_rn(pick(A, s.ky), __dmul_rn(s.Sy, Akz));
+  const double Bx = __dsub_rn(pick(B, s.kx), __dmul_rn(s.Sx, Bkz)), By = __dsub_rn(pick(B, s.ky), __dmul_rn(s.Sy, Bkz));
+  const double Cx = __dsub_rn(pick(C, s.kx), __dmul_rn(s.Sx, Ckz)), Cy = __dsub_rn(pick(C, s.ky), __dmul_rn(s.Sy, Ckz));
+  const double U = __dsub_rn(__dmul_rn(Cx, By), __dmul_rn(Cy, Bx));
+  const double V = __dsub_rn(__dmul_rn(Ax, Cy), __dmul_rn(Ay, Cx));
+  const double W = __dsub_rn(__dmul_rn(Bx, Ay), __dmul_rn(By, Ax));
+  if ((U < 0.0 || V < 0.0 || W < 0.0) && (U > 0.0 || V > 0.0 || W > 0.0)) return 0;
+  const double det = __dadd_rn(__dadd_rn(U, V), W);
+  if (det == 0.0) return 0;
+  const double Az = __dmul_rn(s.Sz, Akz), Bz = __dmul_rn(s.Sz, Bkz), Cz = __dmul_rn(s.Sz, Ckz);
+  const double num = __dadd_rn(__dadd_rn(__dmul_rn(U, Az), __dmul_rn(V, Bz)), __dmul_rn(W, Cz));
+  t_out = num / det;
+  return det > 0.0 ? 1 : -1;
+}
+
+struct Interval {
+  double a, b;
+  int solid;
+};
+
+// All hits of the full line with one mesh via its BVH, sorted, duplicate-collapsed and paired into intervals.
+// Returns 1 = ok, 0 = degenerate sequence, -1 = capacity overflow.
+__device__ int mesh_intervals(const DSolid& S, int solid, Vec3 o, Vec3 d, Interval* iv, int& n_iv) {
+  // clip the line to the mesh box in fp64; the fp32 box walk uses a ray re-origined at the box entry so that
+  // its rounding errors scale with the mesh size, not with the distance to the source
+  double tmin = -CUDART_INF, tmax = CUDART_INF;
+  if (!clip_axis(o.x, d.x, S.root_lo[0], S.root_hi[0], tmin, tmax)) return 1;
+  if (!clip_axis(o.y, d.y, S.root_lo[1], S.root_hi[1], tmin, tmax)) return 1;
+  if (!clip_axis(o.z, d.z, S.root_lo[2], S.root_hi[2], tmin, tmax)) return 1;
+  if (!(tmin < tmax)) return 1;
+  const Vec3 e = o + tmin * d;
+  const float ox = (float)e.x, oy = (float)e.y, oz = (float)e.z;
+  const float big = 3.0e38f;
+  const float ix = d.x != 0.0 ? (float)(1.0 / d.x) : big, iy = d.y != 0.0 ? (float)(1.0 / d.y) : big,
+              iz = d.z != 0.0 ? (float)(1.0 / d.z) : big;
+  const Shear sh = make_shear(d);
+  double ht[kMaxHits];
+  signed char ho[kMaxHits];
+  int nh = 0;
+  bool overflow = false;
+  int stack[kBvhStack];
+  int sp = 0;
+  int node = 0;
+  const BvhNode* __restrict__ nodes = S.nodes;
+  while (true) {
+    const BvhNode nd = nodes[node];
+    // slab test of the full line against the padded fp32 box (no t range: the line is tested, as in step 9)
+    const float tx0 = (nd.lo[0] - ox) * ix, tx1 = (nd.hi[0] - ox) * ix;
+    const float ty0 = (nd.lo[1] - oy) * iy, ty1 = (nd.hi[1] - oy) * iy;
+    const float tz0 = (nd.lo[2] - oz) * iz, tz1 = (nd.hi[2] - oz) * iz;
+    const float tn = fmaxf(fmaxf(fminf(tx0, tx1), fminf(ty0, ty1)), fminf(tz0, tz1));
+    const float tf = fminf(fminf(fmaxf(tx0, tx1), fmaxf(ty0, ty1)), fmaxf(tz0, tz1));
+    bool pop = true;
+    if (tn <= tf) {
+      if (nd.count > 0) {
+        for (int k = 0; k < nd.count; ++k) {
+          double t;
+          const int r = ray_triangle(sh, o, S.tris + 9 * (size_t)(nd.first + k), t);
+          if (r != 0) {
+            if (nh < kMaxHits) { ht[nh] = t; ho[nh] = (signed char)r; ++nh; } else overflow = true;
+          }
+        }
+      } else {
+        if (sp < kBvhStack) stack[sp++] = nd.first + 1; else overflow = true;
+        node = nd.first;
+        pop = false;
+      }
+    }
+    if (pop) {
+      if (sp == 0) break;
+      node = stack[--sp];
+    }
+  }
+  if (overflow) return -1;
+  if (nh == 0) return 1;
+  // insertion sort by (t, enter before exit)
+  for (int a = 1; a < nh; ++a) {
+    const double t = ht[a];
+    const signed char orr = ho[a];
+    int b = a - 1;
+    while (b >= 0 && (ht[b] > t || (ht[b] == t && ho[b] < orr))) { ht[b + 1] = ht[b]; ho[b + 1] = ho[b]; --b; }
+    ht[b + 1] = t;
+    ho[b + 1] = orr;
+  }
+  // collapse consecutive same-orientation hits; what is left must alternate enter, exit, ...
+  int m = 0;
+  for (int a = 0; a < nh; ++a)
+    if (m == 0 || ho[m - 1] != ho[a]) { ht[m] = ht[a]; ho[m] = ho[a]; ++m; }
+  if ((m & 1) || ho[0] != 1) return 0;
+  for (int a = 0; a < m; a += 2) {
+    if (n_iv >= kMaxIntervals) return -1;
+    iv[n_iv++] = Interval{ht[a], ht[a + 1], solid};
+  }
+  return 1;
+}
+
+// Steps 8-10 for one solids group.  Returns 1 = continue, 0 = degenerate, -1 = capacity overflow.
+template <bool MESH>
+__device__ int trace_solids(const DInstrument& I, const DComponent& C, Ray& ray) {
+  const DSolids& G = C.u.solids;
+  Interval iv[kMaxIntervals];
+  int n_iv = 0;
+  for (int s = 0; s < G.n_solids; ++s) {
+    const DSolid& S = G.solids[s];
+    const Vec3 o = to_local(S.pose, ray.r);
+    const Vec3 d = rotate(S.pose.R, ray.d);
+    if (MESH && S.shape == MCX_MESH) {
+      const int rc = mesh_intervals(S, s, o, d, iv, n_iv);
+      if (rc != 1) return rc;
+    } else {
+      double a, b;
+      if (primitive_interval(S, o, d, a, b)) {
+        if (n_iv >= kMaxIntervals) return -1;
+        iv[n_iv++] = Interval{a, b, s};
+      }
+    }
+  }
+  // clip to t >= 0, drop empty intervals
+  int m = 0;
+  for (int k = 0; k < n_iv; ++k) {
+    Interval x = iv[k];
+    if (x.a < 0.0) x.a = 0.0;
+    if (x.b > x.a) iv[m++] = x;
+  }
+  n_iv = m;
+  if (n_iv == 0) return 1;
+  // step 10: sort all endpoints, classify every elementary segment by its midpoint
+  double ts[2 * kMaxIntervals];
+  for (int k = 0; k < n_iv; ++k) { ts[2 * k] = iv[k].a; ts[2 * k + 1] = iv[k].b; }
+  const int nt = 2 * n_iv;
+  for (int a = 1; a < nt; ++a) {
+    const double t = ts[a];
+    int b = a - 1;
+    while (b >= 0 && ts[b] > t) { ts[b + 1] = ts[b]; --b; }
+    ts[b + 1] = t;
+  }
+  const double lnE = log(ray.E);
+  double tau = 0.0;
+  int last_mat = -1;
+  double last_mu = 0.0;
+  for (int k = 0; k + 1 < nt; ++k) {
+    const double ta = ts[k], tb = ts[k + 1];
+    if (!(tb > ta)) continue;
+    const double mid = 0.5 * (ta + tb);
+    int owner = -1, best = 0;
+    for (int q = 0; q < n_iv; ++q)
+      if (iv[q].a <= mid && mid <= iv[q].b) {
+        const int pr = G.solids[iv[q].solid].priority;
+        if (owner < 0 || pr > best) { owner = iv[q].solid; best = pr; }
+      }
+    if (owner < 0) continue;
+    const int mat = G.solids[owner].material;
+    if (mat != last_mat) { last_mu = mu_of(I.mats[mat], ray.E, lnE); last_mat = mat; }
+    tau += last_mu * (tb - ta);
+  }
+  ray.p *= exp(-tau);
+  return 1;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Step 11: exact traversal of the voxel grid (Amanatides & Woo 1987).  tau = sum over the voxels crossed of
+// mu[id] * length.  The product is taken once per RUN of equal material IDs (same real number, fewer roundings):
+// PAPER.md:186-188 names this loop ("steps reach into the thousands") as where the EDXCT time goes.
+// mu_s: per-thread mu of every material, shared memory, element m at mu_s[m * kBlock].
+// ------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void trace_voxels(const DInstrument& I, const DComponent& C, Ray& ray, double* mu_s) {
+  const DVoxels& V = C.u.voxels;
+  const Vec3 ol = to_local(C.pose, ray.r);
+  const Vec3 dl = rotate(C.pose.R, ray.d);
+  const double h = V.h;
+  double t0 = -CUDART_INF, t1 = CUDART_INF;
+  if (!clip_axis(ol.x, dl.x, 0.0, (double)V.n[0] * h, t0, t1)) return;
+  if (!clip_axis(ol.y, dl.y, 0.0, (double)V.n[1] * h, t0, t1)) return;
+  if (!clip_axis(ol.z, dl.z, 0.0, (double)V.n[2] * h, t0, t1)) return;
+  if (t0 < 0.0) t0 = 0.0;
+  if (!(t0 < t1)) return;
+  // per-ray mu of every material (step 7)
+  const double lnE = log(ray.E);
+  for (int m = 0; m < I.n_mats; ++m) mu_s[m * kBlock] = mu_of(I.mats[m], ray.E, lnE);
+  // axis order: f = the axis stored fastest (the one most aligned with the beam), then a1, a2
+  const int f = V.fast, a1 = V.a1, a2 = V.a2;
+  const double of = pick(ol, f), o1 = pick(ol, a1), o2 = pick(ol, a2);
+  const double df = pick(dl, f), d1 = pick(dl, a1), d2 = pick(dl, a2);
+  const int nf = V.n[f], n1 = V.n[a1], n2 = V.n[a2];
+  int i_f, i_1, i_2, s_f, s_1, s_2;
+  double tm_f, tm_1, tm_2, td_f, td_1, td_2;
+#define MCX_AXIS_INIT(o, d, n, idx, stp, tmax, tdel)                                 \
+  {                                                                                   \
+    const double q = o + t0 * d;                                                      \
+    idx = min(n - 1, max(0, (int)floor(q / h)));                                      \
+    if (d > 0.0) { stp = 1; tmax = ((double)(idx + 1) * h - o) / d; tdel = h / d; }   \
+    else if (d < 0.0) { stp = -1; tmax = ((double)idx * h - o) / d; tdel = -h / d; }  \
+    else { stp = 0; tmax = CUDART_INF; tdel = CUDART_INF; }                           \
+  }
+  MCX_AXIS_INIT(of, df, nf, i_f, s_f, tm_f, td_f)
+  MCX_AXIS_INIT(o1, d1, n1, i_1, s_1, tm_1, td_1)
+  MCX_AXIS_INIT(o2, d2, n2, i_2, s_2, tm_2, td_2)
+#undef MCX_AXIS_INIT
+  const uint8_t* __restrict__ ids = V.ids;
+  const int pitch = V.pitch;
+  long long row = ((long long)i_2 * n1 + i_1) * pitch;  // address of (i_2, i_1, 0)
+  const long long row_step1 = (long long)s_1 * pitch, row_step2 = (long long)s_2 * n1 * pitch;
+  int cur = ids[row + i_f];
+  double tau = 0.0, t_run = t0;
+  // Tie rule of step 11: the lowest of (x, y, z) wins.  Ties only order zero-length visits, so the traversal
+  // order (f, a1, a2) used here gives the same tau.
+  while (true) {
+    double tn;
+    if (tm_f <= tm_1 && tm_f <= tm_2) {
+      tn = tm_f;
+      i_f += s_f;
+      if ((unsigned)i_f >= (unsigned)nf) { tn = fmin(tn, t1); tau += mu_s[cur * kBlock] * (tn - t_run); break; }
+      tm_f += td_f;
+    } else if (tm_1 <= tm_2) {
+      tn = tm_1;
+      i_1 += s_1;
+      if ((unsigned)i_1 >= (unsigned)n1) { tn = fmin(tn, t1); tau += mu_s[cur * kBlock] * (tn - t_run); break; }
+      tm_1 += td_1;
+      row += row_step1;
+    } else {
+      tn = tm_2;
+      i_2 += s_2;
+      if ((unsigned)i_2 >= (unsigned)n2) { tn = fmin(tn, t1); tau += mu_s[cur * kBlock] * (tn - t_run); break; }
+      tm_2 += td_2;
+      row += row_step2;
+    }
+    const int id = ids[row + i_f];
+    if (id != cur) {
+      tau += mu_s[cur * kBlock] * (tn - t_run);
+      t_run = tn;
+      cur = id;
+    }
+  }
+  ray.p *= exp(-tau);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Step 12: elliptic-cylinder mirror.  Mirror frame: origin at the pole, z tangential, y = surface normal,
+// x sagittal.  Returns true if reflected.
+// ------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double reflectivity(const DMirror& M, double theta, double E) {
+  const int nt = M.n_theta, ne = M.n_e;
+  double ft = (theta - M.theta_min) / (M.theta_max - M.theta_min) * (double)(nt - 1);
+  double fe = (E - M.e_min) / (M.e_max - M.e_min) * (double)(ne - 1);
+  ft = fmin(fmax(ft, 0.0), (double)(nt - 1));
+  fe = fmin(fmax(fe, 0.0), (double)(ne - 1));
+  const int it = min((int)floor(ft), nt - 2), ie = min((int)floor(fe), ne - 2);
+  const double wt = ft - (double)it, we = fe - (double)ie;
+  const double* __restrict__ row0 = M.table + (size_t)it * ne + ie;
+  const double* __restrict__ row1 = row0 + ne;
+  const double r00 = row0[0], r01 = row0[1], r10 = row1[0], r11 = row1[1];
+  return (1.0 - wt) * ((1.0 - we) * r00 + we * r01) + wt * ((1.0 - we) * r10 + we * r11);
+}
+
+__device__ __forceinline__ bool trace_mirror(const DComponent& C, Ray& ray) {
+  const DMirror& M = C.u.mirror;
+  const Vec3 o = to_local(C.pose, ray.r);
+  const Vec3 d = rotate(C.pose.R, ray.d);
+  // into the ellipse's principal frame (Z, Y)
+  const double oZ = M.Z0 + o.z * M.tZ + o.y * M.nZ, oY = M.Y0 + o.z * M.tY + o.y * M.nY;
+  const double dZ = d.z * M.tZ + d.y * M.nZ, dY = d.z * M.tY + d.y * M.nY;
+  const double A = dZ * dZ * M.inv_a2 + dY * dY * M.inv_b2;
+  const double B = oZ * dZ * M.inv_a2 + oY * dY * M.inv_b2;
+  const double Cc = oZ * oZ * M.inv_a2 + oY * oY * M.inv_b2 - 1.0;
+  if (A == 0.0) return false;
+  const double disc = B * B - A * Cc;
+  if (!(disc >= 0.0)) return false;
+  const double qq = -(B + (B >= 0.0 ? 1.0 : -1.0) * sqrt(disc));  // stable roots of A t^2 + 2 B t + C = 0
+  double ta = qq / A, tb = (qq != 0.0) ? Cc / qq : ta;
+  if (ta > tb) { const double t = ta; ta = tb; tb = t; }
+#pragma unroll
+  for (int r = 0; r < 2; ++r) {
+    const double t = r == 0 ? ta : tb;
+    if (!(t > 0.0)) continue;
+    const Vec3 hp = o + t * d;
+    if (fabs(hp.z) > M.half_length || fabs(hp.x) > M.half_width) continue;
+    const double hZ = M.Z0 + hp.z * M.tZ + hp.y * M.nZ, hY = M.Y0 + hp.z * M.tY + hp.y * M.nY;
+    if (!(hY < 0.0)) continue;  // the arc near the pole only
+    const double gZ = hZ * M.inv_a2, gY = hY * M.inv_b2;
+    const double gn = sqrt(gZ * gZ + gY * gY);
+    const double nZ = -gZ / gn, nY = -gY / gn;  // inward normal in (Z, Y)
+    const Vec3 nrm{0.0, nZ * M.nZ + nY * M.nY, nZ * M.tZ + nY * M.tY};
+    const double dn = dot(d, nrm);
+    if (!(dn < 0.0)) return false;
+    const double theta = asin(-dn);
+    if (theta > M.theta_max) return false;
+    ray.p *= reflectivity(M, theta, ray.E);
+    const Vec3 dr = d - (2.0 * dn) * nrm;
+    ray.r = to_lab(C.pose, hp);
+    ray.d = rotate_back(C.pose.R, dr);
+    return true;
+  }
+  return false;
+}
+
+// Step 13: symmetric Bragg reflection off a thick non-absorbing crystal (Darwin curve).
+__device__ __forceinline__ bool trace_crystal(const DComponent& C, Ray& ray) {
+  const DCrystal& X = C.u.crystal;
+  const Vec3 o = to_local(C.pose, ray.r);
+  const Vec3 d = rotate(C.pose.R, ray.d);
+  if (!(d.y < 0.0)) return false;
+  const double t = -o.y / d.y;
+  if (!(t > 0.0)) return false;
+  const Vec3 hp = o + t * d;
+  if (fabs(hp.z) > X.half_length || fabs(hp.x) > X.half_width) return false;
+  const double theta = asin(-d.y);
+  const double lambda = 12.398419843 / ray.E;  // h c in keV Angstrom
+  const double s = lambda / (2.0 * X.d_hkl);
+  if (!(s < 1.0)) return false;
+  const double theta_b = asin(s);
+  const double w_d = X.zeta * tan(theta_b);
+  const double eta = fabs((theta - theta_b - X.delta0) / (0.5 * w_d));
+  if (eta > 1.0) {
+    const double g = eta + sqrt(eta * eta - 1.0);
+    ray.p *= 1.0 / (g * g);
+  }
+  ray.r = to_lab(C.pose, Vec3{hp.x, 0.0, hp.z});
+  ray.d = rotate_back(C.pose.R, Vec3{d.x, -d.y, d.z});
+  return true;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// The megakernel.  FEAT selects which component kinds are compiled in; DUMP writes per-ray fates instead of
+// tallying.  Shared memory: the instrument image, per-block ray-accounting counters, spectrum CDFs are read through
+// the read-only path (L1), per-thread mu[] for the voxel walk.
+// ------------------------------------------------------------------------------------------------------------
+template <int FEAT, bool DUMP>
+__global__ void __launch_bounds__(kBlock) trace_kernel(const DInstrument* __restrict__ g_inst, uint64_t first, uint64_t n,
+                                                       uint64_t seed, mcx_ray_fate* __restrict__ dump) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  DInstrument& I = *reinterpret_cast<DInstrument*>(smem_raw);
+  unsigned int* s_cnt = reinterpret_cast<unsigned int*>(smem_raw + sizeof(DInstrument));  // [MCX_MAX_COMPONENTS + 4]
+  double* mu_s = reinterpret_cast<double*>(smem_raw + sizeof(DInstrument) + 128) + threadIdx.x;
+  {
+    const int4* src = reinterpret_cast<const int4*>(g_inst);
+    int4* dst = reinterpret_cast<int4*>(smem_raw);
+    for (int k = threadIdx.x; k < (int)(sizeof(DInstrument) / sizeof(int4)); k += kBlock) dst[k] = src[k];
+    if (threadIdx.x < MCX_MAX_COMPONENTS + 4) s_cnt[threadIdx.x] = 0u;
+  }
+  __syncthreads();
+  const int n_comps = I.n_comps;
+  const int lane = threadIdx.x & 31;
+  const uint64_t stride = (uint64_t)gridDim.x * kBlock;
+  // whole warps iterate together so that the ballots below are always full-warp
+  const uint64_t n_round = (n + 31u) & ~(uint64_t)31u;
+  for (uint64_t q = (uint64_t)blockIdx.x * kBlock + threadIdx.x; q < n_round; q += stride) {
+    const bool valid = q < n;
+    Ray ray;
+    int fate = MCX_FATE_MISSED;
+    long long bin = -1;
+    bool alive = valid;
+    if (valid) sample_source(I.comps[0], seed, first + q, ray);
+    for (int c = 1; c < n_comps; ++c) {
+      const DComponent& C = I.comps[c];
+      const int kind = C.kind;  // warp-uniform
+      bool pass = true;
+      if (alive) {
+        if (kind == MCX_SLIT_RECT) {
+          Vec3 h;
+          pass = plane_hit(C.pose, ray, h) && fabs(h.x) <= C.u.slit.half_x && fabs(h.y) <= C.u.slit.half_y;
+        } else if (kind == MCX_SLIT_CIRC) {
+          Vec3 h;
+          pass = plane_hit(C.pose, ray, h) && h.x * h.x + h.y * h.y <= C.u.slit.radius2;
+        } else if ((FEAT & F_SOLIDS) && kind == MCX_SOLIDS) {
+          const int rc = trace_solids<(FEAT & F_MESH) != 0>(I, C, ray);
+          if (rc != 1) {
+            pass = false;
+            fate = MCX_FATE_DEGENERATE;
+            if (rc < 0 && !DUMP) atomicAdd(&s_cnt[MCX_MAX_COMPONENTS + CNT_OVERFLOW], 1u);
+          }
+        } else if ((FEAT & F_VOXELS) && kind == MCX_VOXELS) {
+          trace_voxels(I, C, ray, mu_s);
+        } else if ((FEAT & F_OPTICS) && kind == MCX_MIRROR_ELLIPTIC) {
+          pass = trace_mirror(C, ray);
+        } else if ((FEAT & F_OPTICS) && kind == MCX_CRYSTAL_BRAGG) {
+          pass = trace_crystal(C, ray);
+        } else if (kind == MCX_DETECTOR) {
+          const long long b = detector_bin(C, ray);
+          if (b >= 0) {
+            bin = b;
+            fate = MCX_FATE_DETECTED;
+            if (!DUMP) {
+              TallyBin* rec = I.tallies[C.u.detector.index] + b;
+              atomicAdd(&rec->N, 1ull);
+              atomicAdd(&rec->P, ray.p);
+              atomicAdd(&rec->P2, ray.p * ray.p);
+            }
+          } else {
+            fate = MCX_FATE_MISSED;  // monitors do not absorb: the ray goes on
+          }
+        }
+        if (kind != MCX_DETECTOR && pass) fate = MCX_FATE_MISSED;  // fate = what the last component said
+        if (!pass) {
+          alive = false;
+          if (fate != MCX_FATE_DEGENERATE) fate = c;
+        }
+      }
+      const unsigned alive_mask = __ballot_sync(0xffffffffu, alive);
+      if (!DUMP) {
+        // warp-aggregated ray accounting: one shared-memory add per warp and component
+        const unsigned died = __ballot_sync(0xffffffffu, !pass && fate == c);
+        if (lane == 0 && died) atomicAdd(&s_cnt[c], (unsigned)__popc(died));
+      }
+      if (alive_mask == 0u) break;
+    }
+    if (DUMP) {
+      if (valid) {
+        mcx_ray_fate f;
+        f.fate = fate;
+        f.reserved = 0;
+        f.bin = fate == MCX_FATE_DETECTED ? bin : -1;
+        f.p = ray.p;
+        dump[q] = f;
+      }
+    } else {
+      const unsigned det = __ballot_sync(0xffffffffu, valid && fate == MCX_FATE_DETECTED);
+      const unsigned mis = __ballot_sync(0xffffffffu, valid && fate == MCX_FATE_MISSED);
+      const unsigned deg = __ballot_sync(0xffffffffu, valid && fate == MCX_FATE_DEGENERATE);
+      if (lane == 0) {
+        if (det) atomicAdd(&s_cnt[MCX_MAX_COMPONENTS + CNT_DETECTED], (unsigned)__popc(det));
+        if (mis) atomicAdd(&s_cnt[MCX_MAX_COMPONENTS + CNT_MISSED], (unsigned)__popc(mis));
+        if (deg) atomicAdd(&s_cnt[MCX_MAX_COMPONENTS + CNT_DEGENERATE], (unsigned)__popc(deg));
+      }
+    }
+  }
+  if (!DUMP) {
+    __syncthreads();
+    if (threadIdx.x < MCX_MAX_COMPONENTS + 4) {
+      const unsigned v = s_cnt[threadIdx.x];
+      if (v) {
+        const int slot = threadIdx.x < MCX_MAX_COMPONENTS ? threadIdx.x : n_comps + (threadIdx.x - MCX_MAX_COMPONENTS);
+        if (threadIdx.x >= MCX_MAX_COMPONENTS || threadIdx.x < n_comps) atomicAdd(&I.counters[slot], (unsigned long long)v);
+      }
+    }
+  }
+}
+
+// Step a14: tally finalise.  De-interleaves the 32-byte records into the three output arrays.
+__global__ void __launch_bounds__(256) tally_read_kernel(const TallyBin* __restrict__ bins, uint64_t n_bins,
+                                                         unsigned long long* __restrict__ N, double* __restrict__ P,
+                                                         double* __restrict__ P2) {
+  const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+  for (uint64_t b = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; b < n_bins; b += stride) {
+    const ulonglong4 rec = *reinterpret_cast<const ulonglong4*>(bins + b);
+    N[b] = rec.x;
+    P[b] = __longlong_as_double((long long)rec.y);
+    P2[b] = __longlong_as_double((long long)rec.z);
+  }
+}
+
+// Voxel volume from the interface layout [iz][iy][ix] into the traversal layout [i_a2][i_a1][i_fast (pitch)].
+__global__ void __launch_bounds__(256) voxel_relayout_kernel(const uint8_t* __restrict__ src, uint8_t* __restrict__ dst,
+                                                             int nx, int ny, int nz, int fast, int a1, int a2, int pitch) {
+  const int n[3] = {nx, ny, nz};
+  const long long total = (long long)n[a2] * n[a1] * pitch;
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < total; k += stride) {
+    const int jf = (int)(k % pitch);
+    const long long rowi = k / pitch;
+    const int j1 = (int)(rowi % n[a1]), j2 = (int)(rowi / n[a1]);
+    uint8_t v = 0;
+    if (jf < n[fast]) {
+      int idx[3];
+      idx[fast] = jf; idx[a1] = j1; idx[a2] = j2;
+      v = src[((long long)idx[2] * ny + idx[1]) * nx + idx[0]];
+    }
+    dst[k] = v;
+  }
+}
+
+// FP64 pipe probe for the ALU roofline: 8 independent DFMA chains per thread.
+__global__ void __launch_bounds__(256) probe_dfma_kernel(double* sink, long long n_iters) {
+  double a0 = threadIdx.x * 1e-9, a1 = a0 + 1.0, a2 = a0 + 2.0, a3 = a0 + 3.0, a4 = a0 + 4.0, a5 = a0 + 5.0, a6 = a0 + 6.0,
+         a7 = a0 + 7.0;
+  const double m = 1.0000000001, c = 1e-12;
+  for (long long k = 0; k < n_iters; ++k) {
+    a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+    a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+  }
+  sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+}
+
+constexpr size_t kSmemBase = sizeof(DInstrument) + 128;
+
+template <int FEAT, bool DUMP>
+cudaError_t launch_one(const DInstrument* d_inst, int n_mats, uint64_t first, uint64_t n, uint64_t seed, mcx_ray_fate* dump,
+                       cudaStream_t stream, int n_sm) {
+  const size_t smem = kSmemBase + ((FEAT & F_VOXELS) ? (size_t)n_mats * kBlock * sizeof(double) : 0);
+  static bool configured = false;
+  static int blocks_per_sm = 1;
+  cudaError_t e;
+  if (!configured) {
+    e = cudaFuncSetAttribute(trace_kernel<FEAT, DUMP>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, trace_kernel<FEAT, DUMP>, kBlock, smem);
+  if (e != cudaSuccess) return e;
+  if (blocks_per_sm < 1) return cudaErrorInvalidConfiguration;
+  const uint64_t want = (n + kBlock - 1) / kBlock;
+  const uint64_t full = (uint64_t)n_sm * blocks_per_sm;  // one resident wave: a multiple of the SM count
+  const unsigned grid = (unsigned)(want < full ? (want ? want : 1) : full);
+  trace_kernel<FEAT, DUMP><<<grid, kBlock, smem, stream>>>(d_inst, first, n, seed, dump);
+  return cudaGetLastError();
+}
+
+int g_n_sm = 0;
+
+}  // namespace
+
+cudaError_t kernels_init() {
+  if (g_n_sm) return cudaSuccess;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  return cudaDeviceGetAttribute(&g_n_sm, cudaDevAttrMultiProcessorCount, dev);
+}
+
+cudaError_t launch_trace(const DInstrument* d_inst, int features, int n_mats, uint64_t first, uint64_t n, uint64_t seed,
+                         mcx_ray_fate* dump, cudaStream_t stream) {
+  cudaError_t e = kernels_init();
+  if (e != cudaSuccess) return e;
+  if (n == 0) return cudaSuccess;
+#define MCX_DISPATCH(F)                                                                                  \
+  return dump ? launch_one<F, true>(d_inst, n_mats, first, n, seed, dump, stream, g_n_sm)                \
+              : launch_one<F, false>(d_inst, n_mats, first, n, seed, dump, stream, g_n_sm);
+  switch (features) {
+    case 0: MCX_DISPATCH(0)
+    case F_SOLIDS: MCX_DISPATCH(F_SOLIDS)
+    case F_SOLIDS | F_MESH: MCX_DISPATCH(F_SOLIDS | F_MESH)
+    case F_VOXELS: MCX_DISPATCH(F_VOXELS)
+    case F_OPTICS: MCX_DISPATCH(F_OPTICS)
+    default: MCX_DISPATCH(F_ALL)
+  }
+#undef MCX_DISPATCH
+}
+
+cudaError_t launch_tally_read(const TallyBin* bins, uint64_t n_bins, unsigned long long* N, double* p, double* p2,
+                              cudaStream_t stream) {
+  cudaError_t e = kernels_init();
+  if (e != cudaSuccess) return e;
+  if (n_bins == 0) return cudaSuccess;
+  const uint64_t want = (n_bins + 255) / 256;
+  const unsigned grid = (unsigned)(want < (uint64_t)g_n_sm * 8 ? want : (uint64_t)g_n_sm * 8);
+  tally_read_kernel<<<grid, 256, 0, stream>>>(bins, n_bins, N, p, p2);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_voxel_relayout(const uint8_t* src, uint8_t* dst, int nx, int ny, int nz, int fast, int a1, int a2,
+                                  int pitch, cudaStream_t stream) {
+  cudaError_t e = kernels_init();
+  if (e != cudaSuccess) return e;
+  voxel_relayout_kernel<<<g_n_sm * 8, 256, 0, stream>>>(src, dst, nx, ny, nz, fast, a1, a2, pitch);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_probe_dfma(double* sink, int n_blocks, long long n_iters, cudaStream_t stream) {
+  probe_dfma_kernel<<<n_blocks, 256, 0, stream>>>(sink, n_iters);
+  return cudaGetLastError();
+}
+
+}  // namespace mcx
