@@ -198,6 +198,16 @@ mcx_status mcx_trace_range(mcx_instrument* inst, uint64_t first_ray, uint64_t n_
 mcx_status mcx_tally_read(mcx_instrument* inst, int detector, uint64_t* N, double* p, double* p2, size_t n_bins,
                           void* cuda_stream);
 
+/* Same, with HOST output arrays (pinned memory if the copy is to be asynchronous): finalises into a staging area of
+ * the workspace and enqueues three device-to-host copies on the stream.  This is the end-to-end read a caller
+ * without device buffers uses (the paper's "update host"). */
+mcx_status mcx_tally_read_host(mcx_instrument* inst, int detector, uint64_t* N, double* p, double* p2, size_t n_bins,
+                               void* cuda_stream);
+
+/* Bytes mcx_instrument_create copied from the host to the device for this handle (instrument image and tables; the
+ * voxel volume is the caller's own upload). */
+uint64_t mcx_upload_bytes(const mcx_instrument* inst);
+
 /* Zeroes all tallies and counters. */
 mcx_status mcx_tally_reset(mcx_instrument* inst, void* cuda_stream);
 

@@ -24,7 +24,7 @@ SHAPE = {"box": 0, "cyl": 1, "sphere": 2, "mesh": 3}
 FATE_DETECTED, FATE_MISSED, FATE_DEGENERATE = -1, -2, -3
 
 EXPORTS = ["mcx_instrument_workspace_size", "mcx_instrument_create", "mcx_trace", "mcx_trace_range", "mcx_tally_read",
-           "mcx_tally_reset", "mcx_counters_read", "mcx_trace_dump", "mcx_launch_count", "mcx_probe_dfma",
+           "mcx_tally_read_host", "mcx_upload_bytes", "mcx_tally_reset", "mcx_counters_read", "mcx_trace_dump", "mcx_launch_count", "mcx_probe_dfma",
            "mcx_instrument_destroy", "mcx_last_error"]
 
 _dp = C.POINTER(C.c_double)
@@ -112,6 +112,9 @@ def lib(strict=False):
     L.mcx_trace.argtypes = [vp, C.c_uint64, C.c_uint64, vp]
     L.mcx_trace_range.argtypes = [vp, C.c_uint64, C.c_uint64, C.c_uint64, vp]
     L.mcx_tally_read.argtypes = [vp, C.c_int, vp, vp, vp, C.c_size_t, vp]
+    L.mcx_tally_read_host.argtypes = [vp, C.c_int, vp, vp, vp, C.c_size_t, vp]
+    L.mcx_upload_bytes.argtypes = [vp]
+    L.mcx_upload_bytes.restype = C.c_uint64
     L.mcx_tally_reset.argtypes = [vp, vp]
     L.mcx_counters_read.argtypes = [vp, vp, C.c_int, vp]
     L.mcx_trace_dump.argtypes = [vp, C.c_uint64, C.c_uint64, C.c_uint64, vp, vp]
@@ -122,7 +125,7 @@ def lib(strict=False):
     L.mcx_instrument_destroy.restype = None
     L.mcx_last_error.restype = C.c_char_p
     for name in ("mcx_instrument_workspace_size", "mcx_instrument_create", "mcx_trace", "mcx_trace_range",
-                 "mcx_tally_read", "mcx_tally_reset", "mcx_counters_read", "mcx_trace_dump", "mcx_probe_dfma"):
+                 "mcx_tally_read", "mcx_tally_read_host", "mcx_tally_reset", "mcx_counters_read", "mcx_trace_dump", "mcx_probe_dfma"):
         getattr(L, name).restype = C.c_int
     _libs[strict] = L
     return L
@@ -229,7 +232,9 @@ def marshal(inst, keep, device_voxels):
 class Instrument:
     """A device-resident instrument (mcx_instrument handle + the torch buffers it lives in)."""
 
-    def __init__(self, inst, device="cuda:0", strict=False):
+    def __init__(self, inst, device="cuda:0", strict=False, voxels_pinned=None, sync=True):
+        """voxels_pinned: optional pinned uint8 torch tensor holding the voxel volume (copied asynchronously instead
+        of inst's numpy array); sync=False leaves the create enqueued on the current stream."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("no CUDA device: the mcx hot path has no CPU fallback")
@@ -243,9 +248,13 @@ class Instrument:
         self.handle = None
         L = self.L = lib(strict)
 
+        self.voxel_upload_bytes = 0
+
         def device_voxels(ids):
-            t = torch.from_numpy(ids).to(self.device)
+            src = voxels_pinned if voxels_pinned is not None else torch.from_numpy(ids)
+            t = src.to(self.device, non_blocking=voxels_pinned is not None)
             self._dev.append(t)
+            self.voxel_upload_bytes += t.numel()
             return t.data_ptr()
 
         with torch.cuda.device(self.device):
@@ -259,9 +268,10 @@ class Instrument:
             _check(L.mcx_instrument_create(comps, self.n_comps, mats, self.n_mats, base, self.workspace_bytes,
                                            self._stream(), C.byref(h)), L)
             self.handle = h
-            torch.cuda.current_stream().synchronize()
+            if sync:
+                torch.cuda.current_stream().synchronize()
+                self._dev.clear()    # the voxel volume was copied into the workspace
         self._keep.clear()   # HOST inputs are consumed by create
-        self._dev.clear()    # the voxel volume was copied into the workspace
 
     def _stream(self):
         return C.c_void_p(self.torch.cuda.current_stream(self.device).cuda_stream)
@@ -283,6 +293,17 @@ class Instrument:
         N, P, P2 = out
         _check(self.L.mcx_tally_read(self.handle, detector, N.data_ptr(), P.data_ptr(), P2.data_ptr(), nb, self._stream()), self.L)
         return N, P, P2
+
+    def tally_host(self, out, detector=0):
+        """mcx_tally_read_host into (N int64, p, p2) pinned host tensors; asynchronous on the current stream."""
+        N, P, P2 = out
+        _check(self.L.mcx_tally_read_host(self.handle, detector, N.data_ptr(), P.data_ptr(), P2.data_ptr(), N.numel(),
+                                          self._stream()), self.L)
+        return out
+
+    def upload_bytes(self):
+        """host -> device bytes moved to build this instrument (tables by create + the voxel volume)."""
+        return int(self.L.mcx_upload_bytes(self.handle)) + self.voxel_upload_bytes
 
     def reset(self):
         _check(self.L.mcx_tally_reset(self.handle, self._stream()), self.L)

@@ -20,6 +20,8 @@ struct mcx_instrument {
   unsigned char* workspace = nullptr;
   size_t workspace_bytes = 0;
   size_t zero_begin = 0, zero_end = 0;  // tallies + counters
+  size_t off_staging = 0;
+  size_t upload_bytes = 0;              // host -> device bytes moved by create
   int n_comps = 0, n_mats = 0, n_dets = 0, features = 0;
   uint64_t det_bins[MCX_MAX_DETECTORS] = {0, 0, 0, 0};
   uint64_t launches = 0;
@@ -136,6 +138,7 @@ struct Plan {
   size_t off_tally[MCX_MAX_DETECTORS];
   size_t off_counters = 0;
   size_t zero_begin = 0, zero_end = 0;
+  size_t off_staging = 0;  // N, p, p2 of the largest detector, for mcx_tally_read_host
   size_t total = 0;
   // blob offsets
   size_t off_mat[MCX_MAX_MATERIALS];      // 4 arrays of n doubles each
@@ -242,6 +245,11 @@ mcx_status make_plan(const mcx_component* comps, int n_comps, const mcx_material
     }
   P->off_counters = A.reserve((size_t)MCX_N_COUNTERS(n_comps) * sizeof(unsigned long long));
   P->zero_end = A.top;
+  size_t max_bins = 0;
+  for (int c = 0; c < n_comps; ++c)
+    if (comps[c].kind == MCX_DETECTOR)
+      max_bins = std::max(max_bins, (size_t)comps[c].u.detector.nx * comps[c].u.detector.ny * comps[c].u.detector.ne);
+  P->off_staging = A.reserve(max_bins * 24);
   P->total = A.top;
   return MCX_OK;
 }
@@ -290,6 +298,7 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
   H->n_mats = n_materials;
   H->zero_begin = P.zero_begin;
   H->zero_end = P.zero_end;
+  H->off_staging = P.off_staging;
   H->blob.assign(P.blob_end - P.blob_begin, 0);
   unsigned char* blob = H->blob.data();
   auto host_ptr = [&](size_t off) { return blob + (off - P.blob_begin); };
@@ -505,6 +514,7 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
     e = cudaMemcpyAsync(ws + P.blob_begin, H->blob.data(), H->blob.size(), cudaMemcpyHostToDevice, stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(ws + P.zero_begin, 0, P.zero_end - P.zero_begin, stream);
   if (e != cudaSuccess) { const mcx_status s_ = cuda_fail(e, "upload of the instrument image"); delete H; return s_; }
+  H->upload_bytes = sizeof(DInstrument) + H->blob.size();
   *out = H;
   return MCX_OK;
 }
@@ -550,6 +560,27 @@ mcx_status mcx_tally_read(mcx_instrument* inst, int detector, uint64_t* N, doubl
   inst->launches++;
   return MCX_OK;
 }
+
+mcx_status mcx_tally_read_host(mcx_instrument* inst, int detector, uint64_t* N, double* p, double* p2, size_t n_bins,
+                               void* cuda_stream) {
+  if (!inst) return fail(MCX_ERR_INVALID_ARG, "inst is null");
+  if (detector < 0 || detector >= inst->n_dets) return fail(MCX_ERR_INVALID_ARG, "detector %d out of range (%d detectors)", detector, inst->n_dets);
+  if (!N || !p || !p2) return fail(MCX_ERR_INVALID_ARG, "null output array");
+  if ((uint64_t)n_bins != inst->det_bins[detector]) return fail(MCX_ERR_INVALID_ARG, "n_bins is %zu, detector has %llu", n_bins, (unsigned long long)inst->det_bins[detector]);
+  unsigned long long* dN = (unsigned long long*)(inst->workspace + inst->off_staging);
+  double* dP = (double*)(dN + n_bins);
+  double* dP2 = dP + n_bins;
+  const mcx_status st = mcx_tally_read(inst, detector, (uint64_t*)dN, dP, dP2, n_bins, cuda_stream);
+  if (st != MCX_OK) return st;
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  cudaError_t e = cudaMemcpyAsync(N, dN, n_bins * sizeof(uint64_t), cudaMemcpyDeviceToHost, stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(p, dP, n_bins * sizeof(double), cudaMemcpyDeviceToHost, stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(p2, dP2, n_bins * sizeof(double), cudaMemcpyDeviceToHost, stream);
+  if (e != cudaSuccess) return cuda_fail(e, "tally copy to the host");
+  return MCX_OK;
+}
+
+uint64_t mcx_upload_bytes(const mcx_instrument* inst) { return inst ? (uint64_t)inst->upload_bytes : 0; }
 
 mcx_status mcx_tally_reset(mcx_instrument* inst, void* cuda_stream) {
   if (!inst) return fail(MCX_ERR_INVALID_ARG, "inst is null");
