@@ -192,9 +192,13 @@ def measured_peaks():
 
 
 # ---------------------------------------------------------------------------------------------------------------
+EXEC_MODE = "auto"   # lane scheduling (mcx_instrument_set_exec); --exec overrides for experiments
+
+
 def bench_instrument(M, torch, inst, n_rays, first, steps, warmup, device, dfma_peak, peaks, with_e2e=True, local_rank=0):
     """Times `steps` steps of mcx_trace + mcx_tally_read for one instrument on the current stream.  Returns a dict."""
     g = M.Instrument(inst, device=device)
+    g.set_exec(EXEC_MODE)
     det = g.dets[-1]
     nb = det["nx"] * det["ny"] * det["nE"]
     last = len(g.dets) - 1
@@ -271,6 +275,7 @@ def bench_e2e(M, torch, inst, n_rays, first, steps, device):
         torch.cuda.synchronize(device)
         t0 = time.perf_counter()
         g = M.Instrument(inst, device=device, voxels_pinned=pinned_vox, sync=False)
+        g.set_exec(EXEC_MODE)
         g.trace(n_rays, first=first)
         g.tally_host(host, len(g.dets) - 1)
         torch.cuda.synchronize(device)
@@ -333,7 +338,10 @@ def main():
     ap.add_argument("--instruments", default="0,2,3,4", help="other configs to report under 'instruments' ('' = none)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="configs[4] throughput sweep 1e6..1e10 rays")
+    ap.add_argument("--exec", default="auto", choices=["auto", "direct", "sorted"], help="lane scheduling (row a13)")
     args = ap.parse_args()
+    global EXEC_MODE
+    EXEC_MODE = args.exec
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         return run_reference(args)

@@ -192,6 +192,16 @@ mcx_status mcx_trace(mcx_instrument* inst, uint64_t n_rays, uint64_t seed, void*
 mcx_status mcx_trace_range(mcx_instrument* inst, uint64_t first_ray, uint64_t n_rays, uint64_t seed,
                            void* cuda_stream);
 
+/* Lane scheduling.  Results do not depend on it beyond the summation order of the tallies:
+ * a ray is a pure function of (instrument, seed, ray index) whatever order rays are traced in.
+ *   MCX_EXEC_DIRECT  rays are traced in index order, 32 consecutive indices per warp;
+ *   MCX_EXEC_SORTED  each chunk of <= 2^24 ray indices is first bucketed by the cell of a grid over the source's
+ *                    direction draw (count, scan, scatter; 4 bytes of workspace per ray of a chunk), so that a warp
+ *                    traces rays aimed at the same spot (coherent voxel / BVH / primitive walks);
+ *   MCX_EXEC_AUTO    (default) SORTED for instruments with a mesh or voxel component, DIRECT otherwise. */
+typedef enum { MCX_EXEC_AUTO = 0, MCX_EXEC_DIRECT = 1, MCX_EXEC_SORTED = 2 } mcx_exec_mode;
+mcx_status mcx_instrument_set_exec(mcx_instrument* inst, int mode);
+
 /* Finalises detector `detector` (ordinal among MCX_DETECTOR components): writes N (ray counts), p (sum of
  * weights) and p2 (sum of squared weights) for all bins, bin = (iy * nx + ix) * ne + ie.
  * N, p, p2: DEVICE [n_bins]; n_bins must equal nx*ny*ne. */

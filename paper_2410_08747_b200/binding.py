@@ -21,10 +21,11 @@ POS_MODE = {"point": 0, "disk": 1, "gauss": 2}
 DIR_MODE = {"target": 0, "gauss": 1}
 ENERGY_MODE = {"mono": 0, "uniform": 1, "spectrum": 2}
 SHAPE = {"box": 0, "cyl": 1, "sphere": 2, "mesh": 3}
+EXEC_MODE = {"auto": 0, "direct": 1, "sorted": 2}
 FATE_DETECTED, FATE_MISSED, FATE_DEGENERATE = -1, -2, -3
 
 EXPORTS = ["mcx_instrument_workspace_size", "mcx_instrument_create", "mcx_trace", "mcx_trace_range", "mcx_tally_read",
-           "mcx_tally_read_host", "mcx_upload_bytes", "mcx_tally_reset", "mcx_counters_read", "mcx_trace_dump", "mcx_launch_count", "mcx_probe_dfma",
+           "mcx_tally_read_host", "mcx_instrument_set_exec", "mcx_upload_bytes", "mcx_tally_reset", "mcx_counters_read", "mcx_trace_dump", "mcx_launch_count", "mcx_probe_dfma",
            "mcx_instrument_destroy", "mcx_last_error"]
 
 _dp = C.POINTER(C.c_double)
@@ -113,6 +114,8 @@ def lib(strict=False):
     L.mcx_trace_range.argtypes = [vp, C.c_uint64, C.c_uint64, C.c_uint64, vp]
     L.mcx_tally_read.argtypes = [vp, C.c_int, vp, vp, vp, C.c_size_t, vp]
     L.mcx_tally_read_host.argtypes = [vp, C.c_int, vp, vp, vp, C.c_size_t, vp]
+    L.mcx_instrument_set_exec.argtypes = [vp, C.c_int]
+    L.mcx_instrument_set_exec.restype = C.c_int
     L.mcx_upload_bytes.argtypes = [vp]
     L.mcx_upload_bytes.restype = C.c_uint64
     L.mcx_tally_reset.argtypes = [vp, vp]
@@ -300,6 +303,10 @@ class Instrument:
         _check(self.L.mcx_tally_read_host(self.handle, detector, N.data_ptr(), P.data_ptr(), P2.data_ptr(), N.numel(),
                                           self._stream()), self.L)
         return out
+
+    def set_exec(self, mode):
+        """mcx_instrument_set_exec: "auto" | "direct" | "sorted" (lane scheduling, row a13)."""
+        _check(self.L.mcx_instrument_set_exec(self.handle, EXEC_MODE[mode]), self.L)
 
     def upload_bytes(self):
         """host -> device bytes moved to build this instrument (tables by create + the voxel volume)."""

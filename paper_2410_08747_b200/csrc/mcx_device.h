@@ -130,9 +130,21 @@ static_assert(sizeof(TallyBin) == 32, "one tally record per 32-byte sector");
 // feature bits: select the kernel instantiation (code for absent component kinds is compiled out)
 enum { F_SOLIDS = 1, F_MESH = 2, F_VOXELS = 4, F_OPTICS = 8, F_ALL = 15 };
 
+// One trace launch: rays first + offset(q) for positions q in [0, n); offset(q) = order[q] if order != null, else q.
+struct TraceArgs {
+  uint64_t first, n, seed;
+  const uint32_t* order;   // detector-tile order of the chunk (launch_sort), or null
+  mcx_ray_fate* dump;      // per-ray records indexed by ray offset, or null = tally
+  unsigned int* ticket;    // [2] work-tile ticket and departure count, zero between launches
+};
+
+// sizes of the sort workspace
+enum { MCX_SORT_MAX_G = 10, MCX_SORT_MAX_BUCKETS = 1 << 20, MCX_SORT_MAX_SCAN_BLOCKS = 512 };
+
 // ---- launch interface (defined in mcx_kernels.cu) ----
-cudaError_t launch_trace(const DInstrument* d_inst, int features, int n_mats, uint64_t first, uint64_t n, uint64_t seed,
-                         mcx_ray_fate* dump, cudaStream_t stream);
+cudaError_t launch_trace(const DInstrument* d_inst, int features, int n_mats, const TraceArgs& args, cudaStream_t stream);
+cudaError_t launch_sort(uint64_t first, uint32_t n, uint64_t seed, int g, unsigned int* cnt, unsigned int* bsum,
+                        uint32_t* order, cudaStream_t stream);
 cudaError_t launch_tally_read(const TallyBin* bins, uint64_t n_bins, unsigned long long* N, double* p, double* p2,
                               cudaStream_t stream);
 cudaError_t launch_voxel_relayout(const uint8_t* src, uint8_t* dst, int nx, int ny, int nz, int fast, int a1, int a2,

@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <limits>
 #include <new>
@@ -25,6 +26,10 @@ struct mcx_instrument {
   int n_comps = 0, n_mats = 0, n_dets = 0, features = 0;
   uint64_t det_bins[MCX_MAX_DETECTORS] = {0, 0, 0, 0};
   uint64_t launches = 0;
+  // lane scheduling (row a13)
+  int exec_mode = MCX_EXEC_AUTO;
+  size_t off_ticket = 0, off_sort_cnt = 0, off_sort_bsum = 0, off_order = 0;
+  uint64_t chunk_rays = 0;  // capacity of the order buffer
 };
 
 namespace {
@@ -130,6 +135,26 @@ struct BvhBuilder {
 
 size_t bvh_node_bound(int64_t n_tris) { return (size_t)(2 * n_tris + 2); }
 
+// Rays per sorted chunk: the order buffer (4 B per ray) of a 2^24-ray chunk is 64 MiB and stays L2-resident between
+// the scatter that writes it and the trace that reads it.  MCX_CHUNK_LOG2 / MCX_SORT_G are tuning knobs for sweeps.
+int env_int(const char* name, int lo, int hi, int dflt) {
+  const char* v = std::getenv(name);
+  if (!v || !*v) return dflt;
+  const long x = std::strtol(v, nullptr, 10);
+  return x < lo || x > hi ? dflt : (int)x;
+}
+uint64_t chunk_capacity() { return (uint64_t)1 << env_int("MCX_CHUNK_LOG2", 14, 30, 24); }
+constexpr uint64_t kSortMinRays = 1u << 14;  // shorter chunks are traced in index order
+
+// bits per axis of the bucket grid: about 32-64 rays per bucket
+int sort_bits(uint64_t n) {
+  const int forced = env_int("MCX_SORT_G", 1, MCX_SORT_MAX_G, 0);
+  if (forced) return forced;
+  int g = 1;
+  while (g < MCX_SORT_MAX_G && ((uint64_t)64 << (2 * (g + 1))) <= n) ++g;
+  return g;
+}
+
 // sizes and offsets of everything in the workspace
 struct Plan {
   size_t off_inst = 0;
@@ -139,6 +164,7 @@ struct Plan {
   size_t off_counters = 0;
   size_t zero_begin = 0, zero_end = 0;
   size_t off_staging = 0;  // N, p, p2 of the largest detector, for mcx_tally_read_host
+  size_t off_ticket = 0, off_sort_cnt = 0, off_sort_bsum = 0, off_order = 0;
   size_t total = 0;
   // blob offsets
   size_t off_mat[MCX_MAX_MATERIALS];      // 4 arrays of n doubles each
@@ -244,12 +270,16 @@ mcx_status make_plan(const mcx_component* comps, int n_comps, const mcx_material
       P->off_tally[d++] = A.reserve((size_t)D.nx * D.ny * D.ne * sizeof(TallyBin));
     }
   P->off_counters = A.reserve((size_t)MCX_N_COUNTERS(n_comps) * sizeof(unsigned long long));
+  P->off_ticket = A.reserve(2 * sizeof(unsigned int));
   P->zero_end = A.top;
   size_t max_bins = 0;
   for (int c = 0; c < n_comps; ++c)
     if (comps[c].kind == MCX_DETECTOR)
       max_bins = std::max(max_bins, (size_t)comps[c].u.detector.nx * comps[c].u.detector.ny * comps[c].u.detector.ne);
   P->off_staging = A.reserve(max_bins * 24);
+  P->off_sort_cnt = A.reserve((size_t)MCX_SORT_MAX_BUCKETS * sizeof(unsigned int));
+  P->off_sort_bsum = A.reserve((size_t)MCX_SORT_MAX_SCAN_BLOCKS * sizeof(unsigned int));
+  P->off_order = A.reserve((size_t)chunk_capacity() * sizeof(uint32_t));
   P->total = A.top;
   return MCX_OK;
 }
@@ -299,6 +329,11 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
   H->zero_begin = P.zero_begin;
   H->zero_end = P.zero_end;
   H->off_staging = P.off_staging;
+  H->off_ticket = P.off_ticket;
+  H->off_sort_cnt = P.off_sort_cnt;
+  H->off_sort_bsum = P.off_sort_bsum;
+  H->off_order = P.off_order;
+  H->chunk_rays = chunk_capacity();
   H->blob.assign(P.blob_end - P.blob_begin, 0);
   unsigned char* blob = H->blob.data();
   auto host_ptr = [&](size_t off) { return blob + (off - P.blob_begin); };
@@ -519,15 +554,66 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
   return MCX_OK;
 }
 
+}  // extern "C"
+
+namespace {
+
+// Rows a13: which order the rays of a call are traced in.  AUTO = detector-tile order where the instrument has a
+// memory-walking component (meshes, voxels: coherent warps pay for the sort many times over), index order otherwise
+// (DESIGN.md 6 "What round 1 measured").
+bool use_sorted(const mcx_instrument* H) {
+  if (H->exec_mode == MCX_EXEC_SORTED) return true;
+  if (H->exec_mode == MCX_EXEC_DIRECT) return false;
+  return (H->features & (F_MESH | F_VOXELS)) != 0;
+}
+
+// Traces rays [first, first + n) chunk by chunk; dump == nullptr tallies.
+mcx_status run_trace(mcx_instrument* H, uint64_t first, uint64_t n, uint64_t seed, mcx_ray_fate* dump, cudaStream_t stream) {
+  const bool sorted = use_sorted(H);
+  const uint64_t cap = sorted ? H->chunk_rays : ((uint64_t)1 << 32);
+  unsigned char* ws = H->workspace;
+  for (uint64_t base = 0; base < n; base += cap) {
+    const uint64_t m = std::min(cap, n - base);
+    TraceArgs A;
+    A.first = first + base;
+    A.n = m;
+    A.seed = seed;
+    A.order = nullptr;
+    A.dump = dump ? dump + base : nullptr;
+    A.ticket = (unsigned int*)(ws + H->off_ticket);
+    if (sorted && m >= kSortMinRays) {
+      const int g = sort_bits(m);
+      unsigned int* cnt = (unsigned int*)(ws + H->off_sort_cnt);
+      cudaError_t e = cudaMemsetAsync(cnt, 0, sizeof(unsigned int) << (2 * g), stream);
+      if (e == cudaSuccess)
+        e = launch_sort(A.first, (uint32_t)m, seed, g, cnt, (unsigned int*)(ws + H->off_sort_bsum), (uint32_t*)(ws + H->off_order), stream);
+      if (e != cudaSuccess) return cuda_fail(e, "ray sort launch");
+      H->launches += 3;
+      A.order = (const uint32_t*)(ws + H->off_order);
+    }
+    const cudaError_t e = launch_trace((const DInstrument*)ws, H->features, H->n_mats, A, stream);
+    if (e != cudaSuccess) return cuda_fail(e, "trace launch");
+    H->launches++;
+  }
+  return MCX_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+mcx_status mcx_instrument_set_exec(mcx_instrument* inst, int mode) {
+  if (!inst) return fail(MCX_ERR_INVALID_ARG, "inst is null");
+  if (mode != MCX_EXEC_AUTO && mode != MCX_EXEC_DIRECT && mode != MCX_EXEC_SORTED) return fail(MCX_ERR_INVALID_ARG, "bad exec mode %d", mode);
+  inst->exec_mode = mode;
+  return MCX_OK;
+}
+
 mcx_status mcx_trace_range(mcx_instrument* inst, uint64_t first_ray, uint64_t n_rays, uint64_t seed, void* cuda_stream) {
   if (!inst) return fail(MCX_ERR_INVALID_ARG, "inst is null");
   mcx_status st = check_sticky();
   if (st != MCX_OK) return st;
-  const cudaError_t e = launch_trace((const DInstrument*)inst->workspace, inst->features, inst->n_mats, first_ray, n_rays, seed,
-                                     nullptr, (cudaStream_t)cuda_stream);
-  if (e != cudaSuccess) return cuda_fail(e, "trace launch");
-  if (n_rays) inst->launches++;
-  return MCX_OK;
+  return run_trace(inst, first_ray, n_rays, seed, nullptr, (cudaStream_t)cuda_stream);
 }
 
 mcx_status mcx_trace(mcx_instrument* inst, uint64_t n_rays, uint64_t seed, void* cuda_stream) {
@@ -540,11 +626,8 @@ mcx_status mcx_trace_dump(mcx_instrument* inst, uint64_t first_ray, uint64_t n_r
   if (!out && n_rays) return fail(MCX_ERR_INVALID_ARG, "out is null");
   mcx_status st = check_sticky();
   if (st != MCX_OK) return st;
-  const cudaError_t e = launch_trace((const DInstrument*)inst->workspace, inst->features, inst->n_mats, first_ray, n_rays, seed,
-                                     out, (cudaStream_t)cuda_stream);
-  if (e != cudaSuccess) return cuda_fail(e, "trace_dump launch");
-  if (n_rays) inst->launches++;
-  return MCX_OK;
+  if (n_rays == 0) return MCX_OK;
+  return run_trace(inst, first_ray, n_rays, seed, out, (cudaStream_t)cuda_stream);
 }
 
 mcx_status mcx_tally_read(mcx_instrument* inst, int detector, uint64_t* N, double* p, double* p2, size_t n_bins,

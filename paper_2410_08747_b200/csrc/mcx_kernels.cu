@@ -599,17 +599,104 @@ __device__ __forceinline__ bool trace_crystal(const DComponent& C, Ray& ray) {
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// The megakernel.  FEAT selects which component kinds are compiled in; DUMP writes per-ray fates instead of
-// tallying.  Shared memory: the instrument image, per-block ray-accounting counters, spectrum CDFs are read through
-// the read-only path (L1), per-thread mu[] for the voxel walk.
+// Detector-tile ordering of a chunk of rays (row a13).  A ray's direction is fixed by its slot-1
+// draw (ua, ub) (step 3), and draws are slot-addressed (step 1), so rays may be traced in any order.  The three
+// kernels below bucket the ray offsets of a chunk by the cell of a 2^g x 2^g grid over (ua, ub) their slot-1 draw
+// falls in (count -> scan -> scatter); trace_kernel then gives each warp 32 consecutive entries = rays aimed at
+// (nearly) the same spot, which walk the same voxel rows / BVH nodes / primitives in lockstep.
+// Cell order: 8 x 8 blocks of cells are contiguous, so a tile of consecutive positions is compact in 2-D.
 // ------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t sort_key(uint64_t seed, uint64_t i, int g) {
+  uint32_t w[4];
+  philox4x32_10((uint32_t)i, (uint32_t)(i >> 32), 1u, 0u, (uint32_t)seed, (uint32_t)(seed >> 32), w);
+  const uint32_t kx = w[0] >> (32 - g), ky = w[2] >> (32 - g);  // top g bits of ua and ub (step 2)
+  if (g >= 3) return ((((ky >> 3) << (g - 3)) | (kx >> 3)) << 6) | ((ky & 7u) << 3) | (kx & 7u);
+  return (ky << g) | kx;
+}
+
+__global__ void __launch_bounds__(256) sort_count_kernel(uint64_t first, uint32_t n, uint64_t seed, int g,
+                                                         unsigned int* __restrict__ cnt) {
+  const uint32_t stride = gridDim.x * blockDim.x;
+  for (uint32_t q = blockIdx.x * blockDim.x + threadIdx.x; q < n; q += stride) atomicAdd(&cnt[sort_key(seed, first + q, g)], 1u);
+}
+
+// In-place exclusive scan of cnt within blocks of kScanBlock entries; bsum[b] = total of block b.
+constexpr int kScanBlock = 2048;
+__global__ void __launch_bounds__(256) sort_scan_kernel(unsigned int* __restrict__ cnt, uint32_t n_buckets,
+                                                        unsigned int* __restrict__ bsum) {
+  __shared__ unsigned int s_w[8];
+  const uint32_t base = blockIdx.x * kScanBlock + threadIdx.x * 8;
+  unsigned int v[8], tot = 0;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) {
+    const unsigned int x = base + k < n_buckets ? cnt[base + k] : 0u;
+    v[k] = tot;
+    tot += x;
+  }
+  unsigned int inc = tot;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const unsigned int y = __shfl_up_sync(0xffffffffu, inc, d);
+    if ((threadIdx.x & 31) >= d) inc += y;
+  }
+  if ((threadIdx.x & 31) == 31) s_w[threadIdx.x >> 5] = inc;
+  __syncthreads();
+  unsigned int off = 0;
+  for (int w = 0; w < (int)(threadIdx.x >> 5); ++w) off += s_w[w];
+  const unsigned int excl = off + inc - tot;
+#pragma unroll
+  for (int k = 0; k < 8; ++k)
+    if (base + k < n_buckets) cnt[base + k] = excl + v[k];
+  if (threadIdx.x == 255) bsum[blockIdx.x] = off + inc;
+}
+
+constexpr int kMaxScanBlocks = 512;  // 2^20 buckets / kScanBlock
+__global__ void __launch_bounds__(256) sort_scatter_kernel(uint64_t first, uint32_t n, uint64_t seed, int g,
+                                                           unsigned int* __restrict__ cnt, const unsigned int* __restrict__ bsum,
+                                                           int n_scan_blocks, uint32_t* __restrict__ order) {
+  __shared__ unsigned int s_pre[kMaxScanBlocks];
+  __shared__ unsigned int s_w[8];
+  {  // exclusive scan of the block totals, two per thread
+    const int t = threadIdx.x;
+    const unsigned int a = 2 * t < n_scan_blocks ? bsum[2 * t] : 0u, b = 2 * t + 1 < n_scan_blocks ? bsum[2 * t + 1] : 0u;
+    unsigned int inc = a + b;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const unsigned int y = __shfl_up_sync(0xffffffffu, inc, d);
+      if ((t & 31) >= d) inc += y;
+    }
+    if ((t & 31) == 31) s_w[t >> 5] = inc;
+    __syncthreads();
+    unsigned int off = 0;
+    for (int w = 0; w < (t >> 5); ++w) off += s_w[w];
+    const unsigned int excl = off + inc - (a + b);
+    s_pre[2 * t] = excl;
+    s_pre[2 * t + 1] = excl + a;
+    __syncthreads();
+  }
+  const uint32_t stride = gridDim.x * blockDim.x;
+  for (uint32_t q = blockIdx.x * blockDim.x + threadIdx.x; q < n; q += stride) {
+    const uint32_t key = sort_key(seed, first + q, g);
+    const uint32_t pos = s_pre[key / kScanBlock] + atomicAdd(&cnt[key], 1u);
+    order[pos] = q;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// The megakernel.  FEAT selects which component kinds are compiled in; DUMP writes per-ray fates instead of
+// tallying.  Shared memory: the instrument image, per-block ray-accounting counters, the solids of every group,
+// per-thread mu[] for the voxel walk.  Spectrum CDFs and mu(E) tables are read through L1.
+// ------------------------------------------------------------------------------------------------------------
+constexpr int kTile = 2048;        // positions per work ticket
+constexpr int kSmemSolids = 32;    // solids staged in shared memory (all groups together)
+
 template <int FEAT, bool DUMP>
-__global__ void __launch_bounds__(kBlock) trace_kernel(const DInstrument* __restrict__ g_inst, uint64_t first, uint64_t n,
-                                                       uint64_t seed, mcx_ray_fate* __restrict__ dump) {
+__global__ void __launch_bounds__(kBlock) trace_kernel(const DInstrument* __restrict__ g_inst, TraceArgs A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   DInstrument& I = *reinterpret_cast<DInstrument*>(smem_raw);
   unsigned int* s_cnt = reinterpret_cast<unsigned int*>(smem_raw + sizeof(DInstrument));  // [MCX_MAX_COMPONENTS + 4]
-  double* mu_s = reinterpret_cast<double*>(smem_raw + sizeof(DInstrument) + 128) + threadIdx.x;
+  unsigned int& s_tile = s_cnt[MCX_MAX_COMPONENTS + 4];
+  unsigned char* s_extra = smem_raw + sizeof(DInstrument) + 128;
   {
     const int4* src = reinterpret_cast<const int4*>(g_inst);
     int4* dst = reinterpret_cast<int4*>(smem_raw);
@@ -618,88 +705,126 @@ __global__ void __launch_bounds__(kBlock) trace_kernel(const DInstrument* __rest
   }
   __syncthreads();
   const int n_comps = I.n_comps;
-  const int lane = threadIdx.x & 31;
-  const uint64_t stride = (uint64_t)gridDim.x * kBlock;
-  // whole warps iterate together so that the ballots below are always full-warp
-  const uint64_t n_round = (n + 31u) & ~(uint64_t)31u;
-  for (uint64_t q = (uint64_t)blockIdx.x * kBlock + threadIdx.x; q < n_round; q += stride) {
-    const bool valid = q < n;
-    Ray ray;
-    int fate = MCX_FATE_MISSED;
-    long long bin = -1;
-    bool alive = valid;
-    if (valid) sample_source(I.comps[0], seed, first + q, ray);
+  if (FEAT & F_SOLIDS) {  // stage the solids (poses, sizes, priorities) of every group and re-point the groups at the copy
+    DSolid* s_solids = reinterpret_cast<DSolid*>(s_extra);
+    s_extra += kSmemSolids * sizeof(DSolid);
+    int used = 0;
     for (int c = 1; c < n_comps; ++c) {
-      const DComponent& C = I.comps[c];
-      const int kind = C.kind;  // warp-uniform
-      bool pass = true;
-      if (alive) {
-        if (kind == MCX_SLIT_RECT) {
-          Vec3 h;
-          pass = plane_hit(C.pose, ray, h) && fabs(h.x) <= C.u.slit.half_x && fabs(h.y) <= C.u.slit.half_y;
-        } else if (kind == MCX_SLIT_CIRC) {
-          Vec3 h;
-          pass = plane_hit(C.pose, ray, h) && h.x * h.x + h.y * h.y <= C.u.slit.radius2;
-        } else if ((FEAT & F_SOLIDS) && kind == MCX_SOLIDS) {
-          const int rc = trace_solids<(FEAT & F_MESH) != 0>(I, C, ray);
-          if (rc != 1) {
-            pass = false;
-            fate = MCX_FATE_DEGENERATE;
-            if (rc < 0 && !DUMP) atomicAdd(&s_cnt[MCX_MAX_COMPONENTS + CNT_OVERFLOW], 1u);
-          }
-        } else if ((FEAT & F_VOXELS) && kind == MCX_VOXELS) {
-          trace_voxels(I, C, ray, mu_s);
-        } else if ((FEAT & F_OPTICS) && kind == MCX_MIRROR_ELLIPTIC) {
-          pass = trace_mirror(C, ray);
-        } else if ((FEAT & F_OPTICS) && kind == MCX_CRYSTAL_BRAGG) {
-          pass = trace_crystal(C, ray);
-        } else if (kind == MCX_DETECTOR) {
-          const long long b = detector_bin(C, ray);
-          if (b >= 0) {
-            bin = b;
-            fate = MCX_FATE_DETECTED;
-            if (!DUMP) {
-              TallyBin* rec = I.tallies[C.u.detector.index] + b;
-              atomicAdd(&rec->N, 1ull);
-              atomicAdd(&rec->P, ray.p);
-              atomicAdd(&rec->P2, ray.p * ray.p);
-            }
-          } else {
-            fate = MCX_FATE_MISSED;  // monitors do not absorb: the ray goes on
-          }
-        }
-        if (kind != MCX_DETECTOR && pass) fate = MCX_FATE_MISSED;  // fate = what the last component said
-        if (!pass) {
-          alive = false;
-          if (fate != MCX_FATE_DEGENERATE) fate = c;
-        }
-      }
-      const unsigned alive_mask = __ballot_sync(0xffffffffu, alive);
-      if (!DUMP) {
-        // warp-aggregated ray accounting: one shared-memory add per warp and component
-        const unsigned died = __ballot_sync(0xffffffffu, !pass && fate == c);
-        if (lane == 0 && died) atomicAdd(&s_cnt[c], (unsigned)__popc(died));
-      }
-      if (alive_mask == 0u) break;
+      if (I.comps[c].kind != MCX_SOLIDS) continue;
+      const int ns = I.comps[c].u.solids.n_solids;
+      if (used + ns > kSmemSolids) continue;
+      const unsigned long long* src = reinterpret_cast<const unsigned long long*>(I.comps[c].u.solids.solids);
+      unsigned long long* dst = reinterpret_cast<unsigned long long*>(s_solids + used);
+      for (int k = threadIdx.x; k < ns * (int)(sizeof(DSolid) / 8); k += kBlock) dst[k] = src[k];
+      __syncthreads();
+      if (threadIdx.x == 0) I.comps[c].u.solids.solids = s_solids + used;
+      used += ns;
     }
-    if (DUMP) {
-      if (valid) {
-        mcx_ray_fate f;
-        f.fate = fate;
-        f.reserved = 0;
-        f.bin = fate == MCX_FATE_DETECTED ? bin : -1;
-        f.p = ray.p;
-        dump[q] = f;
+    __syncthreads();
+  }
+  double* mu_s = reinterpret_cast<double*>(s_extra) + threadIdx.x;
+  const int lane = threadIdx.x & 31;
+  const uint64_t first = A.first, n = A.n, seed = A.seed;
+  const uint32_t* __restrict__ order = A.order;
+  mcx_ray_fate* __restrict__ dump = A.dump;
+  // Lane scheduling (row a13): blocks pull tiles of kTile consecutive positions from a ticket counter, so the tail of
+  // a launch is one tile long whatever the per-ray cost.  With `order` set, position q holds the q-th ray of the
+  // chunk in detector-tile order (kernels above); whole warps iterate together so the ballots are full-warp.
+  for (;;) {
+    if (threadIdx.x == 0) s_tile = atomicAdd(A.ticket, 1u);
+    __syncthreads();
+    const uint64_t tile_begin = (uint64_t)s_tile * kTile;
+    __syncthreads();
+    if (tile_begin >= n) break;
+    for (uint64_t q = tile_begin + threadIdx.x; q < tile_begin + kTile; q += kBlock) {
+      if (q - lane >= n) break;  // the whole warp is beyond the end
+      const bool valid = q < n;
+      const uint64_t qi = valid ? (order ? (uint64_t)order[q] : q) : 0;  // position in the chunk -> ray offset
+      Ray ray;
+      int fate = MCX_FATE_MISSED;
+      long long bin = -1;
+      bool alive = valid;
+      if (valid) sample_source(I.comps[0], seed, first + qi, ray);
+      for (int c = 1; c < n_comps; ++c) {
+        const DComponent& C = I.comps[c];
+        const int kind = C.kind;  // warp-uniform
+        bool pass = true;
+        if (alive) {
+          if (kind == MCX_SLIT_RECT) {
+            Vec3 h;
+            pass = plane_hit(C.pose, ray, h) && fabs(h.x) <= C.u.slit.half_x && fabs(h.y) <= C.u.slit.half_y;
+          } else if (kind == MCX_SLIT_CIRC) {
+            Vec3 h;
+            pass = plane_hit(C.pose, ray, h) && h.x * h.x + h.y * h.y <= C.u.slit.radius2;
+          } else if ((FEAT & F_SOLIDS) && kind == MCX_SOLIDS) {
+            const int rc = trace_solids<(FEAT & F_MESH) != 0>(I, C, ray);
+            if (rc != 1) {
+              pass = false;
+              fate = MCX_FATE_DEGENERATE;
+              if (rc < 0 && !DUMP) atomicAdd(&s_cnt[MCX_MAX_COMPONENTS + CNT_OVERFLOW], 1u);
+            }
+          } else if ((FEAT & F_VOXELS) && kind == MCX_VOXELS) {
+            trace_voxels(I, C, ray, mu_s);
+          } else if ((FEAT & F_OPTICS) && kind == MCX_MIRROR_ELLIPTIC) {
+            pass = trace_mirror(C, ray);
+          } else if ((FEAT & F_OPTICS) && kind == MCX_CRYSTAL_BRAGG) {
+            pass = trace_crystal(C, ray);
+          } else if (kind == MCX_DETECTOR) {
+            const long long b = detector_bin(C, ray);
+            if (b >= 0) {
+              bin = b;
+              fate = MCX_FATE_DETECTED;
+              if (!DUMP) {
+                TallyBin* rec = I.tallies[C.u.detector.index] + b;
+                atomicAdd(&rec->N, 1ull);
+                atomicAdd(&rec->P, ray.p);
+                atomicAdd(&rec->P2, ray.p * ray.p);
+              }
+            } else {
+              fate = MCX_FATE_MISSED;  // monitors do not absorb: the ray goes on
+            }
+          }
+          if (kind != MCX_DETECTOR && pass) fate = MCX_FATE_MISSED;  // fate = what the last component said
+          if (!pass) {
+            alive = false;
+            if (fate != MCX_FATE_DEGENERATE) fate = c;
+          }
+        }
+        const unsigned alive_mask = __ballot_sync(0xffffffffu, alive);
+        if (!DUMP) {
+          // warp-aggregated ray accounting: one shared-memory add per warp and component
+          const unsigned died = __ballot_sync(0xffffffffu, !pass && fate == c);
+          if (lane == 0 && died) atomicAdd(&s_cnt[c], (unsigned)__popc(died));
+        }
+        if (alive_mask == 0u) break;
       }
-    } else {
-      const unsigned det = __ballot_sync(0xffffffffu, valid && fate == MCX_FATE_DETECTED);
-      const unsigned mis = __ballot_sync(0xffffffffu, valid && fate == MCX_FATE_MISSED);
-      const unsigned deg = __ballot_sync(0xffffffffu, valid && fate == MCX_FATE_DEGENERATE);
-      if (lane == 0) {
-        if (det) atomicAdd(&s_cnt[MCX_MAX_COMPONENTS + CNT_DETECTED], (unsigned)__popc(det));
-        if (mis) atomicAdd(&s_cnt[MCX_MAX_COMPONENTS + CNT_MISSED], (unsigned)__popc(mis));
-        if (deg) atomicAdd(&s_cnt[MCX_MAX_COMPONENTS + CNT_DEGENERATE], (unsigned)__popc(deg));
+      if (DUMP) {
+        if (valid) {
+          mcx_ray_fate f;
+          f.fate = fate;
+          f.reserved = 0;
+          f.bin = fate == MCX_FATE_DETECTED ? bin : -1;
+          f.p = ray.p;
+          dump[qi] = f;
+        }
+      } else {
+        const unsigned det = __ballot_sync(0xffffffffu, valid && fate == MCX_FATE_DETECTED);
+        const unsigned mis = __ballot_sync(0xffffffffu, valid && fate == MCX_FATE_MISSED);
+        const unsigned deg = __ballot_sync(0xffffffffu, valid && fate == MCX_FATE_DEGENERATE);
+        if (lane == 0) {
+          if (det) atomicAdd(&s_cnt[MCX_MAX_COMPONENTS + CNT_DETECTED], (unsigned)__popc(det));
+          if (mis) atomicAdd(&s_cnt[MCX_MAX_COMPONENTS + CNT_MISSED], (unsigned)__popc(mis));
+          if (deg) atomicAdd(&s_cnt[MCX_MAX_COMPONENTS + CNT_DEGENERATE], (unsigned)__popc(deg));
+        }
       }
+    }
+  }
+  // the last block to leave re-arms the ticket counter for the next launch
+  if (threadIdx.x == 0) {
+    __threadfence();
+    if (atomicAdd(A.ticket + 1, 1u) == gridDim.x - 1) {
+      A.ticket[0] = 0u;
+      A.ticket[1] = 0u;
     }
   }
   if (!DUMP) {
@@ -762,11 +887,11 @@ __global__ void __launch_bounds__(256) probe_dfma_kernel(double* sink, long long
 constexpr size_t kSmemBase = sizeof(DInstrument) + 128;
 
 template <int FEAT, bool DUMP>
-cudaError_t launch_one(const DInstrument* d_inst, int n_mats, uint64_t first, uint64_t n, uint64_t seed, mcx_ray_fate* dump,
-                       cudaStream_t stream, int n_sm) {
-  const size_t smem = kSmemBase + ((FEAT & F_VOXELS) ? (size_t)n_mats * kBlock * sizeof(double) : 0);
+cudaError_t launch_one(const DInstrument* d_inst, int n_mats, const TraceArgs& A, cudaStream_t stream, int n_sm) {
+  const size_t smem = kSmemBase + ((FEAT & F_SOLIDS) ? kSmemSolids * sizeof(DSolid) : 0) +
+                      ((FEAT & F_VOXELS) ? (size_t)n_mats * kBlock * sizeof(double) : 0);
   static bool configured = false;
-  static int blocks_per_sm = 1;
+  int blocks_per_sm = 1;
   cudaError_t e;
   if (!configured) {
     e = cudaFuncSetAttribute(trace_kernel<FEAT, DUMP>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
@@ -776,10 +901,10 @@ cudaError_t launch_one(const DInstrument* d_inst, int n_mats, uint64_t first, ui
   e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, trace_kernel<FEAT, DUMP>, kBlock, smem);
   if (e != cudaSuccess) return e;
   if (blocks_per_sm < 1) return cudaErrorInvalidConfiguration;
-  const uint64_t want = (n + kBlock - 1) / kBlock;
+  const uint64_t want = (A.n + kTile - 1) / kTile;
   const uint64_t full = (uint64_t)n_sm * blocks_per_sm;  // one resident wave: a multiple of the SM count
   const unsigned grid = (unsigned)(want < full ? (want ? want : 1) : full);
-  trace_kernel<FEAT, DUMP><<<grid, kBlock, smem, stream>>>(d_inst, first, n, seed, dump);
+  trace_kernel<FEAT, DUMP><<<grid, kBlock, smem, stream>>>(d_inst, A);
   return cudaGetLastError();
 }
 
@@ -795,14 +920,14 @@ cudaError_t kernels_init() {
   return cudaDeviceGetAttribute(&g_n_sm, cudaDevAttrMultiProcessorCount, dev);
 }
 
-cudaError_t launch_trace(const DInstrument* d_inst, int features, int n_mats, uint64_t first, uint64_t n, uint64_t seed,
-                         mcx_ray_fate* dump, cudaStream_t stream) {
+cudaError_t launch_trace(const DInstrument* d_inst, int features, int n_mats, const TraceArgs& A, cudaStream_t stream) {
   cudaError_t e = kernels_init();
   if (e != cudaSuccess) return e;
-  if (n == 0) return cudaSuccess;
-#define MCX_DISPATCH(F)                                                                                  \
-  return dump ? launch_one<F, true>(d_inst, n_mats, first, n, seed, dump, stream, g_n_sm)                \
-              : launch_one<F, false>(d_inst, n_mats, first, n, seed, dump, stream, g_n_sm);
+  if (A.n == 0) return cudaSuccess;
+  if (A.n > ((uint64_t)1 << 40)) return cudaErrorInvalidValue;  // tile tickets are 32-bit; the host chunks below this
+#define MCX_DISPATCH(F)                                                              \
+  return A.dump ? launch_one<F, true>(d_inst, n_mats, A, stream, g_n_sm)             \
+                : launch_one<F, false>(d_inst, n_mats, A, stream, g_n_sm);
   switch (features) {
     case 0: MCX_DISPATCH(0)
     case F_SOLIDS: MCX_DISPATCH(F_SOLIDS)
@@ -812,6 +937,22 @@ cudaError_t launch_trace(const DInstrument* d_inst, int features, int n_mats, ui
     default: MCX_DISPATCH(F_ALL)
   }
 #undef MCX_DISPATCH
+}
+
+// count -> scan -> scatter of one chunk (n <= 2^32 - 1 rays, 4^g buckets); cnt must be zero on entry
+cudaError_t launch_sort(uint64_t first, uint32_t n, uint64_t seed, int g, unsigned int* cnt, unsigned int* bsum,
+                        uint32_t* order, cudaStream_t stream) {
+  cudaError_t e = kernels_init();
+  if (e != cudaSuccess) return e;
+  const uint32_t n_buckets = 1u << (2 * g);
+  const int n_scan_blocks = (int)((n_buckets + kScanBlock - 1) / kScanBlock);
+  if (g < 1 || g > 10 || n_scan_blocks > kMaxScanBlocks) return cudaErrorInvalidValue;
+  const unsigned want = (n + 255u) / 256u;
+  const unsigned grid = want < (unsigned)g_n_sm * 8u ? (want ? want : 1u) : (unsigned)g_n_sm * 8u;
+  sort_count_kernel<<<grid, 256, 0, stream>>>(first, n, seed, g, cnt);
+  sort_scan_kernel<<<n_scan_blocks, 256, 0, stream>>>(cnt, n_buckets, bsum);
+  sort_scatter_kernel<<<grid, 256, 0, stream>>>(first, n, seed, g, cnt, bsum, n_scan_blocks, order);
+  return cudaGetLastError();
 }
 
 cudaError_t launch_tally_read(const TallyBin* bins, uint64_t n_bins, unsigned long long* N, double* p, double* p2,

@@ -18,8 +18,9 @@ def M():
     return m
 
 
-def run_gpu(M, inst, n, first, seed, strict):
+def run_gpu(M, inst, n, first, seed, strict, mode="auto"):
     g = M.Instrument(inst, strict=strict)
+    g.set_exec(mode)
     gdump = g.trace_dump(first, n, seed)
     g.trace(n, seed, first)
     gt = [tuple(t.cpu().numpy() for t in g.tally(d)) for d in range(len(g.dets))]
@@ -31,17 +32,19 @@ def run_gpu(M, inst, n, first, seed, strict):
 
 def check(M, O, W, inst, n, exact_counts=False, first=0, seed=None, mesh_accel=0):
     """Traces rays [first, first+n) with the oracle and with both builds of the CUDA library (default, and
-    -fmad=false = 'strict') and holds each against the parity bar of _parity.py."""
+    -fmad=false = 'strict'), in both lane schedules (index order and detector-tile order),
+    and holds each against the parity bar of _parity.py."""
     seed = inst["seed"] if seed is None else seed
     o = O.trace(inst, first=first, n=n, seed=seed, dump=True, mesh_accel=mesh_accel)
     out = {}
     for strict in (True, False):
-        out[strict] = check_one(M, W, inst, n, o, exact_counts, first, seed, strict)
+        for mode in ("direct", "sorted"):
+            out[strict] = check_one(M, W, inst, n, o, exact_counts, first, seed, strict, mode)
     return out[False]
 
 
-def check_one(M, W, inst, n, o, exact_counts, first, seed, strict):
-    gdump, gt, gc = run_gpu(M, inst, n, first, seed, strict)
+def check_one(M, W, inst, n, o, exact_counts, first, seed, strict, mode="auto"):
+    gdump, gt, gc = run_gpu(M, inst, n, first, seed, strict, mode)
     st = assert_dump_parity(gdump, o["dump"], strict=strict)
     nb = [W.n_bins(d) for d in W.detectors_of(inst)]
     if st["n_diff"] == 0:
@@ -105,6 +108,28 @@ def test_c3_mesh_larger_prefix(M, O, W):
 def test_c4_voxels(M, O, W):
     check(M, O, W, W.config4(small=True), 100_001)
     check(M, O, W, W.config4(small=True, n_vox=96), 30_000)
+
+
+def test_sorted_order_is_a_permutation_over_several_chunks(M, O, W, monkeypatch):
+    """Detector-tile order with chunks of 2^15 rays: 100 003 rays = three full chunks + a ragged one that is still
+    sorted + (in the second case) a tail short enough to be traced in index order.  Every ray must be traced exactly
+    once: the dump equals the oracle's ray by ray and the tallies equal the sums of the dump."""
+    monkeypatch.setenv("MCX_CHUNK_LOG2", "15")
+    inst = W.config1(small=True)
+    for n in (100_003, 3 * 32768 + 1000):
+        o = O.trace(inst, first=7, n=n, dump=True)
+        check_one(M, W, inst, n, o, False, 7, inst["seed"], True, "sorted")
+    inst = W.config0()
+    o = O.trace(inst, first=0, n=200_000, dump=True)
+    st = check_one(M, W, inst, 200_000, o, True, 0, inst["seed"], False, "sorted")
+    assert st["n_diff"] == 0
+
+
+def test_exec_mode_argument_is_checked(M, W):
+    g = M.Instrument(W.config0())
+    with pytest.raises(M.McxError):
+        M.binding._check(g.L.mcx_instrument_set_exec(g.handle, 7), g.L)
+    g.close()
 
 
 def test_empty_trace_and_accumulation(M, O, W):
