@@ -67,8 +67,8 @@ struct DVoxels {
   double h;
   int n[3];       // nx, ny, nz
   int fast;       // axis stored fastest in the traversal layout
-  int a1, a2;     // the other two axes: address = (i[a2] * n[a1] + i[a1]) * pitch + i[fast]
-  int pitch;      // n[fast] rounded up to a multiple of 16
+  int a1, a2;     // the other two axes: offset = ((i[a2]+1) * (n[a1]+2) + i[a1]+1) * pitch + i[fast]+1 (guard border)
+  int pitch;      // n[fast] + 2 rounded up to a multiple of 16
   const uint8_t* ids;
 };
 

@@ -175,7 +175,9 @@ struct Plan {
   size_t off_tris[MCX_MAX_COMPONENTS][MCX_MAX_SOLIDS];
 };
 
-int voxel_pitch(int64_t n_fast) { return (int)((n_fast + 15) / 16 * 16); }
+// traversal layout of a voxel volume: one guard cell on every side, rows padded to 16 bytes
+int voxel_pitch(int64_t n_fast) { return (int)((n_fast + 2 + 15) / 16 * 16); }
+size_t voxel_bytes(int64_t n_fast, int64_t n_1, int64_t n_2) { return (size_t)(n_2 + 2) * (size_t)(n_1 + 2) * (size_t)voxel_pitch(n_fast); }
 
 // chooses the axis stored fastest: the voxel axis most aligned with the line from the source to the volume centre
 void voxel_axes(const mcx_component& src, const mcx_component& vox, int* fast, int* a1, int* a2) {
@@ -260,7 +262,10 @@ mcx_status make_plan(const mcx_component* comps, int n_comps, const mcx_material
       int f, a1, a2;
       voxel_axes(comps[0], comps[c], &f, &a1, &a2);
       const int64_t n[3] = {V.nx, V.ny, V.nz};
-      P->off_voxels[c] = A.reserve((size_t)n[a2] * n[a1] * voxel_pitch(n[f]));
+      if (voxel_bytes(n[f], n[a1], n[a2]) > 0xFFFFFFFFull)
+        return fail(MCX_ERR_UNSUPPORTED, "component %d: voxel volume above 4 GiB (the walk uses 32-bit voxel offsets)", c);
+      // twice the size: create shifts the volume past a 4 GiB address boundary if it would straddle one
+      P->off_voxels[c] = A.reserve(2 * voxel_bytes(n[f], n[a1], n[a2]));
     }
   P->zero_begin = A.top;
   int d = 0;
@@ -481,8 +486,13 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
         d.n[0] = (int)V.nx; d.n[1] = (int)V.ny; d.n[2] = (int)V.nz;
         voxel_axes(components[0], C, &d.fast, &d.a1, &d.a2);
         d.pitch = voxel_pitch(d.n[d.fast]);
-        d.ids = (const uint8_t*)dev_ptr(P.off_voxels[c]);
-        const cudaError_t e = launch_voxel_relayout(V.ids, (uint8_t*)dev_ptr(P.off_voxels[c]), d.n[0], d.n[1], d.n[2], d.fast,
+        {  // keep [ids, ids + bytes) inside one 4 GiB window of the address space (32-bit stepping in the walk)
+          const size_t bytes = voxel_bytes(d.n[d.fast], d.n[d.a1], d.n[d.a2]);
+          uintptr_t p0 = (uintptr_t)dev_ptr(P.off_voxels[c]);
+          if ((p0 >> 32) != ((p0 + bytes - 1) >> 32)) p0 = ((p0 >> 32) + 1) << 32;
+          d.ids = (const uint8_t*)p0;
+        }
+        const cudaError_t e = launch_voxel_relayout(V.ids, (uint8_t*)d.ids, d.n[0], d.n[1], d.n[2], d.fast,
                                                     d.a1, d.a2, d.pitch, stream);
         if (e != cudaSuccess) { const mcx_status s_ = cuda_fail(e, "voxel relayout"); delete H; return s_; }
         H->launches++;

@@ -15,6 +15,7 @@ constexpr int kBlock = 256;
 constexpr int kMaxIntervals = 32;  // per ray and solids group
 constexpr int kMaxHits = 32;       // per ray and mesh
 constexpr int kBvhStack = 64;
+constexpr unsigned kVoxelGuard = 255u;  // ID of the guard cells around the voxel volume (material IDs are < MCX_MAX_MATERIALS)
 
 // ------------------------------------------------------------------------------------------------------------
 // Step 1: Philox4x32-10 (Salmon et al., SC'11); key = seed, counter = (i lo, i hi, slot, component).
@@ -440,8 +441,23 @@ __device__ int trace_solids(const DInstrument& I, const DComponent& C, Ray& ray)
 // Step 11: exact traversal of the voxel grid (Amanatides & Woo 1987).  tau = sum over the voxels crossed of
 // mu[id] * length.  The product is taken once per RUN of equal material IDs (same real number, fewer roundings):
 // PAPER.md:186-188 names this loop ("steps reach into the thousands") as where the EDXCT time goes.
+//
+// The volume sits in the workspace in traversal layout with a one-voxel guard border of kVoxelGuard on every
+// side (DVoxels), so the walk needs no index or bounds arithmetic: a step adds one of three constant offsets to
+// a 32-bit voxel offset, and stepping onto a guard cell ends the walk.  One iteration = one face crossing and is
+// branch-free apart from the (rare) change of material: three compares pick the axis with the nearest face
+// (the same fp64 face parameters, accumulated by the same additions, as the oracle's), three predicated adds
+// advance it.  Rays of one warp differ in where they cross the lateral faces, and a predicated step costs the same
+// whichever axis a lane takes, so there is nothing to diverge on.
 // mu_s: per-thread mu of every material, shared memory, element m at mu_s[m * kBlock].
 // ------------------------------------------------------------------------------------------------------------
+// x += p ? y : 0 in two instructions (one select, one DADD): when p is false the HIGH word of the addend is zeroed,
+// which leaves a denormal below 2^-1022; for the face parameters here (x >= 2^-1000 or so) x + denormal == x exactly,
+// so the result is bit-identical to not adding.  (A predicated add compiles to an add and two selects.)
+__device__ __forceinline__ void add_if(double& x, double y, bool p) {
+  x += __hiloint2double(p ? __double2hiint(y) : 0, __double2loint(y));
+}
+
 __device__ __forceinline__ void trace_voxels(const DInstrument& I, const DComponent& C, Ray& ray, double* mu_s) {
   const DVoxels& V = C.u.voxels;
   const Vec3 ol = to_local(C.pose, ray.r);
@@ -475,40 +491,33 @@ __device__ __forceinline__ void trace_voxels(const DInstrument& I, const DCompon
   MCX_AXIS_INIT(o1, d1, n1, i_1, s_1, tm_1, td_1)
   MCX_AXIS_INIT(o2, d2, n2, i_2, s_2, tm_2, td_2)
 #undef MCX_AXIS_INIT
-  const uint8_t* __restrict__ ids = V.ids;
-  const int pitch = V.pitch;
-  long long row = ((long long)i_2 * n1 + i_1) * pitch;  // address of (i_2, i_1, 0)
-  const long long row_step1 = (long long)s_1 * pitch, row_step2 = (long long)s_2 * n1 * pitch;
-  int cur = ids[row + i_f];
+  const unsigned pitch = (unsigned)V.pitch, slab = (unsigned)(n1 + 2) * pitch;
+  const unsigned so_f = (unsigned)s_f, so_1 = (unsigned)s_1 * pitch, so_2 = (unsigned)s_2 * slab;  // mod 2^32
+  // The volume does not straddle a 4 GiB address boundary (mcx_instrument_create places it so): the walk keeps the
+  // low address word only and a step is one 32-bit add.
+  const unsigned long long base = (unsigned long long)V.ids;
+  const unsigned long long hi = base & 0xFFFFFFFF00000000ull;
+  unsigned lo = (unsigned)base + (unsigned)(i_2 + 1) * slab + (unsigned)(i_1 + 1) * pitch + (unsigned)(i_f + 1);
+  unsigned cur = __ldg(reinterpret_cast<const uint8_t*>(hi | lo));
   double tau = 0.0, t_run = t0;
   // Tie rule of step 11: the lowest of (x, y, z) wins.  Ties only order zero-length visits, so the traversal
   // order (f, a1, a2) used here gives the same tau.
-  while (true) {
-    double tn;
-    if (tm_f <= tm_1 && tm_f <= tm_2) {
-      tn = tm_f;
-      i_f += s_f;
-      if ((unsigned)i_f >= (unsigned)nf) { tn = fmin(tn, t1); tau += mu_s[cur * kBlock] * (tn - t_run); break; }
-      tm_f += td_f;
-    } else if (tm_1 <= tm_2) {
-      tn = tm_1;
-      i_1 += s_1;
-      if ((unsigned)i_1 >= (unsigned)n1) { tn = fmin(tn, t1); tau += mu_s[cur * kBlock] * (tn - t_run); break; }
-      tm_1 += td_1;
-      row += row_step1;
-    } else {
-      tn = tm_2;
-      i_2 += s_2;
-      if ((unsigned)i_2 >= (unsigned)n2) { tn = fmin(tn, t1); tau += mu_s[cur * kBlock] * (tn - t_run); break; }
-      tm_2 += td_2;
-      row += row_step2;
-    }
-    const int id = ids[row + i_f];
-    if (id != cur) {
+  for (;;) {
+    const bool pf = tm_f <= tm_1 && tm_f <= tm_2;
+    const bool p1 = !pf && tm_1 <= tm_2;
+    const bool p2 = !pf && !p1;
+    lo += pf ? so_f : (p1 ? so_1 : so_2);
+    const unsigned id = __ldg(reinterpret_cast<const uint8_t*>(hi | lo));
+    if (id != cur) {  // a run of equal IDs ends at the face just crossed (or, on a guard cell, at the exit t1)
+      const double tn = fmin(pf ? tm_f : (p1 ? tm_1 : tm_2), t1);
       tau += mu_s[cur * kBlock] * (tn - t_run);
       t_run = tn;
       cur = id;
+      if (id == kVoxelGuard) break;  // left the grid
     }
+    add_if(tm_f, td_f, pf);
+    add_if(tm_1, td_1, p1);
+    add_if(tm_2, td_2, p2);
   }
   ray.p *= exp(-tau);
 }
@@ -852,18 +861,19 @@ __global__ void __launch_bounds__(256) tally_read_kernel(const TallyBin* __restr
   }
 }
 
-// Voxel volume from the interface layout [iz][iy][ix] into the traversal layout [i_a2][i_a1][i_fast (pitch)].
+// Voxel volume from the interface layout [iz][iy][ix] into the traversal layout [i_a2 + 1][i_a1 + 1][i_fast + 1]
+// (rows of `pitch` bytes) with a guard border of kVoxelGuard around it.
 __global__ void __launch_bounds__(256) voxel_relayout_kernel(const uint8_t* __restrict__ src, uint8_t* __restrict__ dst,
                                                              int nx, int ny, int nz, int fast, int a1, int a2, int pitch) {
   const int n[3] = {nx, ny, nz};
-  const long long total = (long long)n[a2] * n[a1] * pitch;
+  const long long total = (long long)(n[a2] + 2) * (n[a1] + 2) * pitch;
   const long long stride = (long long)gridDim.x * blockDim.x;
   for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < total; k += stride) {
-    const int jf = (int)(k % pitch);
+    const int jf = (int)(k % pitch) - 1;
     const long long rowi = k / pitch;
-    const int j1 = (int)(rowi % n[a1]), j2 = (int)(rowi / n[a1]);
-    uint8_t v = 0;
-    if (jf < n[fast]) {
+    const int j1 = (int)(rowi % (n[a1] + 2)) - 1, j2 = (int)(rowi / (n[a1] + 2)) - 1;
+    uint8_t v = (uint8_t)kVoxelGuard;
+    if (jf >= 0 && jf < n[fast] && j1 >= 0 && j1 < n[a1] && j2 >= 0 && j2 < n[a2]) {
       int idx[3];
       idx[fast] = jf; idx[a1] = j1; idx[a2] = j2;
       v = src[((long long)idx[2] * ny + idx[1]) * nx + idx[0]];
