@@ -69,6 +69,8 @@ struct DVoxels {
   int fast;       // axis stored fastest in the traversal layout
   int a1, a2;     // the other two axes: offset = ((i[a2]+1) * (n[a1]+2) + i[a1]+1) * pitch + i[fast]+1 (guard border)
   int pitch;      // n[fast] + 2 rounded up to a multiple of 16
+  unsigned slab;  // (n[a1] + 2) * pitch
+  unsigned mg_pitch, sh_pitch, mg_slab, sh_slab;  // x / pitch, x / slab by multiplication (fast_div in mcx_kernels.cu)
   const uint8_t* ids;
 };
 

@@ -178,6 +178,18 @@ struct Plan {
 // traversal layout of a voxel volume: one guard cell on every side, rows padded to 16 bytes
 int voxel_pitch(int64_t n_fast) { return (int)((n_fast + 2 + 15) / 16 * 16); }
 size_t voxel_bytes(int64_t n_fast, int64_t n_1, int64_t n_2) { return (size_t)(n_2 + 2) * (size_t)(n_1 + 2) * (size_t)voxel_pitch(n_fast); }
+// The walk issues the loads of the slab after the one it is looking at; past a guard cell these reach at most one step
+// along every axis further.  That much of the workspace on either side of the volume belongs to the volume.
+size_t voxel_pad(int64_t n_fast, int64_t n_1) { return align_up((size_t)(n_1 + 3) * (size_t)voxel_pitch(n_fast) + 16); }
+
+// n / d == (t + ((n - t) >> 1)) >> sh with t = mulhi(m, n), for every 32-bit n and d >= 2 (Granlund & Montgomery 1994,
+// "Division by invariant integers using multiplication", the 33-bit multiplier case)
+void fast_div_constants(unsigned d, unsigned* m, unsigned* sh) {
+  unsigned L = 0;
+  while (((uint64_t)1 << L) < d) ++L;  // ceil(log2 d) >= 1
+  *m = (unsigned)((((uint64_t)1 << 32) * (((uint64_t)1 << L) - d)) / d + 1);
+  *sh = L - 1;
+}
 
 // chooses the axis stored fastest: the voxel axis most aligned with the line from the source to the volume centre
 void voxel_axes(const mcx_component& src, const mcx_component& vox, int* fast, int* a1, int* a2) {
@@ -262,10 +274,10 @@ mcx_status make_plan(const mcx_component* comps, int n_comps, const mcx_material
       int f, a1, a2;
       voxel_axes(comps[0], comps[c], &f, &a1, &a2);
       const int64_t n[3] = {V.nx, V.ny, V.nz};
-      if (voxel_bytes(n[f], n[a1], n[a2]) > 0xFFFFFFFFull)
+      if (voxel_bytes(n[f], n[a1], n[a2]) + 2 * voxel_pad(n[f], n[a1]) > 0xFFFFFFFFull)
         return fail(MCX_ERR_UNSUPPORTED, "component %d: voxel volume above 4 GiB (the walk uses 32-bit voxel offsets)", c);
       // twice the size: create shifts the volume past a 4 GiB address boundary if it would straddle one
-      P->off_voxels[c] = A.reserve(2 * voxel_bytes(n[f], n[a1], n[a2]));
+      P->off_voxels[c] = A.reserve(2 * voxel_bytes(n[f], n[a1], n[a2]) + 4 * voxel_pad(n[f], n[a1]));
     }
   P->zero_begin = A.top;
   int d = 0;
@@ -486,10 +498,14 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
         d.n[0] = (int)V.nx; d.n[1] = (int)V.ny; d.n[2] = (int)V.nz;
         voxel_axes(components[0], C, &d.fast, &d.a1, &d.a2);
         d.pitch = voxel_pitch(d.n[d.fast]);
-        {  // keep [ids, ids + bytes) inside one 4 GiB window of the address space (32-bit stepping in the walk)
+        d.slab = (unsigned)(d.n[d.a1] + 2) * (unsigned)d.pitch;
+        fast_div_constants((unsigned)d.pitch, &d.mg_pitch, &d.sh_pitch);
+        fast_div_constants(d.slab, &d.mg_slab, &d.sh_slab);
+        {  // keep [ids - pad, ids + bytes + pad) inside one 4 GiB window of the address space (32-bit stepping in the walk)
           const size_t bytes = voxel_bytes(d.n[d.fast], d.n[d.a1], d.n[d.a2]);
-          uintptr_t p0 = (uintptr_t)dev_ptr(P.off_voxels[c]);
-          if ((p0 >> 32) != ((p0 + bytes - 1) >> 32)) p0 = ((p0 >> 32) + 1) << 32;
+          const size_t pad = voxel_pad(d.n[d.fast], d.n[d.a1]);
+          uintptr_t p0 = (uintptr_t)dev_ptr(P.off_voxels[c]) + pad;
+          if (((p0 - pad) >> 32) != ((p0 + bytes + pad - 1) >> 32)) p0 = ((((p0 + bytes + pad - 1) >> 32)) << 32) + pad;
           d.ids = (const uint8_t*)p0;
         }
         const cudaError_t e = launch_voxel_relayout(V.ids, (uint8_t*)d.ids, d.n[0], d.n[1], d.n[2], d.fast,

@@ -439,85 +439,220 @@ __device__ int trace_solids(const DInstrument& I, const DComponent& C, Ray& ray)
 
 // ------------------------------------------------------------------------------------------------------------
 // Step 11: exact traversal of the voxel grid (Amanatides & Woo 1987).  tau = sum over the voxels crossed of
-// mu[id] * length.  The product is taken once per RUN of equal material IDs (same real number, fewer roundings):
-// PAPER.md:186-188 names this loop ("steps reach into the thousands") as where the EDXCT time goes.
+// mu[id] * length; PAPER.md:186-188 names this loop ("steps reach into the thousands") as where the EDXCT time goes.
 //
-// The volume sits in the workspace in traversal layout with a one-voxel guard border of kVoxelGuard on every
-// side (DVoxels), so the walk needs no index or bounds arithmetic: a step adds one of three constant offsets to
-// a 32-bit voxel offset, and stepping onto a guard cell ends the walk.  One iteration = one face crossing and is
-// branch-free apart from the (rare) change of material: three compares pick the axis with the nearest face
-// (the same fp64 face parameters, accumulated by the same additions, as the oracle's), three predicated adds
-// advance it.  Rays of one warp differ in where they cross the lateral faces, and a predicated step costs the same
-// whichever axis a lane takes, so there is nothing to diverge on.
-// mu_s: per-thread mu of every material, shared memory, element m at mu_s[m * kBlock].
+// The volume sits in the workspace in traversal layout with a one-voxel guard border of kVoxelGuard on every side
+// (DVoxels), so the walk needs no bounds arithmetic: a step adds a constant to the voxel address, and stepping onto a
+// guard cell ends the walk.
+//
+// The walk is organised by slabs of the ray's own dominant axis w (|d_w| >= |d_u|, |d_v|; in c4 w is the beam axis =
+// the axis stored fastest, and 512 of the ~553 faces a ray crosses are w faces).  Per slab the ray crosses one w face
+// and at most one face of each lateral axis, because the lateral coordinate, in voxels, advances by a = |d_u / d_w|
+// <= 1 per slab.  That coordinate is carried as a 64-bit binary fraction: "does the ray cross a u face in this slab"
+// is the carry of one 64-bit integer add, exact (no rounding accumulates over the slabs; the only rounding is that of
+// a itself and of the starting fraction, ~1e-13 voxel, which can reorder two crossings closer than that, i.e. move a
+// zero-length visit).  A slab therefore costs two add-with-carry pairs, two byte loads (the voxel after the lateral
+// step, if any, and the voxel after the w face) and two compares, all on the integer pipe and free of branches as
+// long as the material does not change; no face parameter is tracked.
+//
+// Attenuation.  Face parameters are needed only where a RUN of equal IDs ends.  There t is computed from the integer
+// index of the face, (face - o) / d, the formula of step 11 itself, and the run's length is added to the path length
+// of its material (len_s, shared memory, element m at len_s[m * kBlock]).  tau = sum_m mu_m(E) * len_m is formed at
+// the end over the materials the ray touched, so mu(E) (a table search and an exp each, step 7) is evaluated only for
+// those -- a ray of c4 meets 3-6 of the 16.  Same real number as summing mu[id] * length voxel by voxel; only the
+// rounding order differs.
 // ------------------------------------------------------------------------------------------------------------
-// x += p ? y : 0 in two instructions (one select, one DADD): when p is false the HIGH word of the addend is zeroed,
-// which leaves a denormal below 2^-1022; for the face parameters here (x >= 2^-1000 or so) x + denormal == x exactly,
-// so the result is bit-identical to not adding.  (A predicated add compiles to an add and two selects.)
-__device__ __forceinline__ void add_if(double& x, double y, bool p) {
-  x += __hiloint2double(p ? __double2hiint(y) : 0, __double2loint(y));
+// 64-bit x += a, returns the carry (0 or 1)
+__device__ __forceinline__ unsigned add_carry(unsigned& lo, unsigned& hi, unsigned alo, unsigned ahi) {
+  unsigned c;
+  asm("add.cc.u32 %0, %0, %3;\n\taddc.cc.u32 %1, %1, %4;\n\taddc.u32 %2, 0, 0;" : "+r"(lo), "+r"(hi), "=r"(c) : "r"(alo), "r"(ahi));
+  return c;
 }
 
-__device__ __forceinline__ void trace_voxels(const DInstrument& I, const DComponent& C, Ray& ray, double* mu_s) {
-  const DVoxels& V = C.u.voxels;
-  const Vec3 ol = to_local(C.pose, ray.r);
-  const Vec3 dl = rotate(C.pose.R, ray.d);
-  const double h = V.h;
-  double t0 = -CUDART_INF, t1 = CUDART_INF;
-  if (!clip_axis(ol.x, dl.x, 0.0, (double)V.n[0] * h, t0, t1)) return;
-  if (!clip_axis(ol.y, dl.y, 0.0, (double)V.n[1] * h, t0, t1)) return;
-  if (!clip_axis(ol.z, dl.z, 0.0, (double)V.n[2] * h, t0, t1)) return;
-  if (t0 < 0.0) t0 = 0.0;
-  if (!(t0 < t1)) return;
-  // per-ray mu of every material (step 7)
-  const double lnE = log(ray.E);
-  for (int m = 0; m < I.n_mats; ++m) mu_s[m * kBlock] = mu_of(I.mats[m], ray.E, lnE);
-  // axis order: f = the axis stored fastest (the one most aligned with the beam), then a1, a2
-  const int f = V.fast, a1 = V.a1, a2 = V.a2;
-  const double of = pick(ol, f), o1 = pick(ol, a1), o2 = pick(ol, a2);
-  const double df = pick(dl, f), d1 = pick(dl, a1), d2 = pick(dl, a2);
-  const int nf = V.n[f], n1 = V.n[a1], n2 = V.n[a2];
-  int i_f, i_1, i_2, s_f, s_1, s_2;
-  double tm_f, tm_1, tm_2, td_f, td_1, td_2;
-#define MCX_AXIS_INIT(o, d, n, idx, stp, tmax, tdel)                                 \
-  {                                                                                   \
-    const double q = o + t0 * d;                                                      \
-    idx = min(n - 1, max(0, (int)floor(q / h)));                                      \
-    if (d > 0.0) { stp = 1; tmax = ((double)(idx + 1) * h - o) / d; tdel = h / d; }   \
-    else if (d < 0.0) { stp = -1; tmax = ((double)idx * h - o) / d; tdel = -h / d; }  \
-    else { stp = 0; tmax = CUDART_INF; tdel = CUDART_INF; }                           \
+// one voxel ID through the read-only path, zero-extended into a 32-bit register
+__device__ __forceinline__ unsigned ld_voxel(unsigned long long addr) {
+  unsigned v;
+  asm("ld.global.nc.u8 %0, [%1];" : "=r"(v) : "l"(addr));
+  return v;
+}
+
+// n / d for any 32-bit n by multiplication (Granlund & Montgomery 1994): m, sh precomputed by mcx_instrument_create
+__device__ __forceinline__ unsigned fast_div(unsigned n, unsigned m, unsigned sh) {
+  const unsigned t = __umulhi(m, n);
+  return (t + ((n - t) >> 1)) >> sh;
+}
+
+// x in [0, 1) -> floor(x 2^64); exact (x 2^64 has at most 53 significant bits)
+__device__ __forceinline__ unsigned long long frac64(double x) { return __double2ull_rz(x * 18446744073709551616.0); }
+
+// Per-ray values the walk needs only where a run of equal IDs ends live in shared memory, not in registers
+// (cold_s, element k at cold_s[k * kBlock]): o and 1/d of the axes w, u, v, and the exit parameter t1.
+enum { VC_O = 0, VC_INVD = 1, VC_T1 = 6, VC_COUNT = 8 };
+
+// One axis of the walk at set-up time
+struct VoxAxis {
+  double o, d;      // ray origin and direction component in the volume frame
+  int idx;          // entry voxel index
+  int dir;          // +1, -1, 0
+  unsigned slot;    // 0, 1, 2: position of this axis in the traversal layout (fast, a1, a2)
+  unsigned stride;  // address step per voxel along this axis
+};
+
+__device__ __forceinline__ VoxAxis vox_axis(const DVoxels& V, Vec3 o, Vec3 d, int g, double t0) {
+  VoxAxis A;
+  A.o = pick(o, g);
+  A.d = pick(d, g);
+  const int n = V.n[g];
+  A.idx = min(n - 1, max(0, (int)floor((A.o + t0 * A.d) / V.h)));
+  A.dir = A.d > 0.0 ? 1 : (A.d < 0.0 ? -1 : 0);
+  A.slot = g == V.fast ? 0u : (g == V.a1 ? 1u : 2u);
+  A.stride = A.slot == 0u ? 1u : (A.slot == 1u ? (unsigned)V.pitch : V.slab);
+  return A;
+}
+
+// Lateral coordinate at the first w face ahead (parameter t_w0), in voxels from the entry voxel's near face in the
+// direction of travel: in [0, 2); >= 1 means the lateral face is crossed within the first (partial) slab (c0 = 1).
+// f = its fraction, a = |d / d_w| <= 1 = advance per slab, both as 64-bit binary fractions.
+__device__ __forceinline__ void lateral_init(const VoxAxis& A, double d_w, double t_w0, double h, unsigned long long& f,
+                                             unsigned long long& a, unsigned& c0) {
+  double pos = 0.0, adv = 0.0;
+  if (A.dir != 0) {
+    const double y = (A.o + t_w0 * A.d) / h;
+    pos = A.dir > 0 ? y - (double)A.idx : (double)(A.idx + 1) - y;
+    pos = fmin(fmax(pos, 0.0), 1.9999999999999998);
+    adv = fabs(A.d / d_w);
   }
-  MCX_AXIS_INIT(of, df, nf, i_f, s_f, tm_f, td_f)
-  MCX_AXIS_INIT(o1, d1, n1, i_1, s_1, tm_1, td_1)
-  MCX_AXIS_INIT(o2, d2, n2, i_2, s_2, tm_2, td_2)
-#undef MCX_AXIS_INIT
-  const unsigned pitch = (unsigned)V.pitch, slab = (unsigned)(n1 + 2) * pitch;
-  const unsigned so_f = (unsigned)s_f, so_1 = (unsigned)s_1 * pitch, so_2 = (unsigned)s_2 * slab;  // mod 2^32
+  c0 = pos >= 1.0 ? 1u : 0u;
+  f = frac64(pos - (double)c0);
+  a = adv >= 1.0 ? 0xFFFFFFFFFFFFFFFFull : frac64(adv);
+}
+
+__device__ __forceinline__ void trace_voxels(const DInstrument& I, const DComponent& C, Ray& ray, double* len_s, double* cold_s) {
+  const DVoxels& V = C.u.voxels;
+  const double h = V.h;
+  unsigned ful, fuh, fvl, fvh, aul, auh, avl, avh, cu0, cv0, so_u, so_v, so_w, meta, lo_start;
+  double t_run;
+  {
+    const Vec3 ol = to_local(C.pose, ray.r);
+    const Vec3 dl = rotate(C.pose.R, ray.d);
+    double t0 = -CUDART_INF, t1 = CUDART_INF;
+    if (!clip_axis(ol.x, dl.x, 0.0, (double)V.n[0] * h, t0, t1)) return;
+    if (!clip_axis(ol.y, dl.y, 0.0, (double)V.n[1] * h, t0, t1)) return;
+    if (!clip_axis(ol.z, dl.z, 0.0, (double)V.n[2] * h, t0, t1)) return;
+    if (t0 < 0.0) t0 = 0.0;
+    if (!(t0 < t1)) return;
+    // the ray's dominant axis w and the two lateral axes u < v
+    int gw = 0;
+    {
+      double m = fabs(dl.x);
+      if (fabs(dl.y) > m) { gw = 1; m = fabs(dl.y); }
+      if (fabs(dl.z) > m) gw = 2;
+    }
+    const int gu = gw == 0 ? 1 : 0, gv = gw == 2 ? 1 : 2;
+    const VoxAxis W = vox_axis(V, ol, dl, gw, t0), U = vox_axis(V, ol, dl, gu, t0), X = vox_axis(V, ol, dl, gv, t0);
+    const double t_w0 = ((double)(W.idx + (W.dir > 0 ? 1 : 0)) * h - W.o) / W.d;  // first w face ahead
+    unsigned long long fu, au, fv, av;
+    lateral_init(U, W.d, t_w0, h, fu, au, cu0);
+    lateral_init(X, W.d, t_w0, h, fv, av, cv0);
+    ful = (unsigned)fu; fuh = (unsigned)(fu >> 32); aul = (unsigned)au; auh = (unsigned)(au >> 32);
+    fvl = (unsigned)fv; fvh = (unsigned)(fv >> 32); avl = (unsigned)av; avh = (unsigned)(av >> 32);
+    so_w = (unsigned)W.dir * W.stride; so_u = (unsigned)U.dir * U.stride; so_v = (unsigned)X.dir * X.stride;
+    // axis k (0 = w, 1 = u, 2 = v): layout slot in bits 2k, 2k+1; "travels in the + direction" in bit 6 + k
+    meta = W.slot | (U.slot << 2) | (X.slot << 4) | (W.dir > 0 ? 64u : 0u) | (U.dir > 0 ? 128u : 0u) | (X.dir > 0 ? 256u : 0u);
+    cold_s[(VC_O + 0) * kBlock] = W.o; cold_s[(VC_INVD + 0) * kBlock] = 1.0 / W.d;
+    cold_s[(VC_O + 2) * kBlock] = U.o; cold_s[(VC_INVD + 2) * kBlock] = 1.0 / U.d;
+    cold_s[(VC_O + 4) * kBlock] = X.o; cold_s[(VC_INVD + 4) * kBlock] = 1.0 / X.d;
+    cold_s[VC_T1 * kBlock] = t1;
+    lo_start = (unsigned)(W.idx + 1) * W.stride + (unsigned)(U.idx + 1) * U.stride + (unsigned)(X.idx + 1) * X.stride;
+    t_run = t0;
+  }
   // The volume does not straddle a 4 GiB address boundary (mcx_instrument_create places it so): the walk keeps the
   // low address word only and a step is one 32-bit add.
   const unsigned long long base = (unsigned long long)V.ids;
   const unsigned long long hi = base & 0xFFFFFFFF00000000ull;
-  unsigned lo = (unsigned)base + (unsigned)(i_2 + 1) * slab + (unsigned)(i_1 + 1) * pitch + (unsigned)(i_f + 1);
-  unsigned cur = __ldg(reinterpret_cast<const uint8_t*>(hi | lo));
-  double tau = 0.0, t_run = t0;
-  // Tie rule of step 11: the lowest of (x, y, z) wins.  Ties only order zero-length visits, so the traversal
-  // order (f, a1, a2) used here gives the same tau.
-  for (;;) {
-    const bool pf = tm_f <= tm_1 && tm_f <= tm_2;
-    const bool p1 = !pf && tm_1 <= tm_2;
-    const bool p2 = !pf && !p1;
-    lo += pf ? so_f : (p1 ? so_1 : so_2);
-    const unsigned id = __ldg(reinterpret_cast<const uint8_t*>(hi | lo));
-    if (id != cur) {  // a run of equal IDs ends at the face just crossed (or, on a guard cell, at the exit t1)
-      const double tn = fmin(pf ? tm_f : (p1 ? tm_1 : tm_2), t1);
-      tau += mu_s[cur * kBlock] * (tn - t_run);
-      t_run = tn;
-      cur = id;
-      if (id == kVoxelGuard) break;  // left the grid
+  lo_start += (unsigned)base;
+#define MCX_VOXEL_AT(lo32) ld_voxel(hi | (lo32))
+  unsigned cur = MCX_VOXEL_AT(lo_start);
+  unsigned touched = 0u;  // bit m: len_s[m] holds this ray's path length in material m
+  // The run of `cur` ends where the ray enters the voxel at address `at` through a face of axis k: the index of that
+  // voxel along the axis comes back out of the address (a guard cell gives -1 or n, i.e. the outer face of the grid),
+  // and the face parameter is (face - o) / d as in step 11 (as a product with 1/d, one more rounding).
+  auto close_run = [&](unsigned at, unsigned k, unsigned id) {
+    const unsigned off = at - (unsigned)base;
+    const unsigned q2 = fast_div(off, V.mg_slab, V.sh_slab), r = off - q2 * V.slab;
+    const unsigned q1 = fast_div(r, V.mg_pitch, V.sh_pitch), q0 = r - q1 * (unsigned)V.pitch;
+    const unsigned slot = (meta >> (2u * k)) & 3u;
+    const int face = (int)(slot == 0u ? q0 : (slot == 1u ? q1 : q2)) - (int)((meta >> (6u + k)) & 1u);  // index - 1 + (dir > 0 ? 0 : 1)
+    const double tf = ((double)face * h - cold_s[(VC_O + 2 * k) * kBlock]) * cold_s[(VC_INVD + 2 * k) * kBlock];
+    const double tn = fmin(tf, cold_s[VC_T1 * kBlock]);
+    const double prev = (touched >> cur) & 1u ? len_s[cur * kBlock] : 0.0;
+    len_s[cur * kBlock] = prev + (tn - t_run);
+    touched |= 1u << cur;
+    t_run = tn;
+    cur = id;
+  };
+  // One slab = the lateral step (if any; the same voxel again if cu = cv = 0) and the w face that ends the slab:
+  // voxel b at address lo_b, then voxel c at lo_c.  The two byte loads of slab k+1 are issued before the bytes of slab
+  // k are looked at (their addresses depend on the carries only), so a load's latency is covered by a whole slab of
+  // work.  If both lateral faces are crossed in one slab (rare) lo_b is the diagonal neighbour and the slow path
+  // visits the voxel in between first.  The loads of the slab after the last one reach at most one more step along
+  // every axis beyond the guard border: mcx_instrument_create pads the volume by that much on both sides.
+  // MCX_SLAB(A, B): issue slab B's loads from slab A's end, then settle slab A.
+#define MCX_SLAB(cuA, cvA, lo_bA, lo_cA, idbA, idcA, cuB, cvB, lo_bB, lo_cB, idbB, idcB)                            \
+  cuB = add_carry(ful, fuh, aul, auh);                                                                              \
+  cvB = add_carry(fvl, fvh, avl, avh);                                                                              \
+  lo_bB = lo_cA + cuB * so_u + cvB * so_v;                                                                          \
+  lo_cB = lo_bB + so_w;                                                                                             \
+  idbB = MCX_VOXEL_AT(lo_bB);                                                                                       \
+  idcB = MCX_VOXEL_AT(lo_cB);                                                                                       \
+  if (idbA != cur || idcA != cur || (cuA & cvA) != 0u) {                                                            \
+    if (settle_slab(cuA, cvA, lo_bA, lo_cA, idbA, idcA)) break;                                                     \
+  }
+  // Settles a slab in which a run ends or both lateral faces are crossed; returns true if the ray left the grid.
+  auto settle_slab = [&](unsigned cuA, unsigned cvA, unsigned lo_bA, unsigned lo_cA, unsigned idbA, unsigned idcA) {
+    unsigned k_lat = cuA ? 1u : 2u, k_first = 0u, lo_a = 0u, ida = cur;
+    if (cuA & cvA) {
+      // The face crossed first is the one with more of the slab left after it: f / a, f the fraction after this
+      // slab's add (ties: u).  Compared as f_u a_v >= f_v a_u on the high 64 bits of the products.  The fractions in
+      // registers are already the next slab's: step back by one increment.
+      const unsigned long long au = ((unsigned long long)auh << 32) | aul, av = ((unsigned long long)avh << 32) | avl;
+      const unsigned long long fu = (((unsigned long long)fuh << 32) | ful) - au, fv = (((unsigned long long)fvh << 32) | fvl) - av;
+      const bool u_first = __umul64hi(fu, av) >= __umul64hi(fv, au);
+      k_first = u_first ? 1u : 2u;
+      k_lat = u_first ? 2u : 1u;
+      lo_a = lo_bA - (u_first ? so_v : so_u);
+      ida = MCX_VOXEL_AT(lo_a);
     }
-    add_if(tm_f, td_f, pf);
-    add_if(tm_1, td_1, p1);
-    add_if(tm_2, td_2, p2);
+    if (ida != cur) {  // the voxel in between the two lateral faces of a double step
+      close_run(lo_a, k_first, ida);
+      if (ida == kVoxelGuard) return true;
+    }
+    if (idbA != cur) {
+      close_run(lo_bA, k_lat, idbA);
+      if (idbA == kVoxelGuard) return true;
+    }
+    if (idcA != cur) {
+      close_run(lo_cA, 0u, idcA);
+      if (idcA == kVoxelGuard) return true;
+    }
+    return false;
+  };
+  unsigned cu_a = cu0, cv_a = cv0, lo_b_a = lo_start + cu0 * so_u + cv0 * so_v, lo_c_a = lo_b_a + so_w;
+  unsigned idb_a = MCX_VOXEL_AT(lo_b_a), idc_a = MCX_VOXEL_AT(lo_c_a);
+  unsigned cu_b, cv_b, lo_b_b, lo_c_b, idb_b, idc_b;
+  for (;;) {
+    MCX_SLAB(cu_a, cv_a, lo_b_a, lo_c_a, idb_a, idc_a, cu_b, cv_b, lo_b_b, lo_c_b, idb_b, idc_b)
+    MCX_SLAB(cu_b, cv_b, lo_b_b, lo_c_b, idb_b, idc_b, cu_a, cv_a, lo_b_a, lo_c_a, idb_a, idc_a)
+  }
+#undef MCX_SLAB
+#undef MCX_VOXEL_AT
+  // tau = sum over the touched materials of mu_m(E) * len_m (step 7 evaluated for those only)
+  const double lnE = log(ray.E);
+  double tau = 0.0;
+  while (touched) {
+    const int m = __ffs(touched) - 1;
+    touched &= touched - 1u;
+    tau += mu_of(I.mats[m], ray.E, lnE) * len_s[m * kBlock];
   }
   ray.p *= exp(-tau);
 }
@@ -699,8 +834,11 @@ __global__ void __launch_bounds__(256) sort_scatter_kernel(uint64_t first, uint3
 constexpr int kTile = 2048;        // positions per work ticket
 constexpr int kSmemSolids = 32;    // solids staged in shared memory (all groups together)
 
+// resident blocks per SM the register budget is held to: the voxel walk hides its byte loads with warps
+constexpr int min_blocks(int feat) { return feat == F_VOXELS ? 3 : 1; }
+
 template <int FEAT, bool DUMP>
-__global__ void __launch_bounds__(kBlock) trace_kernel(const DInstrument* __restrict__ g_inst, TraceArgs A) {
+__global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const DInstrument* __restrict__ g_inst, TraceArgs A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   DInstrument& I = *reinterpret_cast<DInstrument*>(smem_raw);
   unsigned int* s_cnt = reinterpret_cast<unsigned int*>(smem_raw + sizeof(DInstrument));  // [MCX_MAX_COMPONENTS + 4]
@@ -731,7 +869,7 @@ __global__ void __launch_bounds__(kBlock) trace_kernel(const DInstrument* __rest
     }
     __syncthreads();
   }
-  double* mu_s = reinterpret_cast<double*>(s_extra) + threadIdx.x;
+  double* len_s = reinterpret_cast<double*>(s_extra) + threadIdx.x;  // per-thread path length per material (voxel walk)
   const int lane = threadIdx.x & 31;
   const uint64_t first = A.first, n = A.n, seed = A.seed;
   const uint32_t* __restrict__ order = A.order;
@@ -773,7 +911,7 @@ __global__ void __launch_bounds__(kBlock) trace_kernel(const DInstrument* __rest
               if (rc < 0 && !DUMP) atomicAdd(&s_cnt[MCX_MAX_COMPONENTS + CNT_OVERFLOW], 1u);
             }
           } else if ((FEAT & F_VOXELS) && kind == MCX_VOXELS) {
-            trace_voxels(I, C, ray, mu_s);
+            trace_voxels(I, C, ray, len_s, len_s + (size_t)I.n_mats * kBlock);
           } else if ((FEAT & F_OPTICS) && kind == MCX_MIRROR_ELLIPTIC) {
             pass = trace_mirror(C, ray);
           } else if ((FEAT & F_OPTICS) && kind == MCX_CRYSTAL_BRAGG) {
@@ -899,7 +1037,7 @@ constexpr size_t kSmemBase = sizeof(DInstrument) + 128;
 template <int FEAT, bool DUMP>
 cudaError_t launch_one(const DInstrument* d_inst, int n_mats, const TraceArgs& A, cudaStream_t stream, int n_sm) {
   const size_t smem = kSmemBase + ((FEAT & F_SOLIDS) ? kSmemSolids * sizeof(DSolid) : 0) +
-                      ((FEAT & F_VOXELS) ? (size_t)n_mats * kBlock * sizeof(double) : 0);
+                      ((FEAT & F_VOXELS) ? (size_t)(n_mats + VC_COUNT) * kBlock * sizeof(double) : 0);
   static bool configured = false;
   int blocks_per_sm = 1;
   cudaError_t e;
