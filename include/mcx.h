@@ -198,7 +198,8 @@ mcx_status mcx_trace_range(mcx_instrument* inst, uint64_t first_ray, uint64_t n_
  *   MCX_EXEC_SORTED  each chunk of <= 2^24 ray indices is first bucketed by the cell of a grid over the source's
  *                    direction draw (count, scan, scatter; 4 bytes of workspace per ray of a chunk), so that a warp
  *                    traces rays aimed at the same spot (coherent voxel / BVH / primitive walks);
- *   MCX_EXEC_AUTO    (default) SORTED for instruments with a mesh or voxel component, DIRECT otherwise. */
+ *   MCX_EXEC_AUTO    (default) SORTED where the source aims at a target rectangle and the instrument has a mesh, a
+ *                    voxel volume or a group of two or more solids, DIRECT otherwise. */
 typedef enum { MCX_EXEC_AUTO = 0, MCX_EXEC_DIRECT = 1, MCX_EXEC_SORTED = 2 } mcx_exec_mode;
 mcx_status mcx_instrument_set_exec(mcx_instrument* inst, int mode);
 

@@ -39,18 +39,20 @@ struct DSlit {
   double half_x, half_y, radius2;
 };
 
-// BVH2 node, 32 bytes.  Boxes are fp32, rounded outward and padded; they only select candidate triangles, the
-// exact fp64 triangle test decides.  Leaf: count > 0, first = first triangle; inner: count == 0, first = index of
-// the left child, right child = first + 1.
+// BVH2 node, 32 bytes, stored in depth-first preorder: the left child of an inner node is the next node, and
+// `escape` is the node to go to when this node's subtree is done or its box is missed (n_nodes = end of the walk), so
+// the walk needs no stack.  Boxes are fp32, rounded outward and padded; they only select candidate triangles, the
+// exact fp64 triangle test decides.  Leaf: tris = first_triangle * 8 + count (count 1..kBvhLeafMax); inner: tris = 0.
 struct BvhNode {
   float lo[3];
-  int first;
+  int escape;
   float hi[3];
-  int count;
+  int tris;
 };
+enum { kBvhLeafMax = 2 };
 
 struct DSolid {
-  int shape, material, priority, n_tris;
+  int shape, material, priority, n_nodes;  // n_nodes: BVH nodes of a mesh
   DPose pose;
   double dims[3];
   double root_lo[3], root_hi[3];  // fp64 AABB of the mesh (solid-local)
@@ -58,6 +60,8 @@ struct DSolid {
   const double* tris;  // [n_tris][9] vertices in BVH leaf order
 };
 
+// The solids of a group are stored in ascending order of precedence (priority, then earlier-listed first among
+// equals, step 10): where several overlap, the one with the highest index owns the segment.
 struct DSolids {
   int n_solids, n_mesh;
   const DSolid* solids;
@@ -135,6 +139,7 @@ enum { F_SOLIDS = 1, F_MESH = 2, F_VOXELS = 4, F_OPTICS = 8, F_ALL = 15 };
 // One trace launch: rays first + offset(q) for positions q in [0, n); offset(q) = order[q] if order != null, else q.
 struct TraceArgs {
   uint64_t first, n, seed;
+  int cap_endpoints;       // interval endpoints per ray and solids group held in shared memory (a multiple of 8)
   const uint32_t* order;   // detector-tile order of the chunk (launch_sort), or null
   mcx_ray_fate* dump;      // per-ray records indexed by ray offset, or null = tally
   unsigned int* ticket;    // [2] work-tile ticket and departure count, zero between launches
@@ -144,7 +149,7 @@ struct TraceArgs {
 enum { MCX_SORT_MAX_G = 10, MCX_SORT_MAX_BUCKETS = 1 << 20, MCX_SORT_MAX_SCAN_BLOCKS = 512 };
 
 // ---- launch interface (defined in mcx_kernels.cu) ----
-cudaError_t launch_trace(const DInstrument* d_inst, int features, int n_mats, const TraceArgs& args, cudaStream_t stream);
+cudaError_t launch_trace(const DInstrument* d_inst, int features, int n_mats, const TraceArgs& args, cudaStream_t stream);  // args.cap_endpoints sizes the shared memory
 cudaError_t launch_sort(uint64_t first, uint32_t n, uint64_t seed, int g, unsigned int* cnt, unsigned int* bsum,
                         uint32_t* order, cudaStream_t stream);
 cudaError_t launch_tally_read(const TallyBin* bins, uint64_t n_bins, unsigned long long* N, double* p, double* p2,

@@ -24,6 +24,8 @@ struct mcx_instrument {
   size_t off_staging = 0;
   size_t upload_bytes = 0;              // host -> device bytes moved by create
   int n_comps = 0, n_mats = 0, n_dets = 0, features = 0;
+  int cap_endpoints = 8;                // interval endpoints per ray and solids group (shared memory of the trace kernel)
+  bool sort_pays = false;               // AUTO lane scheduling: detector-tile order
   uint64_t det_bins[MCX_MAX_DETECTORS] = {0, 0, 0, 0};
   uint64_t launches = 0;
   // lane scheduling (row a13)
@@ -74,10 +76,10 @@ void copy_pose(DPose* d, const mcx_pose& s) {
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// BVH over one mesh: top-down, median split of the triangle centroids along the widest axis, <= 4 triangles
-// per leaf.  Node boxes are stored in fp32 rounded outward and padded by 2^-16 of the mesh scale, far above the
-// fp32 rounding of the box walk (<= a few 2^-24 of the scale), so the walk never loses a triangle the exact
-// fp64 test would hit.
+// BVH over one mesh: top-down, median split of the triangle centroids along the widest axis, <= kBvhLeafMax
+// triangles per leaf, nodes emitted in depth-first preorder with escape links (BvhNode).  Node boxes are stored in
+// fp32 rounded outward and padded by 2^-16 of the mesh scale, far above the fp32 rounding of the box walk (<= a few
+// 2^-24 of the scale), so the walk never loses a triangle the exact fp64 test would hit.
 // ---------------------------------------------------------------------------------------------------------
 struct TriRef {
   double c[3], lo[3], hi[3];
@@ -99,7 +101,10 @@ struct BvhBuilder {
   std::vector<TriRef>& refs;
   std::vector<BvhNode>& nodes;
   double pad;
-  void build(int node, int begin, int end) {
+  // builds the subtree over refs[begin, end) at the end of `nodes`; escape links are set by link() afterwards
+  void build(int begin, int end) {
+    const int node = (int)nodes.size();
+    nodes.push_back(BvhNode{});
     double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
     double clo[3] = {1e300, 1e300, 1e300}, chi[3] = {-1e300, -1e300, -1e300};
     for (int k = begin; k < end; ++k)
@@ -112,9 +117,8 @@ struct BvhBuilder {
       nodes[node].hi[a] = round_up(hi[a] + pad);
     }
     const int count = end - begin;
-    if (count <= 4) {
-      nodes[node].first = begin;
-      nodes[node].count = count;
+    if (count <= kBvhLeafMax) {
+      nodes[node].tris = begin * 8 + count;
       return;
     }
     int axis = 0;
@@ -123,13 +127,15 @@ struct BvhBuilder {
     const int mid = begin + count / 2;
     std::nth_element(refs.begin() + begin, refs.begin() + mid, refs.begin() + end,
                      [axis](const TriRef& x, const TriRef& y) { return x.c[axis] < y.c[axis]; });
-    const int left = (int)nodes.size();
-    nodes.push_back(BvhNode{});
-    nodes.push_back(BvhNode{});
-    nodes[node].first = left;
-    nodes[node].count = 0;
-    build(left, begin, mid);
-    build(left + 1, mid, end);
+    nodes[node].tris = 0;
+    build(begin, mid);  // left child = node + 1
+    build(mid, end);
+  }
+  // escape(node) = the first node after its subtree in preorder; returns it
+  int link(int node) {
+    if (nodes[node].tris != 0) return nodes[node].escape = node + 1;
+    const int right = link(node + 1);
+    return nodes[node].escape = link(right);
   }
 };
 
@@ -359,7 +365,7 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
   std::memset(&I, 0, sizeof(I));
   I.n_comps = n_components;
   I.n_mats = n_materials;
-  int features = 0;
+  int features = 0, cap_endpoints = 8;
 
 #define MCX_BAIL(status, ...) do { const mcx_status s_ = fail(status, __VA_ARGS__); delete H; return s_; } while (0)
 
@@ -437,9 +443,24 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
         DSolid* hs = (DSolid*)host_ptr(P.off_solids[c]);
         D.u.solids.n_solids = (int)G.n_solids;
         D.u.solids.solids = (const DSolid*)dev_ptr(P.off_solids[c]);
+        // device order = ascending precedence: by priority, among equals the LATER-listed first (step 10: the earlier
+        // solid wins a tie), so that the owner of an overlap is the solid with the highest device index
+        int pos[MCX_MAX_SOLIDS];
+        {
+          int order[MCX_MAX_SOLIDS];
+          for (int k = 0; k < (int)G.n_solids; ++k) order[k] = k;
+          std::sort(order, order + G.n_solids, [&](int x, int y) {
+            if (G.solids[x].priority != G.solids[y].priority) return G.solids[x].priority < G.solids[y].priority;
+            return x > y;
+          });
+          for (int k = 0; k < (int)G.n_solids; ++k) pos[order[k]] = k;
+        }
+        int n_prim = 0, n_mesh = 0;
+        for (int64_t s = 0; s < G.n_solids; ++s) (G.solids[s].shape == MCX_MESH ? n_mesh : n_prim)++;
+        cap_endpoints = std::max(cap_endpoints, std::min(48, (2 * n_prim + 8 * n_mesh + 7) / 8 * 8));
         for (int64_t s = 0; s < G.n_solids; ++s) {
           const mcx_solid& S = G.solids[s];
-          DSolid& d = hs[s];
+          DSolid& d = hs[pos[s]];
           if (S.shape < 0 || S.shape > 3) MCX_BAIL(MCX_ERR_INVALID_ARG, "component %d solid %d: bad shape", c, (int)s);
           if (S.material < 0 || S.material >= n_materials) MCX_BAIL(MCX_ERR_INVALID_ARG, "component %d solid %d: material out of range", c, (int)s);
           if (!pose_ok(S.pose)) MCX_BAIL(MCX_ERR_INVALID_ARG, "component %d solid %d: pose is not finite", c, (int)s);
@@ -472,10 +493,11 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
           const double pad = scale * (1.0 / 65536.0);
           std::vector<BvhNode> nodes;
           nodes.reserve(bvh_node_bound(nt));
-          nodes.push_back(BvhNode{});
           BvhBuilder B{refs, nodes, pad};
-          B.build(0, 0, nt);
+          B.build(0, nt);
+          B.link(0);
           if (nodes.size() > bvh_node_bound(nt)) MCX_BAIL(MCX_ERR_UNSUPPORTED, "BVH node bound exceeded");
+          if ((size_t)nt >= ((size_t)1 << 27)) MCX_BAIL(MCX_ERR_UNSUPPORTED, "component %d solid %d: more than 2^27 triangles", c, (int)s);
           std::memcpy(host_ptr(P.off_nodes[c][s]), nodes.data(), nodes.size() * sizeof(BvhNode));
           double* tri = (double*)host_ptr(P.off_tris[c][s]);
           for (int t = 0; t < nt; ++t)
@@ -483,7 +505,7 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
               for (int a = 0; a < 3; ++a)
                 tri[9 * (size_t)t + 3 * v + a] = S.vertices[3 * (size_t)S.triangles[3 * (size_t)refs[t].idx + v] + a];
           for (int a = 0; a < 3; ++a) { d.root_lo[a] = lo[a] - pad; d.root_hi[a] = hi[a] + pad; }
-          d.n_tris = nt;
+          d.n_nodes = (int)nodes.size();
           d.nodes = (const BvhNode*)dev_ptr(P.off_nodes[c][s]);
           d.tris = (const double*)dev_ptr(P.off_tris[c][s]);
         }
@@ -569,6 +591,14 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
   I.counters = (unsigned long long*)dev_ptr(P.off_counters);
   H->n_dets = n_dets;
   H->features = features;
+  H->cap_endpoints = cap_endpoints;
+  {  // Detector-tile order needs a source whose slot-1 draw is a target point (step 3) and pays where neighbouring rays
+     // share work: voxels, meshes, groups of several solids (measured: c1 1.4x, c3 5x, c4 3x; c0 and c2 nothing)
+    bool shared_work = (features & (F_MESH | F_VOXELS)) != 0;
+    for (int c = 0; c < n_components; ++c)
+      if (components[c].kind == MCX_SOLIDS && components[c].u.solids.n_solids >= 2) shared_work = true;
+    H->sort_pays = components[0].u.source.dir_mode == MCX_DIR_TARGET && shared_work;
+  }
 
   cudaError_t e = cudaMemcpyAsync(ws + P.off_inst, &H->host_image, sizeof(DInstrument), cudaMemcpyHostToDevice, stream);
   if (e == cudaSuccess && !H->blob.empty())
@@ -584,13 +614,12 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
 
 namespace {
 
-// Rows a13: which order the rays of a call are traced in.  AUTO = detector-tile order where the instrument has a
-// memory-walking component (meshes, voxels: coherent warps pay for the sort many times over), index order otherwise
-// (DESIGN.md 6 "What round 1 measured").
+// Rows a13: which order the rays of a call are traced in.  AUTO = detector-tile order where neighbouring rays share
+// work (mcx_instrument_create decides, see sort_pays), index order otherwise (DESIGN.md 6 "What round 1 measured").
 bool use_sorted(const mcx_instrument* H) {
   if (H->exec_mode == MCX_EXEC_SORTED) return true;
   if (H->exec_mode == MCX_EXEC_DIRECT) return false;
-  return (H->features & (F_MESH | F_VOXELS)) != 0;
+  return H->sort_pays;
 }
 
 // Traces rays [first, first + n) chunk by chunk; dump == nullptr tallies.
@@ -604,6 +633,7 @@ mcx_status run_trace(mcx_instrument* H, uint64_t first, uint64_t n, uint64_t see
     A.first = first + base;
     A.n = m;
     A.seed = seed;
+    A.cap_endpoints = H->cap_endpoints;
     A.order = nullptr;
     A.dump = dump ? dump + base : nullptr;
     A.ticket = (unsigned int*)(ws + H->off_ticket);

@@ -12,9 +12,6 @@ namespace mcx {
 namespace {
 
 constexpr int kBlock = 256;
-constexpr int kMaxIntervals = 32;  // per ray and solids group
-constexpr int kMaxHits = 32;       // per ray and mesh
-constexpr int kBvhStack = 64;
 constexpr unsigned kVoxelGuard = 255u;  // ID of the guard cells around the voxel volume (material IDs are < MCX_MAX_MATERIALS)
 
 // ------------------------------------------------------------------------------------------------------------
@@ -293,14 +290,53 @@ __device__ __forceinline__ int ray_triangle(const Shear& s, Vec3 o, const double
   return det > 0.0 ? 1 : -1;
 }
 
-struct Interval {
-  double a, b;
-  int solid;
+// ------------------------------------------------------------------------------------------------------------
+// Steps 8-10 work on one list of interval END POINTS per ray and solids group, held in shared memory (element k of
+// thread tid at [k * kBlock + tid]: conflict-free, dynamically indexable, no local memory): the parameter t and a tag
+// byte = index of the solid in the group (device order = ascending precedence, DSolids) | 0x80 for an exit.
+// ------------------------------------------------------------------------------------------------------------
+struct Endpoints {
+  double* t;
+  unsigned char* tag;
+  int cap;
 };
+constexpr unsigned char kTagExit = 0x80;
+constexpr int kTriQueue = 16;  // candidate triangles per thread between two rounds of exact tests
 
-// All hits of the full line with one mesh via its BVH, sorted, duplicate-collapsed and paired into intervals.
+__device__ __forceinline__ bool ep_push(const Endpoints& E, int& n, double t, unsigned tag) {
+  if (n >= E.cap) return false;
+  E.t[n * kBlock] = t;
+  E.tag[n * kBlock] = (unsigned char)tag;
+  ++n;
+  return true;
+}
+
+// insertion sort of E[begin, end) by t; exits_last: among equal t an entry comes before an exit (step 9)
+__device__ __forceinline__ void ep_sort(const Endpoints& E, int begin, int end, bool exits_last) {
+  for (int a = begin + 1; a < end; ++a) {
+    const double t = E.t[a * kBlock];
+    const unsigned tag = E.tag[a * kBlock];
+    int b = a - 1;
+    while (b >= begin) {
+      const double tb = E.t[b * kBlock];
+      const unsigned tagb = E.tag[b * kBlock];
+      if (!(tb > t || (exits_last && tb == t && (tagb & kTagExit) > (tag & kTagExit)))) break;
+      E.t[(b + 1) * kBlock] = tb;
+      E.tag[(b + 1) * kBlock] = (unsigned char)tagb;
+      --b;
+    }
+    E.t[(b + 1) * kBlock] = t;
+    E.tag[(b + 1) * kBlock] = (unsigned char)tag;
+  }
+}
+
+// All crossings of the full line with one mesh, appended to E as sorted, duplicate-collapsed, paired end points clipped
+// to t >= 0.  The BVH is walked without a stack (preorder + escape links, any order will do since every hit is wanted);
+// leaves only queue their triangles, and the exact tests run over the queue afterwards, so that the lanes of a warp
+// do box tests together and triangle tests together instead of waiting for one another at every leaf.
 // Returns 1 = ok, 0 = degenerate sequence, -1 = capacity overflow.
-__device__ int mesh_intervals(const DSolid& S, int solid, Vec3 o, Vec3 d, Interval* iv, int& n_iv) {
+__device__ __forceinline__ int mesh_endpoints(const DSolid& S, unsigned solid, Vec3 o, Vec3 d, const Endpoints& E, int& ne,
+                                              unsigned* __restrict__ queue) {
   // clip the line to the mesh box in fp64; the fp32 box walk uses a ray re-origined at the box entry so that
   // its rounding errors scale with the mesh size, not with the distance to the source
   double tmin = -CUDART_INF, tmax = CUDART_INF;
@@ -314,124 +350,109 @@ __device__ int mesh_intervals(const DSolid& S, int solid, Vec3 o, Vec3 d, Interv
   const float ix = d.x != 0.0 ? (float)(1.0 / d.x) : big, iy = d.y != 0.0 ? (float)(1.0 / d.y) : big,
               iz = d.z != 0.0 ? (float)(1.0 / d.z) : big;
   const Shear sh = make_shear(d);
-  double ht[kMaxHits];
-  signed char ho[kMaxHits];
-  int nh = 0;
+  const int begin = ne, n_nodes = S.n_nodes;
+  const float4* __restrict__ nodes = reinterpret_cast<const float4*>(S.nodes);
+  const double* __restrict__ tris = S.tris;
   bool overflow = false;
-  int stack[kBvhStack];
-  int sp = 0;
   int node = 0;
-  const BvhNode* __restrict__ nodes = S.nodes;
-  while (true) {
-    const BvhNode nd = nodes[node];
-    // slab test of the full line against the padded fp32 box (no t range: the line is tested, as in step 9)
-    const float tx0 = (nd.lo[0] - ox) * ix, tx1 = (nd.hi[0] - ox) * ix;
-    const float ty0 = (nd.lo[1] - oy) * iy, ty1 = (nd.hi[1] - oy) * iy;
-    const float tz0 = (nd.lo[2] - oz) * iz, tz1 = (nd.hi[2] - oz) * iz;
-    const float tn = fmaxf(fmaxf(fminf(tx0, tx1), fminf(ty0, ty1)), fminf(tz0, tz1));
-    const float tf = fminf(fminf(fmaxf(tx0, tx1), fmaxf(ty0, ty1)), fmaxf(tz0, tz1));
-    bool pop = true;
-    if (tn <= tf) {
-      if (nd.count > 0) {
-        for (int k = 0; k < nd.count; ++k) {
-          double t;
-          const int r = ray_triangle(sh, o, S.tris + 9 * (size_t)(nd.first + k), t);
-          if (r != 0) {
-            if (nh < kMaxHits) { ht[nh] = t; ho[nh] = (signed char)r; ++nh; } else overflow = true;
-          }
-        }
-      } else {
-        if (sp < kBvhStack) stack[sp++] = nd.first + 1; else overflow = true;
-        node = nd.first;
-        pop = false;
+  do {
+    int nq = 0;
+    while (node < n_nodes && nq <= kTriQueue - kBvhLeafMax) {
+      const float4 a = __ldg(nodes + 2 * node), b = __ldg(nodes + 2 * node + 1);  // lo.xyz, escape | hi.xyz, tris
+      // slab test of the full line against the padded fp32 box (no t range: the line is tested, as in step 9)
+      const float tx0 = (a.x - ox) * ix, tx1 = (b.x - ox) * ix;
+      const float ty0 = (a.y - oy) * iy, ty1 = (b.y - oy) * iy;
+      const float tz0 = (a.z - oz) * iz, tz1 = (b.z - oz) * iz;
+      const float tn = fmaxf(fmaxf(fminf(tx0, tx1), fminf(ty0, ty1)), fminf(tz0, tz1));
+      const float tf = fminf(fminf(fmaxf(tx0, tx1), fmaxf(ty0, ty1)), fmaxf(tz0, tz1));
+      const bool hit = tn <= tf;
+      const int leaf = __float_as_int(b.w);
+      if (hit && leaf != 0) {
+        queue[nq * kBlock] = (unsigned)(leaf >> 3);
+        ++nq;
+        if ((leaf & 7) > 1) { queue[nq * kBlock] = (unsigned)(leaf >> 3) + 1u; ++nq; }
       }
+      node = (hit && leaf == 0) ? node + 1 : __float_as_int(a.w);
     }
-    if (pop) {
-      if (sp == 0) break;
-      node = stack[--sp];
+    for (int k = 0; k < nq; ++k) {
+      double t;
+      const int r = ray_triangle(sh, o, tris + 9 * (size_t)queue[k * kBlock], t);
+      if (r != 0 && !ep_push(E, ne, t, solid | (r < 0 ? kTagExit : 0u))) overflow = true;
     }
-  }
+  } while (node < n_nodes);
   if (overflow) return -1;
-  if (nh == 0) return 1;
-  // insertion sort by (t, enter before exit)
-  for (int a = 1; a < nh; ++a) {
-    const double t = ht[a];
-    const signed char orr = ho[a];
-    int b = a - 1;
-    while (b >= 0 && (ht[b] > t || (ht[b] == t && ho[b] < orr))) { ht[b + 1] = ht[b]; ho[b + 1] = ho[b]; --b; }
-    ht[b + 1] = t;
-    ho[b + 1] = orr;
+  if (ne == begin) return 1;
+  ep_sort(E, begin, ne, true);
+  // collapse consecutive same-orientation hits (shared-edge duplicates); what is left must alternate enter, exit, ...
+  int m = begin;
+  for (int a = begin; a < ne; ++a) {
+    const unsigned tag = E.tag[a * kBlock];
+    if (m == begin || E.tag[(m - 1) * kBlock] != tag) {
+      E.t[m * kBlock] = E.t[a * kBlock];
+      E.tag[m * kBlock] = (unsigned char)tag;
+      ++m;
+    }
   }
-  // collapse consecutive same-orientation hits; what is left must alternate enter, exit, ...
-  int m = 0;
-  for (int a = 0; a < nh; ++a)
-    if (m == 0 || ho[m - 1] != ho[a]) { ht[m] = ht[a]; ho[m] = ho[a]; ++m; }
-  if ((m & 1) || ho[0] != 1) return 0;
-  for (int a = 0; a < m; a += 2) {
-    if (n_iv >= kMaxIntervals) return -1;
-    iv[n_iv++] = Interval{ht[a], ht[a + 1], solid};
+  if (((m - begin) & 1) || (E.tag[begin * kBlock] & kTagExit)) { ne = begin; return 0; }
+  // clip the pairs to t >= 0 and drop the empty ones
+  int w = begin;
+  for (int a = begin; a < m; a += 2) {
+    const double ta = fmax(E.t[a * kBlock], 0.0), tb = E.t[(a + 1) * kBlock];
+    if (tb > ta) {
+      E.t[w * kBlock] = ta; E.tag[w * kBlock] = (unsigned char)solid;
+      E.t[(w + 1) * kBlock] = tb; E.tag[(w + 1) * kBlock] = (unsigned char)(solid | kTagExit);
+      w += 2;
+    }
   }
+  ne = w;
   return 1;
 }
 
 // Steps 8-10 for one solids group.  Returns 1 = continue, 0 = degenerate, -1 = capacity overflow.
 template <bool MESH>
-__device__ int trace_solids(const DInstrument& I, const DComponent& C, Ray& ray) {
+__device__ __forceinline__ int trace_solids(const DInstrument& I, const DComponent& C, Ray& ray, const Endpoints& E,
+                                            unsigned* __restrict__ queue) {
   const DSolids& G = C.u.solids;
-  Interval iv[kMaxIntervals];
-  int n_iv = 0;
+  int ne = 0;
   for (int s = 0; s < G.n_solids; ++s) {
     const DSolid& S = G.solids[s];
     const Vec3 o = to_local(S.pose, ray.r);
     const Vec3 d = rotate(S.pose.R, ray.d);
     if (MESH && S.shape == MCX_MESH) {
-      const int rc = mesh_intervals(S, s, o, d, iv, n_iv);
+      const int rc = mesh_endpoints(S, (unsigned)s, o, d, E, ne, queue);
       if (rc != 1) return rc;
     } else {
       double a, b;
-      if (primitive_interval(S, o, d, a, b)) {
-        if (n_iv >= kMaxIntervals) return -1;
-        iv[n_iv++] = Interval{a, b, s};
+      if (primitive_interval(S, o, d, a, b)) {  // clip to t >= 0, drop if empty
+        a = fmax(a, 0.0);
+        if (b > a) {
+          if (!ep_push(E, ne, a, (unsigned)s)) return -1;
+          if (!ep_push(E, ne, b, (unsigned)s | kTagExit)) return -1;
+        }
       }
     }
   }
-  // clip to t >= 0, drop empty intervals
-  int m = 0;
-  for (int k = 0; k < n_iv; ++k) {
-    Interval x = iv[k];
-    if (x.a < 0.0) x.a = 0.0;
-    if (x.b > x.a) iv[m++] = x;
-  }
-  n_iv = m;
-  if (n_iv == 0) return 1;
-  // step 10: sort all endpoints, classify every elementary segment by its midpoint
-  double ts[2 * kMaxIntervals];
-  for (int k = 0; k < n_iv; ++k) { ts[2 * k] = iv[k].a; ts[2 * k + 1] = iv[k].b; }
-  const int nt = 2 * n_iv;
-  for (int a = 1; a < nt; ++a) {
-    const double t = ts[a];
-    int b = a - 1;
-    while (b >= 0 && ts[b] > t) { ts[b + 1] = ts[b]; --b; }
-    ts[b + 1] = t;
-  }
+  if (ne == 0) return 1;
+  // Step 10.  Between two consecutive end points the set of solids the ray is inside of is constant, so sweeping the
+  // sorted end points with that set as a bit mask classifies every elementary segment exactly as its midpoint would;
+  // the owner is the solid of highest precedence in the set = the highest bit (DSolids).  Equal end points only
+  // make zero-length segments, whatever their order.
+  ep_sort(E, 0, ne, false);
   const double lnE = log(ray.E);
-  double tau = 0.0;
+  double tau = 0.0, t_prev = 0.0, last_mu = 0.0;
   int last_mat = -1;
-  double last_mu = 0.0;
-  for (int k = 0; k + 1 < nt; ++k) {
-    const double ta = ts[k], tb = ts[k + 1];
-    if (!(tb > ta)) continue;
-    const double mid = 0.5 * (ta + tb);
-    int owner = -1, best = 0;
-    for (int q = 0; q < n_iv; ++q)
-      if (iv[q].a <= mid && mid <= iv[q].b) {
-        const int pr = G.solids[iv[q].solid].priority;
-        if (owner < 0 || pr > best) { owner = iv[q].solid; best = pr; }
-      }
-    if (owner < 0) continue;
-    const int mat = G.solids[owner].material;
-    if (mat != last_mat) { last_mu = mu_of(I.mats[mat], ray.E, lnE); last_mat = mat; }
-    tau += last_mu * (tb - ta);
+  unsigned inside = 0u;
+  for (int k = 0; k < ne; ++k) {
+    const double t = E.t[k * kBlock];
+    const unsigned tag = E.tag[k * kBlock];
+    if (inside != 0u && t > t_prev) {
+      const int mat = G.solids[31 - __clz(inside)].material;
+      if (mat != last_mat) { last_mu = mu_of(I.mats[mat], ray.E, lnE); last_mat = mat; }
+      tau += last_mu * (t - t_prev);
+    }
+    t_prev = t;
+    const unsigned bit = 1u << (tag & 31u);
+    inside = (tag & kTagExit) ? (inside & ~bit) : (inside | bit);
   }
   ray.p *= exp(-tau);
   return 1;
@@ -869,6 +890,19 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
     }
     __syncthreads();
   }
+  Endpoints ep{nullptr, nullptr, 0};
+  unsigned* tri_queue = nullptr;
+  if (FEAT & F_SOLIDS) {  // per-thread interval end points (and, with meshes, the candidate-triangle queue)
+    ep.cap = A.cap_endpoints;
+    ep.t = reinterpret_cast<double*>(s_extra) + threadIdx.x;
+    s_extra += (size_t)ep.cap * kBlock * sizeof(double);
+    ep.tag = s_extra + threadIdx.x;
+    s_extra += (size_t)ep.cap * kBlock;
+    if (FEAT & F_MESH) {
+      tri_queue = reinterpret_cast<unsigned*>(s_extra) + threadIdx.x;
+      s_extra += (size_t)kTriQueue * kBlock * sizeof(unsigned);
+    }
+  }
   double* len_s = reinterpret_cast<double*>(s_extra) + threadIdx.x;  // per-thread path length per material (voxel walk)
   const int lane = threadIdx.x & 31;
   const uint64_t first = A.first, n = A.n, seed = A.seed;
@@ -904,7 +938,7 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
             Vec3 h;
             pass = plane_hit(C.pose, ray, h) && h.x * h.x + h.y * h.y <= C.u.slit.radius2;
           } else if ((FEAT & F_SOLIDS) && kind == MCX_SOLIDS) {
-            const int rc = trace_solids<(FEAT & F_MESH) != 0>(I, C, ray);
+            const int rc = trace_solids<(FEAT & F_MESH) != 0>(I, C, ray, ep, tri_queue);
             if (rc != 1) {
               pass = false;
               fate = MCX_FATE_DEGENERATE;
@@ -1036,13 +1070,14 @@ constexpr size_t kSmemBase = sizeof(DInstrument) + 128;
 
 template <int FEAT, bool DUMP>
 cudaError_t launch_one(const DInstrument* d_inst, int n_mats, const TraceArgs& A, cudaStream_t stream, int n_sm) {
-  const size_t smem = kSmemBase + ((FEAT & F_SOLIDS) ? kSmemSolids * sizeof(DSolid) : 0) +
+  const size_t smem = kSmemBase + ((FEAT & F_SOLIDS) ? kSmemSolids * sizeof(DSolid) + (size_t)A.cap_endpoints * kBlock * 9 : 0) +
+                      ((FEAT & F_MESH) ? (size_t)kTriQueue * kBlock * sizeof(unsigned) : 0) +
                       ((FEAT & F_VOXELS) ? (size_t)(n_mats + VC_COUNT) * kBlock * sizeof(double) : 0);
   static bool configured = false;
   int blocks_per_sm = 1;
   cudaError_t e;
   if (!configured) {
-    e = cudaFuncSetAttribute(trace_kernel<FEAT, DUMP>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    e = cudaFuncSetAttribute(trace_kernel<FEAT, DUMP>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e != cudaSuccess) return e;
     configured = true;
   }
