@@ -195,7 +195,7 @@ mcx_status mcx_trace_range(mcx_instrument* inst, uint64_t first_ray, uint64_t n_
 /* Lane scheduling.  Results do not depend on it beyond the summation order of the tallies:
  * a ray is a pure function of (instrument, seed, ray index) whatever order rays are traced in.
  *   MCX_EXEC_DIRECT  rays are traced in index order, 32 consecutive indices per warp;
- *   MCX_EXEC_SORTED  each chunk of <= 2^24 ray indices is first bucketed by the cell of a grid over the source's
+ *   MCX_EXEC_SORTED  each chunk of <= 2^26 ray indices is first bucketed by the cell of a grid over the source's
  *                    direction draw (count, scan, scatter; 4 bytes of workspace per ray of a chunk), so that a warp
  *                    traces rays aimed at the same spot (coherent voxel / BVH / primitive walks);
  *   MCX_EXEC_AUTO    (default) SORTED where the source aims at a target rectangle and the instrument has a mesh, a

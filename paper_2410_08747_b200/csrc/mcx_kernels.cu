@@ -856,7 +856,7 @@ constexpr int kTile = 2048;        // positions per work ticket
 constexpr int kSmemSolids = 32;    // solids staged in shared memory (all groups together)
 
 // resident blocks per SM the register budget is held to: the voxel walk hides its byte loads with warps
-constexpr int min_blocks(int feat) { return feat == F_VOXELS ? 3 : 1; }
+constexpr int min_blocks(int feat) { return feat == F_VOXELS || feat == F_SOLIDS || feat == (F_SOLIDS | F_MESH) ? 3 : 1; }
 
 template <int FEAT, bool DUMP>
 __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const DInstrument* __restrict__ g_inst, TraceArgs A) {
