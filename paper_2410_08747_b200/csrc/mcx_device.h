@@ -33,7 +33,9 @@ struct DSource {
   double target_w, target_h, target_dist, div_x, div_y;
   double e0, de_rel, spec_emin, spec_bin_w;
   const double* cdf;  // [spec_n + 1] running sum of the spectrum
+  const int* guide;   // [kSpecGuide + 1]: guide[k] <= the bin holding v = (k / kSpecGuide) cdf[spec_n] (starts the search)
 };
+enum { kSpecGuide = 2048 };
 
 struct DSlit {
   double half_x, half_y, radius2;
@@ -139,6 +141,7 @@ enum { F_SOLIDS = 1, F_MESH = 2, F_VOXELS = 4, F_OPTICS = 8, F_ALL = 15 };
 // One trace launch: rays first + offset(q) for positions q in [0, n); offset(q) = order[q] if order != null, else q.
 struct TraceArgs {
   uint64_t first, n, seed;
+  unsigned tile;           // positions per work ticket (set by launch_trace)
   int cap_endpoints;       // interval endpoints per ray and solids group held in shared memory (a multiple of 8)
   const uint32_t* order;   // detector-tile order of the chunk (launch_sort), or null
   mcx_ray_fate* dump;      // per-ray records indexed by ray offset, or null = tally

@@ -177,6 +177,7 @@ struct Plan {
   // blob offsets
   size_t off_mat[MCX_MAX_MATERIALS];      // 4 arrays of n doubles each
   size_t off_cdf[MCX_MAX_COMPONENTS];
+  size_t off_guide[MCX_MAX_COMPONENTS];
   size_t off_table[MCX_MAX_COMPONENTS];
   size_t off_solids[MCX_MAX_COMPONENTS];  // DSolid array
   size_t off_nodes[MCX_MAX_COMPONENTS][MCX_MAX_SOLIDS];
@@ -244,6 +245,7 @@ mcx_status make_plan(const mcx_component* comps, int n_comps, const mcx_material
         if (C.u.source.energy_mode == MCX_E_SPECTRUM) {
           if (C.u.source.spec_n < 1) return fail(MCX_ERR_INVALID_ARG, "source: empty spectrum");
           P->off_cdf[c] = A.reserve((size_t)(C.u.source.spec_n + 1) * sizeof(double));
+          P->off_guide[c] = A.reserve((size_t)(kSpecGuide + 1) * sizeof(int));
         }
         break;
       case MCX_SLIT_RECT: case MCX_SLIT_CIRC: case MCX_CRYSTAL_BRAGG: break;
@@ -429,6 +431,17 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
           d.spec_emin = S.spec_emin;
           d.spec_bin_w = (S.spec_emax - S.spec_emin) / (double)S.spec_n;
           d.cdf = (const double*)dev_ptr(P.off_cdf[c]);
+          // guide table: where the inverse-CDF search of step 3 may start for v in [k, k+1) / kSpecGuide of the total
+          // (one bin below the exact answer for the lower edge; the kernel verifies its bracket and falls back to
+          // the whole table, so the table only has to be nearly right)
+          int* guide = (int*)host_ptr(P.off_guide[c]);
+          int64_t j = 0;
+          for (int k = 0; k <= kSpecGuide; ++k) {
+            const double v = ((double)k / (double)kSpecGuide) * cdf[S.spec_n];
+            while (j + 1 < S.spec_n && cdf[j + 1] <= v) ++j;
+            guide[k] = (int)std::max<int64_t>(j - 1, 0);
+          }
+          d.guide = (const int*)dev_ptr(P.off_guide[c]);
         }
         break;
       }
