@@ -69,15 +69,19 @@ struct DSolids {
   const DSolid* solids;
 };
 
+// Voxel volume in traversal layout: 2 bytes per cell, {material ID, run}, where run = how many cells FOLLOWING this one
+// along the fast axis in the beam's direction (run_dir) hold the same ID (capped at 255).  Cells are addressed as
+// ((i[a2]+1) * (n[a1]+2) + i[a1]+1) * pitch + i[fast]+1, with a one-cell guard border of ID kVoxelGuard all around.
 struct DVoxels {
   double h;
   int n[3];       // nx, ny, nz
   int fast;       // axis stored fastest in the traversal layout
-  int a1, a2;     // the other two axes: offset = ((i[a2]+1) * (n[a1]+2) + i[a1]+1) * pitch + i[fast]+1 (guard border)
-  int pitch;      // n[fast] + 2 rounded up to a multiple of 16
-  unsigned slab;  // (n[a1] + 2) * pitch
+  int a1, a2;     // the other two axes
+  int pitch;      // cells per row: n[fast] + 2 rounded up to a multiple of 16
+  unsigned slab;  // cells per slab: (n[a1] + 2) * pitch
   unsigned mg_pitch, sh_pitch, mg_slab, sh_slab;  // x / pitch, x / slab by multiplication (fast_div in mcx_kernels.cu)
-  const uint8_t* ids;
+  int run_dir;    // +1 / -1: the direction along the fast axis the runs are counted in (source -> volume)
+  const uint8_t* ids;  // cell k at ids[2 k] (ID) and ids[2 k + 1] (run)
 };
 
 struct DMirror {
@@ -158,7 +162,7 @@ cudaError_t launch_sort(uint64_t first, uint32_t n, uint64_t seed, int g, unsign
 cudaError_t launch_tally_read(const TallyBin* bins, uint64_t n_bins, unsigned long long* N, double* p, double* p2,
                               cudaStream_t stream);
 cudaError_t launch_voxel_relayout(const uint8_t* src, uint8_t* dst, int nx, int ny, int nz, int fast, int a1, int a2,
-                                  int pitch, cudaStream_t stream);
+                                  int pitch, int run_dir, cudaStream_t stream);
 cudaError_t launch_probe_dfma(double* sink, int n_blocks, long long n_iters, cudaStream_t stream);
 cudaError_t kernels_init();
 

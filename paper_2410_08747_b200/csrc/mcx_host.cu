@@ -186,10 +186,10 @@ struct Plan {
 
 // traversal layout of a voxel volume: one guard cell on every side, rows padded to 16 bytes
 int voxel_pitch(int64_t n_fast) { return (int)((n_fast + 2 + 15) / 16 * 16); }
-size_t voxel_bytes(int64_t n_fast, int64_t n_1, int64_t n_2) { return (size_t)(n_2 + 2) * (size_t)(n_1 + 2) * (size_t)voxel_pitch(n_fast); }
+size_t voxel_bytes(int64_t n_fast, int64_t n_1, int64_t n_2) { return 2 * (size_t)(n_2 + 2) * (size_t)(n_1 + 2) * (size_t)voxel_pitch(n_fast); }
 // The walk issues the loads of the slab after the one it is looking at; past a guard cell these reach at most one step
 // along every axis further.  That much of the workspace on either side of the volume belongs to the volume.
-size_t voxel_pad(int64_t n_fast, int64_t n_1) { return align_up((size_t)(n_1 + 3) * (size_t)voxel_pitch(n_fast) + 16); }
+size_t voxel_pad(int64_t n_fast, int64_t n_1) { return align_up(2 * ((size_t)(n_1 + 3) * (size_t)voxel_pitch(n_fast) + 16)); }
 
 // n / d == (t + ((n - t) >> 1)) >> sh with t = mulhi(m, n), for every 32-bit n and d >= 2 (Granlund & Montgomery 1994,
 // "Division by invariant integers using multiplication", the 33-bit multiplier case)
@@ -201,7 +201,7 @@ void fast_div_constants(unsigned d, unsigned* m, unsigned* sh) {
 }
 
 // chooses the axis stored fastest: the voxel axis most aligned with the line from the source to the volume centre
-void voxel_axes(const mcx_component& src, const mcx_component& vox, int* fast, int* a1, int* a2) {
+void voxel_axes(const mcx_component& src, const mcx_component& vox, int* fast, int* a1, int* a2, int* run_dir) {
   const mcx_voxels_params& V = vox.u.voxels;
   const double half[3] = {0.5 * V.nx * V.h, 0.5 * V.ny * V.h, 0.5 * V.nz * V.h};
   // volume centre in lab coordinates: origin + R^T half
@@ -213,9 +213,10 @@ void voxel_axes(const mcx_component& src, const mcx_component& vox, int* fast, i
   }
   double best = -1.0;
   *fast = 2;
+  *run_dir = 1;
   for (int k = 0; k < 3; ++k) {
-    const double comp = std::fabs(vox.pose.rot[3 * k] * dirl[0] + vox.pose.rot[3 * k + 1] * dirl[1] + vox.pose.rot[3 * k + 2] * dirl[2]);
-    if (comp > best) { best = comp; *fast = k; }
+    const double comp = vox.pose.rot[3 * k] * dirl[0] + vox.pose.rot[3 * k + 1] * dirl[1] + vox.pose.rot[3 * k + 2] * dirl[2];
+    if (std::fabs(comp) > best) { best = std::fabs(comp); *fast = k; *run_dir = comp < 0.0 ? -1 : 1; }
   }
   *a1 = (*fast + 1) % 3;
   *a2 = (*fast + 2) % 3;
@@ -282,10 +283,11 @@ mcx_status make_plan(const mcx_component* comps, int n_comps, const mcx_material
       if (V.nx < 1 || V.ny < 1 || V.nz < 1 || V.nx > 4096 || V.ny > 4096 || V.nz > 4096 || !(V.h > 0.0))
         return fail(MCX_ERR_INVALID_ARG, "component %d: bad voxel grid", c);
       int f, a1, a2;
-      voxel_axes(comps[0], comps[c], &f, &a1, &a2);
+      int run_dir;
+      voxel_axes(comps[0], comps[c], &f, &a1, &a2, &run_dir);
       const int64_t n[3] = {V.nx, V.ny, V.nz};
       if (voxel_bytes(n[f], n[a1], n[a2]) + 2 * voxel_pad(n[f], n[a1]) > 0xFFFFFFFFull)
-        return fail(MCX_ERR_UNSUPPORTED, "component %d: voxel volume above 4 GiB (the walk uses 32-bit voxel offsets)", c);
+        return fail(MCX_ERR_UNSUPPORTED, "component %d: voxel volume above 2^31 cells (the walk uses 32-bit byte offsets, 2 bytes per cell)", c);
       // twice the size: create shifts the volume past a 4 GiB address boundary if it would straddle one
       P->off_voxels[c] = A.reserve(2 * voxel_bytes(n[f], n[a1], n[a2]) + 4 * voxel_pad(n[f], n[a1]));
     }
@@ -533,7 +535,7 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
         DVoxels& d = D.u.voxels;
         d.h = V.h;
         d.n[0] = (int)V.nx; d.n[1] = (int)V.ny; d.n[2] = (int)V.nz;
-        voxel_axes(components[0], C, &d.fast, &d.a1, &d.a2);
+        voxel_axes(components[0], C, &d.fast, &d.a1, &d.a2, &d.run_dir);
         d.pitch = voxel_pitch(d.n[d.fast]);
         d.slab = (unsigned)(d.n[d.a1] + 2) * (unsigned)d.pitch;
         fast_div_constants((unsigned)d.pitch, &d.mg_pitch, &d.sh_pitch);
@@ -546,9 +548,9 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
           d.ids = (const uint8_t*)p0;
         }
         const cudaError_t e = launch_voxel_relayout(V.ids, (uint8_t*)d.ids, d.n[0], d.n[1], d.n[2], d.fast,
-                                                    d.a1, d.a2, d.pitch, stream);
+                                                    d.a1, d.a2, d.pitch, d.run_dir, stream);
         if (e != cudaSuccess) { const mcx_status s_ = cuda_fail(e, "voxel relayout"); delete H; return s_; }
-        H->launches++;
+        H->launches += 2;
         break;
       }
       case MCX_MIRROR_ELLIPTIC: {

@@ -501,6 +501,13 @@ __device__ __forceinline__ unsigned ld_voxel(unsigned long long addr) {
   return v;
 }
 
+// one cell {ID, run} of the voxel volume as ID | run << 8
+__device__ __forceinline__ unsigned ld_cell(unsigned long long addr) {
+  unsigned short v;
+  asm("ld.global.nc.u16 %0, [%1];" : "=h"(v) : "l"(addr));
+  return v;
+}
+
 // n / d for any 32-bit n by multiplication (Granlund & Montgomery 1994): m, sh precomputed by mcx_instrument_create
 __device__ __forceinline__ unsigned fast_div(unsigned n, unsigned m, unsigned sh) {
   const unsigned t = __umulhi(m, n);
@@ -520,7 +527,7 @@ struct VoxAxis {
   int idx;          // entry voxel index
   int dir;          // +1, -1, 0
   unsigned slot;    // 0, 1, 2: position of this axis in the traversal layout (fast, a1, a2)
-  unsigned stride;  // address step per voxel along this axis
+  unsigned stride;  // address step (bytes) per voxel along this axis
 };
 
 __device__ __forceinline__ VoxAxis vox_axis(const DVoxels& V, Vec3 o, Vec3 d, int g, double t0) {
@@ -531,7 +538,7 @@ __device__ __forceinline__ VoxAxis vox_axis(const DVoxels& V, Vec3 o, Vec3 d, in
   A.idx = min(n - 1, max(0, (int)floor((A.o + t0 * A.d) / V.h)));
   A.dir = A.d > 0.0 ? 1 : (A.d < 0.0 ? -1 : 0);
   A.slot = g == V.fast ? 0u : (g == V.a1 ? 1u : 2u);
-  A.stride = A.slot == 0u ? 1u : (A.slot == 1u ? (unsigned)V.pitch : V.slab);
+  A.stride = 2u * (A.slot == 0u ? 1u : (A.slot == 1u ? (unsigned)V.pitch : V.slab));  // bytes, 2 per cell
   return A;
 }
 
@@ -555,7 +562,7 @@ __device__ __forceinline__ void lateral_init(const VoxAxis& A, double d_w, doubl
 __device__ __forceinline__ void trace_voxels(const DInstrument& I, const DComponent& C, Ray& ray, double* len_s, double* cold_s) {
   const DVoxels& V = C.u.voxels;
   const double h = V.h;
-  unsigned ful, fuh, fvl, fvh, aul, auh, avl, avh, cu0, cv0, so_u, so_v, so_w, meta, lo_start;
+  unsigned ful, fuh, fvl, fvh, aul, auh, avl, avh, cu0, cv0, so_u, so_v, so_w, meta, lo_start, inv_u, inv_v;
   double t_run;
   {
     const Vec3 ol = to_local(C.pose, ray.r);
@@ -588,6 +595,12 @@ __device__ __forceinline__ void trace_voxels(const DInstrument& I, const DCompon
     cold_s[(VC_O + 2) * kBlock] = U.o; cold_s[(VC_INVD + 2) * kBlock] = 1.0 / U.d;
     cold_s[(VC_O + 4) * kBlock] = X.o; cold_s[(VC_INVD + 4) * kBlock] = 1.0 / X.d;
     cold_s[VC_T1 * kBlock] = t1;
+    {  // skipping (see the loop below): only along the fast axis in the direction the runs were counted in
+      const bool can_skip = W.slot == 0u && W.dir == V.run_dir;
+      // inv <= 2^32 / (a_hi + 1): float quotient less a relative 1e-6 (its own error is 2^-22)
+      inv_u = can_skip ? __float2uint_rz(__fdividef(4294967296.0f, (float)auh + 1.0f) * 0.999999f) : 0u;
+      inv_v = can_skip ? __float2uint_rz(__fdividef(4294967296.0f, (float)avh + 1.0f) * 0.999999f) : 0u;
+    }
     lo_start = (unsigned)(W.idx + 1) * W.stride + (unsigned)(U.idx + 1) * U.stride + (unsigned)(X.idx + 1) * X.stride;
     t_run = t0;
   }
@@ -603,7 +616,7 @@ __device__ __forceinline__ void trace_voxels(const DInstrument& I, const DCompon
   // voxel along the axis comes back out of the address (a guard cell gives -1 or n, i.e. the outer face of the grid),
   // and the face parameter is (face - o) / d as in step 11 (as a product with 1/d, one more rounding).
   auto close_run = [&](unsigned at, unsigned k, unsigned id) {
-    const unsigned off = at - (unsigned)base;
+    const unsigned off = (at - (unsigned)base) >> 1;  // cell index
     const unsigned q2 = fast_div(off, V.mg_slab, V.sh_slab), r = off - q2 * V.slab;
     const unsigned q1 = fast_div(r, V.mg_pitch, V.sh_pitch), q0 = r - q1 * (unsigned)V.pitch;
     const unsigned slot = (meta >> (2u * k)) & 3u;
@@ -616,39 +629,29 @@ __device__ __forceinline__ void trace_voxels(const DInstrument& I, const DCompon
     t_run = tn;
     cur = id;
   };
-  // One slab = the lateral step (if any; the same voxel again if cu = cv = 0) and the w face that ends the slab:
-  // voxel b at address lo_b, then voxel c at lo_c.  The two byte loads of slab k+1 are issued before the bytes of slab
-  // k are looked at (their addresses depend on the carries only), so a load's latency is covered by a whole slab of
-  // work.  If both lateral faces are crossed in one slab (rare) lo_b is the diagonal neighbour and the slow path
-  // visits the voxel in between first.  The loads of the slab after the last one reach at most one more step along
-  // every axis beyond the guard border: mcx_instrument_create pads the volume by that much on both sides.
-  // MCX_SLAB(A, B): issue slab B's loads from slab A's end, then settle slab A.
-#define MCX_SLAB(cuA, cvA, lo_bA, lo_cA, idbA, idcA, cuB, cvB, lo_bB, lo_cB, idbB, idcB)                            \
-  cuB = add_carry(ful, fuh, aul, auh);                                                                              \
-  cvB = add_carry(fvl, fvh, avl, avh);                                                                              \
-  lo_bB = lo_cA + cuB * so_u + cvB * so_v;                                                                          \
-  lo_cB = lo_bB + so_w;                                                                                             \
-  idbB = MCX_VOXEL_AT(lo_bB);                                                                                       \
-  idcB = MCX_VOXEL_AT(lo_cB);                                                                                       \
-  if (idbA != cur || idcA != cur || (cuA & cvA) != 0u) {                                                            \
-    if (settle_slab(cuA, cvA, lo_bA, lo_cA, idbA, idcA)) break;                                                     \
-  }
-  // Settles a slab in which a run ends or both lateral faces are crossed; returns true if the ray left the grid.
+  // One iteration = one slab, then a skip.
+  //  Slab: the lateral step (if any; the same cell again if cu = cv = 0) and the w face that ends the slab: cell b at
+  //  lo_b, then cell c at lo_c.  If both lateral faces are crossed in one slab (rare) lo_b is the diagonal neighbour
+  //  and the slow path visits the cell in between first.
+  //  Skip: standing in cell c (same ID as the run), the ray may cross s more w faces without looking at anything if
+  //  the next s cells of the row hold the same ID (the cell's run) and no lateral face comes in those s slabs, i.e.
+  //  s additions of a leave the fraction below 1: s <= (2^64 - 1 - f) / a, taken conservatively from the high words
+  //  as mulhi(~f_hi, inv) with inv <= 2^32 / (a_hi + 1).  Then f += s a exactly and the address moves s cells on.
+  //  inv = 0 (no skipping) unless the ray runs along the fast axis in the direction the runs were counted in.
   auto settle_slab = [&](unsigned cuA, unsigned cvA, unsigned lo_bA, unsigned lo_cA, unsigned idbA, unsigned idcA) {
     unsigned k_lat = cuA ? 1u : 2u, k_first = 0u, lo_a = 0u, ida = cur;
     if (cuA & cvA) {
       // The face crossed first is the one with more of the slab left after it: f / a, f the fraction after this
-      // slab's add (ties: u).  Compared as f_u a_v >= f_v a_u on the high 64 bits of the products.  The fractions in
-      // registers are already the next slab's: step back by one increment.
+      // slab's add (ties: u).  Compared as f_u a_v >= f_v a_u on the high 64 bits of the products.
       const unsigned long long au = ((unsigned long long)auh << 32) | aul, av = ((unsigned long long)avh << 32) | avl;
-      const unsigned long long fu = (((unsigned long long)fuh << 32) | ful) - au, fv = (((unsigned long long)fvh << 32) | fvl) - av;
+      const unsigned long long fu = ((unsigned long long)fuh << 32) | ful, fv = ((unsigned long long)fvh << 32) | fvl;
       const bool u_first = __umul64hi(fu, av) >= __umul64hi(fv, au);
       k_first = u_first ? 1u : 2u;
       k_lat = u_first ? 2u : 1u;
       lo_a = lo_bA - (u_first ? so_v : so_u);
       ida = MCX_VOXEL_AT(lo_a);
     }
-    if (ida != cur) {  // the voxel in between the two lateral faces of a double step
+    if (ida != cur) {  // the cell in between the two lateral faces of a double step
       close_run(lo_a, k_first, ida);
       if (ida == kVoxelGuard) return true;
     }
@@ -662,14 +665,25 @@ __device__ __forceinline__ void trace_voxels(const DInstrument& I, const DCompon
     }
     return false;
   };
-  unsigned cu_a = cu0, cv_a = cv0, lo_b_a = lo_start + cu0 * so_u + cv0 * so_v, lo_c_a = lo_b_a + so_w;
-  unsigned idb_a = MCX_VOXEL_AT(lo_b_a), idc_a = MCX_VOXEL_AT(lo_c_a);
-  unsigned cu_b, cv_b, lo_b_b, lo_c_b, idb_b, idc_b;
+  unsigned cu = cu0, cv = cv0, lo = lo_start;
   for (;;) {
-    MCX_SLAB(cu_a, cv_a, lo_b_a, lo_c_a, idb_a, idc_a, cu_b, cv_b, lo_b_b, lo_c_b, idb_b, idc_b)
-    MCX_SLAB(cu_b, cv_b, lo_b_b, lo_c_b, idb_b, idc_b, cu_a, cv_a, lo_b_a, lo_c_a, idb_a, idc_a)
+    const unsigned lo_b = lo + cu * so_u + cv * so_v, lo_c = lo_b + so_w;
+    const unsigned idb = MCX_VOXEL_AT(lo_b);
+    const unsigned cell_c = ld_cell(hi | lo_c);
+    const unsigned idc = cell_c & 0xffu;
+    if (idb != cur || idc != cur || (cu & cv) != 0u) {
+      if (settle_slab(cu, cv, lo_b, lo_c, idb, idc)) break;
+    }
+    const unsigned s = min(min(cell_c >> 8, __umulhi(~fuh, inv_u)), __umulhi(~fvh, inv_v));
+    lo = lo_c + s * so_w;
+    {
+      const unsigned long long tu = (unsigned long long)s * aul + ful, tv = (unsigned long long)s * avl + fvl;
+      ful = (unsigned)tu; fuh += s * auh + (unsigned)(tu >> 32);
+      fvl = (unsigned)tv; fvh += s * avh + (unsigned)(tv >> 32);
+    }
+    cu = add_carry(ful, fuh, aul, auh);
+    cv = add_carry(fvl, fvh, avl, avh);
   }
-#undef MCX_SLAB
 #undef MCX_VOXEL_AT
   // tau = sum over the touched materials of mu_m(E) * len_m (step 7 evaluated for those only)
   const double lnE = log(ray.E);
@@ -1054,7 +1068,8 @@ __global__ void __launch_bounds__(256) tally_read_kernel(const TallyBin* __restr
 }
 
 // Voxel volume from the interface layout [iz][iy][ix] into the traversal layout [i_a2 + 1][i_a1 + 1][i_fast + 1]
-// (rows of `pitch` bytes) with a guard border of kVoxelGuard around it.
+// (rows of `pitch` cells of 2 bytes: ID, run) with a guard border of kVoxelGuard around it.  Runs are filled in by
+// voxel_runs_kernel.
 __global__ void __launch_bounds__(256) voxel_relayout_kernel(const uint8_t* __restrict__ src, uint8_t* __restrict__ dst,
                                                              int nx, int ny, int nz, int fast, int a1, int a2, int pitch) {
   const int n[3] = {nx, ny, nz};
@@ -1064,13 +1079,30 @@ __global__ void __launch_bounds__(256) voxel_relayout_kernel(const uint8_t* __re
     const int jf = (int)(k % pitch) - 1;
     const long long rowi = k / pitch;
     const int j1 = (int)(rowi % (n[a1] + 2)) - 1, j2 = (int)(rowi / (n[a1] + 2)) - 1;
-    uint8_t v = (uint8_t)kVoxelGuard;
+    unsigned v = kVoxelGuard;
     if (jf >= 0 && jf < n[fast] && j1 >= 0 && j1 < n[a1] && j2 >= 0 && j2 < n[a2]) {
       int idx[3];
       idx[fast] = jf; idx[a1] = j1; idx[a2] = j2;
       v = src[((long long)idx[2] * ny + idx[1]) * nx + idx[0]];
     }
-    dst[k] = v;
+    reinterpret_cast<uint16_t*>(dst)[k] = (uint16_t)v;  // run = 0
+  }
+}
+
+// run of a cell = number of cells following it along the row in direction run_dir that hold the same ID, capped at
+// 255.  One thread per row, walking against run_dir.
+__global__ void __launch_bounds__(256) voxel_runs_kernel(uint8_t* __restrict__ cells, long long n_rows, int pitch, int run_dir) {
+  const long long row = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (row >= n_rows) return;
+  uint8_t* r = cells + 2 * row * pitch;
+  int j = run_dir > 0 ? pitch - 1 : 0;
+  unsigned prev_id = r[2 * j], run = 0u;
+  for (int k = 1; k < pitch; ++k) {
+    j -= run_dir;
+    const unsigned id = r[2 * j];
+    run = id == prev_id ? min(run + 1u, 255u) : 0u;
+    r[2 * j + 1] = (uint8_t)run;
+    prev_id = id;
   }
 }
 
@@ -1173,10 +1205,13 @@ cudaError_t launch_tally_read(const TallyBin* bins, uint64_t n_bins, unsigned lo
 }
 
 cudaError_t launch_voxel_relayout(const uint8_t* src, uint8_t* dst, int nx, int ny, int nz, int fast, int a1, int a2,
-                                  int pitch, cudaStream_t stream) {
+                                  int pitch, int run_dir, cudaStream_t stream) {
   cudaError_t e = kernels_init();
   if (e != cudaSuccess) return e;
   voxel_relayout_kernel<<<g_n_sm * 8, 256, 0, stream>>>(src, dst, nx, ny, nz, fast, a1, a2, pitch);
+  const int n[3] = {nx, ny, nz};
+  const long long n_rows = (long long)(n[a2] + 2) * (n[a1] + 2);
+  voxel_runs_kernel<<<(unsigned)((n_rows + 255) / 256), 256, 0, stream>>>(dst, n_rows, pitch, run_dir);
   return cudaGetLastError();
 }
 
