@@ -24,7 +24,7 @@ struct mcx_instrument {
   size_t off_staging = 0;
   size_t upload_bytes = 0;              // host -> device bytes moved by create
   int n_comps = 0, n_mats = 0, n_dets = 0, features = 0;
-  int cap_endpoints = 8;                // interval endpoints per ray and solids group (shared memory of the trace kernel)
+  int cap_endpoints = 16;               // interval endpoints per ray and solids group (shared memory of the trace kernel)
   bool sort_pays = false;               // AUTO lane scheduling: detector-tile order
   uint64_t det_bins[MCX_MAX_DETECTORS] = {0, 0, 0, 0};
   uint64_t launches = 0;
@@ -371,7 +371,7 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
   std::memset(&I, 0, sizeof(I));
   I.n_comps = n_components;
   I.n_mats = n_materials;
-  int features = 0, cap_endpoints = 8;
+  int features = 0, cap_endpoints = 16;  // a ray through a mesh vertex makes one hit per triangle around it, on both sides
 
 #define MCX_BAIL(status, ...) do { const mcx_status s_ = fail(status, __VA_ARGS__); delete H; return s_; } while (0)
 
