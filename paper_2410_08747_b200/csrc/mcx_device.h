@@ -153,7 +153,7 @@ struct TraceArgs {
 };
 
 // sizes of the sort workspace
-enum { MCX_SORT_MAX_G = 10, MCX_SORT_MAX_BUCKETS = 1 << 20, MCX_SORT_MAX_SCAN_BLOCKS = 512 };
+enum { MCX_SORT_MAX_G = 11, MCX_SORT_MAX_BUCKETS = 1 << 22, MCX_SORT_MAX_SCAN_BLOCKS = 2048 };
 
 // ---- launch interface (defined in mcx_kernels.cu) ----
 cudaError_t launch_trace(const DInstrument* d_inst, int features, int n_mats, const TraceArgs& args, cudaStream_t stream);  // args.cap_endpoints sizes the shared memory

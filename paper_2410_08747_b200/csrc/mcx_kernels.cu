@@ -833,16 +833,22 @@ __global__ void __launch_bounds__(256) sort_scan_kernel(unsigned int* __restrict
   if (threadIdx.x == 255) bsum[blockIdx.x] = off + inc;
 }
 
-constexpr int kMaxScanBlocks = 512;  // 2^20 buckets / kScanBlock
+constexpr int kMaxScanBlocks = MCX_SORT_MAX_SCAN_BLOCKS;  // 2^22 buckets / kScanBlock
 __global__ void __launch_bounds__(256) sort_scatter_kernel(uint64_t first, uint32_t n, uint64_t seed, int g,
                                                            unsigned int* __restrict__ cnt, const unsigned int* __restrict__ bsum,
                                                            int n_scan_blocks, uint32_t* __restrict__ order) {
   __shared__ unsigned int s_pre[kMaxScanBlocks];
   __shared__ unsigned int s_w[8];
-  {  // exclusive scan of the block totals, two per thread
+  {  // exclusive scan of the block totals, kMaxScanBlocks / 256 consecutive ones per thread
+    constexpr int kPer = kMaxScanBlocks / 256;
     const int t = threadIdx.x;
-    const unsigned int a = 2 * t < n_scan_blocks ? bsum[2 * t] : 0u, b = 2 * t + 1 < n_scan_blocks ? bsum[2 * t + 1] : 0u;
-    unsigned int inc = a + b;
+    unsigned int v[kPer], tot = 0;
+#pragma unroll
+    for (int k = 0; k < kPer; ++k) {
+      v[k] = tot;
+      tot += kPer * t + k < n_scan_blocks ? bsum[kPer * t + k] : 0u;
+    }
+    unsigned int inc = tot;
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
       const unsigned int y = __shfl_up_sync(0xffffffffu, inc, d);
@@ -852,9 +858,9 @@ __global__ void __launch_bounds__(256) sort_scatter_kernel(uint64_t first, uint3
     __syncthreads();
     unsigned int off = 0;
     for (int w = 0; w < (t >> 5); ++w) off += s_w[w];
-    const unsigned int excl = off + inc - (a + b);
-    s_pre[2 * t] = excl;
-    s_pre[2 * t + 1] = excl + a;
+    const unsigned int excl = off + inc - tot;
+#pragma unroll
+    for (int k = 0; k < kPer; ++k) s_pre[kPer * t + k] = excl + v[k];
     __syncthreads();
   }
   const uint32_t stride = gridDim.x * blockDim.x;
@@ -1184,7 +1190,7 @@ cudaError_t launch_sort(uint64_t first, uint32_t n, uint64_t seed, int g, unsign
   if (e != cudaSuccess) return e;
   const uint32_t n_buckets = 1u << (2 * g);
   const int n_scan_blocks = (int)((n_buckets + kScanBlock - 1) / kScanBlock);
-  if (g < 1 || g > 10 || n_scan_blocks > kMaxScanBlocks) return cudaErrorInvalidValue;
+  if (g < 1 || g > MCX_SORT_MAX_G || n_scan_blocks > kMaxScanBlocks) return cudaErrorInvalidValue;
   const unsigned want = (n + 255u) / 256u;
   const unsigned grid = want < (unsigned)g_n_sm * 8u ? (want ? want : 1u) : (unsigned)g_n_sm * 8u;
   sort_count_kernel<<<grid, 256, 0, stream>>>(first, n, seed, g, cnt);
