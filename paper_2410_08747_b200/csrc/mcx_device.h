@@ -146,6 +146,7 @@ enum { F_SOLIDS = 1, F_MESH = 2, F_VOXELS = 4, F_OPTICS = 8, F_ALL = 15 };
 struct TraceArgs {
   uint64_t first, n, seed;
   unsigned tile;           // positions per work ticket (set by launch_trace)
+  int gate_max;            // components 1..gate_max are slits / mirrors / crystals: candidates for the absorber gate; 0 = off
   int cap_endpoints;       // interval endpoints per ray and solids group held in shared memory (a multiple of 8)
   const uint32_t* order;   // detector-tile order of the chunk (launch_sort), or null
   mcx_ray_fate* dump;      // per-ray records indexed by ray offset, or null = tally

@@ -25,6 +25,7 @@ struct mcx_instrument {
   size_t upload_bytes = 0;              // host -> device bytes moved by create
   int n_comps = 0, n_mats = 0, n_dets = 0, features = 0;
   int cap_endpoints = 16;               // interval endpoints per ray and solids group (shared memory of the trace kernel)
+  int gate_max = 0;                     // leading slits / mirrors / crystals of the chain (TraceArgs::gate_max)
   bool sort_pays = false;               // AUTO lane scheduling: detector-tile order
   uint64_t det_bins[MCX_MAX_DETECTORS] = {0, 0, 0, 0};
   uint64_t launches = 0;
@@ -612,6 +613,12 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
   H->n_dets = n_dets;
   H->features = features;
   H->cap_endpoints = cap_endpoints;
+  if (env_int("MCX_GATE", 0, 1, 1))
+    for (int c = 1; c + 1 < n_components; ++c) {
+      const int k = components[c].kind;
+      if (k != MCX_SLIT_RECT && k != MCX_SLIT_CIRC && k != MCX_MIRROR_ELLIPTIC && k != MCX_CRYSTAL_BRAGG) break;
+      H->gate_max = c;
+    }
   {  // Detector-tile order needs a source whose slot-1 draw is a target point (step 3) and pays where neighbouring rays
      // share work: voxels, meshes, groups of several solids (measured: c1 1.4x, c3 5x, c4 3x; c0 and c2 nothing)
     bool shared_work = (features & (F_MESH | F_VOXELS)) != 0;
@@ -654,6 +661,7 @@ mcx_status run_trace(mcx_instrument* H, uint64_t first, uint64_t n, uint64_t see
     A.n = m;
     A.seed = seed;
     A.cap_endpoints = H->cap_endpoints;
+    A.gate_max = H->gate_max;
     A.order = nullptr;
     A.dump = dump ? dump + base : nullptr;
     A.ticket = (unsigned int*)(ws + H->off_ticket);

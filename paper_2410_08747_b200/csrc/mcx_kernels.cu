@@ -876,6 +876,7 @@ __global__ void __launch_bounds__(256) sort_scatter_kernel(uint64_t first, uint3
 // tallying.  Shared memory: the instrument image, per-block ray-accounting counters, the solids of every group,
 // per-thread mu[] for the voxel walk.  Spectrum CDFs and mu(E) tables are read through L1.
 // ------------------------------------------------------------------------------------------------------------
+constexpr size_t kRingBytes = (kBlock / 32) * 64 * sizeof(unsigned);  // per-warp rings of gate survivors
 constexpr unsigned kTileMax = 8192;  // positions per work ticket (a power of two >= kBlock; smaller for short launches)
 constexpr int kSmemSolids = 32;    // solids staged in shared memory (all groups together)
 
@@ -888,7 +889,7 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
   DInstrument& I = *reinterpret_cast<DInstrument*>(smem_raw);
   unsigned int* s_cnt = reinterpret_cast<unsigned int*>(smem_raw + sizeof(DInstrument));  // [MCX_MAX_COMPONENTS + 4]
   unsigned int* s_sched = s_cnt + MCX_MAX_COMPONENTS + 4;  // [0..1] tile tickets, [2..3] slice counters (ping-pong)
-  unsigned char* s_extra = smem_raw + sizeof(DInstrument) + 128;
+  unsigned char* s_extra = smem_raw + sizeof(DInstrument) + 128 + kRingBytes;
   {
     const int4* src = reinterpret_cast<const int4*>(g_inst);
     int4* dst = reinterpret_cast<int4*>(smem_raw);
@@ -943,29 +944,56 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
     s_sched[2] = 0u;
   }
   __syncthreads();
+  // Absorber gate (row a13, "warp-level compaction of absorbed rays").  Where the chain starts with slits, mirrors or
+  // crystals (A.gate_max of them) and few rays survive those (c0 loses 84 % at its slit, c2 87 % at its two mirrors),
+  // fresh rays are traced through components 1..gate only, and the offsets of the survivors go into a per-warp ring
+  // in shared memory (ballot + prefix count); whenever the ring holds 32 the warp traces those through the WHOLE chain
+  // from the source again, all lanes alive at the gate.  Legal because a ray is a pure function of its index
+  // (slot-addressed draws), cheap because the replayed part is the source and a few apertures.  Rays absorbed up to
+  // the gate are accounted in the first pass, everything a queued ray does in the second (it is counted there whatever
+  // happens to it), so every ray is counted once.  The block picks the gate itself from what its first tile (traced
+  // ungated) lost where: the first component after which at most 35 % of the rays are left, if there is one.
+  int gate = 0;
+  unsigned* ring = reinterpret_cast<unsigned*>(smem_raw + sizeof(DInstrument) + 128) + (threadIdx.x >> 5) * 64;
+  unsigned ring_head = 0u, ring_n = 0u;  // warp-uniform
   for (unsigned it = 0;; ++it) {
     const unsigned par = it & 1u;
     const uint64_t tile_begin = (uint64_t)s_sched[par] * tile;
-    if (tile_begin >= n) break;
-    if (threadIdx.x == 0) {
+    const bool last = tile_begin >= n;  // no tile left: drain the ring and leave
+    if (!last && threadIdx.x == 0) {
       s_sched[par ^ 1u] = atomicAdd(A.ticket, 1u);
       s_sched[2 + (par ^ 1u)] = 0u;
     }
     for (;;) {
-      unsigned slice = 0u;
-      if (lane == 0) slice = atomicAdd(&s_sched[2 + par], 32u);
-      slice = __shfl_sync(0xffffffffu, slice, 0);
-      if (slice >= tile) break;
-      const uint64_t q = tile_begin + slice + lane;
-      if (q - lane >= n) break;  // the whole warp is beyond the end
-      const bool valid = q < n;
-      const uint64_t qi = valid ? (order ? (uint64_t)order[q] : q) : 0;  // position in the chunk -> ray offset
+      bool valid, final_pass;
+      uint64_t qi;
+      if (ring_n >= 32u || (last && ring_n > 0u)) {  // a warp-load of gate survivors
+        const unsigned take = min(ring_n, 32u);
+        valid = (unsigned)lane < take;
+        qi = ring[(ring_head + lane) & 63u];
+        ring_head = (ring_head + take) & 63u;
+        ring_n -= take;
+        final_pass = true;
+      } else if (!last) {
+        unsigned slice = 0u;
+        if (lane == 0) slice = atomicAdd(&s_sched[2 + par], 32u);
+        slice = __shfl_sync(0xffffffffu, slice, 0);
+        if (slice >= tile) break;
+        const uint64_t q = tile_begin + slice + lane;
+        if (q - lane >= n) break;  // the whole warp is beyond the end
+        valid = q < n;
+        qi = valid ? (order ? (uint64_t)order[q] : q) : 0;  // position in the chunk -> ray offset
+        final_pass = gate == 0;
+      } else {
+        break;
+      }
+      const int c_end = final_pass ? n_comps : gate + 1;
       Ray ray;
       int fate = MCX_FATE_MISSED;
       long long bin = -1;
       bool alive = valid;
       if (valid) sample_source(I.comps[0], seed, first + qi, ray);
-      for (int c = 1; c < n_comps; ++c) {
+      for (int c = 1; c < c_end; ++c) {
         const DComponent& C = I.comps[c];
         const int kind = C.kind;  // warp-uniform
         bool pass = true;
@@ -1018,8 +1046,14 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
         }
         if (alive_mask == 0u) break;
       }
+      if (!final_pass) {  // survivors of the gate: queue their offsets for the full pass
+        const unsigned live = __ballot_sync(0xffffffffu, alive);
+        if (alive) ring[(ring_head + ring_n + __popc(live & ((1u << lane) - 1u))) & 63u] = (unsigned)qi;
+        ring_n += __popc(live);
+        __syncwarp();
+      }
       if (DUMP) {
-        if (valid) {
+        if (valid && (final_pass || !alive)) {
           mcx_ray_fate f;
           f.fate = fate;
           f.reserved = 0;
@@ -1028,9 +1062,9 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
           dump[qi] = f;
         }
       } else {
-        const unsigned det = __ballot_sync(0xffffffffu, valid && fate == MCX_FATE_DETECTED);
-        const unsigned mis = __ballot_sync(0xffffffffu, valid && fate == MCX_FATE_MISSED);
-        const unsigned deg = __ballot_sync(0xffffffffu, valid && fate == MCX_FATE_DEGENERATE);
+        const unsigned det = __ballot_sync(0xffffffffu, valid && final_pass && fate == MCX_FATE_DETECTED);
+        const unsigned mis = __ballot_sync(0xffffffffu, valid && final_pass && fate == MCX_FATE_MISSED);
+        const unsigned deg = __ballot_sync(0xffffffffu, valid && final_pass && fate == MCX_FATE_DEGENERATE);
         if (lane == 0) {
           if (det) atomicAdd(&s_cnt[MCX_MAX_COMPONENTS + CNT_DETECTED], (unsigned)__popc(det));
           if (mis) atomicAdd(&s_cnt[MCX_MAX_COMPONENTS + CNT_MISSED], (unsigned)__popc(mis));
@@ -1038,7 +1072,22 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
         }
       }
     }
+    if (last) break;
     __syncthreads();  // the tile is done and the next ticket is in place
+    if (it == 0u && A.gate_max > 0 && !DUMP) {
+      if (threadIdx.x == 0) {
+        const uint64_t left_in_range = n - tile_begin;
+        const unsigned traced = left_in_range < tile ? (unsigned)left_in_range : tile;
+        unsigned alive_after = traced, pick = 0u;
+        for (int c = 1; c <= A.gate_max && pick == 0u; ++c) {
+          alive_after -= s_cnt[c];
+          if (100u * alive_after <= 35u * traced) pick = (unsigned)c;
+        }
+        s_sched[4] = pick;
+      }
+      __syncthreads();
+      gate = (int)s_sched[4];
+    }
   }
   // the last block to leave re-arms the ticket counter for the next launch
   if (threadIdx.x == 0) {
@@ -1124,7 +1173,7 @@ __global__ void __launch_bounds__(256) probe_dfma_kernel(double* sink, long long
   sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
 }
 
-constexpr size_t kSmemBase = sizeof(DInstrument) + 128;
+constexpr size_t kSmemBase = sizeof(DInstrument) + 128 + kRingBytes;
 
 template <int FEAT, bool DUMP>
 cudaError_t launch_one(const DInstrument* d_inst, int n_mats, const TraceArgs& A, cudaStream_t stream, int n_sm) {
