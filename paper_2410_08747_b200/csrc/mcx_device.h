@@ -57,6 +57,7 @@ struct DSolid {
   int shape, material, priority, n_nodes;  // n_nodes: BVH nodes of a mesh
   DPose pose;
   double dims[3];
+  double bound2;                  // primitives: (radius of the bounding sphere about the solid's origin, plus 1e-9)^2
   double root_lo[3], root_hi[3];  // fp64 AABB of the mesh (solid-local)
   const BvhNode* nodes;
   const double* tris;  // [n_tris][9] vertices in BVH leaf order

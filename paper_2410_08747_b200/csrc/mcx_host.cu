@@ -488,6 +488,11 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
           d.shape = S.shape; d.material = S.material; d.priority = S.priority;
           copy_pose(&d.pose, S.pose);
           for (int k = 0; k < 3; ++k) d.dims[k] = S.dims[k];
+          {  // bounding sphere about the solid's origin: box half-diagonal, sphere radius, cylinder (radius, half height)
+            const double r2 = S.shape == MCX_BOX ? S.dims[0] * S.dims[0] + S.dims[1] * S.dims[1] + S.dims[2] * S.dims[2]
+                            : S.shape == MCX_SPHERE ? S.dims[0] * S.dims[0] : S.dims[0] * S.dims[0] + S.dims[1] * S.dims[1];
+            d.bound2 = r2 * (1.0 + 2e-9);
+          }
           if (S.shape != MCX_MESH) continue;
           features |= F_MESH;
           D.u.solids.n_mesh++;

@@ -350,9 +350,15 @@ __device__ __forceinline__ int mesh_endpoints(const DSolid& S, unsigned solid, V
   if (!(tmin < tmax)) return 1;
   const Vec3 e = o + tmin * d;
   const float ox = (float)e.x, oy = (float)e.y, oz = (float)e.z;
-  const float big = 3.0e38f;
-  const float ix = d.x != 0.0 ? (float)(1.0 / d.x) : big, iy = d.y != 0.0 ? (float)(1.0 / d.y) : big,
-              iz = d.z != 0.0 ? (float)(1.0 / d.z) : big;
+  // 1/d, held to +-1e30 so that the products below stay finite (a ray parallel to a pair of planes gets huge
+  // parameters of the right signs instead of infinities)
+  const float big = 1.0e30f;
+  const float ix = d.x != 0.0 ? fminf(fmaxf((float)(1.0 / d.x), -big), big) : big;
+  const float iy = d.y != 0.0 ? fminf(fmaxf((float)(1.0 / d.y), -big), big) : big;
+  const float iz = d.z != 0.0 ? fminf(fmaxf((float)(1.0 / d.z), -big), big) : big;
+  // (x - o) / d as one fused multiply-add per plane: x * (1/d) + (-o/d).  Its rounding error is below 2^-22 of the
+  // mesh scale times |1/d|, the boxes are padded by 2^-16 of the scale (times |1/d| in t): the test stays conservative.
+  const float bx = -ox * ix, by = -oy * iy, bz = -oz * iz;
   const Shear sh = make_shear(d);
   const int begin = ne, n_nodes = S.n_nodes;
   const float4* __restrict__ nodes = reinterpret_cast<const float4*>(S.nodes);
@@ -364,9 +370,9 @@ __device__ __forceinline__ int mesh_endpoints(const DSolid& S, unsigned solid, V
     while (node < n_nodes && nq <= kTriQueue - kBvhLeafMax) {
       const float4 a = __ldg(nodes + 2 * node), b = __ldg(nodes + 2 * node + 1);  // lo.xyz, escape | hi.xyz, tris
       // slab test of the full line against the padded fp32 box (no t range: the line is tested, as in step 9)
-      const float tx0 = (a.x - ox) * ix, tx1 = (b.x - ox) * ix;
-      const float ty0 = (a.y - oy) * iy, ty1 = (b.y - oy) * iy;
-      const float tz0 = (a.z - oz) * iz, tz1 = (b.z - oz) * iz;
+      const float tx0 = fmaf(a.x, ix, bx), tx1 = fmaf(b.x, ix, bx);
+      const float ty0 = fmaf(a.y, iy, by), ty1 = fmaf(b.y, iy, by);
+      const float tz0 = fmaf(a.z, iz, bz), tz1 = fmaf(b.z, iz, bz);
       const float tn = fmaxf(fmaxf(fminf(tx0, tx1), fminf(ty0, ty1)), fminf(tz0, tz1));
       const float tf = fminf(fminf(fmaxf(tx0, tx1), fmaxf(ty0, ty1)), fmaxf(tz0, tz1));
       const bool hit = tn <= tf;
@@ -420,6 +426,13 @@ __device__ __forceinline__ int trace_solids(const DInstrument& I, const DCompone
   int ne = 0;
   for (int s = 0; s < G.n_solids; ++s) {
     const DSolid& S = G.solids[s];
+    if (!MESH) {  // (the mesh kernels run at the register limit and do without)
+      // the line misses the solid's bounding sphere, by more than the rounding of this test (1e-9 of the radius^2 in
+      // bound2, 1e-14 of the squared distance for the cancellation): no interval, no need for the solid's frame
+      const Vec3 oc = Vec3{S.pose.T[0], S.pose.T[1], S.pose.T[2]} - ray.r;
+      const double along = dot(oc, ray.d), oc2 = dot(oc, oc);
+      if (oc2 - along * along > S.bound2 + 1e-14 * oc2) continue;
+    }
     const Vec3 o = to_local(S.pose, ray.r);
     const Vec3 d = rotate(S.pose.R, ray.d);
     if (MESH && S.shape == MCX_MESH) {
@@ -883,13 +896,13 @@ constexpr int kSmemSolids = 32;    // solids staged in shared memory (all groups
 // resident blocks per SM the register budget is held to: the voxel walk hides its byte loads with warps
 constexpr int min_blocks(int feat) { return feat == F_VOXELS || feat == F_SOLIDS || feat == (F_SOLIDS | F_MESH) ? 3 : 1; }
 
-template <int FEAT, bool DUMP>
+template <int FEAT, bool DUMP, bool GATE>
 __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const DInstrument* __restrict__ g_inst, TraceArgs A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   DInstrument& I = *reinterpret_cast<DInstrument*>(smem_raw);
   unsigned int* s_cnt = reinterpret_cast<unsigned int*>(smem_raw + sizeof(DInstrument));  // [MCX_MAX_COMPONENTS + 4]
   unsigned int* s_sched = s_cnt + MCX_MAX_COMPONENTS + 4;  // [0..1] tile tickets, [2..3] slice counters (ping-pong)
-  unsigned char* s_extra = smem_raw + sizeof(DInstrument) + 128 + kRingBytes;
+  unsigned char* s_extra = smem_raw + sizeof(DInstrument) + 128 + (GATE ? kRingBytes : 0);
   {
     const int4* src = reinterpret_cast<const int4*>(g_inst);
     int4* dst = reinterpret_cast<int4*>(smem_raw);
@@ -956,137 +969,164 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
   int gate = 0;
   unsigned* ring = reinterpret_cast<unsigned*>(smem_raw + sizeof(DInstrument) + 128) + (threadIdx.x >> 5) * 64;
   unsigned ring_head = 0u, ring_n = 0u;  // warp-uniform
-  for (unsigned it = 0;; ++it) {
-    const unsigned par = it & 1u;
-    const uint64_t tile_begin = (uint64_t)s_sched[par] * tile;
-    const bool last = tile_begin >= n;  // no tile left: drain the ring and leave
-    if (!last && threadIdx.x == 0) {
-      s_sched[par ^ 1u] = atomicAdd(A.ticket, 1u);
-      s_sched[2 + (par ^ 1u)] = 0u;
+  // One warp-load of rays through components 1 .. (final_pass ? the end : the gate); see the loops below.
+  auto trace_item = [&](const bool valid, const uint64_t qi, const bool final_pass) {
+    const int c_end = final_pass ? n_comps : gate + 1;
+    Ray ray;
+    int fate = MCX_FATE_MISSED;
+    long long bin = -1;
+    bool alive = valid;
+    if (valid) sample_source(I.comps[0], seed, first + qi, ray);
+    for (int c = 1; c < c_end; ++c) {
+      const DComponent& C = I.comps[c];
+      const int kind = C.kind;  // warp-uniform
+      bool pass = true;
+      if (alive) {
+        if (kind == MCX_SLIT_RECT) {
+          Vec3 h;
+          pass = plane_hit(C.pose, ray, h) && fabs(h.x) <= C.u.slit.half_x && fabs(h.y) <= C.u.slit.half_y;
+        } else if (kind == MCX_SLIT_CIRC) {
+          Vec3 h;
+          pass = plane_hit(C.pose, ray, h) && h.x * h.x + h.y * h.y <= C.u.slit.radius2;
+        } else if ((FEAT & F_SOLIDS) && kind == MCX_SOLIDS) {
+          const int rc = trace_solids<(FEAT & F_MESH) != 0>(I, C, ray, ep, tri_queue);
+          if (rc != 1) {
+            pass = false;
+            fate = MCX_FATE_DEGENERATE;
+            if (rc < 0 && !DUMP) atomicAdd(&s_cnt[MCX_MAX_COMPONENTS + CNT_OVERFLOW], 1u);
+          }
+        } else if ((FEAT & F_VOXELS) && kind == MCX_VOXELS) {
+          trace_voxels(I, C, ray, len_s, len_s + (size_t)I.n_mats * kBlock);
+        } else if ((FEAT & F_OPTICS) && kind == MCX_MIRROR_ELLIPTIC) {
+          pass = trace_mirror(C, ray);
+        } else if ((FEAT & F_OPTICS) && kind == MCX_CRYSTAL_BRAGG) {
+          pass = trace_crystal(C, ray);
+        } else if (kind == MCX_DETECTOR) {
+          const long long b = detector_bin(C, ray);
+          if (b >= 0) {
+            bin = b;
+            fate = MCX_FATE_DETECTED;
+            if (!DUMP) {
+              TallyBin* rec = I.tallies[C.u.detector.index] + b;
+              atomicAdd(&rec->N, 1ull);
+              atomicAdd(&rec->P, ray.p);
+              atomicAdd(&rec->P2, ray.p * ray.p);
+            }
+          } else {
+            fate = MCX_FATE_MISSED;  // monitors do not absorb: the ray goes on
+          }
+        }
+        if (kind != MCX_DETECTOR && pass) fate = MCX_FATE_MISSED;  // fate = what the last component said
+        if (!pass) {
+          alive = false;
+          if (fate != MCX_FATE_DEGENERATE) fate = c;
+        }
+      }
+      const unsigned alive_mask = __ballot_sync(0xffffffffu, alive);
+      if (!DUMP) {
+        // warp-aggregated ray accounting: one shared-memory add per warp and component
+        const unsigned died = __ballot_sync(0xffffffffu, !pass && fate == c);
+        if (lane == 0 && died) atomicAdd(&s_cnt[c], (unsigned)__popc(died));
+      }
+      if (alive_mask == 0u) break;
     }
-    for (;;) {
-      bool valid, final_pass;
-      uint64_t qi;
-      if (ring_n >= 32u || (last && ring_n > 0u)) {  // a warp-load of gate survivors
-        const unsigned take = min(ring_n, 32u);
-        valid = (unsigned)lane < take;
-        qi = ring[(ring_head + lane) & 63u];
-        ring_head = (ring_head + take) & 63u;
-        ring_n -= take;
-        final_pass = true;
-      } else if (!last) {
+    if (GATE && !final_pass) {  // survivors of the gate: queue their offsets for the full pass
+      const unsigned live = __ballot_sync(0xffffffffu, alive);
+      if (alive) ring[(ring_head + ring_n + __popc(live & ((1u << lane) - 1u))) & 63u] = (unsigned)qi;
+      ring_n += __popc(live);
+      __syncwarp();
+    }
+    if (DUMP) {
+      if (valid && (final_pass || !alive)) {
+        mcx_ray_fate f;
+        f.fate = fate;
+        f.reserved = 0;
+        f.bin = fate == MCX_FATE_DETECTED ? bin : -1;
+        f.p = ray.p;
+        dump[qi] = f;
+      }
+    } else {
+      const unsigned det = __ballot_sync(0xffffffffu, valid && final_pass && fate == MCX_FATE_DETECTED);
+      const unsigned mis = __ballot_sync(0xffffffffu, valid && final_pass && fate == MCX_FATE_MISSED);
+      const unsigned deg = __ballot_sync(0xffffffffu, valid && final_pass && fate == MCX_FATE_DEGENERATE);
+      if (lane == 0) {
+        if (det) atomicAdd(&s_cnt[MCX_MAX_COMPONENTS + CNT_DETECTED], (unsigned)__popc(det));
+        if (mis) atomicAdd(&s_cnt[MCX_MAX_COMPONENTS + CNT_MISSED], (unsigned)__popc(mis));
+        if (deg) atomicAdd(&s_cnt[MCX_MAX_COMPONENTS + CNT_DEGENERATE], (unsigned)__popc(deg));
+      }
+    }
+  };
+  if (!GATE) {
+    for (unsigned it = 0;; ++it) {
+      const unsigned par = it & 1u;
+      const uint64_t tile_begin = (uint64_t)s_sched[par] * tile;
+      if (tile_begin >= n) break;
+      if (threadIdx.x == 0) {
+        s_sched[par ^ 1u] = atomicAdd(A.ticket, 1u);
+        s_sched[2 + (par ^ 1u)] = 0u;
+      }
+      for (;;) {
         unsigned slice = 0u;
         if (lane == 0) slice = atomicAdd(&s_sched[2 + par], 32u);
         slice = __shfl_sync(0xffffffffu, slice, 0);
         if (slice >= tile) break;
         const uint64_t q = tile_begin + slice + lane;
         if (q - lane >= n) break;  // the whole warp is beyond the end
-        valid = q < n;
-        qi = valid ? (order ? (uint64_t)order[q] : q) : 0;  // position in the chunk -> ray offset
-        final_pass = gate == 0;
-      } else {
-        break;
+        const bool valid = q < n;
+        trace_item(valid, valid ? (order ? (uint64_t)order[q] : q) : 0, true);  // position in the chunk -> ray offset
       }
-      const int c_end = final_pass ? n_comps : gate + 1;
-      Ray ray;
-      int fate = MCX_FATE_MISSED;
-      long long bin = -1;
-      bool alive = valid;
-      if (valid) sample_source(I.comps[0], seed, first + qi, ray);
-      for (int c = 1; c < c_end; ++c) {
-        const DComponent& C = I.comps[c];
-        const int kind = C.kind;  // warp-uniform
-        bool pass = true;
-        if (alive) {
-          if (kind == MCX_SLIT_RECT) {
-            Vec3 h;
-            pass = plane_hit(C.pose, ray, h) && fabs(h.x) <= C.u.slit.half_x && fabs(h.y) <= C.u.slit.half_y;
-          } else if (kind == MCX_SLIT_CIRC) {
-            Vec3 h;
-            pass = plane_hit(C.pose, ray, h) && h.x * h.x + h.y * h.y <= C.u.slit.radius2;
-          } else if ((FEAT & F_SOLIDS) && kind == MCX_SOLIDS) {
-            const int rc = trace_solids<(FEAT & F_MESH) != 0>(I, C, ray, ep, tri_queue);
-            if (rc != 1) {
-              pass = false;
-              fate = MCX_FATE_DEGENERATE;
-              if (rc < 0 && !DUMP) atomicAdd(&s_cnt[MCX_MAX_COMPONENTS + CNT_OVERFLOW], 1u);
-            }
-          } else if ((FEAT & F_VOXELS) && kind == MCX_VOXELS) {
-            trace_voxels(I, C, ray, len_s, len_s + (size_t)I.n_mats * kBlock);
-          } else if ((FEAT & F_OPTICS) && kind == MCX_MIRROR_ELLIPTIC) {
-            pass = trace_mirror(C, ray);
-          } else if ((FEAT & F_OPTICS) && kind == MCX_CRYSTAL_BRAGG) {
-            pass = trace_crystal(C, ray);
-          } else if (kind == MCX_DETECTOR) {
-            const long long b = detector_bin(C, ray);
-            if (b >= 0) {
-              bin = b;
-              fate = MCX_FATE_DETECTED;
-              if (!DUMP) {
-                TallyBin* rec = I.tallies[C.u.detector.index] + b;
-                atomicAdd(&rec->N, 1ull);
-                atomicAdd(&rec->P, ray.p);
-                atomicAdd(&rec->P2, ray.p * ray.p);
-              }
-            } else {
-              fate = MCX_FATE_MISSED;  // monitors do not absorb: the ray goes on
-            }
-          }
-          if (kind != MCX_DETECTOR && pass) fate = MCX_FATE_MISSED;  // fate = what the last component said
-          if (!pass) {
-            alive = false;
-            if (fate != MCX_FATE_DEGENERATE) fate = c;
-          }
-        }
-        const unsigned alive_mask = __ballot_sync(0xffffffffu, alive);
-        if (!DUMP) {
-          // warp-aggregated ray accounting: one shared-memory add per warp and component
-          const unsigned died = __ballot_sync(0xffffffffu, !pass && fate == c);
-          if (lane == 0 && died) atomicAdd(&s_cnt[c], (unsigned)__popc(died));
-        }
-        if (alive_mask == 0u) break;
-      }
-      if (!final_pass) {  // survivors of the gate: queue their offsets for the full pass
-        const unsigned live = __ballot_sync(0xffffffffu, alive);
-        if (alive) ring[(ring_head + ring_n + __popc(live & ((1u << lane) - 1u))) & 63u] = (unsigned)qi;
-        ring_n += __popc(live);
-        __syncwarp();
-      }
-      if (DUMP) {
-        if (valid && (final_pass || !alive)) {
-          mcx_ray_fate f;
-          f.fate = fate;
-          f.reserved = 0;
-          f.bin = fate == MCX_FATE_DETECTED ? bin : -1;
-          f.p = ray.p;
-          dump[qi] = f;
-        }
-      } else {
-        const unsigned det = __ballot_sync(0xffffffffu, valid && final_pass && fate == MCX_FATE_DETECTED);
-        const unsigned mis = __ballot_sync(0xffffffffu, valid && final_pass && fate == MCX_FATE_MISSED);
-        const unsigned deg = __ballot_sync(0xffffffffu, valid && final_pass && fate == MCX_FATE_DEGENERATE);
-        if (lane == 0) {
-          if (det) atomicAdd(&s_cnt[MCX_MAX_COMPONENTS + CNT_DETECTED], (unsigned)__popc(det));
-          if (mis) atomicAdd(&s_cnt[MCX_MAX_COMPONENTS + CNT_MISSED], (unsigned)__popc(mis));
-          if (deg) atomicAdd(&s_cnt[MCX_MAX_COMPONENTS + CNT_DEGENERATE], (unsigned)__popc(deg));
-        }
-      }
+      __syncthreads();  // the tile is done and the next ticket is in place
     }
-    if (last) break;
-    __syncthreads();  // the tile is done and the next ticket is in place
-    if (it == 0u && A.gate_max > 0 && !DUMP) {
-      if (threadIdx.x == 0) {
-        const uint64_t left_in_range = n - tile_begin;
-        const unsigned traced = left_in_range < tile ? (unsigned)left_in_range : tile;
-        unsigned alive_after = traced, pick = 0u;
-        for (int c = 1; c <= A.gate_max && pick == 0u; ++c) {
-          alive_after -= s_cnt[c];
-          if (100u * alive_after <= 35u * traced) pick = (unsigned)c;
-        }
-        s_sched[4] = pick;
+  } else {
+    for (unsigned it = 0;; ++it) {
+      const unsigned par = it & 1u;
+      const uint64_t tile_begin = (uint64_t)s_sched[par] * tile;
+      const bool last = tile_begin >= n;  // no tile left: drain the ring and leave
+      if (!last && threadIdx.x == 0) {
+        s_sched[par ^ 1u] = atomicAdd(A.ticket, 1u);
+        s_sched[2 + (par ^ 1u)] = 0u;
       }
-      __syncthreads();
-      gate = (int)s_sched[4];
+      for (;;) {
+        bool valid, final_pass;
+        uint64_t qi;
+        if (GATE && (ring_n >= 32u || (last && ring_n > 0u))) {  // a warp-load of gate survivors
+          const unsigned take = min(ring_n, 32u);
+          valid = (unsigned)lane < take;
+          qi = ring[(ring_head + lane) & 63u];
+          ring_head = (ring_head + take) & 63u;
+          ring_n -= take;
+          final_pass = true;
+        } else if (!last) {
+          unsigned slice = 0u;
+          if (lane == 0) slice = atomicAdd(&s_sched[2 + par], 32u);
+          slice = __shfl_sync(0xffffffffu, slice, 0);
+          if (slice >= tile) break;
+          const uint64_t q = tile_begin + slice + lane;
+          if (q - lane >= n) break;  // the whole warp is beyond the end
+          valid = q < n;
+          qi = valid ? (order ? (uint64_t)order[q] : q) : 0;  // position in the chunk -> ray offset
+          final_pass = !GATE || gate == 0;
+        } else {
+          break;
+        }
+        trace_item(valid, qi, final_pass);
+      }
+      if (last) break;
+      __syncthreads();  // the tile is done and the next ticket is in place
+      if (GATE && it == 0u) {
+        if (threadIdx.x == 0) {
+          const uint64_t left_in_range = n - tile_begin;
+          const unsigned traced = left_in_range < tile ? (unsigned)left_in_range : tile;
+          unsigned alive_after = traced, pick = 0u;
+          for (int c = 1; c <= A.gate_max && pick == 0u; ++c) {
+            alive_after -= s_cnt[c];
+            if (100u * alive_after <= 35u * traced) pick = (unsigned)c;
+          }
+          s_sched[4] = pick;
+        }
+        __syncthreads();
+        gate = (int)s_sched[4];
+      }
     }
   }
   // the last block to leave re-arms the ticket counter for the next launch
@@ -1173,22 +1213,22 @@ __global__ void __launch_bounds__(256) probe_dfma_kernel(double* sink, long long
   sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
 }
 
-constexpr size_t kSmemBase = sizeof(DInstrument) + 128 + kRingBytes;
+constexpr size_t kSmemBase = sizeof(DInstrument) + 128;
 
-template <int FEAT, bool DUMP>
+template <int FEAT, bool DUMP, bool GATE>
 cudaError_t launch_one(const DInstrument* d_inst, int n_mats, const TraceArgs& A, cudaStream_t stream, int n_sm) {
-  const size_t smem = kSmemBase + ((FEAT & F_SOLIDS) ? kSmemSolids * sizeof(DSolid) + (size_t)A.cap_endpoints * kBlock * 9 : 0) +
+  const size_t smem = kSmemBase + (GATE ? kRingBytes : 0) + ((FEAT & F_SOLIDS) ? kSmemSolids * sizeof(DSolid) + (size_t)A.cap_endpoints * kBlock * 9 : 0) +
                       ((FEAT & F_MESH) ? (size_t)kTriQueue * kBlock * sizeof(unsigned) : 0) +
                       ((FEAT & F_VOXELS) ? (size_t)(n_mats + VC_COUNT) * kBlock * sizeof(double) : 0);
   static bool configured = false;
   int blocks_per_sm = 1;
   cudaError_t e;
   if (!configured) {
-    e = cudaFuncSetAttribute(trace_kernel<FEAT, DUMP>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    e = cudaFuncSetAttribute(trace_kernel<FEAT, DUMP, GATE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e != cudaSuccess) return e;
     configured = true;
   }
-  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, trace_kernel<FEAT, DUMP>, kBlock, smem);
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, trace_kernel<FEAT, DUMP, GATE>, kBlock, smem);
   if (e != cudaSuccess) return e;
   if (blocks_per_sm < 1) return cudaErrorInvalidConfiguration;
   const uint64_t full = (uint64_t)n_sm * blocks_per_sm;  // one resident wave: a multiple of the SM count
@@ -1197,7 +1237,7 @@ cudaError_t launch_one(const DInstrument* d_inst, int n_mats, const TraceArgs& A
   while (B.tile > (unsigned)kBlock && A.n / B.tile < 4 * full) B.tile >>= 1;
   const uint64_t want = (A.n + B.tile - 1) / B.tile;
   const unsigned grid = (unsigned)(want < full ? (want ? want : 1) : full);
-  trace_kernel<FEAT, DUMP><<<grid, kBlock, smem, stream>>>(d_inst, B);
+  trace_kernel<FEAT, DUMP, GATE><<<grid, kBlock, smem, stream>>>(d_inst, B);
   return cudaGetLastError();
 }
 
@@ -1218,18 +1258,25 @@ cudaError_t launch_trace(const DInstrument* d_inst, int features, int n_mats, co
   if (e != cudaSuccess) return e;
   if (A.n == 0) return cudaSuccess;
   if (A.n > ((uint64_t)1 << 40)) return cudaErrorInvalidValue;  // tile tickets are 32-bit; the host chunks below this
+  // the absorber gate is compiled into the tallying kernels of the chains that can start with absorbers and stay light
+  // (no mesh, no voxels: those run at the register limit and their chains start at the sample)
 #define MCX_DISPATCH(F)                                                              \
-  return A.dump ? launch_one<F, true>(d_inst, n_mats, A, stream, g_n_sm)             \
-                : launch_one<F, false>(d_inst, n_mats, A, stream, g_n_sm);
+  return A.dump ? launch_one<F, true, false>(d_inst, n_mats, A, stream, g_n_sm)      \
+                : launch_one<F, false, false>(d_inst, n_mats, A, stream, g_n_sm);
+#define MCX_DISPATCH_GATED(F)                                                        \
+  return A.dump         ? launch_one<F, true, false>(d_inst, n_mats, A, stream, g_n_sm)  \
+         : A.gate_max > 0 ? launch_one<F, false, true>(d_inst, n_mats, A, stream, g_n_sm) \
+                          : launch_one<F, false, false>(d_inst, n_mats, A, stream, g_n_sm);
   switch (features) {
-    case 0: MCX_DISPATCH(0)
-    case F_SOLIDS: MCX_DISPATCH(F_SOLIDS)
+    case 0: MCX_DISPATCH_GATED(0)
+    case F_SOLIDS: MCX_DISPATCH_GATED(F_SOLIDS)
     case F_SOLIDS | F_MESH: MCX_DISPATCH(F_SOLIDS | F_MESH)
     case F_VOXELS: MCX_DISPATCH(F_VOXELS)
-    case F_OPTICS: MCX_DISPATCH(F_OPTICS)
-    default: MCX_DISPATCH(F_ALL)
+    case F_OPTICS: MCX_DISPATCH_GATED(F_OPTICS)
+    default: MCX_DISPATCH_GATED(F_ALL)
   }
 #undef MCX_DISPATCH
+#undef MCX_DISPATCH_GATED
 }
 
 // count -> scan -> scatter of one chunk (n <= 2^32 - 1 rays, 4^g buckets); cnt must be zero on entry
