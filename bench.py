@@ -41,8 +41,8 @@ OPS_VOXEL_ENTRY, OPS_VOXEL_STEP = 100, 6
 OPS_TRI_TEST, OPS_BVH_NODE = 45, 14
 NOMINAL_FP64_LANES_PER_SM, N_SM = 64, 148
 # DRAM bytes per ray of trace_kernel (dram__bytes_read.sum + dram__bytes_write.sum of one launch of 2^26 rays / 2^26) from
-# the ncu --set full captures summarised in profiles/r01c_README.md; None where no capture was taken.
-NCU_DRAM_BYTES_PER_RAY = {"c1_polychromatic": 10.6, "c3_mesh": 17.3, "c4_edxct": 27.8}
+# the ncu --set full captures summarised in profiles/r01d_README.md (c0, c2: whole run / n_rays; their tallies stay in L2).
+NCU_DRAM_BYTES_PER_RAY = {"c0_minimal": 0.001, "c1_polychromatic": 10.5, "c2_beamline": 0.01, "c3_mesh": 17.3, "c4_edxct": 29.0}
 
 
 def reached_per_component(n_rays, absorbed):
@@ -251,7 +251,7 @@ def bench_instrument(M, torch, inst, n_rays, first, steps, warmup, device, dfma_
     res["work_per_ray"] = work
     bpr = NCU_DRAM_BYTES_PER_RAY.get(inst["name"])
     traffic = None if bpr is None else bpr * n_rays      # bytes per step (all launches of the step)
-    traffic_src = None if bpr is None else f"ncu dram bytes {bpr} B/ray (profiles/r01c_README.md) x n_rays"
+    traffic_src = None if bpr is None else f"ncu dram bytes {bpr} B/ray (profiles/r01d_README.md) x n_rays"
     res["roofline"] = {"bound": "alu", "achieved": ops / sec / 1e12, "peak": dfma_peak / 1e12, "unit": "Tlane-op/s (fp64)",
                        "frac": alu_frac, "traffic": traffic, "traffic_source": traffic_src, "kernel": "trace_kernel",
                        "ops_per_ray": ops / n_rays, "peak_source": "mcx_probe_dfma, measured in this run",
