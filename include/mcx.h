@@ -120,7 +120,8 @@ typedef struct mcx_solids_params {
 typedef struct mcx_voxels_params {
   double h;                 /* voxel edge; the component origin is the outer corner of voxel (0,0,0) */
   int64_t nx, ny, nz;
-  const uint8_t* ids;       /* DEVICE [nz][ny][nx], x fastest; values index the materials array.
+  const uint8_t* ids;       /* DEVICE [nz][ny][nx], x fastest; values index the materials array (a value >=
+                               n_materials is not a material and is traced as material 0, vacuum).
                                Read once by create (copied into the workspace in the traversal layout). */
 } mcx_voxels_params;
 

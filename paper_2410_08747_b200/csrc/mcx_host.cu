@@ -557,7 +557,7 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
           d.ids = (const uint8_t*)p0;
         }
         const cudaError_t e = launch_voxel_relayout(V.ids, (uint8_t*)d.ids, d.n[0], d.n[1], d.n[2], d.fast,
-                                                    d.a1, d.a2, d.pitch, d.run_dir, stream);
+                                                    d.a1, d.a2, d.pitch, d.run_dir, n_materials, stream);
         if (e != cudaSuccess) { const mcx_status s_ = cuda_fail(e, "voxel relayout"); delete H; return s_; }
         H->launches += 2;
         break;

@@ -1166,7 +1166,8 @@ __global__ void __launch_bounds__(256) tally_read_kernel(const TallyBin* __restr
 // (rows of `pitch` cells of 2 bytes: ID, run) with a guard border of kVoxelGuard around it.  Runs are filled in by
 // voxel_runs_kernel.
 __global__ void __launch_bounds__(256) voxel_relayout_kernel(const uint8_t* __restrict__ src, uint8_t* __restrict__ dst,
-                                                             int nx, int ny, int nz, int fast, int a1, int a2, int pitch) {
+                                                             int nx, int ny, int nz, int fast, int a1, int a2, int pitch,
+                                                             int n_mats) {
   const int n[3] = {nx, ny, nz};
   const long long total = (long long)(n[a2] + 2) * (n[a1] + 2) * pitch;
   const long long stride = (long long)gridDim.x * blockDim.x;
@@ -1179,6 +1180,7 @@ __global__ void __launch_bounds__(256) voxel_relayout_kernel(const uint8_t* __re
       int idx[3];
       idx[fast] = jf; idx[a1] = j1; idx[a2] = j2;
       v = src[((long long)idx[2] * ny + idx[1]) * nx + idx[0]];
+      if (v >= (unsigned)n_mats) v = 0u;  // not a material: vacuum (include/mcx.h)
     }
     reinterpret_cast<uint16_t*>(dst)[k] = (uint16_t)v;  // run = 0
   }
@@ -1307,10 +1309,10 @@ cudaError_t launch_tally_read(const TallyBin* bins, uint64_t n_bins, unsigned lo
 }
 
 cudaError_t launch_voxel_relayout(const uint8_t* src, uint8_t* dst, int nx, int ny, int nz, int fast, int a1, int a2,
-                                  int pitch, int run_dir, cudaStream_t stream) {
+                                  int pitch, int run_dir, int n_mats, cudaStream_t stream) {
   cudaError_t e = kernels_init();
   if (e != cudaSuccess) return e;
-  voxel_relayout_kernel<<<g_n_sm * 8, 256, 0, stream>>>(src, dst, nx, ny, nz, fast, a1, a2, pitch);
+  voxel_relayout_kernel<<<g_n_sm * 8, 256, 0, stream>>>(src, dst, nx, ny, nz, fast, a1, a2, pitch, n_mats);
   const int n[3] = {nx, ny, nz};
   const long long n_rows = (long long)(n[a2] + 2) * (n[a1] + 2);
   voxel_runs_kernel<<<(unsigned)((n_rows + 255) / 256), 256, 0, stream>>>(dst, n_rows, pitch, run_dir);

@@ -85,3 +85,26 @@ def test_long_runs_beyond_the_run_cap(M, O, W):
     ids = np.full((4, 4, 600), 2, dtype=np.uint8)
     ids[:, :, 300:310] = 1
     check(M, O, W, voxel_instrument(W, ids, 1.0e-3, np.eye(3), (0.0, 0.0, 1.0), target=0.02), 30_000)
+
+
+def test_ids_beyond_the_materials_are_vacuum(M, O, W):
+    """include/mcx.h: a voxel value >= n_materials is traced as material 0.  The GPU gets the raw volume, the oracle
+    the volume with those values replaced."""
+    rng = np.random.default_rng(15)
+    ids = blobs(rng, (32, 32, 32))
+    raw = ids.copy()
+    raw[4:9, 10:20, 3:30] = 200
+    raw[20:25, 5:9, 8:12] = 254
+    clean = np.where(raw >= 6, 0, raw).astype(np.uint8)       # blobs() uses IDs 0..5 -> 6 materials
+    inst_clean = voxel_instrument(W, clean, 4.0e-3, np.eye(3), (0.0, 0.0, 1.0))
+    assert len(inst_clean["materials"]) == 6
+    inst_raw = dict(inst_clean)                                # same source, tables and detector; only the volume differs
+    inst_raw["components"] = [dict(c) for c in inst_clean["components"]]
+    inst_raw["components"][1]["ids"] = np.ascontiguousarray(raw)
+    n = 30_000
+    o = O.trace(inst_clean, first=0, n=n, dump=True)
+    g = M.Instrument(inst_raw)
+    d = g.trace_dump(0, n)
+    g.close()
+    assert np.array_equal(d["fate"], o["dump"]["fate"]) and np.array_equal(d["bin"], o["dump"]["bin"])
+    assert np.allclose(d["p"], o["dump"]["p"], rtol=1e-9, atol=0)
