@@ -200,7 +200,9 @@ mcx_status mcx_trace_range(mcx_instrument* inst, uint64_t first_ray, uint64_t n_
  *                    direction draw (count, scan, scatter; 4 bytes of workspace per ray of a chunk), so that a warp
  *                    traces rays aimed at the same spot (coherent voxel / BVH / primitive walks);
  *   MCX_EXEC_AUTO    (default) SORTED where the source aims at a target rectangle and the instrument has a mesh, a
- *                    voxel volume or a group of two or more solids, DIRECT otherwise. */
+ *                    voxel volume or a group of two or more solids, DIRECT otherwise.
+ * In either order, a chain that starts with slits, mirrors or crystals is traced through those first and only the
+ * survivors, compacted warp by warp, through the whole chain (absorber gate); same results. */
 typedef enum { MCX_EXEC_AUTO = 0, MCX_EXEC_DIRECT = 1, MCX_EXEC_SORTED = 2 } mcx_exec_mode;
 mcx_status mcx_instrument_set_exec(mcx_instrument* inst, int mode);
 
