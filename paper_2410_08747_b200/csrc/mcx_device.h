@@ -152,6 +152,7 @@ struct TraceArgs {
   const uint32_t* order;   // detector-tile order of the chunk (launch_sort), or null
   mcx_ray_fate* dump;      // per-ray records indexed by ray offset, or null = tally
   unsigned int* ticket;    // [2] work-tile ticket and departure count, zero between launches
+  unsigned int* gate_known;  // the absorber gate an earlier launch on this instrument settled on, plus 1 (0 = not yet)
 };
 
 // sizes of the sort workspace

@@ -31,7 +31,7 @@ struct mcx_instrument {
   uint64_t launches = 0;
   // lane scheduling (row a13)
   int exec_mode = MCX_EXEC_AUTO;
-  size_t off_ticket = 0, off_sort_cnt = 0, off_sort_bsum = 0, off_order = 0;
+  size_t off_ticket = 0, off_gate = 0, off_sort_cnt = 0, off_sort_bsum = 0, off_order = 0;
   uint64_t chunk_rays = 0;  // capacity of the order buffer
 };
 
@@ -176,7 +176,7 @@ struct Plan {
   size_t off_counters = 0;
   size_t zero_begin = 0, zero_end = 0;
   size_t off_staging = 0;  // N, p, p2 of the largest detector, for mcx_tally_read_host
-  size_t off_ticket = 0, off_sort_cnt = 0, off_sort_bsum = 0, off_order = 0;
+  size_t off_ticket = 0, off_gate = 0, off_sort_cnt = 0, off_sort_bsum = 0, off_order = 0;
   size_t total = 0;
   // blob offsets
   size_t off_mat[MCX_MAX_MATERIALS];      // 4 arrays of n doubles each
@@ -305,6 +305,7 @@ mcx_status make_plan(const mcx_component* comps, int n_comps, const mcx_material
   P->off_counters = A.reserve((size_t)MCX_N_COUNTERS(n_comps) * sizeof(unsigned long long));
   P->off_ticket = A.reserve(2 * sizeof(unsigned int));
   P->zero_end = A.top;
+  P->off_gate = A.reserve(sizeof(unsigned int));  // zeroed by create only: survives mcx_tally_reset
   size_t max_bins = 0;
   for (int c = 0; c < n_comps; ++c)
     if (comps[c].kind == MCX_DETECTOR)
@@ -363,6 +364,7 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
   H->zero_end = P.zero_end;
   H->off_staging = P.off_staging;
   H->off_ticket = P.off_ticket;
+  H->off_gate = P.off_gate;
   H->off_sort_cnt = P.off_sort_cnt;
   H->off_sort_bsum = P.off_sort_bsum;
   H->off_order = P.off_order;
@@ -636,6 +638,7 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
   if (e == cudaSuccess && !H->blob.empty())
     e = cudaMemcpyAsync(ws + P.blob_begin, H->blob.data(), H->blob.size(), cudaMemcpyHostToDevice, stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(ws + P.zero_begin, 0, P.zero_end - P.zero_begin, stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(ws + P.off_gate, 0, sizeof(unsigned int), stream);
   if (e != cudaSuccess) { const mcx_status s_ = cuda_fail(e, "upload of the instrument image"); delete H; return s_; }
   H->upload_bytes = sizeof(DInstrument) + H->blob.size();
   *out = H;
@@ -670,6 +673,7 @@ mcx_status run_trace(mcx_instrument* H, uint64_t first, uint64_t n, uint64_t see
     A.order = nullptr;
     A.dump = dump ? dump + base : nullptr;
     A.ticket = (unsigned int*)(ws + H->off_ticket);
+    A.gate_known = (unsigned int*)(ws + H->off_gate);
     if (sorted && m >= kSortMinRays) {
       const int g = sort_bits(m, H->features);
       unsigned int* cnt = (unsigned int*)(ws + H->off_sort_cnt);

@@ -965,8 +965,10 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
   // (slot-addressed draws), cheap because the replayed part is the source and a few apertures.  Rays absorbed up to
   // the gate are accounted in the first pass, everything a queued ray does in the second (it is counted there whatever
   // happens to it), so every ray is counted once.  The block picks the gate itself from what its first tile (traced
-  // ungated) lost where: the first component after which at most 35 % of the rays are left, if there is one.
-  int gate = 0;
+  // ungated) lost where: the first component after which at most 35 % of the rays are left, if there is one; the
+  // choice is left in the workspace, and later launches on the instrument start with it.
+  const unsigned known_gate = GATE ? *A.gate_known : 0u;
+  int gate = known_gate ? (int)known_gate - 1 : 0;
   unsigned* ring = reinterpret_cast<unsigned*>(smem_raw + sizeof(DInstrument) + 128) + (threadIdx.x >> 5) * 64;
   unsigned ring_head = 0u, ring_n = 0u;  // warp-uniform
   // One warp-load of rays through components 1 .. (final_pass ? the end : the gate); see the loops below.
@@ -1113,7 +1115,7 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
       }
       if (last) break;
       __syncthreads();  // the tile is done and the next ticket is in place
-      if (GATE && it == 0u) {
+      if (GATE && it == 0u && known_gate == 0u) {
         if (threadIdx.x == 0) {
           const uint64_t left_in_range = n - tile_begin;
           const unsigned traced = left_in_range < tile ? (unsigned)left_in_range : tile;
@@ -1123,6 +1125,7 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
             if (100u * alive_after <= 35u * traced) pick = (unsigned)c;
           }
           s_sched[4] = pick;
+          *A.gate_known = pick + 1u;
         }
         __syncthreads();
         gate = (int)s_sched[4];
@@ -1236,7 +1239,7 @@ cudaError_t launch_one(const DInstrument* d_inst, int n_mats, const TraceArgs& A
   const uint64_t full = (uint64_t)n_sm * blocks_per_sm;  // one resident wave: a multiple of the SM count
   TraceArgs B = A;
   B.tile = kTileMax;  // at least ~4 tiles per resident block, so that the tail of the launch is short
-  while (B.tile > (unsigned)kBlock && A.n / B.tile < 4 * full) B.tile >>= 1;
+  while (B.tile > (unsigned)kBlock && A.n / B.tile < 2 * full) B.tile >>= 1;
   const uint64_t want = (A.n + B.tile - 1) / B.tile;
   const unsigned grid = (unsigned)(want < full ? (want ? want : 1) : full);
   trace_kernel<FEAT, DUMP, GATE><<<grid, kBlock, smem, stream>>>(d_inst, B);
