@@ -532,7 +532,7 @@ __device__ __forceinline__ unsigned long long frac64(double x) { return __double
 
 // Per-ray values the walk needs only where a run of equal IDs ends live in shared memory, not in registers
 // (cold_s, element k at cold_s[k * kBlock]): o and 1/d of the axes w, u, v, and the exit parameter t1.
-enum { VC_O = 0, VC_INVD = 1, VC_T1 = 6, VC_COUNT = 8 };
+enum { VC_O = 0, VC_INVD = 1, VC_T1 = 6, VC_WFACE = 7, VC_COUNT = 8 };
 
 // One axis of the walk at set-up time
 struct VoxAxis {
@@ -608,6 +608,8 @@ __device__ __forceinline__ void trace_voxels(const DInstrument& I, const DCompon
     cold_s[(VC_O + 2) * kBlock] = U.o; cold_s[(VC_INVD + 2) * kBlock] = 1.0 / U.d;
     cold_s[(VC_O + 4) * kBlock] = X.o; cold_s[(VC_INVD + 4) * kBlock] = 1.0 / X.d;
     cold_s[VC_T1 * kBlock] = t1;
+    // index of the first w face ahead and the walk's direction along w, as one 8-byte slot
+    cold_s[VC_WFACE * kBlock] = __hiloint2double(W.dir, W.idx + (W.dir > 0 ? 1 : 0));
     {  // skipping (see the loop below): only along the fast axis in the direction the runs were counted in
       const bool can_skip = W.slot == 0u && W.dir == V.run_dir;
       // inv <= 2^32 / (a_hi + 1): float quotient less a relative 1e-6 (its own error is 2^-22)
@@ -628,12 +630,20 @@ __device__ __forceinline__ void trace_voxels(const DInstrument& I, const DCompon
   // The run of `cur` ends where the ray enters the voxel at address `at` through a face of axis k: the index of that
   // voxel along the axis comes back out of the address (a guard cell gives -1 or n, i.e. the outer face of the grid),
   // and the face parameter is (face - o) / d as in step 11 (as a product with 1/d, one more rounding).
+  // (For w faces, most of them, the index is simply counted: w_crossed faces lie behind the current slab.)
+  unsigned w_crossed = 0u;
   auto close_run = [&](unsigned at, unsigned k, unsigned id) {
-    const unsigned off = (at - (unsigned)base) >> 1;  // cell index
-    const unsigned q2 = fast_div(off, V.mg_slab, V.sh_slab), r = off - q2 * V.slab;
-    const unsigned q1 = fast_div(r, V.mg_pitch, V.sh_pitch), q0 = r - q1 * (unsigned)V.pitch;
-    const unsigned slot = (meta >> (2u * k)) & 3u;
-    const int face = (int)(slot == 0u ? q0 : (slot == 1u ? q1 : q2)) - (int)((meta >> (6u + k)) & 1u);  // index - 1 + (dir > 0 ? 0 : 1)
+    int face;
+    if (k == 0u) {
+      const double wf = cold_s[VC_WFACE * kBlock];
+      face = __double2loint(wf) + __double2hiint(wf) * (int)w_crossed;
+    } else {
+      const unsigned off = (at - (unsigned)base) >> 1;  // cell index
+      const unsigned q2 = fast_div(off, V.mg_slab, V.sh_slab), r = off - q2 * V.slab;
+      const unsigned q1 = fast_div(r, V.mg_pitch, V.sh_pitch), q0 = r - q1 * (unsigned)V.pitch;
+      const unsigned slot = (meta >> (2u * k)) & 3u;
+      face = (int)(slot == 0u ? q0 : (slot == 1u ? q1 : q2)) - (int)((meta >> (6u + k)) & 1u);  // index - 1 + (dir > 0 ? 0 : 1)
+    }
     const double tf = ((double)face * h - cold_s[(VC_O + 2 * k) * kBlock]) * cold_s[(VC_INVD + 2 * k) * kBlock];
     const double tn = fmin(tf, cold_s[VC_T1 * kBlock]);
     const double prev = (touched >> cur) & 1u ? len_s[cur * kBlock] : 0.0;
@@ -689,6 +699,7 @@ __device__ __forceinline__ void trace_voxels(const DInstrument& I, const DCompon
     }
     const unsigned s = min(min(cell_c >> 8, __umulhi(~fuh, inv_u)), __umulhi(~fvh, inv_v));
     lo = lo_c + s * so_w;
+    w_crossed += s + 1u;
     {
       const unsigned long long tu = (unsigned long long)s * aul + ful, tv = (unsigned long long)s * avl + fvl;
       ful = (unsigned)tu; fuh += s * auh + (unsigned)(tu >> 32);
