@@ -74,7 +74,7 @@ struct DSolids {
 // along the fast axis in the beam's direction (run_dir) hold the same ID (capped at 255).  Cells are addressed as
 // ((i[a2]+1) * (n[a1]+2) + i[a1]+1) * pitch + i[fast]+1, with a one-cell guard border of ID kVoxelGuard all around.
 struct DVoxels {
-  double h;
+  double h, inv_h;
   int n[3];       // nx, ny, nz
   int fast;       // axis stored fastest in the traversal layout
   int a1, a2;     // the other two axes

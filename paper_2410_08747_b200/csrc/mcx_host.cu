@@ -545,6 +545,7 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
         if (!V.ids) MCX_BAIL(MCX_ERR_INVALID_ARG, "component %d: ids is null", c);
         DVoxels& d = D.u.voxels;
         d.h = V.h;
+        d.inv_h = 1.0 / V.h;
         d.n[0] = (int)V.nx; d.n[1] = (int)V.ny; d.n[2] = (int)V.nz;
         voxel_axes(components[0], C, &d.fast, &d.a1, &d.a2, &d.run_dir);
         d.pitch = voxel_pitch(d.n[d.fast]);

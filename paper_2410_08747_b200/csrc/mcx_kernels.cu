@@ -537,18 +537,20 @@ enum { VC_O = 0, VC_INVD = 1, VC_T1 = 6, VC_WFACE = 7, VC_COUNT = 8 };
 // One axis of the walk at set-up time
 struct VoxAxis {
   double o, d;      // ray origin and direction component in the volume frame
+  double inv_d;     // 1 / d (the walk's set-up divides once per axis and multiplies from there on)
   int idx;          // entry voxel index
   int dir;          // +1, -1, 0
   unsigned slot;    // 0, 1, 2: position of this axis in the traversal layout (fast, a1, a2)
   unsigned stride;  // address step (bytes) per voxel along this axis
 };
 
-__device__ __forceinline__ VoxAxis vox_axis(const DVoxels& V, Vec3 o, Vec3 d, int g, double t0) {
+__device__ __forceinline__ VoxAxis vox_axis(const DVoxels& V, Vec3 o, Vec3 d, Vec3 inv_d, int g, double t0) {
   VoxAxis A;
   A.o = pick(o, g);
   A.d = pick(d, g);
+  A.inv_d = pick(inv_d, g);
   const int n = V.n[g];
-  A.idx = min(n - 1, max(0, (int)floor((A.o + t0 * A.d) / V.h)));
+  A.idx = min(n - 1, max(0, (int)floor((A.o + t0 * A.d) * V.inv_h)));
   A.dir = A.d > 0.0 ? 1 : (A.d < 0.0 ? -1 : 0);
   A.slot = g == V.fast ? 0u : (g == V.a1 ? 1u : 2u);
   A.stride = 2u * (A.slot == 0u ? 1u : (A.slot == 1u ? (unsigned)V.pitch : V.slab));  // bytes, 2 per cell
@@ -558,14 +560,14 @@ __device__ __forceinline__ VoxAxis vox_axis(const DVoxels& V, Vec3 o, Vec3 d, in
 // Lateral coordinate at the first w face ahead (parameter t_w0), in voxels from the entry voxel's near face in the
 // direction of travel: in [0, 2); >= 1 means the lateral face is crossed within the first (partial) slab (c0 = 1).
 // f = its fraction, a = |d / d_w| <= 1 = advance per slab, both as 64-bit binary fractions.
-__device__ __forceinline__ void lateral_init(const VoxAxis& A, double d_w, double t_w0, double h, unsigned long long& f,
+__device__ __forceinline__ void lateral_init(const VoxAxis& A, double inv_dw, double t_w0, double inv_h, unsigned long long& f,
                                              unsigned long long& a, unsigned& c0) {
   double pos = 0.0, adv = 0.0;
   if (A.dir != 0) {
-    const double y = (A.o + t_w0 * A.d) / h;
+    const double y = (A.o + t_w0 * A.d) * inv_h;
     pos = A.dir > 0 ? y - (double)A.idx : (double)(A.idx + 1) - y;
     pos = fmin(fmax(pos, 0.0), 1.9999999999999998);
-    adv = fabs(A.d / d_w);
+    adv = fabs(A.d * inv_dw);
   }
   c0 = pos >= 1.0 ? 1u : 0u;
   f = frac64(pos - (double)c0);
@@ -580,10 +582,18 @@ __device__ __forceinline__ void trace_voxels(const DInstrument& I, const DCompon
   {
     const Vec3 ol = to_local(C.pose, ray.r);
     const Vec3 dl = rotate(C.pose.R, ray.d);
+    const Vec3 inv_d{1.0 / dl.x, 1.0 / dl.y, 1.0 / dl.z};  // the only divisions of the set-up (+-inf where d = 0: unused)
     double t0 = -CUDART_INF, t1 = CUDART_INF;
-    if (!clip_axis(ol.x, dl.x, 0.0, (double)V.n[0] * h, t0, t1)) return;
-    if (!clip_axis(ol.y, dl.y, 0.0, (double)V.n[1] * h, t0, t1)) return;
-    if (!clip_axis(ol.z, dl.z, 0.0, (double)V.n[2] * h, t0, t1)) return;
+    auto clip = [&](double o, double d, double inv, double top) {  // slab [0, top] of one axis, as clip_axis
+      if (d == 0.0) return o > 0.0 && o < top;
+      const double ta = -o * inv, tb = (top - o) * inv;
+      t0 = fmax(t0, fmin(ta, tb));
+      t1 = fmin(t1, fmax(ta, tb));
+      return true;
+    };
+    if (!clip(ol.x, dl.x, inv_d.x, (double)V.n[0] * h)) return;
+    if (!clip(ol.y, dl.y, inv_d.y, (double)V.n[1] * h)) return;
+    if (!clip(ol.z, dl.z, inv_d.z, (double)V.n[2] * h)) return;
     if (t0 < 0.0) t0 = 0.0;
     if (!(t0 < t1)) return;
     // the ray's dominant axis w and the two lateral axes u < v
@@ -594,19 +604,19 @@ __device__ __forceinline__ void trace_voxels(const DInstrument& I, const DCompon
       if (fabs(dl.z) > m) gw = 2;
     }
     const int gu = gw == 0 ? 1 : 0, gv = gw == 2 ? 1 : 2;
-    const VoxAxis W = vox_axis(V, ol, dl, gw, t0), U = vox_axis(V, ol, dl, gu, t0), X = vox_axis(V, ol, dl, gv, t0);
-    const double t_w0 = ((double)(W.idx + (W.dir > 0 ? 1 : 0)) * h - W.o) / W.d;  // first w face ahead
+    const VoxAxis W = vox_axis(V, ol, dl, inv_d, gw, t0), U = vox_axis(V, ol, dl, inv_d, gu, t0), X = vox_axis(V, ol, dl, inv_d, gv, t0);
+    const double t_w0 = ((double)(W.idx + (W.dir > 0 ? 1 : 0)) * h - W.o) * W.inv_d;  // first w face ahead
     unsigned long long fu, au, fv, av;
-    lateral_init(U, W.d, t_w0, h, fu, au, cu0);
-    lateral_init(X, W.d, t_w0, h, fv, av, cv0);
+    lateral_init(U, W.inv_d, t_w0, V.inv_h, fu, au, cu0);
+    lateral_init(X, W.inv_d, t_w0, V.inv_h, fv, av, cv0);
     ful = (unsigned)fu; fuh = (unsigned)(fu >> 32); aul = (unsigned)au; auh = (unsigned)(au >> 32);
     fvl = (unsigned)fv; fvh = (unsigned)(fv >> 32); avl = (unsigned)av; avh = (unsigned)(av >> 32);
     so_w = (unsigned)W.dir * W.stride; so_u = (unsigned)U.dir * U.stride; so_v = (unsigned)X.dir * X.stride;
     // axis k (0 = w, 1 = u, 2 = v): layout slot in bits 2k, 2k+1; "travels in the + direction" in bit 6 + k
     meta = W.slot | (U.slot << 2) | (X.slot << 4) | (W.dir > 0 ? 64u : 0u) | (U.dir > 0 ? 128u : 0u) | (X.dir > 0 ? 256u : 0u);
-    cold_s[(VC_O + 0) * kBlock] = W.o; cold_s[(VC_INVD + 0) * kBlock] = 1.0 / W.d;
-    cold_s[(VC_O + 2) * kBlock] = U.o; cold_s[(VC_INVD + 2) * kBlock] = 1.0 / U.d;
-    cold_s[(VC_O + 4) * kBlock] = X.o; cold_s[(VC_INVD + 4) * kBlock] = 1.0 / X.d;
+    cold_s[(VC_O + 0) * kBlock] = W.o; cold_s[(VC_INVD + 0) * kBlock] = W.inv_d;
+    cold_s[(VC_O + 2) * kBlock] = U.o; cold_s[(VC_INVD + 2) * kBlock] = U.inv_d;
+    cold_s[(VC_O + 4) * kBlock] = X.o; cold_s[(VC_INVD + 4) * kBlock] = X.inv_d;
     cold_s[VC_T1 * kBlock] = t1;
     // index of the first w face ahead and the walk's direction along w, as one 8-byte slot
     cold_s[VC_WFACE * kBlock] = __hiloint2double(W.dir, W.idx + (W.dir > 0 ? 1 : 0));
