@@ -100,6 +100,7 @@ struct DCrystal {
 
 struct DDetector {
   double xmin, xmax, ymin, ymax, emin, emax;
+  double sx, sy, se;  // bins per unit: nx / (xmax - xmin), ...
   int nx, ny, ne, index;
   uint64_t n_bins;
 };

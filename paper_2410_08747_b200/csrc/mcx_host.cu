@@ -605,6 +605,7 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
         DDetector& d = D.u.detector;
         d.xmin = T.xmin; d.xmax = T.xmax; d.ymin = T.ymin; d.ymax = T.ymax; d.emin = T.emin; d.emax = T.emax;
         d.nx = (int)T.nx; d.ny = (int)T.ny; d.ne = (int)T.ne; d.index = n_dets;
+        d.sx = (double)T.nx / (T.xmax - T.xmin); d.sy = (double)T.ny / (T.ymax - T.ymin); d.se = (double)T.ne / (T.emax - T.emin);
         d.n_bins = (uint64_t)T.nx * T.ny * T.ne;
         H->det_bins[n_dets] = d.n_bins;
         I.tallies[n_dets] = (TallyBin*)dev_ptr(P.off_tally[n_dets]);
