@@ -212,12 +212,21 @@ __device__ __forceinline__ bool clip_axis(double o, double d, double lo, double 
   return true;
 }
 
+// the same with 1/d supplied (one division per axis and solid instead of two; one more rounding per plane)
+__device__ __forceinline__ bool clip_axis_inv(double o, double d, double inv, double lo, double hi, double& tmin, double& tmax) {
+  if (d == 0.0) return o > lo && o < hi;
+  const double ta = (lo - o) * inv, tb = (hi - o) * inv;
+  tmin = fmax(tmin, fmin(ta, tb));
+  tmax = fmin(tmax, fmax(ta, tb));
+  return true;
+}
+
 __device__ __forceinline__ bool primitive_interval(const DSolid& S, Vec3 o, Vec3 d, double& tin, double& tout) {
   double tmin = -CUDART_INF, tmax = CUDART_INF;
   if (S.shape == MCX_BOX) {
-    if (!clip_axis(o.x, d.x, -S.dims[0], S.dims[0], tmin, tmax)) return false;
-    if (!clip_axis(o.y, d.y, -S.dims[1], S.dims[1], tmin, tmax)) return false;
-    if (!clip_axis(o.z, d.z, -S.dims[2], S.dims[2], tmin, tmax)) return false;
+    if (!clip_axis_inv(o.x, d.x, 1.0 / d.x, -S.dims[0], S.dims[0], tmin, tmax)) return false;
+    if (!clip_axis_inv(o.y, d.y, 1.0 / d.y, -S.dims[1], S.dims[1], tmin, tmax)) return false;
+    if (!clip_axis_inv(o.z, d.z, 1.0 / d.z, -S.dims[2], S.dims[2], tmin, tmax)) return false;
   } else if (S.shape == MCX_SPHERE) {
     const double b = dot(o, d);
     const double c = dot(o, o) - S.dims[0] * S.dims[0];
@@ -235,11 +244,11 @@ __device__ __forceinline__ bool primitive_interval(const DSolid& S, Vec3 o, Vec3
       const double b = o.x * d.x + o.z * d.z;
       const double disc = b * b - a * c;
       if (!(disc > 0.0)) return false;
-      const double s = sqrt(disc);
-      tmin = (-b - s) / a;
-      tmax = (-b + s) / a;
+      const double s = sqrt(disc), inv_a = 1.0 / a;
+      tmin = (-b - s) * inv_a;
+      tmax = (-b + s) * inv_a;
     }
-    if (!clip_axis(o.y, d.y, -S.dims[1], S.dims[1], tmin, tmax)) return false;
+    if (!clip_axis_inv(o.y, d.y, 1.0 / d.y, -S.dims[1], S.dims[1], tmin, tmax)) return false;
   }
   if (!(tmin < tmax)) return false;
   tin = tmin;
@@ -259,7 +268,7 @@ struct Shear {
 
 __device__ __forceinline__ double pick(Vec3 v, int k) { return k == 0 ? v.x : (k == 1 ? v.y : v.z); }
 
-__device__ __forceinline__ Shear make_shear(Vec3 d) {
+__device__ __forceinline__ Shear make_shear(Vec3 d, Vec3 inv_d) {
   Shear s;
   s.kz = 0;
   double m = fabs(d.x);
@@ -269,9 +278,11 @@ __device__ __forceinline__ Shear make_shear(Vec3 d) {
   s.ky = s.kx == 2 ? 0 : s.kx + 1;
   const double dz = pick(d, s.kz);
   if (dz < 0.0) { const int t = s.kx; s.kx = s.ky; s.ky = t; }
-  s.Sx = pick(d, s.kx) / dz;
-  s.Sy = pick(d, s.ky) / dz;
-  s.Sz = 1.0 / dz;
+  // the same constants serve every triangle of the ray, which is all watertightness needs; as products with 1/d_kz
+  // they are within an ulp of the quotients
+  s.Sz = pick(inv_d, s.kz);
+  s.Sx = pick(d, s.kx) * s.Sz;
+  s.Sy = pick(d, s.ky) * s.Sz;
   return s;
 }
 
@@ -345,23 +356,24 @@ __device__ __forceinline__ int mesh_endpoints(const DSolid& S, unsigned solid, V
                                               unsigned* __restrict__ queue) {
   // clip the line to the mesh box in fp64; the fp32 box walk uses a ray re-origined at the box entry so that
   // its rounding errors scale with the mesh size, not with the distance to the source
+  const Vec3 inv_d{1.0 / d.x, 1.0 / d.y, 1.0 / d.z};  // the only divisions of the set-up (+-inf where d = 0: unused)
   double tmin = -CUDART_INF, tmax = CUDART_INF;
-  if (!clip_axis(o.x, d.x, S.root_lo[0], S.root_hi[0], tmin, tmax)) return 1;
-  if (!clip_axis(o.y, d.y, S.root_lo[1], S.root_hi[1], tmin, tmax)) return 1;
-  if (!clip_axis(o.z, d.z, S.root_lo[2], S.root_hi[2], tmin, tmax)) return 1;
+  if (!clip_axis_inv(o.x, d.x, inv_d.x, S.root_lo[0], S.root_hi[0], tmin, tmax)) return 1;
+  if (!clip_axis_inv(o.y, d.y, inv_d.y, S.root_lo[1], S.root_hi[1], tmin, tmax)) return 1;
+  if (!clip_axis_inv(o.z, d.z, inv_d.z, S.root_lo[2], S.root_hi[2], tmin, tmax)) return 1;
   if (!(tmin < tmax)) return 1;
   const Vec3 e = o + tmin * d;
   const float ox = (float)e.x, oy = (float)e.y, oz = (float)e.z;
   // 1/d, held to +-1e30 so that the products below stay finite (a ray parallel to a pair of planes gets huge
   // parameters of the right signs instead of infinities)
   const float big = 1.0e30f;
-  const float ix = d.x != 0.0 ? fminf(fmaxf((float)(1.0 / d.x), -big), big) : big;
-  const float iy = d.y != 0.0 ? fminf(fmaxf((float)(1.0 / d.y), -big), big) : big;
-  const float iz = d.z != 0.0 ? fminf(fmaxf((float)(1.0 / d.z), -big), big) : big;
+  const float ix = d.x != 0.0 ? fminf(fmaxf((float)inv_d.x, -big), big) : big;
+  const float iy = d.y != 0.0 ? fminf(fmaxf((float)inv_d.y, -big), big) : big;
+  const float iz = d.z != 0.0 ? fminf(fmaxf((float)inv_d.z, -big), big) : big;
   // (x - o) / d as one fused multiply-add per plane: x * (1/d) + (-o/d).  Its rounding error is below 2^-22 of the
   // mesh scale times |1/d|, the boxes are padded by 2^-16 of the scale (times |1/d| in t): the test stays conservative.
   const float bx = -ox * ix, by = -oy * iy, bz = -oz * iz;
-  const Shear sh = make_shear(d);
+  const Shear sh = make_shear(d, inv_d);
   const int begin = ne, n_nodes = S.n_nodes;
   const float4* __restrict__ nodes = reinterpret_cast<const float4*>(S.nodes);
   const double* __restrict__ tris = S.tris;
