@@ -51,7 +51,7 @@ struct BvhNode {
   float hi[3];
   int tris;
 };
-enum { kBvhLeafMax = 2 };
+enum { kBvhLeafMax = 1 };
 
 struct DSolid {
   int shape, material, priority, n_nodes;  // n_nodes: BVH nodes of a mesh
