@@ -42,7 +42,7 @@ OPS_TRI_TEST, OPS_BVH_NODE = 45, 14
 NOMINAL_FP64_LANES_PER_SM, N_SM = 64, 148
 # DRAM bytes per ray of trace_kernel (dram__bytes_read.sum + dram__bytes_write.sum of one launch of 2^26 rays / 2^26) from
 # the ncu --set full captures summarised in profiles/r01d_README.md (c0, c2: whole run / n_rays; their tallies stay in L2).
-NCU_DRAM_BYTES_PER_RAY = {"c0_minimal": 0.001, "c1_polychromatic": 10.5, "c2_beamline": 0.01, "c3_mesh": 17.3, "c4_edxct": 29.0}
+NCU_DRAM_BYTES_PER_RAY = {"c0_minimal": 0.001, "c1_polychromatic": 10.5, "c2_beamline": 0.01, "c3_mesh": 17.3, "c4_edxct": 28.6}
 
 
 def reached_per_component(n_rays, absorbed):
