@@ -1,8 +1,8 @@
 // mcx_kernels.cu -- the ray-tracing megakernel and its helper kernels, hand-written for sm_100a.
 //
 // One thread traces one ray at a time through the whole component chain with its state (r, d, E, p) in fp64
-// registers; a grid of 148 x k blocks strides over the ray-index range.  Step numbers are
-// those of DESIGN.md "Readings".  This file shares no code with oracle/.
+// registers; a grid of 148 x k resident blocks pulls tiles of ray positions from a ticket counter.
+// Step numbers are those of DESIGN.md "Readings".  This file shares no code with oracle/.
 #include <math_constants.h>
 
 #include "mcx_device.h"
@@ -921,8 +921,10 @@ __global__ void __launch_bounds__(256) sort_scatter_kernel(uint64_t first, uint3
 
 // ------------------------------------------------------------------------------------------------------------
 // The megakernel.  FEAT selects which component kinds are compiled in; DUMP writes per-ray fates instead of
-// tallying.  Shared memory: the instrument image, per-block ray-accounting counters, the solids of every group,
-// per-thread mu[] for the voxel walk.  Spectrum CDFs and mu(E) tables are read through L1.
+// tallying; GATE compiles in the absorber gate.  Shared memory: the instrument image, per-block ray-accounting and
+// scheduling counters, (GATE) per-warp rings of survivors, the solids of every group, per-thread interval end
+// points and candidate-triangle queue, per-thread path lengths per material and run-end scratch of the voxel walk.
+// Spectrum CDFs, guide tables and mu(E) tables are read through L1.
 // ------------------------------------------------------------------------------------------------------------
 constexpr size_t kRingBytes = (kBlock / 32) * 64 * sizeof(unsigned);  // per-warp rings of gate survivors
 constexpr unsigned kTileMax = 8192;  // positions per work ticket (a power of two >= kBlock; smaller for short launches)
