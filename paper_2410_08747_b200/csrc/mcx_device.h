@@ -41,26 +41,27 @@ struct DSlit {
   double half_x, half_y, radius2;
 };
 
-// BVH2 node, 32 bytes, stored in depth-first preorder: the left child of an inner node is the next node, and
-// `escape` is the node to go to when this node's subtree is done or its box is missed (n_nodes = end of the walk), so
-// the walk needs no stack.  Boxes are fp32, rounded outward and padded; they only select candidate triangles, the
-// exact fp64 triangle test decides.  Leaf: tris = first_triangle * 8 + count (count 1..kBvhLeafMax); inner: tris = 0.
+// BVH2 node, 32 bytes.  The tree over a mesh is a COMPLETE binary tree of depth D = ceil(log2(n_triangles)), stored in
+// heap order with node i at slot i + 1 (children 2i+1, 2i+2 share one 64-byte line), leaves all at level D, leaf
+// number p = i - (2^D - 1) holding triangle slot p (slots without a triangle, and subtrees without one, have count 0
+// and are never entered).  Nothing needs a pointer: the walk keeps (i, level) and one bit per level for "the right
+// sibling is still to be visited", so it needs no stack either.  Boxes are fp32, rounded outward and padded; they only
+// select candidate triangles, the exact fp64 triangle test decides.
 struct BvhNode {
   float lo[3];
-  int escape;
+  int count;   // triangles below this node
   float hi[3];
-  int tris;
+  int unused;
 };
-enum { kBvhLeafMax = 1 };
 
 struct DSolid {
-  int shape, material, priority, n_nodes;  // n_nodes: BVH nodes of a mesh
+  int shape, material, priority, depth;  // depth: D of a mesh's BVH
   DPose pose;
   double dims[3];
   double bound2;                  // primitives: (radius of the bounding sphere about the solid's origin, plus 1e-9)^2
   double root_lo[3], root_hi[3];  // fp64 AABB of the mesh (solid-local)
   const BvhNode* nodes;
-  const double* tris;  // [n_tris][9] vertices in BVH leaf order
+  const double* tris;  // [2^D][9] vertices by leaf number (zeros where a leaf holds no triangle)
 };
 
 // The solids of a group are stored in ascending order of precedence (priority, then earlier-listed first among

@@ -77,10 +77,10 @@ void copy_pose(DPose* d, const mcx_pose& s) {
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// BVH over one mesh: top-down, median split of the triangle centroids along the widest axis, <= kBvhLeafMax
-// triangles per leaf, nodes emitted in depth-first preorder with escape links (BvhNode).  Node boxes are stored in
-// fp32 rounded outward and padded by 2^-16 of the mesh scale, far above the fp32 rounding of the box walk (<= a few
-// 2^-24 of the scale), so the walk never loses a triangle the exact fp64 test would hit.
+// BVH over one mesh: a complete binary tree in heap order (BvhNode), built top-down by splitting the triangles of a
+// node at the median of their centroids along the widest axis, the left child taking the larger half.  Node boxes
+// are stored in fp32 rounded outward and padded by 2^-16 of the mesh scale, far above the fp32 rounding of the box
+// walk (<= a few 2^-24 of the scale), so the walk never loses a triangle the exact fp64 test would hit.
 // ---------------------------------------------------------------------------------------------------------
 struct TriRef {
   double c[3], lo[3], hi[3];
@@ -98,14 +98,24 @@ float round_up(double x) {
   return f;
 }
 
+int bvh_depth(int64_t n_tris) {
+  int d = 0;
+  while (((int64_t)1 << d) < n_tris) ++d;
+  return d;
+}
+size_t bvh_node_bound(int64_t n_tris) { return (size_t)2 << bvh_depth(n_tris); }  // slots: node i at slot i + 1
+size_t bvh_leaf_count(int64_t n_tris) { return (size_t)1 << bvh_depth(n_tris); }
+
 struct BvhBuilder {
   std::vector<TriRef>& refs;
-  std::vector<BvhNode>& nodes;
+  std::vector<BvhNode>& slots;  // zero-initialised: count 0 everywhere
+  std::vector<int>& leaf_tri;   // triangle (index into the caller's array) of every leaf, -1 = none
   double pad;
-  // builds the subtree over refs[begin, end) at the end of `nodes`; escape links are set by link() afterwards
-  void build(int begin, int end) {
-    const int node = (int)nodes.size();
-    nodes.push_back(BvhNode{});
+  int depth;
+  void build(int64_t i, int begin, int end, int level) {
+    const int count = end - begin;
+    if (count == 0) return;
+    BvhNode& N = slots[(size_t)i + 1];
     double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
     double clo[3] = {1e300, 1e300, 1e300}, chi[3] = {-1e300, -1e300, -1e300};
     for (int k = begin; k < end; ++k)
@@ -114,33 +124,25 @@ struct BvhBuilder {
         clo[a] = std::min(clo[a], refs[k].c[a]); chi[a] = std::max(chi[a], refs[k].c[a]);
       }
     for (int a = 0; a < 3; ++a) {
-      nodes[node].lo[a] = round_down(lo[a] - pad);
-      nodes[node].hi[a] = round_up(hi[a] + pad);
+      N.lo[a] = round_down(lo[a] - pad);
+      N.hi[a] = round_up(hi[a] + pad);
     }
-    const int count = end - begin;
-    if (count <= kBvhLeafMax) {
-      nodes[node].tris = begin * 8 + count;
+    N.count = count;
+    if (level == depth) {  // count == 1: 2^(depth - level) bounds the triangles of a node
+      leaf_tri[(size_t)(i - (((int64_t)1 << depth) - 1))] = refs[begin].idx;
       return;
     }
     int axis = 0;
     if (chi[1] - clo[1] > chi[axis] - clo[axis]) axis = 1;
     if (chi[2] - clo[2] > chi[axis] - clo[axis]) axis = 2;
-    const int mid = begin + count / 2;
-    std::nth_element(refs.begin() + begin, refs.begin() + mid, refs.begin() + end,
-                     [axis](const TriRef& x, const TriRef& y) { return x.c[axis] < y.c[axis]; });
-    nodes[node].tris = 0;
-    build(begin, mid);  // left child = node + 1
-    build(mid, end);
-  }
-  // escape(node) = the first node after its subtree in preorder; returns it
-  int link(int node) {
-    if (nodes[node].tris != 0) return nodes[node].escape = node + 1;
-    const int right = link(node + 1);
-    return nodes[node].escape = link(right);
+    const int mid = begin + (count + 1) / 2;
+    if (mid < end)
+      std::nth_element(refs.begin() + begin, refs.begin() + mid, refs.begin() + end,
+                       [axis](const TriRef& x, const TriRef& y) { return x.c[axis] < y.c[axis]; });
+    build(2 * i + 1, begin, mid, level + 1);
+    build(2 * i + 2, mid, end, level + 1);
   }
 };
-
-size_t bvh_node_bound(int64_t n_tris) { return (size_t)(2 * n_tris + 2); }
 
 // Rays per sorted chunk.  The more rays a chunk holds the closer together the 32 rays of a warp land (the bucket grid
 // is capped at 2^10 x 2^10 cells, so past 2^24 rays the buckets only get fuller and a warp spans less of one): c4
@@ -263,7 +265,7 @@ mcx_status make_plan(const mcx_component* comps, int n_comps, const mcx_material
           if (G.solids[s].shape == MCX_MESH) {
             if (G.solids[s].n_triangles < 1 || G.solids[s].n_vertices < 3) return fail(MCX_ERR_INVALID_ARG, "component %d solid %d: empty mesh", c, (int)s);
             P->off_nodes[c][s] = A.reserve(bvh_node_bound(G.solids[s].n_triangles) * sizeof(BvhNode));
-            P->off_tris[c][s] = A.reserve((size_t)G.solids[s].n_triangles * 9 * sizeof(double));
+            P->off_tris[c][s] = A.reserve(bvh_leaf_count(G.solids[s].n_triangles) * 9 * sizeof(double));
           }
         break;
       }
@@ -519,21 +521,20 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
           double scale = 0.0;
           for (int a = 0; a < 3; ++a) scale = std::max(scale, std::max(std::fabs(lo[a]), std::fabs(hi[a])));
           const double pad = scale * (1.0 / 65536.0);
-          std::vector<BvhNode> nodes;
-          nodes.reserve(bvh_node_bound(nt));
-          BvhBuilder B{refs, nodes, pad};
-          B.build(0, nt);
-          B.link(0);
-          if (nodes.size() > bvh_node_bound(nt)) MCX_BAIL(MCX_ERR_UNSUPPORTED, "BVH node bound exceeded");
           if ((size_t)nt >= ((size_t)1 << 27)) MCX_BAIL(MCX_ERR_UNSUPPORTED, "component %d solid %d: more than 2^27 triangles", c, (int)s);
-          std::memcpy(host_ptr(P.off_nodes[c][s]), nodes.data(), nodes.size() * sizeof(BvhNode));
-          double* tri = (double*)host_ptr(P.off_tris[c][s]);
-          for (int t = 0; t < nt; ++t)
-            for (int v = 0; v < 3; ++v)
-              for (int a = 0; a < 3; ++a)
-                tri[9 * (size_t)t + 3 * v + a] = S.vertices[3 * (size_t)S.triangles[3 * (size_t)refs[t].idx + v] + a];
+          std::vector<BvhNode> slots(bvh_node_bound(nt), BvhNode{});
+          std::vector<int> leaf_tri(bvh_leaf_count(nt), -1);
+          BvhBuilder B{refs, slots, leaf_tri, pad, bvh_depth(nt)};
+          B.build(0, 0, nt, 0);
+          std::memcpy(host_ptr(P.off_nodes[c][s]), slots.data(), slots.size() * sizeof(BvhNode));
+          double* tri = (double*)host_ptr(P.off_tris[c][s]);  // zero-filled blob: leaves without a triangle stay zero
+          for (size_t leaf = 0; leaf < leaf_tri.size(); ++leaf)
+            if (leaf_tri[leaf] >= 0)
+              for (int v = 0; v < 3; ++v)
+                for (int a = 0; a < 3; ++a)
+                  tri[9 * leaf + 3 * v + a] = S.vertices[3 * (size_t)S.triangles[3 * (size_t)leaf_tri[leaf] + v] + a];
           for (int a = 0; a < 3; ++a) { d.root_lo[a] = lo[a] - pad; d.root_hi[a] = hi[a] + pad; }
-          d.n_nodes = (int)nodes.size();
+          d.depth = bvh_depth(nt);
           d.nodes = (const BvhNode*)dev_ptr(P.off_nodes[c][s]);
           d.tris = (const double*)dev_ptr(P.off_tris[c][s]);
         }

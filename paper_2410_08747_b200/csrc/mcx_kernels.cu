@@ -374,36 +374,60 @@ __device__ __forceinline__ int mesh_endpoints(const DSolid& S, unsigned solid, V
   // mesh scale times |1/d|, the boxes are padded by 2^-16 of the scale (times |1/d| in t): the test stays conservative.
   const float bx = -ox * ix, by = -oy * iy, bz = -oz * iz;
   const Shear sh = make_shear(d, inv_d);
-  const int begin = ne, n_nodes = S.n_nodes;
+  const int begin = ne, depth = S.depth, leaf_base = (1 << depth) - 1;
   const float4* __restrict__ nodes = reinterpret_cast<const float4*>(S.nodes);
   const double* __restrict__ tris = S.tris;
   bool overflow = false;
-  int node = 0;
+  // Walk of the complete tree (BvhNode): at node i of `level`, already known to be hit, both children are tested at
+  // once (one 64-byte line); bit `level` of `trail` says the right child was hit too and waits while the left
+  // subtree is walked.  Going back up needs no memory: the ancestor of i at level m is ((i + 1) >> (level - m)) - 1.
+  int i = 0, level = 0;
+  unsigned trail = 0u;
+  bool walking = true;
+  auto next_pending = [&]() {  // to the deepest right sibling still to be visited, or done
+    if (trail == 0u) { walking = false; return; }
+    const int l = 31 - __clz(trail);
+    trail ^= 1u << l;
+    i = ((i + 1) >> (level - (l + 1)));  // = (left child at level l + 1) + 1 = its right sibling
+    level = l + 1;
+  };
   do {
     int nq = 0;
-    while (node < n_nodes && nq <= kTriQueue - kBvhLeafMax) {
-      const float4 a = __ldg(nodes + 2 * node), b = __ldg(nodes + 2 * node + 1);  // lo.xyz, escape | hi.xyz, tris
-      // slab test of the full line against the padded fp32 box (no t range: the line is tested, as in step 9)
-      const float tx0 = fmaf(a.x, ix, bx), tx1 = fmaf(b.x, ix, bx);
-      const float ty0 = fmaf(a.y, iy, by), ty1 = fmaf(b.y, iy, by);
-      const float tz0 = fmaf(a.z, iz, bz), tz1 = fmaf(b.z, iz, bz);
-      const float tn = fmaxf(fmaxf(fminf(tx0, tx1), fminf(ty0, ty1)), fminf(tz0, tz1));
-      const float tf = fminf(fminf(fmaxf(tx0, tx1), fmaxf(ty0, ty1)), fmaxf(tz0, tz1));
-      const bool hit = tn <= tf;
-      const int leaf = __float_as_int(b.w);
-      if (hit && leaf != 0) {
-        queue[nq * kBlock] = (unsigned)(leaf >> 3);
+    while (walking && nq < kTriQueue) {
+      if (level == depth) {  // a leaf whose box the line hits: queue its triangle
+        queue[nq * kBlock] = (unsigned)(i - leaf_base);
         ++nq;
-        if ((leaf & 7) > 1) { queue[nq * kBlock] = (unsigned)(leaf >> 3) + 1u; ++nq; }
+        next_pending();
+        continue;
       }
-      node = (hit && leaf == 0) ? node + 1 : __float_as_int(a.w);
+      const float4* pair = nodes + 2 * (2 * i + 2);  // children 2i+1, 2i+2 sit in slots 2i+2, 2i+3
+      const float4 a0 = __ldg(pair), b0 = __ldg(pair + 1), a1 = __ldg(pair + 2), b1 = __ldg(pair + 3);
+      // slab tests of the full line against the padded fp32 boxes (no t range: the line is tested, as in step 9)
+      const float x00 = fmaf(a0.x, ix, bx), x01 = fmaf(b0.x, ix, bx), x10 = fmaf(a1.x, ix, bx), x11 = fmaf(b1.x, ix, bx);
+      const float y00 = fmaf(a0.y, iy, by), y01 = fmaf(b0.y, iy, by), y10 = fmaf(a1.y, iy, by), y11 = fmaf(b1.y, iy, by);
+      const float z00 = fmaf(a0.z, iz, bz), z01 = fmaf(b0.z, iz, bz), z10 = fmaf(a1.z, iz, bz), z11 = fmaf(b1.z, iz, bz);
+      const float n0 = fmaxf(fmaxf(fminf(x00, x01), fminf(y00, y01)), fminf(z00, z01));
+      const float f0 = fminf(fminf(fmaxf(x00, x01), fmaxf(y00, y01)), fmaxf(z00, z01));
+      const float n1 = fmaxf(fmaxf(fminf(x10, x11), fminf(y10, y11)), fminf(z10, z11));
+      const float f1 = fminf(fminf(fmaxf(x10, x11), fmaxf(y10, y11)), fmaxf(z10, z11));
+      const bool hit0 = n0 <= f0 && __float_as_int(a0.w) != 0, hit1 = n1 <= f1 && __float_as_int(a1.w) != 0;
+      if (hit0) {
+        if (hit1) trail |= 1u << level;
+        i = 2 * i + 1;
+        ++level;
+      } else if (hit1) {
+        i = 2 * i + 2;
+        ++level;
+      } else {
+        next_pending();
+      }
     }
     for (int k = 0; k < nq; ++k) {
       double t;
       const int r = ray_triangle(sh, o, tris + 9 * (size_t)queue[k * kBlock], t);
       if (r != 0 && !ep_push(E, ne, t, solid | (r < 0 ? kTagExit : 0u))) overflow = true;
     }
-  } while (node < n_nodes);
+  } while (walking);
   if (overflow) return -1;
   if (ne == begin) return 1;
   ep_sort(E, begin, ne, true);
