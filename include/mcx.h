@@ -242,6 +242,12 @@ uint64_t mcx_launch_count(const mcx_instrument* inst);
  * Lane-ops performed = n_blocks * 256 * n_iters * 8. */
 mcx_status mcx_probe_dfma(double* sink, int n_blocks, int64_t n_iters, void* cuda_stream);
 
+/* Tally-reduction probe for the atomics roofline ("measure random red.add.f64 rate"): every thread of a
+ * (n_blocks x 256) grid does n_iters rounds of the three reductions of a detected ray (u64 count, two fp64 sums)
+ * into one pseudo-random 32-byte record of `table` (DEVICE, n_records * 32 bytes, n_records a power of two; contents
+ * are garbage afterwards).  Records updated = n_blocks * 256 * n_iters. */
+mcx_status mcx_probe_tally(void* table, uint64_t n_records, int n_blocks, int64_t n_iters, void* cuda_stream);
+
 void mcx_instrument_destroy(mcx_instrument* inst);
 
 const char* mcx_last_error(void);

@@ -25,7 +25,7 @@ EXEC_MODE = {"auto": 0, "direct": 1, "sorted": 2}
 FATE_DETECTED, FATE_MISSED, FATE_DEGENERATE = -1, -2, -3
 
 EXPORTS = ["mcx_instrument_workspace_size", "mcx_instrument_create", "mcx_trace", "mcx_trace_range", "mcx_tally_read",
-           "mcx_tally_read_host", "mcx_instrument_set_exec", "mcx_upload_bytes", "mcx_tally_reset", "mcx_counters_read", "mcx_trace_dump", "mcx_launch_count", "mcx_probe_dfma",
+           "mcx_tally_read_host", "mcx_instrument_set_exec", "mcx_upload_bytes", "mcx_tally_reset", "mcx_counters_read", "mcx_trace_dump", "mcx_launch_count", "mcx_probe_dfma", "mcx_probe_tally",
            "mcx_instrument_destroy", "mcx_last_error"]
 
 _dp = C.POINTER(C.c_double)
@@ -124,11 +124,12 @@ def lib(strict=False):
     L.mcx_launch_count.argtypes = [vp]
     L.mcx_launch_count.restype = C.c_uint64
     L.mcx_probe_dfma.argtypes = [vp, C.c_int, C.c_int64, vp]
+    L.mcx_probe_tally.argtypes = [vp, C.c_uint64, C.c_int, C.c_int64, vp]
     L.mcx_instrument_destroy.argtypes = [vp]
     L.mcx_instrument_destroy.restype = None
     L.mcx_last_error.restype = C.c_char_p
     for name in ("mcx_instrument_workspace_size", "mcx_instrument_create", "mcx_trace", "mcx_trace_range",
-                 "mcx_tally_read", "mcx_tally_read_host", "mcx_tally_reset", "mcx_counters_read", "mcx_trace_dump", "mcx_probe_dfma"):
+                 "mcx_tally_read", "mcx_tally_read_host", "mcx_tally_reset", "mcx_counters_read", "mcx_trace_dump", "mcx_probe_dfma", "mcx_probe_tally"):
         getattr(L, name).restype = C.c_int
     _libs[strict] = L
     return L
@@ -347,6 +348,23 @@ class Instrument:
             self.close()
         except Exception:
             pass
+
+
+def probe_tally(n_records, n_blocks, n_iters, device="cuda:0"):
+    """mcx_probe_tally: returns tally records updated per second (3 reductions each) into a table of n_records x 32 B."""
+    import torch
+    dev = torch.device(device)
+    with torch.cuda.device(dev):
+        table = torch.zeros(n_records * 4, dtype=torch.int64, device=dev)
+        st = C.c_void_p(torch.cuda.current_stream(dev).cuda_stream)
+        _check(lib().mcx_probe_tally(table.data_ptr(), n_records, n_blocks, max(1, n_iters // 4), st))
+        torch.cuda.synchronize(dev)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        _check(lib().mcx_probe_tally(table.data_ptr(), n_records, n_blocks, n_iters, st))
+        e1.record()
+        torch.cuda.synchronize(dev)
+        return n_blocks * 256 * n_iters / (e0.elapsed_time(e1) * 1e-3)
 
 
 def probe_dfma(n_blocks, n_iters, device="cuda:0"):

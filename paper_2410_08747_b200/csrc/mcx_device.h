@@ -169,6 +169,7 @@ cudaError_t launch_tally_read(const TallyBin* bins, uint64_t n_bins, unsigned lo
 cudaError_t launch_voxel_relayout(const uint8_t* src, uint8_t* dst, int nx, int ny, int nz, int fast, int a1, int a2,
                                   int pitch, int run_dir, int n_mats, cudaStream_t stream);
 cudaError_t launch_probe_dfma(double* sink, int n_blocks, long long n_iters, cudaStream_t stream);
+cudaError_t launch_probe_tally(void* table, unsigned long long n_records, int n_blocks, long long n_iters, cudaStream_t stream);
 cudaError_t kernels_init();
 
 }  // namespace mcx

@@ -789,6 +789,14 @@ mcx_status mcx_probe_dfma(double* sink, int n_blocks, int64_t n_iters, void* cud
   return MCX_OK;
 }
 
+mcx_status mcx_probe_tally(void* table, uint64_t n_records, int n_blocks, int64_t n_iters, void* cuda_stream) {
+  if (!table || n_records == 0 || (n_records & (n_records - 1)) != 0 || n_blocks < 1 || n_iters < 0)
+    return fail(MCX_ERR_INVALID_ARG, "bad probe arguments (n_records must be a power of two)");
+  const cudaError_t e = launch_probe_tally(table, n_records, n_blocks, (long long)n_iters, (cudaStream_t)cuda_stream);
+  if (e != cudaSuccess) return cuda_fail(e, "probe launch");
+  return MCX_OK;
+}
+
 void mcx_instrument_destroy(mcx_instrument* inst) { delete inst; }
 
 }  // extern "C"

@@ -1383,6 +1383,24 @@ cudaError_t launch_voxel_relayout(const uint8_t* src, uint8_t* dst, int nx, int 
   return cudaGetLastError();
 }
 
+// Tally probe for the atomics roofline: every thread does n_iters rounds of the three reductions of step 14 (u64 count,
+// two fp64 sums) into one pseudo-random 32-byte record of a table of n_records (a power of two).
+__global__ void __launch_bounds__(256) probe_tally_kernel(TallyBin* table, unsigned long long mask, long long n_iters) {
+  unsigned long long x = ((unsigned long long)blockIdx.x * blockDim.x + threadIdx.x) * 0x9E3779B97F4A7C15ull + 0x2545F4914F6CDD1Dull;
+  for (long long k = 0; k < n_iters; ++k) {
+    x ^= x >> 12; x ^= x << 25; x ^= x >> 27;  // xorshift64*
+    TallyBin* rec = table + ((x * 0x2545F4914F6CDD1Dull) >> 20 & mask);
+    atomicAdd(&rec->N, 1ull);
+    atomicAdd(&rec->P, 0.5);
+    atomicAdd(&rec->P2, 0.25);
+  }
+}
+
+cudaError_t launch_probe_tally(void* table, unsigned long long n_records, int n_blocks, long long n_iters, cudaStream_t stream) {
+  probe_tally_kernel<<<n_blocks, 256, 0, stream>>>(reinterpret_cast<TallyBin*>(table), n_records - 1, n_iters);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_probe_dfma(double* sink, int n_blocks, long long n_iters, cudaStream_t stream) {
   probe_dfma_kernel<<<n_blocks, 256, 0, stream>>>(sink, n_iters);
   return cudaGetLastError();
