@@ -259,8 +259,18 @@ def bench_instrument(M, torch, inst, n_rays, first, steps, warmup, device, dfma_
                                "bytes_per_ray": byt / n_rays,
                                "peak_source": "MEASURED_PEAKS.json" if peaks else "fallback 6650 GB/s"}}
     if with_e2e:
+        # the second candidate roofline: random tally-record updates at this detector's footprint
+        n_rec = 1 << (int(nb).bit_length() - 1)
+        g.close()
+        g = None
+        torch.cuda.empty_cache()
+        tally_peak = max(M.probe_tally(n_rec, N_SM * 8, 128, device=str(device)) for _ in range(2))
+        det_rate = res["detected_fraction"] * n_rays / sec
+        res["roofline"]["tally"] = {"achieved": det_rate, "peak": tally_peak, "unit": "records/s", "frac": det_rate / tally_peak,
+                                    "peak_source": f"mcx_probe_tally, {n_rec} random 32-byte records, measured in this run"}
         res["e2e"] = bench_e2e(M, torch, inst, n_rays, first, max(2, min(steps, 3)), device)
-    g.close()
+    if g is not None:
+        g.close()
     del flush, out
     torch.cuda.empty_cache()
     return res
