@@ -16,9 +16,12 @@
 //
 // Pins (tests/test_oracle_*.py, -m "not gpu"): Philox known answers, u01 end points, slab exp(-mu L),
 // slit acceptance 0.16, weight conservation, ray accounting, power-law mu(E), sphere/box/cylinder chords,
-// cube-mesh == box, icosphere vs analytic sphere, grid accelerator == brute force, voxel closed forms and
-// the paper's fixed-step marching as a convergence cross-check, ellipse focal property,
-// bilinear exactness, Darwin closed forms, detector binning.
+// cube-mesh == box (random rays, and rays exactly through face diagonals, edges and vertices: duplicate-hit
+// collapse; rays grazing an edge or vertex: enter-before-exit tie order; open and inward-wound meshes: the
+// DEGENERATE return), icosphere vs analytic sphere (levels 5 and 6), grid accelerator == brute force, no degenerate
+// ray in 1e6 through closed meshes, voxel closed forms and the paper's fixed-step marching as a
+// convergence cross-check, ellipse focal property, bilinear exactness, Darwin closed forms, detector binning, the
+// fate rule of chains with several monitors against plane geometry written out in numpy.
 // Whole-config tallies of c1..c4 have no closed form: "parity unpinned" beyond those part-wise pins
 // (SURVEY.md 8(c) last row).
 #include <algorithm>

@@ -117,3 +117,50 @@ def test_slits(O, W):
     # the slit does not change the ray
     rc, st, _ = O.apply(s, [0.1e-3, 0.2e-3, 0, 0, 0, 1, 20, 0.7])
     assert rc == 1 and np.array_equal(st, [0.1e-3, 0.2e-3, 0, 0, 0, 1, 20, 0.7])
+
+
+def test_fate_with_several_detectors_is_what_the_last_component_said(O, W):
+    """DESIGN.md section 2, step 14 (a reading; the paper only says monitors measure "at given points"):
+    a monitor never ends a ray, every monitor the ray crosses tallies it, and the ray's FATE is decided by where the
+    chain ends for it -- absorbed at component c, else DETECTED / MISSED by the LAST component of the chain (MISSED if
+    that is not a detector).  Pinned against plain plane geometry written out here in numpy."""
+    src = W.source("point", "target", "mono", target_w=20e-3, target_h=20e-3, target_dist=1.0, E0=20.0)
+    detA = W.detector(-3e-3, 3e-3, -3e-3, 3e-3, 6, 6, 0.0, 40.0, 1, T=(0, 0, 0.4))
+    slit = W.slit_rect(8e-3, 8e-3, T=(0, 0, 0.6))
+    detB = W.detector(-5e-3, 5e-3, -5e-3, 5e-3, 10, 10, 0.0, 40.0, 1, T=(0, 0, 1.0))
+    n = 6000
+    inst = W.instrument("two_monitors", [src, detA, slit, detB], [None], n)
+    r = O.trace(inst, dump=True)
+    rays = np.array([O.source_ray(src, inst["seed"], i) for i in range(n)])
+    at = lambda z: rays[:, 3:5] / rays[:, 5:6] * z                     # (x, y) where the line meets the plane z
+    a, s, b = at(0.4), at(0.6), at(1.0)
+    inA = np.all((a >= -3e-3) & (a < 3e-3), axis=1)
+    passes = np.all(np.abs(s) <= 4e-3, axis=1)
+    inB = np.all((b >= -5e-3) & (b < 5e-3), axis=1)
+    expect = np.where(~passes, 2, np.where(inB, O.F_DETECTED, O.F_MISSED))
+    assert np.array_equal(r["dump"]["fate"], expect)
+    assert (inA & ~passes).sum() > 100 and (inA & passes & inB).sum() > 100 and (~passes).sum() > 100 and (passes & ~inB).sum() > 100
+    # both monitors tally every ray that crosses them, whatever happens to it afterwards
+    assert int(r["N"][0].sum()) == inA.sum() and int(r["N"][1].sum()) == (passes & inB).sum() == r["detected"]
+    binB = (np.floor((b[:, 1] + 5e-3) / 1e-3) * 10 + np.floor((b[:, 0] + 5e-3) / 1e-3)).astype(np.int64)
+    sel = expect == O.F_DETECTED
+    assert np.array_equal(r["dump"]["bin"][sel], binB[sel]) and np.all(r["dump"]["bin"][~sel] == -1)
+    # a slit AFTER the first monitor that absorbs rays the monitor has already counted
+    tight = W.slit_rect(2e-3, 2e-3, T=(0, 0, 0.6))
+    r2 = O.trace(W.instrument("monitor_then_slit", [src, detA, tight, detB], [None], n), dump=True)
+    passes2 = np.all(np.abs(s) <= 1e-3, axis=1)
+    assert (inA & ~passes2).sum() > 100
+    assert np.array_equal(r2["dump"]["fate"], np.where(~passes2, 2, O.F_DETECTED))      # a passing ray always lands in B
+    assert int(r2["N"][0].sum()) == inA.sum() and int(r2["absorbed"][2]) == (~passes2).sum()
+    # a chain that ENDS with a non-detector: nobody is DETECTED although monitor A has counted its rays
+    r3 = O.trace(W.instrument("monitor_not_last", [src, detA, slit], [None], n), dump=True)
+    assert np.array_equal(r3["dump"]["fate"], np.where(passes, O.F_MISSED, 2))
+    assert r3["detected"] == 0 and r3["missed"] == passes.sum() and int(r3["N"][0].sum()) == inA.sum()
+    assert np.all(r3["dump"]["bin"] == -1)
+
+
+def test_closed_meshes_never_degenerate_over_a_million_rays(O, W):
+    # SURVEY.md 8(c) "Pins", mesh row: an even, alternating crossing count for every ray of a closed outward-wound mesh
+    inst = W.config3(small=True)
+    r = O.trace(inst, n=1_000_000, mesh_accel=1)
+    assert r["degenerate"] == 0 and r["detected"] + r["missed"] == 1_000_000

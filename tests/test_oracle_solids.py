@@ -272,3 +272,142 @@ def test_nested_meshes_priority(O, W):
     Lo, Li = t_out[-1] - t_out[0], t_in[-1] - t_in[0]
     assert abs(_tau(O, W, [outer, inner], ray, mats) - (50 * (Lo - Li) + 400 * Li)) < 1e-12
     assert 0.039 < Lo <= 0.04 + 1e-15 and 0.0195 < Li <= 0.02 + 1e-15
+
+
+# ------------------------------------------------------------------ step 9, second half: hits -> intervals
+# Coordinates below are dyadic (exact in fp64) and the direction ratios are +-1 or 0, so the rays go EXACTLY through
+# the shared diagonal of a cube face, through a cube edge or through a cube vertex: every edge function that
+# should vanish is an exact zero, and the duplicate hits really occur.  What the mathematics fixes is the chord of
+# the box, which the box primitive pins independently (test_box_hand_values).
+H_DYADIC = (1 / 64, 3 / 128, 1 / 128)
+
+
+def _tau_rc(O, W, solids, ray, mats):
+    rc, st, _ = O.apply(W.solids(solids), ray, materials=mats)
+    return rc, (-np.log(st[7] / ray[7]) if rc == 1 else None)
+
+
+def test_mesh_duplicate_hits_on_diagonal_edge_vertex_collapse_to_box_chord(O, W):
+    mats = [None, _flat(80.0)]
+    hx, hy, hz = H_DYADIC
+    V, F = W.cube_mesh(hx, hy, hz)
+    mesh, box = W.solid_mesh(V, F, 1, 0), W.solid_box(H_DYADIC, 1, 0)
+    s2 = np.sqrt(2.0)
+    cases = [
+        # (origin, direction, hits of the full line: t-multiplicities (enter, exit), chord)
+        ([0, 0, -1], [0, 0, 1], (2, 2), 2 * hz),                          # both face diagonals (shared edge of 2 triangles)
+        ([1 / 256, 3 / 512, -1], [0, 0, 1], (2, 2), 2 * hz),              # another point of the same diagonals
+        ([2 * hx, 1 / 256, -hz - hx], [-1, 0, 1], (2, 1), 2 * hz * s2),   # in through the edge x = hx, z = -hz
+    ]
+    for o, d, mult, chord in cases:
+        d = unit(d)
+        t, orient, _ = O.mesh_hits(mesh, o, d)
+        assert (int((orient == 1).sum()), int((orient == -1).sum())) == mult, (o, orient)   # the duplicates are there
+        ray = [*o, *d, 30.0, 1.0]
+        rc_m, tau_m = _tau_rc(O, W, [mesh], ray, mats)
+        rc_b, tau_b = _tau_rc(O, W, [box], ray, mats)
+        assert rc_m == 1 and rc_b == 1
+        assert abs(tau_m - 80.0 * chord) < 1e-13 and abs(tau_m - tau_b) < 1e-13
+    # through two opposite vertices of a cube (six triangles meet the ray at either end)
+    hc = 1 / 64
+    Vc, Fc = W.cube_mesh(hc, hc, hc)
+    o, d = [-2 * hc] * 3, unit([1, 1, 1])
+    t, orient, _ = O.mesh_hits(W.solid_mesh(Vc, Fc, 1, 0), o, d)
+    assert (orient == 1).sum() >= 3 and (orient == -1).sum() >= 3
+    rc, tau = _tau_rc(O, W, [W.solid_mesh(Vc, Fc, 1, 0)], [*o, *d, 30.0, 1.0], mats)
+    assert rc == 1 and abs(tau - 80.0 * 2 * hc * np.sqrt(3.0)) < 1e-13
+    # the same rays against a rotated and shifted cube (not exact any more, still the box chord)
+    Rm = W.random_rotation(np.random.default_rng(70))
+    T = np.array([1e-3, -2e-3, 0.5])
+    mesh_r, box_r = W.solid_mesh(V, F, 1, 0, R=Rm, T=T), W.solid_box(H_DYADIC, 1, 0, R=Rm, T=T)
+    for o, d, _, chord in cases:
+        ol, dl = Rm.T @ np.asarray(o, float) + T, Rm.T @ unit(d)
+        ray = [*ol, *dl, 30.0, 1.0]
+        rc_m, tau_m = _tau_rc(O, W, [mesh_r], ray, mats)
+        rc_b, tau_b = _tau_rc(O, W, [box_r], ray, mats)
+        assert rc_m == 1 and abs(tau_m - tau_b) < 1e-12 and abs(tau_b - 80.0 * chord) < 1e-11
+
+
+def test_mesh_grazing_edge_and_vertex_enter_sorts_before_exit(O, W):
+    # A ray that only touches a cube edge (or vertex) from outside hits an entering and an exiting face at the SAME t.
+    # With "enter before exit on ties" that is an interval of zero length (tau = 0, as for the box, whose chord is
+    # empty); the opposite tie order would start the sequence with an exit and call the mesh degenerate.
+    mats = [None, _flat(80.0)]
+    hx, hy, hz = H_DYADIC
+    V, F = W.cube_mesh(hx, hy, hz)
+    mesh, box = W.solid_mesh(V, F, 1, 0), W.solid_box(H_DYADIC, 1, 0)
+    for o, d in (([0, 1 / 256, -hz - hx], [1, 0, 1]),              # touches the edge x = hx, z = -hz
+                 ([0, hy - hx, -hz - hx], [1, 1, 1])):             # touches the vertex (hx, hy, -hz)
+        d = unit(d)
+        t, orient, _ = O.mesh_hits(mesh, o, d)
+        assert len(t) >= 2 and (orient == 1).any() and (orient == -1).any() and np.ptp(t) == 0.0
+        ray = [*o, *d, 30.0, 1.0]
+        assert _tau_rc(O, W, [mesh], ray, mats) == (1, 0.0)
+        assert _tau_rc(O, W, [box], ray, mats) == (1, 0.0)
+
+
+def test_open_or_inward_wound_mesh_is_degenerate(O, W):
+    # step 9: a hit sequence that does not alternate enter, exit, ... starting with enter drops the ray (rc -3)
+    mats = [None, _flat(80.0)]
+    V, F = W.cube_mesh(*H_DYADIC)
+    top = np.array([all(V[v][2] > 0 for v in f) for f in F])
+    assert top.sum() == 2
+    opened = W.solid_mesh(V, F[~top], 1, 0)                        # cube without its face z = +hz
+    through_hole = [1e-3, 2e-3, -1, 0, 0, 1, 30.0, 1.0]            # in through z = -hz, out through the hole: 1 hit
+    sideways = [-1, 2e-3, 1e-3, 1, 0, 0, 30.0, 1.0]                # in and out through the x faces: still closed there
+    assert _tau_rc(O, W, [opened], through_hole, mats) == (-3, None)
+    rc, tau = _tau_rc(O, W, [opened], sideways, mats)
+    assert rc == 1 and abs(tau - 80.0 * 2 * H_DYADIC[0]) < 1e-13
+    assert _tau_rc(O, W, [opened], [0.1, 0, -1, 0, 0, 1, 30.0, 1.0], mats) == (1, 0.0)       # misses it altogether
+    inward = W.solid_mesh(V, F[:, [0, 2, 1]], 1, 0)                # every triangle flipped: the first hit is an exit
+    assert _tau_rc(O, W, [inward], through_hole, mats) == (-3, None)
+    assert _tau_rc(O, W, [inward], sideways, mats) == (-3, None)
+    assert _tau_rc(O, W, [inward], [0.1, 0, -1, 0, 0, 1, 30.0, 1.0], mats) == (1, 0.0)
+    # a closed, outward-wound mesh never is: 2000 random lines through a bumpy sphere, and whole chains count them
+    rng = np.random.default_rng(12)
+    Vb, Fb = W.bumpy_sphere(rng, 3, 20e-3)
+    closed = W.solid_mesh(Vb, Fb, 1, 0)
+    for _ in range(2000):
+        o = unit(rng.normal(size=3)) * 0.1
+        d = unit(rng.normal(size=3) * 0.012 - o)
+        assert O.apply(W.solids([closed]), [*o, *d, 30.0, 1.0], materials=mats)[0] == 1
+    # in a chain the ray is dropped and counted: fate -3, no tally, counters still add up
+    src = W.source("point", "target", "mono", target_w=0.2, target_h=0.2, target_dist=1.0, E0=30.0)
+    det = W.detector(-0.1, 0.1, -0.1, 0.1, 8, 8, 0.0, 60.0, 1, T=(0, 0, 1.0))
+    opened_at = W.solid_mesh(V, F[~top], 1, 0, T=(0, 0, 0.5))
+    r = O.trace(W.instrument("open", [src, W.solids([opened_at]), det], mats, 4000), dump=True)
+    # degenerate = the rays through the missing face (2 hx x 2 hy at z = 0.5 + hz), seen from the point source
+    zf = 0.5 + H_DYADIC[2]
+    frac = (2 * H_DYADIC[0] / zf) * (2 * H_DYADIC[1] / zf) / 0.2 ** 2
+    assert abs(r["degenerate"] / 4000 - frac) < 4 * np.sqrt(frac * (1 - frac) / 4000)
+    assert r["degenerate"] + r["detected"] + r["missed"] + int(r["absorbed"].sum()) == 4000
+    assert int(r["N"][0].sum()) == r["detected"] == int((r["dump"]["fate"] == O.F_DETECTED).sum())
+    assert np.all(r["dump"]["p"][r["dump"]["fate"] == O.F_DEGENERATE] == 1.0)      # dropped before any attenuation
+
+
+def test_icosphere_level6_chord_vs_analytic_sphere(O, W):
+    # SURVEY.md 8(c) "Pins", mesh row: the unperturbed level-6 icosphere (the outer mesh of configs[3]) is inscribed in
+    # the sphere.  Its faces lie 5.6e-5 R .. 7.1e-5 R below the sphere at their centres (computed here from the
+    # generator's vertices; the survey's "5.0e-5 R" was an estimate), so away from grazing (impact parameter <= R/4,
+    # incidence <= 14.5 deg) a chord is SHORT of the analytic 2 sqrt(R^2 - b^2) by at most 2 x 7.2e-5 R / cos(14.5 deg)
+    # = 1.5e-4 R, and never longer.
+    R = 20e-3
+    V, F = W.icosphere(6)
+    assert len(F) == 81920
+    ctr = (V[F[:, 0]] + V[F[:, 1]] + V[F[:, 2]]) / 3.0
+    sag = 1.0 - np.linalg.norm(ctr, axis=1)
+    assert 5.5e-5 < sag.min() and sag.max() < 7.2e-5
+    mesh = W.solid_mesh(V * R, F, 1, 0)
+    rng = np.random.default_rng(90)
+    worst = 0.0
+    for _ in range(25):
+        n = unit(rng.normal(size=3))
+        e = unit(np.cross(n, rng.normal(size=3)))
+        b = rng.uniform(0.0, 0.25) * R
+        o = b * e - 0.5 * n
+        t, orient, ntest = O.mesh_hits(mesh, o, n, use_grid=False)
+        assert ntest == len(F) and len(t) >= 2 and orient[0] == +1 and orient[-1] == -1
+        deficit = 2 * np.sqrt(R * R - b * b) - (t[-1] - t[0])
+        assert 0.0 <= deficit < 1.5e-4 * R
+        worst = max(worst, deficit)
+    assert worst > 1e-5 * R                                        # it IS a polyhedron, not the sphere
