@@ -22,7 +22,11 @@
  *
  * Errors.  Every call returns an mcx_status; mcx_last_error() gives a thread-local message for the last failure.
  * Argument and range errors are found synchronously at create.  A sticky CUDA error is reported by the next call
- * as MCX_ERR_CUDA.  A handle must be used from one host thread at a time; distinct handles are independent.
+ * as MCX_ERR_CUDA.  Errors of the asynchronous trace itself surface the same way: if a ray overflowed its per-ray
+ * scratch capacity (MCX_ERR_CAPACITY below), every later call on the handle that finds the overflowing trace finished
+ * on the device -- mcx_trace*, mcx_tally_read*, mcx_counters_read -- still does its work and returns MCX_ERR_CAPACITY,
+ * until mcx_tally_reset; mcx_trace_status synchronises the stream first and is therefore definitive.
+ * A handle must be used from one host thread at a time; distinct handles are independent.
  */
 #ifndef MCX_H_
 #define MCX_H_
@@ -40,10 +44,14 @@ typedef enum {
   MCX_OK = 0,
   MCX_ERR_INVALID_ARG = 1, /* null pointer, bad enum, chain not starting with a source, ... */
   MCX_ERR_UNSUPPORTED = 2, /* a limit of this build exceeded (see MCX_MAX_*) */
-  MCX_ERR_RANGE = 3,       /* a source energy range not covered by a reflectivity table grid, bad table order */
+  MCX_ERR_RANGE = 3,       /* a table that is not strictly increasing / positive, an empty grid or bin range */
   MCX_ERR_WORKSPACE = 4,   /* workspace too small or misaligned (needs 256-byte alignment) */
   MCX_ERR_CUDA = 5,        /* a CUDA runtime call failed */
-  MCX_ERR_CAPACITY = 6     /* a per-ray scratch capacity (intervals, mesh hits) overflowed during a trace */
+  MCX_ERR_CAPACITY = 6     /* during a trace some ray produced more interval end points in one solids group than the
+                              per-ray scratch holds (2 per primitive + 8 per mesh, at least 16, at most 48: e.g. a ray
+                              through the apex of a fan of more triangles than that).  Such rays are dropped as
+                              MCX_FATE_DEGENERATE and counted in the capacity_overflows counter; the tallies hold
+                              every other ray. */
 } mcx_status;
 
 enum { MCX_MAX_COMPONENTS = 16, MCX_MAX_DETECTORS = 4, MCX_MAX_MATERIALS = 32, MCX_MAX_SOLIDS = 16 };
@@ -206,6 +214,18 @@ mcx_status mcx_trace_range(mcx_instrument* inst, uint64_t first_ray, uint64_t n_
 typedef enum { MCX_EXEC_AUTO = 0, MCX_EXEC_DIRECT = 1, MCX_EXEC_SORTED = 2 } mcx_exec_mode;
 mcx_status mcx_instrument_set_exec(mcx_instrument* inst, int mode);
 
+/* Tuning of the lane scheduling, for sweeps and tests; 0 in a field = keep the library's choice.  Results never depend
+ * on it beyond the summation order of the tallies.
+ *   chunk_log2      rays per sorted chunk = 2^chunk_log2, 14..26 (default 26: the workspace always holds the order
+ *                   buffer of a 2^26 chunk, 256 MiB, whatever is set here);
+ *   sort_grid_bits  bits per axis of the bucket grid of MCX_EXEC_SORTED, 1..11 (default: by chunk length, at most 9
+ *                   for instruments of analytic solids only, else 10);
+ *   absorber_gate   1 = on (default), 2 = off. */
+typedef struct mcx_tuning {
+  int32_t chunk_log2, sort_grid_bits, absorber_gate, reserved;
+} mcx_tuning;
+mcx_status mcx_instrument_set_tuning(mcx_instrument* inst, const mcx_tuning* tuning);
+
 /* Finalises detector `detector` (ordinal among MCX_DETECTOR components): writes N (ray counts), p (sum of
  * weights) and p2 (sum of squared weights) for all bins, bin = (iy * nx + ix) * ne + ie.
  * N, p, p2: DEVICE [n_bins]; n_bins must equal nx*ny*ne. */
@@ -229,6 +249,11 @@ mcx_status mcx_tally_reset(mcx_instrument* inst, void* cuda_stream);
  * absorbed + detected + missed + degenerate equals the number of rays traced since the last reset. */
 mcx_status mcx_counters_read(mcx_instrument* inst, uint64_t* counters, int n, void* cuda_stream);
 
+/* Waits for everything enqueued on `cuda_stream` and reports what the traces since the last mcx_tally_reset did:
+ * MCX_OK, MCX_ERR_CAPACITY (mcx_last_error gives the number of rays dropped) or MCX_ERR_CUDA (an asynchronous fault).
+ * The one call that synchronises. */
+mcx_status mcx_trace_status(mcx_instrument* inst, void* cuda_stream);
+
 /* Traces rays [first_ray, first_ray + n_rays) and writes one record per ray to `out` (DEVICE [n_rays]) instead of
  * tallying: tallies and counters are left untouched.  For parity tests. */
 mcx_status mcx_trace_dump(mcx_instrument* inst, uint64_t first_ray, uint64_t n_rays, uint64_t seed,
@@ -247,6 +272,19 @@ mcx_status mcx_probe_dfma(double* sink, int n_blocks, int64_t n_iters, void* cud
  * into one pseudo-random 32-byte record of `table` (DEVICE, n_records * 32 bytes, n_records a power of two; contents
  * are garbage afterwards).  Records updated = n_blocks * 256 * n_iters. */
 mcx_status mcx_probe_tally(void* table, uint64_t n_records, int n_blocks, int64_t n_iters, void* cuda_stream);
+
+/* Memory-side probes for the rooflines of the mesh and voxel paths ("measure L2 sector
+ * peak").  Both read `table` (DEVICE, n_bytes, a power of two >= 4096; contents irrelevant for mcx_probe_l2, overwritten
+ * with a pointer chain by mcx_probe_latency) and write one value per thread to `sink` (DEVICE [n_blocks * 256] uint32).
+ *   mcx_probe_l2       every thread does n_iters independent loads of one pseudo-random aligned 32-byte sector (the
+ *                      size of a BVH node; read through L1 with ld.global.nc as the walk does) --
+ *                      sectors read = n_blocks * 256 * n_iters;
+ *   mcx_probe_latency  every thread chases a dependent chain of n_iters 8-byte loads through a random cyclic
+ *                      permutation of the table's 32-byte sectors -- loads in flight per thread = 1;
+ *                      n_blocks x 256 threads (use 1 block of 32 for the unloaded latency). */
+mcx_status mcx_probe_l2(const void* table, uint64_t n_bytes, uint32_t* sink, int n_blocks, int64_t n_iters, void* cuda_stream);
+mcx_status mcx_probe_latency(void* table, uint64_t n_bytes, uint32_t* sink, int n_blocks, int n_threads, int64_t n_iters,
+                             void* cuda_stream);
 
 void mcx_instrument_destroy(mcx_instrument* inst);
 

@@ -25,8 +25,10 @@ EXEC_MODE = {"auto": 0, "direct": 1, "sorted": 2}
 FATE_DETECTED, FATE_MISSED, FATE_DEGENERATE = -1, -2, -3
 
 EXPORTS = ["mcx_instrument_workspace_size", "mcx_instrument_create", "mcx_trace", "mcx_trace_range", "mcx_tally_read",
-           "mcx_tally_read_host", "mcx_instrument_set_exec", "mcx_upload_bytes", "mcx_tally_reset", "mcx_counters_read", "mcx_trace_dump", "mcx_launch_count", "mcx_probe_dfma", "mcx_probe_tally",
-           "mcx_instrument_destroy", "mcx_last_error"]
+           "mcx_tally_read_host", "mcx_instrument_set_exec", "mcx_instrument_set_tuning", "mcx_upload_bytes", "mcx_tally_reset",
+           "mcx_counters_read", "mcx_trace_status", "mcx_trace_dump", "mcx_launch_count", "mcx_probe_dfma", "mcx_probe_tally",
+           "mcx_probe_l2", "mcx_probe_latency", "mcx_instrument_destroy", "mcx_last_error"]
+MCX_ERR_CAPACITY = 6
 
 _dp = C.POINTER(C.c_double)
 _u64p = C.POINTER(C.c_uint64)
@@ -92,6 +94,10 @@ class McxComponent(C.Structure):
     _fields_ = [("kind", C.c_int32), ("reserved", C.c_int32), ("pose", McxPose), ("u", McxParamsUnion)]
 
 
+class McxTuning(C.Structure):
+    _fields_ = [("chunk_log2", C.c_int32), ("sort_grid_bits", C.c_int32), ("absorber_gate", C.c_int32), ("reserved", C.c_int32)]
+
+
 FATE_DTYPE = np.dtype([("fate", np.int32), ("reserved", np.int32), ("bin", np.int64), ("p", np.float64)])
 
 _libs = {}
@@ -116,6 +122,14 @@ def lib(strict=False):
     L.mcx_tally_read_host.argtypes = [vp, C.c_int, vp, vp, vp, C.c_size_t, vp]
     L.mcx_instrument_set_exec.argtypes = [vp, C.c_int]
     L.mcx_instrument_set_exec.restype = C.c_int
+    L.mcx_instrument_set_tuning.argtypes = [vp, C.POINTER(McxTuning)]
+    L.mcx_instrument_set_tuning.restype = C.c_int
+    L.mcx_trace_status.argtypes = [vp, vp]
+    L.mcx_trace_status.restype = C.c_int
+    L.mcx_probe_l2.argtypes = [vp, C.c_uint64, vp, C.c_int, C.c_int64, vp]
+    L.mcx_probe_l2.restype = C.c_int
+    L.mcx_probe_latency.argtypes = [vp, C.c_uint64, vp, C.c_int, C.c_int, C.c_int64, vp]
+    L.mcx_probe_latency.restype = C.c_int
     L.mcx_upload_bytes.argtypes = [vp]
     L.mcx_upload_bytes.restype = C.c_uint64
     L.mcx_tally_reset.argtypes = [vp, vp]
@@ -309,6 +323,16 @@ class Instrument:
         """mcx_instrument_set_exec: "auto" | "direct" | "sorted" (lane scheduling, row a13)."""
         _check(self.L.mcx_instrument_set_exec(self.handle, EXEC_MODE[mode]), self.L)
 
+    def set_tuning(self, chunk_log2=0, sort_grid_bits=0, absorber_gate=0):
+        """mcx_instrument_set_tuning; 0 = keep the library's choice."""
+        t = McxTuning(int(chunk_log2), int(sort_grid_bits), int(absorber_gate), 0)
+        _check(self.L.mcx_instrument_set_tuning(self.handle, C.byref(t)), self.L)
+
+    def status(self):
+        """mcx_trace_status: synchronises the current stream; raises McxError (MCX_ERR_CAPACITY / MCX_ERR_CUDA) if a
+        trace since the last reset went wrong."""
+        _check(self.L.mcx_trace_status(self.handle, self._stream()), self.L)
+
     def upload_bytes(self):
         """host -> device bytes moved to build this instrument (tables by create + the voxel volume)."""
         return int(self.L.mcx_upload_bytes(self.handle)) + self.voxel_upload_bytes
@@ -316,12 +340,15 @@ class Instrument:
     def reset(self):
         _check(self.L.mcx_tally_reset(self.handle, self._stream()), self.L)
 
-    def counters(self):
-        """mcx_counters_read -> dict(absorbed=[n_comps], detected, missed, degenerate, overflows); synchronises."""
+    def counters(self, allow_capacity=False):
+        """mcx_counters_read -> dict(absorbed=[n_comps], detected, missed, degenerate, overflows); synchronises.
+        allow_capacity: return the counters even if the call reports MCX_ERR_CAPACITY (overflows > 0 says so)."""
         torch = self.torch
         n = self.n_comps + 4
         buf = torch.empty(n, dtype=torch.int64, device=self.device)
-        _check(self.L.mcx_counters_read(self.handle, buf.data_ptr(), n, self._stream()), self.L)
+        st = self.L.mcx_counters_read(self.handle, buf.data_ptr(), n, self._stream())
+        if not (allow_capacity and st == MCX_ERR_CAPACITY):
+            _check(st, self.L)
         v = buf.cpu().numpy()
         return {"absorbed": v[:self.n_comps].copy(), "detected": int(v[self.n_comps]), "missed": int(v[self.n_comps + 1]),
                 "degenerate": int(v[self.n_comps + 2]), "overflows": int(v[self.n_comps + 3])}
@@ -382,3 +409,40 @@ def probe_dfma(n_blocks, n_iters, device="cuda:0"):
         e1.record()
         torch.cuda.synchronize(dev)
         return n_blocks * 256 * n_iters * 8 / (e0.elapsed_time(e1) * 1e-3)
+
+
+def probe_l2(n_bytes, n_blocks, n_iters, device="cuda:0"):
+    """mcx_probe_l2: returns random 32-byte sectors read per second from a table of n_bytes (CUDA-event timed)."""
+    import torch
+    dev = torch.device(device)
+    with torch.cuda.device(dev):
+        table = torch.zeros(n_bytes // 8, dtype=torch.int64, device=dev)
+        sink = torch.empty(n_blocks * 256, dtype=torch.int32, device=dev)
+        st = C.c_void_p(torch.cuda.current_stream(dev).cuda_stream)
+        _check(lib().mcx_probe_l2(table.data_ptr(), n_bytes, sink.data_ptr(), n_blocks, max(4, n_iters // 4), st))
+        torch.cuda.synchronize(dev)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        _check(lib().mcx_probe_l2(table.data_ptr(), n_bytes, sink.data_ptr(), n_blocks, n_iters, st))
+        e1.record()
+        torch.cuda.synchronize(dev)
+        return n_blocks * 256 * n_iters / (e0.elapsed_time(e1) * 1e-3)
+
+
+def probe_latency(n_bytes, n_blocks, n_threads, n_iters, device="cuda:0"):
+    """mcx_probe_latency: returns seconds per dependent load (one chain per thread) in a table of n_bytes."""
+    import torch
+    dev = torch.device(device)
+    with torch.cuda.device(dev):
+        table = torch.zeros(n_bytes // 8, dtype=torch.int64, device=dev)
+        sink = torch.empty(n_blocks * 256, dtype=torch.int32, device=dev)
+        st = C.c_void_p(torch.cuda.current_stream(dev).cuda_stream)
+        _check(lib().mcx_probe_latency(table.data_ptr(), n_bytes, sink.data_ptr(), n_blocks, n_threads, max(1, n_iters // 4), st))
+        torch.cuda.synchronize(dev)
+        # the init launch of the second call is timed too: one pass over the table, small against n_iters dependent loads
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        _check(lib().mcx_probe_latency(table.data_ptr(), n_bytes, sink.data_ptr(), n_blocks, n_threads, n_iters, st))
+        e1.record()
+        torch.cuda.synchronize(dev)
+        return e0.elapsed_time(e1) * 1e-3 / n_iters

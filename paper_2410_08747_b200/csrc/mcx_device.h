@@ -155,6 +155,8 @@ struct TraceArgs {
   mcx_ray_fate* dump;      // per-ray records indexed by ray offset, or null = tally
   unsigned int* ticket;    // [2] work-tile ticket and departure count, zero between launches
   unsigned int* gate_known;  // the absorber gate an earlier launch on this instrument settled on, plus 1 (0 = not yet)
+  unsigned int* host_flag;   // mapped pinned host word: receives epoch + 1 when a ray overflowed its scratch capacity
+  unsigned int epoch;        // number of mcx_tally_reset calls on the handle so far
 };
 
 // sizes of the sort workspace
@@ -170,7 +172,10 @@ cudaError_t launch_voxel_relayout(const uint8_t* src, uint8_t* dst, int nx, int 
                                   int pitch, int run_dir, int n_mats, cudaStream_t stream);
 cudaError_t launch_probe_dfma(double* sink, int n_blocks, long long n_iters, cudaStream_t stream);
 cudaError_t launch_probe_tally(void* table, unsigned long long n_records, int n_blocks, long long n_iters, cudaStream_t stream);
-cudaError_t kernels_init();
+cudaError_t launch_probe_l2(const void* table, unsigned long long n_bytes, uint32_t* sink, int n_blocks, long long n_iters,
+                            cudaStream_t stream);
+cudaError_t launch_probe_latency(void* table, unsigned long long n_bytes, uint32_t* sink, int n_blocks, int n_threads,
+                                 long long n_iters, cudaStream_t stream);
 
 }  // namespace mcx
 #endif

@@ -17,7 +17,6 @@ using namespace mcx;
 
 struct mcx_instrument {
   DInstrument host_image;            // what sits at workspace offset 0
-  std::vector<unsigned char> blob;   // host copy of the table section (kept alive for the async H2D copy)
   unsigned char* workspace = nullptr;
   size_t workspace_bytes = 0;
   size_t zero_begin = 0, zero_end = 0;  // tallies + counters
@@ -32,7 +31,13 @@ struct mcx_instrument {
   // lane scheduling (row a13)
   int exec_mode = MCX_EXEC_AUTO;
   size_t off_ticket = 0, off_gate = 0, off_sort_cnt = 0, off_sort_bsum = 0, off_order = 0;
-  uint64_t chunk_rays = 0;  // capacity of the order buffer
+  uint64_t chunk_rays = 0;  // rays per sorted chunk (<= kChunkCapacity, the order buffer in the workspace)
+  int sort_grid_bits = 0;   // 0 = by chunk length (sort_bits)
+  bool gate_enabled = true;
+  // MCX_ERR_CAPACITY: a mapped pinned host word the trace kernel writes (epoch + 1) when a ray overflows its scratch
+  unsigned int* host_flag = nullptr;
+  unsigned int epoch = 0;   // resets so far: an overflow of an earlier epoch is forgotten
+  ~mcx_instrument() { if (host_flag) cudaFreeHost(host_flag); }
 };
 
 namespace {
@@ -147,21 +152,15 @@ struct BvhBuilder {
 // Rays per sorted chunk.  The more rays a chunk holds the closer together the 32 rays of a warp land (the bucket grid
 // is capped at 2^10 x 2^10 cells, so past 2^24 rays the buckets only get fuller and a warp spans less of one): c4
 // gains 6 % from 2^24 to 2^26 and 1 % more at 2^28; the order buffer (4 B per ray, 256 MiB) is streamed once each
-// way.  MCX_CHUNK_LOG2 / MCX_SORT_G are tuning knobs for sweeps.
-int env_int(const char* name, int lo, int hi, int dflt) {
-  const char* v = std::getenv(name);
-  if (!v || !*v) return dflt;
-  const long x = std::strtol(v, nullptr, 10);
-  return x < lo || x > hi ? dflt : (int)x;
-}
-uint64_t chunk_capacity() { return (uint64_t)1 << env_int("MCX_CHUNK_LOG2", 14, 30, 26); }
+// way.  mcx_instrument_set_tuning can shorten the chunks (tests, sweeps); the workspace always holds a full one.
+constexpr int kChunkLog2Max = 26, kChunkLog2Min = 14;
+constexpr uint64_t kChunkCapacity = (uint64_t)1 << kChunkLog2Max;
 constexpr uint64_t kSortMinRays = 1u << 14;  // shorter chunks are traced in index order
 
 // Bits per axis of the bucket grid: at least 64 rays per bucket, at most 2^10 x 2^10 cells (a finer grid measured no
 // gain on c3 / c4), and 2^9 x 2^9 where the instrument has only analytic solids: there coherence of the branches is
 // all the order buys, and the coarser grid keeps the scatter's write fronts L2-resident (c1: 7 % faster than 2^10).
-int sort_bits(uint64_t n, int features) {
-  const int forced = env_int("MCX_SORT_G", 1, MCX_SORT_MAX_G, 0);
+int sort_bits(uint64_t n, int features, int forced) {
   if (forced) return forced;
   const int g_max = (features & (F_MESH | F_VOXELS)) ? 10 : 9;
   int g = 1;
@@ -315,7 +314,7 @@ mcx_status make_plan(const mcx_component* comps, int n_comps, const mcx_material
   P->off_staging = A.reserve(max_bins * 24);
   P->off_sort_cnt = A.reserve((size_t)MCX_SORT_MAX_BUCKETS * sizeof(unsigned int));
   P->off_sort_bsum = A.reserve((size_t)MCX_SORT_MAX_SCAN_BLOCKS * sizeof(unsigned int));
-  P->off_order = A.reserve((size_t)chunk_capacity() * sizeof(uint32_t));
+  P->off_order = A.reserve((size_t)kChunkCapacity * sizeof(uint32_t));
   P->total = A.top;
   return MCX_OK;
 }
@@ -324,6 +323,16 @@ mcx_status check_sticky() {
   const cudaError_t e = cudaPeekAtLastError();
   if (e != cudaSuccess) return cuda_fail(e, "earlier CUDA error");
   return MCX_OK;
+}
+
+// include/mcx.h "Errors": has a trace of the current reset epoch, finished on the device, overflowed a per-ray capacity?
+bool capacity_overflowed(const mcx_instrument* H) {
+  return H->host_flag && *reinterpret_cast<volatile unsigned int*>(H->host_flag) == H->epoch + 1u;
+}
+mcx_status capacity_status(const mcx_instrument* H) {
+  if (!capacity_overflowed(H)) return MCX_OK;
+  return fail(MCX_ERR_CAPACITY, "rays overflowed the per-ray end-point capacity (%d) of a solids group and were dropped as "
+              "degenerate; mcx_trace_status / mcx_counters_read give the count", H->cap_endpoints);
 }
 
 }  // namespace
@@ -370,9 +379,11 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
   H->off_sort_cnt = P.off_sort_cnt;
   H->off_sort_bsum = P.off_sort_bsum;
   H->off_order = P.off_order;
-  H->chunk_rays = chunk_capacity();
-  H->blob.assign(P.blob_end - P.blob_begin, 0);
-  unsigned char* blob = H->blob.data();
+  H->chunk_rays = kChunkCapacity;
+  // host copy of the table section; consumed by the upload below (a copy from pageable memory has been staged when
+  // cudaMemcpyAsync returns), so it lives only as long as this call
+  std::vector<unsigned char> blob_storage(P.blob_end - P.blob_begin, 0);
+  unsigned char* blob = blob_storage.data();
   auto host_ptr = [&](size_t off) { return blob + (off - P.blob_begin); };
   auto dev_ptr = [&](size_t off) { return ws + off; };
   DInstrument& I = H->host_image;
@@ -544,6 +555,7 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
         features |= F_VOXELS;
         const mcx_voxels_params& V = C.u.voxels;
         if (!V.ids) MCX_BAIL(MCX_ERR_INVALID_ARG, "component %d: ids is null", c);
+        if (n_materials < 1) MCX_BAIL(MCX_ERR_INVALID_ARG, "component %d: a voxel volume needs a materials array (ID 0 = materials[0])", c);
         DVoxels& d = D.u.voxels;
         d.h = V.h;
         d.inv_h = 1.0 / V.h;
@@ -623,12 +635,11 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
   H->n_dets = n_dets;
   H->features = features;
   H->cap_endpoints = cap_endpoints;
-  if (env_int("MCX_GATE", 0, 1, 1))
-    for (int c = 1; c + 1 < n_components; ++c) {
+  for (int c = 1; c + 1 < n_components; ++c) {
       const int k = components[c].kind;
-      if (k != MCX_SLIT_RECT && k != MCX_SLIT_CIRC && k != MCX_MIRROR_ELLIPTIC && k != MCX_CRYSTAL_BRAGG) break;
-      H->gate_max = c;
-    }
+    if (k != MCX_SLIT_RECT && k != MCX_SLIT_CIRC && k != MCX_MIRROR_ELLIPTIC && k != MCX_CRYSTAL_BRAGG) break;
+    H->gate_max = c;
+  }
   {  // Detector-tile order needs a source whose slot-1 draw is a target point (step 3) and pays where neighbouring rays
      // share work: voxels, meshes, groups of several solids (measured: c1 1.4x, c3 5x, c4 3x; c0 and c2 nothing)
     bool shared_work = (features & (F_MESH | F_VOXELS)) != 0;
@@ -637,13 +648,16 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
     H->sort_pays = components[0].u.source.dir_mode == MCX_DIR_TARGET && shared_work;
   }
 
-  cudaError_t e = cudaMemcpyAsync(ws + P.off_inst, &H->host_image, sizeof(DInstrument), cudaMemcpyHostToDevice, stream);
-  if (e == cudaSuccess && !H->blob.empty())
-    e = cudaMemcpyAsync(ws + P.blob_begin, H->blob.data(), H->blob.size(), cudaMemcpyHostToDevice, stream);
+  cudaError_t e = cudaHostAlloc((void**)&H->host_flag, 64, cudaHostAllocMapped | cudaHostAllocPortable);
+  if (e != cudaSuccess) { H->host_flag = nullptr; const mcx_status s_ = cuda_fail(e, "pinned status word"); delete H; return s_; }
+  *H->host_flag = 0u;
+  e = cudaMemcpyAsync(ws + P.off_inst, &H->host_image, sizeof(DInstrument), cudaMemcpyHostToDevice, stream);
+  if (e == cudaSuccess && !blob_storage.empty())
+    e = cudaMemcpyAsync(ws + P.blob_begin, blob_storage.data(), blob_storage.size(), cudaMemcpyHostToDevice, stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(ws + P.zero_begin, 0, P.zero_end - P.zero_begin, stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(ws + P.off_gate, 0, sizeof(unsigned int), stream);
   if (e != cudaSuccess) { const mcx_status s_ = cuda_fail(e, "upload of the instrument image"); delete H; return s_; }
-  H->upload_bytes = sizeof(DInstrument) + H->blob.size();
+  H->upload_bytes = sizeof(DInstrument) + blob_storage.size();
   *out = H;
   return MCX_OK;
 }
@@ -672,13 +686,15 @@ mcx_status run_trace(mcx_instrument* H, uint64_t first, uint64_t n, uint64_t see
     A.n = m;
     A.seed = seed;
     A.cap_endpoints = H->cap_endpoints;
-    A.gate_max = H->gate_max;
+    A.gate_max = H->gate_enabled ? H->gate_max : 0;
+    A.host_flag = H->host_flag;
+    A.epoch = H->epoch;
     A.order = nullptr;
     A.dump = dump ? dump + base : nullptr;
     A.ticket = (unsigned int*)(ws + H->off_ticket);
     A.gate_known = (unsigned int*)(ws + H->off_gate);
     if (sorted && m >= kSortMinRays) {
-      const int g = sort_bits(m, H->features);
+      const int g = sort_bits(m, H->features, H->sort_grid_bits);
       unsigned int* cnt = (unsigned int*)(ws + H->off_sort_cnt);
       cudaError_t e = cudaMemsetAsync(cnt, 0, sizeof(unsigned int) << (2 * g), stream);
       if (e == cudaSuccess)
@@ -709,7 +725,8 @@ mcx_status mcx_trace_range(mcx_instrument* inst, uint64_t first_ray, uint64_t n_
   if (!inst) return fail(MCX_ERR_INVALID_ARG, "inst is null");
   mcx_status st = check_sticky();
   if (st != MCX_OK) return st;
-  return run_trace(inst, first_ray, n_rays, seed, nullptr, (cudaStream_t)cuda_stream);
+  st = run_trace(inst, first_ray, n_rays, seed, nullptr, (cudaStream_t)cuda_stream);
+  return st != MCX_OK ? st : capacity_status(inst);
 }
 
 mcx_status mcx_trace(mcx_instrument* inst, uint64_t n_rays, uint64_t seed, void* cuda_stream) {
@@ -737,7 +754,7 @@ mcx_status mcx_tally_read(mcx_instrument* inst, int detector, uint64_t* N, doubl
   const cudaError_t e = launch_tally_read(inst->host_image.tallies[detector], n_bins, (unsigned long long*)N, p, p2, (cudaStream_t)cuda_stream);
   if (e != cudaSuccess) return cuda_fail(e, "tally_read launch");
   inst->launches++;
-  return MCX_OK;
+  return capacity_status(inst);
 }
 
 mcx_status mcx_tally_read_host(mcx_instrument* inst, int detector, uint64_t* N, double* p, double* p2, size_t n_bins,
@@ -750,13 +767,13 @@ mcx_status mcx_tally_read_host(mcx_instrument* inst, int detector, uint64_t* N, 
   double* dP = (double*)(dN + n_bins);
   double* dP2 = dP + n_bins;
   const mcx_status st = mcx_tally_read(inst, detector, (uint64_t*)dN, dP, dP2, n_bins, cuda_stream);
-  if (st != MCX_OK) return st;
+  if (st != MCX_OK && st != MCX_ERR_CAPACITY) return st;
   cudaStream_t stream = (cudaStream_t)cuda_stream;
   cudaError_t e = cudaMemcpyAsync(N, dN, n_bins * sizeof(uint64_t), cudaMemcpyDeviceToHost, stream);
   if (e == cudaSuccess) e = cudaMemcpyAsync(p, dP, n_bins * sizeof(double), cudaMemcpyDeviceToHost, stream);
   if (e == cudaSuccess) e = cudaMemcpyAsync(p2, dP2, n_bins * sizeof(double), cudaMemcpyDeviceToHost, stream);
   if (e != cudaSuccess) return cuda_fail(e, "tally copy to the host");
-  return MCX_OK;
+  return st;
 }
 
 uint64_t mcx_upload_bytes(const mcx_instrument* inst) { return inst ? (uint64_t)inst->upload_bytes : 0; }
@@ -767,6 +784,7 @@ mcx_status mcx_tally_reset(mcx_instrument* inst, void* cuda_stream) {
   if (st != MCX_OK) return st;
   const cudaError_t e = cudaMemsetAsync(inst->workspace + inst->zero_begin, 0, inst->zero_end - inst->zero_begin, (cudaStream_t)cuda_stream);
   if (e != cudaSuccess) return cuda_fail(e, "tally reset");
+  inst->epoch++;  // an overflow reported by a trace enqueued before this reset no longer counts
   return MCX_OK;
 }
 
@@ -777,6 +795,31 @@ mcx_status mcx_counters_read(mcx_instrument* inst, uint64_t* counters, int n, vo
   if (st != MCX_OK) return st;
   const cudaError_t e = cudaMemcpyAsync(counters, inst->host_image.counters, (size_t)n * sizeof(uint64_t), cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream);
   if (e != cudaSuccess) return cuda_fail(e, "counters copy");
+  return capacity_status(inst);
+}
+
+mcx_status mcx_trace_status(mcx_instrument* inst, void* cuda_stream) {
+  if (!inst) return fail(MCX_ERR_INVALID_ARG, "inst is null");
+  cudaError_t e = cudaStreamSynchronize((cudaStream_t)cuda_stream);
+  if (e != cudaSuccess) return cuda_fail(e, "stream synchronize");
+  if ((e = cudaGetLastError()) != cudaSuccess) return cuda_fail(e, "asynchronous CUDA error");
+  if (!capacity_overflowed(inst)) return MCX_OK;
+  unsigned long long dropped = 0;
+  e = cudaMemcpy(&dropped, inst->host_image.counters + inst->n_comps + CNT_OVERFLOW, sizeof(dropped), cudaMemcpyDeviceToHost);
+  if (e != cudaSuccess) return cuda_fail(e, "overflow counter copy");
+  return fail(MCX_ERR_CAPACITY, "%llu rays overflowed the per-ray end-point capacity (%d) of a solids group and were dropped as degenerate",
+              dropped, inst->cap_endpoints);
+}
+
+mcx_status mcx_instrument_set_tuning(mcx_instrument* inst, const mcx_tuning* t) {
+  if (!inst || !t) return fail(MCX_ERR_INVALID_ARG, "null argument");
+  if (t->chunk_log2 != 0 && (t->chunk_log2 < kChunkLog2Min || t->chunk_log2 > kChunkLog2Max))
+    return fail(MCX_ERR_INVALID_ARG, "chunk_log2 %d outside %d..%d", t->chunk_log2, kChunkLog2Min, kChunkLog2Max);
+  if (t->sort_grid_bits < 0 || t->sort_grid_bits > MCX_SORT_MAX_G) return fail(MCX_ERR_INVALID_ARG, "sort_grid_bits %d outside 1..%d", t->sort_grid_bits, MCX_SORT_MAX_G);
+  if (t->absorber_gate < 0 || t->absorber_gate > 2) return fail(MCX_ERR_INVALID_ARG, "absorber_gate must be 0, 1 or 2");
+  if (t->chunk_log2) inst->chunk_rays = (uint64_t)1 << t->chunk_log2;
+  if (t->sort_grid_bits) inst->sort_grid_bits = t->sort_grid_bits;
+  if (t->absorber_gate) inst->gate_enabled = t->absorber_gate == 1;
   return MCX_OK;
 }
 
@@ -793,6 +836,23 @@ mcx_status mcx_probe_tally(void* table, uint64_t n_records, int n_blocks, int64_
   if (!table || n_records == 0 || (n_records & (n_records - 1)) != 0 || n_blocks < 1 || n_iters < 0)
     return fail(MCX_ERR_INVALID_ARG, "bad probe arguments (n_records must be a power of two)");
   const cudaError_t e = launch_probe_tally(table, n_records, n_blocks, (long long)n_iters, (cudaStream_t)cuda_stream);
+  if (e != cudaSuccess) return cuda_fail(e, "probe launch");
+  return MCX_OK;
+}
+
+mcx_status mcx_probe_l2(const void* table, uint64_t n_bytes, uint32_t* sink, int n_blocks, int64_t n_iters, void* cuda_stream) {
+  if (!table || !sink || n_bytes < 4096 || (n_bytes & (n_bytes - 1)) != 0 || n_blocks < 1 || n_iters < 0)
+    return fail(MCX_ERR_INVALID_ARG, "bad probe arguments (n_bytes must be a power of two >= 4096)");
+  const cudaError_t e = launch_probe_l2(table, n_bytes, sink, n_blocks, (long long)n_iters, (cudaStream_t)cuda_stream);
+  if (e != cudaSuccess) return cuda_fail(e, "probe launch");
+  return MCX_OK;
+}
+
+mcx_status mcx_probe_latency(void* table, uint64_t n_bytes, uint32_t* sink, int n_blocks, int n_threads, int64_t n_iters,
+                             void* cuda_stream) {
+  if (!table || !sink || n_bytes < 4096 || (n_bytes & (n_bytes - 1)) != 0 || n_blocks < 1 || n_threads < 1 || n_threads > 256 || n_iters < 0)
+    return fail(MCX_ERR_INVALID_ARG, "bad probe arguments (n_bytes must be a power of two >= 4096, n_threads <= 256)");
+  const cudaError_t e = launch_probe_latency(table, n_bytes, sink, n_blocks, n_threads, (long long)n_iters, (cudaStream_t)cuda_stream);
   if (e != cudaSuccess) return cuda_fail(e, "probe launch");
   return MCX_OK;
 }

@@ -5,6 +5,8 @@
 // Step numbers are those of DESIGN.md "Readings".  This file shares no code with oracle/.
 #include <math_constants.h>
 
+#include <atomic>
+
 #include "mcx_device.h"
 
 namespace mcx {
@@ -348,7 +350,7 @@ __device__ __forceinline__ void ep_sort(const Endpoints& E, int begin, int end, 
 }
 
 // All crossings of the full line with one mesh, appended to E as sorted, duplicate-collapsed, paired end points clipped
-// to t >= 0.  The BVH is walked without a stack (preorder + escape links, any order will do since every hit is wanted);
+// to t >= 0.  The BVH is walked without a stack (complete tree in heap order + a bit trail; any order will do since every hit is wanted);
 // leaves only queue their triangles, and the exact tests run over the queue afterwards, so that the lanes of a warp
 // do box tests together and triangle tests together instead of waiting for one another at every leaf.
 // Returns 1 = ok, 0 = degenerate sequence, -1 = capacity overflow.
@@ -1016,6 +1018,9 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
   if (threadIdx.x == 0) {
     s_sched[0] = atomicAdd(A.ticket, 1u);
     s_sched[2] = 0u;
+    // one read per block, before the barrier: every warp of the block must see the same value (it decides whether the
+    // block takes the extra barrier after its first tile), whatever other blocks store meanwhile
+    if (GATE) s_sched[5] = *reinterpret_cast<volatile unsigned int*>(A.gate_known);
   }
   __syncthreads();
   // Absorber gate (row a13, "warp-level compaction of absorbed rays").  Where the chain starts with slits, mirrors or
@@ -1027,8 +1032,9 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
   // the gate are accounted in the first pass, everything a queued ray does in the second (it is counted there whatever
   // happens to it), so every ray is counted once.  The block picks the gate itself from what its first tile (traced
   // ungated) lost where: the first component after which at most 35 % of the rays are left, if there is one; the
-  // choice is left in the workspace, and later launches on the instrument start with it.
-  const unsigned known_gate = GATE ? *A.gate_known : 0u;
+  // choice (the first block's to finish a tile: one compare-and-swap decides for all) is left in the workspace, and
+  // later launches on the instrument start with it.
+  const unsigned known_gate = GATE ? s_sched[5] : 0u;
   int gate = known_gate ? (int)known_gate - 1 : 0;
   unsigned* ring = reinterpret_cast<unsigned*>(smem_raw + sizeof(DInstrument) + 128) + (threadIdx.x >> 5) * 64;
   unsigned ring_head = 0u, ring_n = 0u;  // warp-uniform
@@ -1185,8 +1191,8 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
             alive_after -= s_cnt[c];
             if (100u * alive_after <= 35u * traced) pick = (unsigned)c;
           }
-          s_sched[4] = pick;
-          *A.gate_known = pick + 1u;
+          const unsigned won = atomicCAS(A.gate_known, 0u, pick + 1u);  // 0: this block's choice stands
+          s_sched[4] = won ? won - 1u : pick;
         }
         __syncthreads();
         gate = (int)s_sched[4];
@@ -1208,6 +1214,11 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
       if (v) {
         const int slot = threadIdx.x < MCX_MAX_COMPONENTS ? threadIdx.x : n_comps + (threadIdx.x - MCX_MAX_COMPONENTS);
         if (threadIdx.x >= MCX_MAX_COMPONENTS || threadIdx.x < n_comps) atomicAdd(&I.counters[slot], (unsigned long long)v);
+        if (threadIdx.x == MCX_MAX_COMPONENTS + CNT_OVERFLOW && A.host_flag) {
+          // MCX_ERR_CAPACITY: tell the host (mapped pinned word) which reset epoch overflowed; include/mcx.h "Errors"
+          *reinterpret_cast<volatile unsigned int*>(A.host_flag) = A.epoch + 1u;
+          __threadfence_system();
+        }
       }
     }
   }
@@ -1286,13 +1297,14 @@ cudaError_t launch_one(const DInstrument* d_inst, int n_mats, const TraceArgs& A
   const size_t smem = kSmemBase + (GATE ? kRingBytes : 0) + ((FEAT & F_SOLIDS) ? kSmemSolids * sizeof(DSolid) + (size_t)A.cap_endpoints * kBlock * 9 : 0) +
                       ((FEAT & F_MESH) ? (size_t)kTriQueue * kBlock * sizeof(unsigned) : 0) +
                       ((FEAT & F_VOXELS) ? (size_t)(n_mats + VC_COUNT) * kBlock * sizeof(double) : 0);
-  static bool configured = false;
-  int blocks_per_sm = 1;
-  cudaError_t e;
-  if (!configured) {
+  static std::atomic<unsigned long long> configured{0ull};  // bit d: the opt-in below was made on device d
+  int blocks_per_sm = 1, dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev >= 64 || !((configured.load(std::memory_order_relaxed) >> dev) & 1ull)) {
     e = cudaFuncSetAttribute(trace_kernel<FEAT, DUMP, GATE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e != cudaSuccess) return e;
-    configured = true;
+    if (dev < 64) configured.fetch_or(1ull << dev, std::memory_order_relaxed);
   }
   e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, trace_kernel<FEAT, DUMP, GATE>, kBlock, smem);
   if (e != cudaSuccess) return e;
@@ -1307,20 +1319,27 @@ cudaError_t launch_one(const DInstrument* d_inst, int n_mats, const TraceArgs& A
   return cudaGetLastError();
 }
 
-int g_n_sm = 0;
+std::atomic<int> g_sm_of_device[64];  // SM count per device, 0 = not asked yet
 
-}  // namespace
-
-cudaError_t kernels_init() {
-  if (g_n_sm) return cudaSuccess;
+// SM count of the current device
+cudaError_t sm_count(int* n_sm) {
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return e;
-  return cudaDeviceGetAttribute(&g_n_sm, cudaDevAttrMultiProcessorCount, dev);
+  if (dev < 64) {
+    const int known = g_sm_of_device[dev].load(std::memory_order_relaxed);
+    if (known) { *n_sm = known; return cudaSuccess; }
+  }
+  e = cudaDeviceGetAttribute(n_sm, cudaDevAttrMultiProcessorCount, dev);
+  if (e == cudaSuccess && dev < 64) g_sm_of_device[dev].store(*n_sm, std::memory_order_relaxed);
+  return e;
 }
 
+}  // namespace
+
 cudaError_t launch_trace(const DInstrument* d_inst, int features, int n_mats, const TraceArgs& A, cudaStream_t stream) {
-  cudaError_t e = kernels_init();
+  int g_n_sm = 0;
+  cudaError_t e = sm_count(&g_n_sm);
   if (e != cudaSuccess) return e;
   if (A.n == 0) return cudaSuccess;
   if (A.n > ((uint64_t)1 << 40)) return cudaErrorInvalidValue;  // tile tickets are 32-bit; the host chunks below this
@@ -1348,7 +1367,8 @@ cudaError_t launch_trace(const DInstrument* d_inst, int features, int n_mats, co
 // count -> scan -> scatter of one chunk (n <= 2^32 - 1 rays, 4^g buckets); cnt must be zero on entry
 cudaError_t launch_sort(uint64_t first, uint32_t n, uint64_t seed, int g, unsigned int* cnt, unsigned int* bsum,
                         uint32_t* order, cudaStream_t stream) {
-  cudaError_t e = kernels_init();
+  int g_n_sm = 0;
+  cudaError_t e = sm_count(&g_n_sm);
   if (e != cudaSuccess) return e;
   const uint32_t n_buckets = 1u << (2 * g);
   const int n_scan_blocks = (int)((n_buckets + kScanBlock - 1) / kScanBlock);
@@ -1363,7 +1383,8 @@ cudaError_t launch_sort(uint64_t first, uint32_t n, uint64_t seed, int g, unsign
 
 cudaError_t launch_tally_read(const TallyBin* bins, uint64_t n_bins, unsigned long long* N, double* p, double* p2,
                               cudaStream_t stream) {
-  cudaError_t e = kernels_init();
+  int g_n_sm = 0;
+  cudaError_t e = sm_count(&g_n_sm);
   if (e != cudaSuccess) return e;
   if (n_bins == 0) return cudaSuccess;
   const uint64_t want = (n_bins + 255) / 256;
@@ -1374,7 +1395,8 @@ cudaError_t launch_tally_read(const TallyBin* bins, uint64_t n_bins, unsigned lo
 
 cudaError_t launch_voxel_relayout(const uint8_t* src, uint8_t* dst, int nx, int ny, int nz, int fast, int a1, int a2,
                                   int pitch, int run_dir, int n_mats, cudaStream_t stream) {
-  cudaError_t e = kernels_init();
+  int g_n_sm = 0;
+  cudaError_t e = sm_count(&g_n_sm);
   if (e != cudaSuccess) return e;
   voxel_relayout_kernel<<<g_n_sm * 8, 256, 0, stream>>>(src, dst, nx, ny, nz, fast, a1, a2, pitch, n_mats);
   const int n[3] = {nx, ny, nz};
@@ -1398,6 +1420,57 @@ __global__ void __launch_bounds__(256) probe_tally_kernel(TallyBin* table, unsig
 
 cudaError_t launch_probe_tally(void* table, unsigned long long n_records, int n_blocks, long long n_iters, cudaStream_t stream) {
   probe_tally_kernel<<<n_blocks, 256, 0, stream>>>(reinterpret_cast<TallyBin*>(table), n_records - 1, n_iters);
+  return cudaGetLastError();
+}
+
+// L2 / L1 sector probe for the roofline of the mesh walk: independent loads of pseudo-random
+// aligned 32-byte sectors (one BVH node) through the read-only path, four in flight per thread.
+__global__ void __launch_bounds__(256) probe_l2_kernel(const uint4* __restrict__ table, unsigned long long sector_mask,
+                                                       uint32_t* __restrict__ sink, long long n_iters) {
+  unsigned long long x = ((unsigned long long)blockIdx.x * blockDim.x + threadIdx.x) * 0x9E3779B97F4A7C15ull + 0x2545F4914F6CDD1Dull;
+  unsigned acc = 0u;
+  for (long long k = 0; k < n_iters; k += 4) {
+    uint4 v[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      x ^= x >> 12; x ^= x << 25; x ^= x >> 27;  // xorshift64*
+      v[u] = __ldg(table + 2 * (((x * 0x2545F4914F6CDD1Dull) >> 24) & sector_mask));
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) acc += v[u].x ^ v[u].w;
+  }
+  sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = acc;
+}
+
+// Dependent-load latency probe: sector i of the table holds the index of the sector to read next (a full-period
+// linear congruential permutation of the n sectors, written by probe_chain_init_kernel).
+__global__ void __launch_bounds__(256) probe_chain_init_kernel(unsigned long long* __restrict__ table, unsigned long long n_sectors) {
+  const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+  for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n_sectors; i += stride)
+    table[4 * i] = (i * 1664525ull + 1013904223ull) & (n_sectors - 1);  // Hull-Dobell: a = 1 mod 4, c odd
+}
+__global__ void __launch_bounds__(256) probe_latency_kernel(const unsigned long long* __restrict__ table, unsigned long long n_sectors,
+                                                            uint32_t* __restrict__ sink, long long n_iters) {
+  unsigned long long i = (((unsigned long long)blockIdx.x * blockDim.x + threadIdx.x) * 0x9E3779B97F4A7C15ull >> 20) & (n_sectors - 1);
+  for (long long k = 0; k < n_iters; ++k) {
+    unsigned long long nxt;
+    asm volatile("ld.global.nc.u64 %0, [%1];" : "=l"(nxt) : "l"(table + 4 * i));
+    i = nxt;
+  }
+  sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = (uint32_t)i;
+}
+
+cudaError_t launch_probe_l2(const void* table, unsigned long long n_bytes, uint32_t* sink, int n_blocks, long long n_iters,
+                            cudaStream_t stream) {
+  probe_l2_kernel<<<n_blocks, 256, 0, stream>>>(reinterpret_cast<const uint4*>(table), n_bytes / 32 - 1, sink, n_iters);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_probe_latency(void* table, unsigned long long n_bytes, uint32_t* sink, int n_blocks, int n_threads,
+                                 long long n_iters, cudaStream_t stream) {
+  const unsigned long long n_sectors = n_bytes / 32;
+  probe_chain_init_kernel<<<1024, 256, 0, stream>>>(reinterpret_cast<unsigned long long*>(table), n_sectors);
+  probe_latency_kernel<<<n_blocks, n_threads, 0, stream>>>(reinterpret_cast<const unsigned long long*>(table), n_sectors, sink, n_iters);
   return cudaGetLastError();
 }
 

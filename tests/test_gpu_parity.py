@@ -18,9 +18,11 @@ def M():
     return m
 
 
-def run_gpu(M, inst, n, first, seed, strict, mode="auto"):
+def run_gpu(M, inst, n, first, seed, strict, mode="auto", tuning=None):
     g = M.Instrument(inst, strict=strict)
     g.set_exec(mode)
+    if tuning:
+        g.set_tuning(**tuning)
     gdump = g.trace_dump(first, n, seed)
     g.trace(n, seed, first)
     gt = [tuple(t.cpu().numpy() for t in g.tally(d)) for d in range(len(g.dets))]
@@ -43,8 +45,8 @@ def check(M, O, W, inst, n, exact_counts=False, first=0, seed=None, mesh_accel=0
     return out[False]
 
 
-def check_one(M, W, inst, n, o, exact_counts, first, seed, strict, mode="auto"):
-    gdump, gt, gc = run_gpu(M, inst, n, first, seed, strict, mode)
+def check_one(M, W, inst, n, o, exact_counts, first, seed, strict, mode="auto", tuning=None):
+    gdump, gt, gc = run_gpu(M, inst, n, first, seed, strict, mode, tuning)
     st = assert_dump_parity(gdump, o["dump"], strict=strict)
     nb = [W.n_bins(d) for d in W.detectors_of(inst)]
     if st["n_diff"] == 0:
@@ -110,25 +112,32 @@ def test_c4_voxels(M, O, W):
     check(M, O, W, W.config4(small=True, n_vox=96), 30_000)
 
 
-def test_sorted_order_is_a_permutation_over_several_chunks(M, O, W, monkeypatch):
+def test_sorted_order_is_a_permutation_over_several_chunks(M, O, W):
     """Detector-tile order with chunks of 2^15 rays: 100 003 rays = three full chunks + a ragged one that is still
     sorted + (in the second case) a tail short enough to be traced in index order.  Every ray must be traced exactly
     once: the dump equals the oracle's ray by ray and the tallies equal the sums of the dump."""
-    monkeypatch.setenv("MCX_CHUNK_LOG2", "15")
+    tuning = {"chunk_log2": 15}
     inst = W.config1(small=True)
     for n in (100_003, 3 * 32768 + 1000):
         o = O.trace(inst, first=7, n=n, dump=True)
-        check_one(M, W, inst, n, o, False, 7, inst["seed"], True, "sorted")
+        check_one(M, W, inst, n, o, False, 7, inst["seed"], True, "sorted", tuning)
     inst = W.config0()
     o = O.trace(inst, first=0, n=200_000, dump=True)
-    st = check_one(M, W, inst, 200_000, o, True, 0, inst["seed"], False, "sorted")
+    st = check_one(M, W, inst, 200_000, o, True, 0, inst["seed"], False, "sorted", tuning)
     assert st["n_diff"] == 0
+    # a forced bucket grid and the absorber gate switched off: the same rays again
+    check_one(M, W, inst, 200_000, o, True, 0, inst["seed"], False, "sorted", {"chunk_log2": 16, "sort_grid_bits": 3, "absorber_gate": 2})
 
 
-def test_exec_mode_argument_is_checked(M, W):
+def test_exec_mode_and_tuning_arguments_are_checked(M, W):
     g = M.Instrument(W.config0())
     with pytest.raises(M.McxError):
         M.binding._check(g.L.mcx_instrument_set_exec(g.handle, 7), g.L)
+    for bad in ({"chunk_log2": 13}, {"chunk_log2": 27}, {"sort_grid_bits": 12}, {"absorber_gate": 3}):
+        with pytest.raises(M.McxError):
+            g.set_tuning(**bad)
+    g.set_tuning()                                                              # all zeros: nothing changes
+    g.status()
     g.close()
 
 
