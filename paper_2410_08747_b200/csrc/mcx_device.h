@@ -58,8 +58,10 @@ struct DSolid {
   int shape, material, priority, depth;  // depth: D of a mesh's BVH
   DPose pose;
   double dims[3];
-  double bound2;                  // primitives: (radius of the bounding sphere about the solid's origin, plus 1e-9)^2
-  double root_lo[3], root_hi[3];  // fp64 AABB of the mesh (solid-local)
+  double bound2;                  // primitives: (radius of the bounding sphere about the solid's origin, plus 1e-9)^2;
+                                  // meshes: the beam limit of the warp-cooperative walk (a length)
+  double ctr[3], radius;          // meshes: bounding sphere of the mesh's (padded) box, solid-local
+  double unused[2];
   const BvhNode* nodes;
   const double* tris;  // [2^D][9] vertices by leaf number (zeros where a leaf holds no triangle)
 };
@@ -143,7 +145,7 @@ static_assert(sizeof(DInstrument) % 16 == 0, "copied to shared memory as int4");
 static_assert(sizeof(TallyBin) == 32, "one tally record per 32-byte sector");
 
 // feature bits: select the kernel instantiation (code for absent component kinds is compiled out)
-enum { F_SOLIDS = 1, F_MESH = 2, F_VOXELS = 4, F_OPTICS = 8, F_ALL = 15 };
+enum { F_SOLIDS = 1, F_MESH = 2, F_VOXELS = 4, F_OPTICS = 8, F_PRIM = 16, F_ALL = 31 };  // F_SOLIDS: a solids group; F_PRIM / F_MESH: what it holds
 
 // One trace launch: rays first + offset(q) for positions q in [0, n); offset(q) = order[q] if order != null, else q.
 struct TraceArgs {

@@ -508,7 +508,7 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
                             : S.shape == MCX_SPHERE ? S.dims[0] * S.dims[0] : S.dims[0] * S.dims[0] + S.dims[1] * S.dims[1];
             d.bound2 = r2 * (1.0 + 2e-9);
           }
-          if (S.shape != MCX_MESH) continue;
+          if (S.shape != MCX_MESH) { features |= F_PRIM; continue; }
           features |= F_MESH;
           D.u.solids.n_mesh++;
           if (!S.vertices || !S.triangles) MCX_BAIL(MCX_ERR_INVALID_ARG, "component %d solid %d: null mesh arrays", c, (int)s);
@@ -544,7 +544,25 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
               for (int v = 0; v < 3; ++v)
                 for (int a = 0; a < 3; ++a)
                   tri[9 * leaf + 3 * v + a] = S.vertices[3 * (size_t)S.triangles[3 * (size_t)leaf_tri[leaf] + v] + a];
-          for (int a = 0; a < 3; ++a) { d.root_lo[a] = lo[a] - pad; d.root_hi[a] = hi[a] + pad; }
+          {  // bounding sphere of the padded box (participation test and parameter range of the mesh walk)
+            double r2 = 0.0;
+            for (int a = 0; a < 3; ++a) {
+              d.ctr[a] = 0.5 * (lo[a] + hi[a]);
+              const double half = 0.5 * (hi[a] - lo[a]) + pad;
+              r2 += half * half;
+            }
+            d.radius = std::sqrt(r2) * (1.0 + 1e-12);
+          }
+          {  // beam limit of the warp-cooperative walk (mesh_endpoints_beam): the rays of a warp may lie apart by up to
+             // half the mean extent of a triangle's box; wider beams collect too many candidates to pay
+            double sum = 0.0;
+            for (int t = 0; t < nt; ++t) {
+              double ext = 0.0;
+              for (int a = 0; a < 3; ++a) ext = std::max(ext, refs[t].hi[a] - refs[t].lo[a]);
+              sum += ext;
+            }
+            d.bound2 = 0.5 * sum / (double)nt;
+          }
           d.depth = bvh_depth(nt);
           d.nodes = (const BvhNode*)dev_ptr(P.off_nodes[c][s]);
           d.tris = (const double*)dev_ptr(P.off_tris[c][s]);

@@ -206,15 +206,7 @@ __device__ __forceinline__ double mu_of(const DMaterial& M, double E, double lnE
 // ------------------------------------------------------------------------------------------------------------
 // Step 8: inside-interval of the ray parameter for the convex primitives, in the solid's own frame.
 // ------------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ bool clip_axis(double o, double d, double lo, double hi, double& tmin, double& tmax) {
-  if (d == 0.0) return o > lo && o < hi;
-  const double ta = (lo - o) / d, tb = (hi - o) / d;
-  tmin = fmax(tmin, fmin(ta, tb));
-  tmax = fmin(tmax, fmax(ta, tb));
-  return true;
-}
-
-// the same with 1/d supplied (one division per axis and solid instead of two; one more rounding per plane)
+// slab of one axis with 1/d supplied (one division per axis and solid instead of two; one more rounding per plane)
 __device__ __forceinline__ bool clip_axis_inv(double o, double d, double inv, double lo, double hi, double& tmin, double& tmax) {
   if (d == 0.0) return o > lo && o < hi;
   const double ta = (lo - o) * inv, tb = (hi - o) * inv;
@@ -266,11 +258,12 @@ __device__ __forceinline__ bool primitive_interval(const DSolid& S, Vec3 o, Vec3
 struct Shear {
   int kx, ky, kz;
   double Sx, Sy, Sz;
+  double ox, oy, oz;  // the ray origin's components kx, ky, kz
 };
 
 __device__ __forceinline__ double pick(Vec3 v, int k) { return k == 0 ? v.x : (k == 1 ? v.y : v.z); }
 
-__device__ __forceinline__ Shear make_shear(Vec3 d, Vec3 inv_d) {
+__device__ __forceinline__ Shear make_shear(Vec3 o, Vec3 d) {
   Shear s;
   s.kz = 0;
   double m = fabs(d.x);
@@ -282,21 +275,22 @@ __device__ __forceinline__ Shear make_shear(Vec3 d, Vec3 inv_d) {
   if (dz < 0.0) { const int t = s.kx; s.kx = s.ky; s.ky = t; }
   // the same constants serve every triangle of the ray, which is all watertightness needs; as products with 1/d_kz
   // they are within an ulp of the quotients
-  s.Sz = pick(inv_d, s.kz);
+  s.Sz = 1.0 / dz;
   s.Sx = pick(d, s.kx) * s.Sz;
   s.Sy = pick(d, s.ky) * s.Sz;
+  s.ox = pick(o, s.kx); s.oy = pick(o, s.ky); s.oz = pick(o, s.kz);
   return s;
 }
 
-// returns 0 = miss, +1 = entering, -1 = exiting
-__device__ __forceinline__ int ray_triangle(const Shear& s, Vec3 o, const double* __restrict__ tri, double& t_out) {
-  const Vec3 A{tri[0] - o.x, tri[1] - o.y, tri[2] - o.z};
-  const Vec3 B{tri[3] - o.x, tri[4] - o.y, tri[5] - o.z};
-  const Vec3 C{tri[6] - o.x, tri[7] - o.y, tri[8] - o.z};
-  const double Akz = pick(A, s.kz), Bkz = pick(B, s.kz), Ckz = pick(C, s.kz);
-  const double Ax = __dsub_rn(pick(A, s.kx), __dmul_rn(s.Sx, Akz)), Ay = __dsub_rn(pick(A, s.ky), __dmul_rn(s.Sy, Akz));
-  const double Bx = __dsub_rn(pick(B, s.kx), __dmul_rn(s.Sx, Bkz)), By = __dsub_rn(pick(B, s.ky), __dmul_rn(s.Sy, Bkz));
-  const double Cx = __dsub_rn(pick(C, s.kx), __dmul_rn(s.Sx, Ckz)), Cy = __dsub_rn(pick(C, s.ky), __dmul_rn(s.Sy, Ckz));
+// returns 0 = miss, +1 = entering, -1 = exiting.  The vertex components are fetched in the ray's own axis order
+// (kx, ky, kz), which saves permuting them in registers.
+__device__ __forceinline__ int ray_triangle(const Shear& s, const double* __restrict__ tri, double& t_out) {
+  const double Akx = tri[s.kx] - s.ox, Aky = tri[s.ky] - s.oy, Akz = tri[s.kz] - s.oz;
+  const double Bkx = tri[3 + s.kx] - s.ox, Bky = tri[3 + s.ky] - s.oy, Bkz = tri[3 + s.kz] - s.oz;
+  const double Ckx = tri[6 + s.kx] - s.ox, Cky = tri[6 + s.ky] - s.oy, Ckz = tri[6 + s.kz] - s.oz;
+  const double Ax = __dsub_rn(Akx, __dmul_rn(s.Sx, Akz)), Ay = __dsub_rn(Aky, __dmul_rn(s.Sy, Akz));
+  const double Bx = __dsub_rn(Bkx, __dmul_rn(s.Sx, Bkz)), By = __dsub_rn(Bky, __dmul_rn(s.Sy, Bkz));
+  const double Cx = __dsub_rn(Ckx, __dmul_rn(s.Sx, Ckz)), Cy = __dsub_rn(Cky, __dmul_rn(s.Sy, Ckz));
   const double U = __dsub_rn(__dmul_rn(Cx, By), __dmul_rn(Cy, Bx));
   const double V = __dsub_rn(__dmul_rn(Ax, Cy), __dmul_rn(Ay, Cx));
   const double W = __dsub_rn(__dmul_rn(Bx, Ay), __dmul_rn(By, Ax));
@@ -349,88 +343,10 @@ __device__ __forceinline__ void ep_sort(const Endpoints& E, int begin, int end, 
   }
 }
 
-// All crossings of the full line with one mesh, appended to E as sorted, duplicate-collapsed, paired end points clipped
-// to t >= 0.  The BVH is walked without a stack (complete tree in heap order + a bit trail; any order will do since every hit is wanted);
-// leaves only queue their triangles, and the exact tests run over the queue afterwards, so that the lanes of a warp
-// do box tests together and triangle tests together instead of waiting for one another at every leaf.
-// Returns 1 = ok, 0 = degenerate sequence, -1 = capacity overflow.
-__device__ __forceinline__ int mesh_endpoints(const DSolid& S, unsigned solid, Vec3 o, Vec3 d, const Endpoints& E, int& ne,
-                                              unsigned* __restrict__ queue) {
-  // clip the line to the mesh box in fp64; the fp32 box walk uses a ray re-origined at the box entry so that
-  // its rounding errors scale with the mesh size, not with the distance to the source
-  const Vec3 inv_d{1.0 / d.x, 1.0 / d.y, 1.0 / d.z};  // the only divisions of the set-up (+-inf where d = 0: unused)
-  double tmin = -CUDART_INF, tmax = CUDART_INF;
-  if (!clip_axis_inv(o.x, d.x, inv_d.x, S.root_lo[0], S.root_hi[0], tmin, tmax)) return 1;
-  if (!clip_axis_inv(o.y, d.y, inv_d.y, S.root_lo[1], S.root_hi[1], tmin, tmax)) return 1;
-  if (!clip_axis_inv(o.z, d.z, inv_d.z, S.root_lo[2], S.root_hi[2], tmin, tmax)) return 1;
-  if (!(tmin < tmax)) return 1;
-  const Vec3 e = o + tmin * d;
-  const float ox = (float)e.x, oy = (float)e.y, oz = (float)e.z;
-  // 1/d, held to +-1e30 so that the products below stay finite (a ray parallel to a pair of planes gets huge
-  // parameters of the right signs instead of infinities)
-  const float big = 1.0e30f;
-  const float ix = d.x != 0.0 ? fminf(fmaxf((float)inv_d.x, -big), big) : big;
-  const float iy = d.y != 0.0 ? fminf(fmaxf((float)inv_d.y, -big), big) : big;
-  const float iz = d.z != 0.0 ? fminf(fmaxf((float)inv_d.z, -big), big) : big;
-  // (x - o) / d as one fused multiply-add per plane: x * (1/d) + (-o/d).  Its rounding error is below 2^-22 of the
-  // mesh scale times |1/d|, the boxes are padded by 2^-16 of the scale (times |1/d| in t): the test stays conservative.
-  const float bx = -ox * ix, by = -oy * iy, bz = -oz * iz;
-  const Shear sh = make_shear(d, inv_d);
-  const int begin = ne, depth = S.depth, leaf_base = (1 << depth) - 1;
-  const float4* __restrict__ nodes = reinterpret_cast<const float4*>(S.nodes);
-  const double* __restrict__ tris = S.tris;
-  bool overflow = false;
-  // Walk of the complete tree (BvhNode): at node i of `level`, already known to be hit, both children are tested at
-  // once (one 64-byte line); bit `level` of `trail` says the right child was hit too and waits while the left
-  // subtree is walked.  Going back up needs no memory: the ancestor of i at level m is ((i + 1) >> (level - m)) - 1.
-  int i = 0, level = 0;
-  unsigned trail = 0u;
-  bool walking = true;
-  auto next_pending = [&]() {  // to the deepest right sibling still to be visited, or done
-    if (trail == 0u) { walking = false; return; }
-    const int l = 31 - __clz(trail);
-    trail ^= 1u << l;
-    i = ((i + 1) >> (level - (l + 1)));  // = (left child at level l + 1) + 1 = its right sibling
-    level = l + 1;
-  };
-  do {
-    int nq = 0;
-    while (walking && nq < kTriQueue) {
-      if (level == depth) {  // a leaf whose box the line hits: queue its triangle
-        queue[nq * kBlock] = (unsigned)(i - leaf_base);
-        ++nq;
-        next_pending();
-        continue;
-      }
-      const float4* pair = nodes + 2 * (2 * i + 2);  // children 2i+1, 2i+2 sit in slots 2i+2, 2i+3
-      const float4 a0 = __ldg(pair), b0 = __ldg(pair + 1), a1 = __ldg(pair + 2), b1 = __ldg(pair + 3);
-      // slab tests of the full line against the padded fp32 boxes (no t range: the line is tested, as in step 9)
-      const float x00 = fmaf(a0.x, ix, bx), x01 = fmaf(b0.x, ix, bx), x10 = fmaf(a1.x, ix, bx), x11 = fmaf(b1.x, ix, bx);
-      const float y00 = fmaf(a0.y, iy, by), y01 = fmaf(b0.y, iy, by), y10 = fmaf(a1.y, iy, by), y11 = fmaf(b1.y, iy, by);
-      const float z00 = fmaf(a0.z, iz, bz), z01 = fmaf(b0.z, iz, bz), z10 = fmaf(a1.z, iz, bz), z11 = fmaf(b1.z, iz, bz);
-      const float n0 = fmaxf(fmaxf(fminf(x00, x01), fminf(y00, y01)), fminf(z00, z01));
-      const float f0 = fminf(fminf(fmaxf(x00, x01), fmaxf(y00, y01)), fmaxf(z00, z01));
-      const float n1 = fmaxf(fmaxf(fminf(x10, x11), fminf(y10, y11)), fminf(z10, z11));
-      const float f1 = fminf(fminf(fmaxf(x10, x11), fmaxf(y10, y11)), fmaxf(z10, z11));
-      const bool hit0 = n0 <= f0 && __float_as_int(a0.w) != 0, hit1 = n1 <= f1 && __float_as_int(a1.w) != 0;
-      if (hit0) {
-        if (hit1) trail |= 1u << level;
-        i = 2 * i + 1;
-        ++level;
-      } else if (hit1) {
-        i = 2 * i + 2;
-        ++level;
-      } else {
-        next_pending();
-      }
-    }
-    for (int k = 0; k < nq; ++k) {
-      double t;
-      const int r = ray_triangle(sh, o, tris + 9 * (size_t)queue[k * kBlock], t);
-      if (r != 0 && !ep_push(E, ne, t, solid | (r < 0 ? kTagExit : 0u))) overflow = true;
-    }
-  } while (walking);
-  if (overflow) return -1;
+// Step 9, second half, on the raw hits E[begin, ne) of one mesh: sort by t (enter before exit on ties), collapse
+// consecutive same-orientation hits (shared-edge / vertex duplicates), check the enter / exit alternation, clip to t >= 0.
+// Returns 1 = ok, 0 = degenerate sequence.
+__device__ __forceinline__ int mesh_finish(const Endpoints& E, int begin, int& ne, unsigned solid) {
   if (ne == begin) return 1;
   ep_sort(E, begin, ne, true);
   // collapse consecutive same-orientation hits (shared-edge duplicates); what is left must alternate enter, exit, ...
@@ -458,14 +374,240 @@ __device__ __forceinline__ int mesh_endpoints(const DSolid& S, unsigned solid, V
   return 1;
 }
 
+
+// ------------------------------------------------------------------------------------------------------------
+// Step 9 for one mesh and one WARP of rays: all crossings of every lane's full line with the mesh, appended to the lane's
+// end-point list as sorted, duplicate-collapsed, paired end points clipped to t >= 0.  Must be called by all 32 lanes
+// (`active` = this lane has a live ray).  Returns per lane 1 = ok, 0 = degenerate sequence, -1 = capacity overflow, or,
+// for the whole warp, 2 = the beam walk met more nodes than its stack holds, nothing was appended: call again with
+// coherent = false.
+//
+// The BVH (a complete binary tree in heap order, BvhNode) only yields CANDIDATE triangles; the exact fp64 watertight
+// test of the lane's own ray decides, so a lane's hit set is what brute force gives it.  Two walks produce candidates:
+//
+//  beam walk (coherent warps: detector-tile order, where a warp's rays are aimed at one spot, far
+//    closer together than a triangle is wide).  The warp walks ONE beam instead of 32 lines: the line of its first
+//    participating lane (the leader), with every node box inflated by delta = the largest distance, per axis, of any
+//    participating lane's line from the leader's at equal parameter inside the mesh's bounding sphere.  If lane l's
+//    line meets a node box at parameter t, the leader's point at t lies within delta of that point, i.e. inside the
+//    inflated box: the leader's line meets every inflated box whose original any lane's line meets, so the candidate set
+//    is a superset of every lane's.  A step expands one pending node by up to five levels at once -- lane l tests
+//    descendant l, 32 boxes of 32 bytes read as one coalesced kilobyte -- so a root-to-leaf path of c3's depth-17 tree
+//    is 4 dependent loads instead of 17, and the node sectors are read once per warp instead of once per lane (c3 is
+//    bound by L2 sector traffic and dependent-load latency, profiles/r02_README.md).  Hit descendants go on a stack
+//    (inner nodes) or the candidate list (leaves), both warp-shared;
+//
+//  lane walk (any warp; also where the beam is too wide to pay, or its stack would overflow).  Every lane walks its
+//    own line: at node i of `level`, already known to be hit, both children are tested at once (one 64-byte line); bit
+//    `level` of `trail` says the right child was hit too and waits while the left subtree is walked; going back up
+//    needs no memory (the ancestor of i at level m is ((i + 1) >> (level - m)) - 1).  Leaves go into the lane's queue.
+//
+// Both use the warp's triangle-queue words in shared memory (kTriQueue words per thread): the lane walk as per-lane
+// queues, the beam walk as warp-shared lists.  The exact tests, the sort and the pairing exist once, behind both.
+// ------------------------------------------------------------------------------------------------------------
+constexpr int kBeamStack = 64, kBeamCand = 64;  // warp-shared words: rows 0-1 and rows 2-3 of the warp's triangle queues
+static_assert(kBeamStack + kBeamCand <= 32 * kTriQueue, "the beam lists live in the warp's triangle-queue words");
+
+__device__ __forceinline__ int mesh_endpoints_warp(const DSolid& S, unsigned solid, bool active, Vec3 o, Vec3 d, const Endpoints& E,
+                                                   int& ne, unsigned* __restrict__ queue, bool coherent) {
+  const unsigned full = 0xffffffffu;
+  const int lane = threadIdx.x & 31;
+  unsigned* __restrict__ wq = queue - lane;  // word j of the warp's list space at wq[(j >> 5) * kBlock + (j & 31)]
+#define MCX_WQ(j) wq[((j) >> 5) * kBlock + ((j) & 31)]
+  // Does this lane's line pass the mesh at all?  Bounding sphere of the mesh box (DSolid::ctr, radius): the line's closest approach to the centre is at parameter tc.
+  const Vec3 ctr{S.ctr[0], S.ctr[1], S.ctr[2]};
+  const double rad = S.radius;
+  const double tc = dot(ctr - o, d);
+  bool part = false;
+  if (active) {
+    const Vec3 q = (o + tc * d) - ctr;
+    part = dot(q, q) <= rad * rad;
+  }
+  const unsigned pmask = __ballot_sync(full, part);
+  if (pmask == 0u) return 1;
+  const int leader = __ffs(pmask) - 1;
+  bool beam = coherent;
+  float ex = 0.0f, ey = 0.0f, ez = 0.0f;
+  if (beam) {
+    // delta per axis: |p_l(t) - p_0(t)| is convex in t, so its maximum over the lane's stretch [tc - rad, tc + rad]
+    // inside the sphere is at an end
+    const Vec3 lo{__shfl_sync(full, o.x, leader), __shfl_sync(full, o.y, leader), __shfl_sync(full, o.z, leader)};
+    const Vec3 ld{__shfl_sync(full, d.x, leader), __shfl_sync(full, d.y, leader), __shfl_sync(full, d.z, leader)};
+    if (part) {
+      const double ta = tc - rad, tb = tc + rad;
+      const Vec3 a = (o + ta * d) - (lo + ta * ld), b = (o + tb * d) - (lo + tb * ld);
+      ex = __double2float_ru(fmax(fabs(a.x), fabs(b.x)));
+      ey = __double2float_ru(fmax(fabs(a.y), fabs(b.y)));
+      ez = __double2float_ru(fmax(fabs(a.z), fabs(b.z)));
+    }
+    // non-negative floats order like their bit patterns
+    ex = __uint_as_float(__reduce_max_sync(full, __float_as_uint(ex)));
+    ey = __uint_as_float(__reduce_max_sync(full, __float_as_uint(ey)));
+    ez = __uint_as_float(__reduce_max_sync(full, __float_as_uint(ez)));
+    beam = fmaxf(fmaxf(ex, ey), ez) <= (float)S.bound2;  // (bound2 of a mesh = its beam limit)
+    // the deviations were rounded up; 2^-20 of them more covers the roundings of the folded constants below
+    ex *= 1.000001f; ey *= 1.000001f; ez *= 1.000001f;
+  }
+  if (!beam) ex = ey = ez = 0.0f;  // the lane walk tests the boxes as they are
+  const Shear sh = make_shear(o, d);
+  const int begin = ne, depth = S.depth, leaf_base = (1 << depth) - 1;
+  const int k_first = depth - 5 * ((depth - 1) / 5);  // levels of the beam's first step, 1..5 (the others take 5)
+  const float4* __restrict__ nodes = reinterpret_cast<const float4*>(S.nodes);
+  const double* __restrict__ tris = S.tris;
+  bool overflow = false;
+  {
+    // The line the boxes are tested against -- the leader's (beam walk) or the lane's own -- in fp32, re-origined just
+    // before the mesh so that rounding errors scale with the mesh size, not with the distance to the source.
+    const int src = beam ? leader : lane;
+    const Vec3 so{__shfl_sync(full, o.x, src), __shfl_sync(full, o.y, src), __shfl_sync(full, o.z, src)};
+    const Vec3 sd{__shfl_sync(full, d.x, src), __shfl_sync(full, d.y, src), __shfl_sync(full, d.z, src)};
+    const Vec3 le = so + (__shfl_sync(full, tc, src) - rad) * sd;
+    // 1/d in fp32, held to +-1e30 so that the products below stay finite (a line parallel to a pair of planes gets huge
+    // parameters of the right signs instead of infinities)
+    const float big = 1.0e30f;
+    const float ix = sd.x != 0.0 ? fminf(fmaxf(1.0f / (float)sd.x, -big), big) : big;
+    const float iy = sd.y != 0.0 ? fminf(fmaxf(1.0f / (float)sd.y, -big), big) : big;
+    const float iz = sd.z != 0.0 ? fminf(fmaxf(1.0f / (float)sd.z, -big), big) : big;
+    // (x -+ e - o) / d as one fused multiply-add per plane: x * (1/d) + (-o/d -+ e/d).  Its rounding error is below
+    // 2^-21 of the mesh scale times |1/d| (1/d itself is within 2^-22 of the exact reciprocal), the boxes are padded by
+    // 2^-16 of the scale (times |1/d| in t): the test stays conservative.
+    const float bx = -(float)le.x * ix, by = -(float)le.y * iy, bz = -(float)le.z * iz;
+    const float bxl = bx - ex * ix, bxh = bx + ex * ix, byl = by - ey * iy, byh = by + ey * iy, bzl = bz - ez * iz, bzh = bz + ez * iz;
+    // beam walk state (warp-uniform)
+    int sn = 0, cn = 0, node = 0;
+    bool walking_w = depth > 0;
+    if (beam && depth == 0) {  // a single triangle
+      if (lane == 0) MCX_WQ(kBeamStack) = 0u;
+      __syncwarp();
+      cn = 1;
+    }
+    // lane walk state
+    int i = 0, level = 0;
+    unsigned trail = 0u;
+    bool walking_l = part;
+    for (;;) {
+      int n_c = 0;  // candidates this lane tests in this round
+      if (beam) {
+        while (walking_w) {
+          const int lv = 31 - __clz(node + 1), k = lv == 0 ? k_first : 5;
+          const bool leaf_step = lv + k == depth;
+          if (leaf_step && cn > kBeamCand - 32) break;  // make room in the candidate list first
+          const int child = ((node + 1) << k) - 1 + lane;
+          bool hit = false;
+          if (lane < (1 << k)) {
+            const float4 a = __ldg(nodes + 2 * (child + 1)), b = __ldg(nodes + 2 * (child + 1) + 1);
+            const float x0 = fmaf(a.x, ix, bxl), x1 = fmaf(b.x, ix, bxh);
+            const float y0 = fmaf(a.y, iy, byl), y1 = fmaf(b.y, iy, byh);
+            const float z0 = fmaf(a.z, iz, bzl), z1 = fmaf(b.z, iz, bzh);
+            const float n0 = fmaxf(fmaxf(fminf(x0, x1), fminf(y0, y1)), fminf(z0, z1));
+            const float f0 = fminf(fminf(fmaxf(x0, x1), fmaxf(y0, y1)), fmaxf(z0, z1));
+            hit = n0 <= f0 && __float_as_int(a.w) != 0;
+          }
+          const unsigned hits = __ballot_sync(full, hit);
+          if (hits) {
+            const int nh = __popc(hits), rank = __popc(hits & ((1u << lane) - 1u));
+            if (leaf_step) {
+              if (hit) MCX_WQ(kBeamStack + cn + rank) = (unsigned)(child - leaf_base);
+              cn += nh;
+            } else {
+              if (sn + nh > kBeamStack) { ne = begin; return 2; }  // (warp-uniform)
+              if (hit) MCX_WQ(sn + rank) = (unsigned)child;
+              sn += nh;
+            }
+            __syncwarp();
+          }
+          if (sn == 0) { walking_w = false; break; }
+          node = (int)MCX_WQ(sn - 1);
+          --sn;
+        }
+        n_c = cn;
+      } else {
+        while (walking_l && n_c < kTriQueue) {
+          if (level == depth) {  // a leaf whose box the line hits: queue its triangle
+            queue[n_c * kBlock] = (unsigned)(i - leaf_base);
+            ++n_c;
+          } else {
+            const float4* pair = nodes + 2 * (2 * i + 2);  // children 2i+1, 2i+2 sit in slots 2i+2, 2i+3
+            const float4 a0 = __ldg(pair), b0 = __ldg(pair + 1), a1 = __ldg(pair + 2), b1 = __ldg(pair + 3);
+            // slab tests of the full line against the padded fp32 boxes (no t range: the line is tested, as in step 9)
+            // (bxl = bxh here: no inflation)
+            const float x00 = fmaf(a0.x, ix, bxl), x01 = fmaf(b0.x, ix, bxh), x10 = fmaf(a1.x, ix, bxl), x11 = fmaf(b1.x, ix, bxh);
+            const float y00 = fmaf(a0.y, iy, byl), y01 = fmaf(b0.y, iy, byh), y10 = fmaf(a1.y, iy, byl), y11 = fmaf(b1.y, iy, byh);
+            const float z00 = fmaf(a0.z, iz, bzl), z01 = fmaf(b0.z, iz, bzh), z10 = fmaf(a1.z, iz, bzl), z11 = fmaf(b1.z, iz, bzh);
+            const float n0 = fmaxf(fmaxf(fminf(x00, x01), fminf(y00, y01)), fminf(z00, z01));
+            const float f0 = fminf(fminf(fmaxf(x00, x01), fmaxf(y00, y01)), fmaxf(z00, z01));
+            const float n1 = fmaxf(fmaxf(fminf(x10, x11), fminf(y10, y11)), fminf(z10, z11));
+            const float f1 = fminf(fminf(fmaxf(x10, x11), fmaxf(y10, y11)), fmaxf(z10, z11));
+            const bool hit0 = n0 <= f0 && __float_as_int(a0.w) != 0, hit1 = n1 <= f1 && __float_as_int(a1.w) != 0;
+            if (hit0) {
+              if (hit1) trail |= 1u << level;
+              i = 2 * i + 1;
+              ++level;
+              continue;
+            }
+            if (hit1) {
+              i = 2 * i + 2;
+              ++level;
+              continue;
+            }
+          }
+          // to the deepest right sibling still to be visited, or done
+          if (trail == 0u) { walking_l = false; break; }
+          const int l = 31 - __clz(trail);
+          trail ^= 1u << l;
+          i = ((i + 1) >> (level - (l + 1)));  // = (left child at level l + 1) + 1 = its right sibling
+          level = l + 1;
+        }
+      }
+      // the exact test of the lane's own ray on the candidates (beam walk: the warp's list, uniform loads)
+      for (int k = 0; k < n_c; ++k) {
+        const unsigned leaf = beam ? MCX_WQ(kBeamStack + k) : queue[k * kBlock];
+        if (part) {
+          double t;
+          const int r = ray_triangle(sh, tris + 9 * (size_t)leaf, t);
+          if (r != 0 && !ep_push(E, ne, t, solid | (r < 0 ? kTagExit : 0u))) overflow = true;
+        }
+      }
+      if (beam) {
+        __syncwarp();
+        cn = 0;
+        if (!walking_w) break;
+      } else if (!walking_l) {
+        break;
+      }
+    }
+  }
+#undef MCX_WQ
+  __syncwarp();
+  if (overflow) return -1;
+  if (!part) return 1;
+  return mesh_finish(E, begin, ne, solid);
+}
+
 // Steps 8-10 for one solids group.  Returns 1 = continue, 0 = degenerate, -1 = capacity overflow.
-template <bool MESH>
+// With meshes (MESH) the function must be called by all 32 lanes of the warp, `active` saying which have a live ray;
+// `coherent` = the warp's rays are neighbours (detector-tile order), so the beam walk of the meshes is tried first.
+// PRIM = some group of the instrument holds a box, cylinder or sphere.
+template <bool MESH, bool PRIM>
 __device__ __forceinline__ int trace_solids(const DInstrument& I, const DComponent& C, Ray& ray, const Endpoints& E,
-                                            unsigned* __restrict__ queue) {
+                                            unsigned* __restrict__ queue, bool active, bool coherent) {
   const DSolids& G = C.u.solids;
-  int ne = 0;
+  int ne = 0, status = 1;
   for (int s = 0; s < G.n_solids; ++s) {
     const DSolid& S = G.solids[s];
+    if (MESH && S.shape == MCX_MESH) {  // warp-uniform branch
+      const bool act = active && status == 1;
+      int rc;
+      for (bool coh = coherent;; coh = false) {  // (a second round only if the beam walk gives up: rc 2, warp-uniform)
+        Vec3 o{0.0, 0.0, 0.0}, d{0.0, 0.0, 1.0};
+        if (act) { o = to_local(S.pose, ray.r); d = rotate(S.pose.R, ray.d); }
+        rc = mesh_endpoints_warp(S, (unsigned)s, act, o, d, E, ne, queue, coh);
+        if (rc != 2) break;
+      }
+      if (act && rc != 1) status = rc;
+      continue;
+    }
+    if (!PRIM || !(active && status == 1)) continue;
     if (!MESH) {  // (the mesh kernels run at the register limit and do without)
       // the line misses the solid's bounding sphere, by more than the rounding of this test (1e-9 of the radius^2 in
       // bound2, 1e-14 of the squared distance for the cancellation): no interval, no need for the solid's frame
@@ -475,20 +617,16 @@ __device__ __forceinline__ int trace_solids(const DInstrument& I, const DCompone
     }
     const Vec3 o = to_local(S.pose, ray.r);
     const Vec3 d = rotate(S.pose.R, ray.d);
-    if (MESH && S.shape == MCX_MESH) {
-      const int rc = mesh_endpoints(S, (unsigned)s, o, d, E, ne, queue);
-      if (rc != 1) return rc;
-    } else {
-      double a, b;
-      if (primitive_interval(S, o, d, a, b)) {  // clip to t >= 0, drop if empty
-        a = fmax(a, 0.0);
-        if (b > a) {
-          if (!ep_push(E, ne, a, (unsigned)s)) return -1;
-          if (!ep_push(E, ne, b, (unsigned)s | kTagExit)) return -1;
-        }
+    double a, b;
+    if (primitive_interval(S, o, d, a, b)) {  // clip to t >= 0, drop if empty
+      a = fmax(a, 0.0);
+      if (b > a) {
+        if (!ep_push(E, ne, a, (unsigned)s)) status = -1;
+        if (!ep_push(E, ne, b, (unsigned)s | kTagExit)) status = -1;
       }
     }
   }
+  if (!active || status != 1) return status;
   if (ne == 0) return 1;
   // Step 10.  Between two consecutive end points the set of solids the ray is inside of is constant, so sweeping the
   // sorted end points with that set as a bit mask classifies every elementary segment exactly as its midpoint would;
@@ -957,7 +1095,9 @@ constexpr unsigned kTileMax = 8192;  // positions per work ticket (a power of tw
 constexpr int kSmemSolids = 32;    // solids staged in shared memory (all groups together)
 
 // resident blocks per SM the register budget is held to: the voxel walk hides its byte loads with warps
-constexpr int min_blocks(int feat) { return feat == F_VOXELS || feat == F_SOLIDS || feat == (F_SOLIDS | F_MESH) ? 3 : 1; }
+constexpr int min_blocks(int feat) {
+  return feat == F_VOXELS || feat == (F_SOLIDS | F_PRIM) || feat == (F_SOLIDS | F_MESH) || feat == (F_SOLIDS | F_MESH | F_PRIM) ? 3 : 1;
+}
 
 template <int FEAT, bool DUMP, bool GATE>
 __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const DInstrument* __restrict__ g_inst, TraceArgs A) {
@@ -1050,20 +1190,20 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
       const DComponent& C = I.comps[c];
       const int kind = C.kind;  // warp-uniform
       bool pass = true;
-      if (alive) {
+      if ((FEAT & F_SOLIDS) && kind == MCX_SOLIDS) {  // whole warp: the mesh walk is warp-cooperative
+        const int rc = trace_solids<(FEAT & F_MESH) != 0, (FEAT & F_PRIM) != 0>(I, C, ray, ep, tri_queue, alive, order != nullptr);
+        if (alive && rc != 1) {
+          pass = false;
+          fate = MCX_FATE_DEGENERATE;
+          if (rc < 0 && !DUMP) atomicAdd(&s_cnt[MCX_MAX_COMPONENTS + CNT_OVERFLOW], 1u);
+        }
+      } else if (alive) {
         if (kind == MCX_SLIT_RECT) {
           Vec3 h;
           pass = plane_hit(C.pose, ray, h) && fabs(h.x) <= C.u.slit.half_x && fabs(h.y) <= C.u.slit.half_y;
         } else if (kind == MCX_SLIT_CIRC) {
           Vec3 h;
           pass = plane_hit(C.pose, ray, h) && h.x * h.x + h.y * h.y <= C.u.slit.radius2;
-        } else if ((FEAT & F_SOLIDS) && kind == MCX_SOLIDS) {
-          const int rc = trace_solids<(FEAT & F_MESH) != 0>(I, C, ray, ep, tri_queue);
-          if (rc != 1) {
-            pass = false;
-            fate = MCX_FATE_DEGENERATE;
-            if (rc < 0 && !DUMP) atomicAdd(&s_cnt[MCX_MAX_COMPONENTS + CNT_OVERFLOW], 1u);
-          }
         } else if ((FEAT & F_VOXELS) && kind == MCX_VOXELS) {
           trace_voxels(I, C, ray, len_s, len_s + (size_t)I.n_mats * kBlock);
         } else if ((FEAT & F_OPTICS) && kind == MCX_MIRROR_ELLIPTIC) {
@@ -1085,6 +1225,8 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
             fate = MCX_FATE_MISSED;  // monitors do not absorb: the ray goes on
           }
         }
+      }
+      if (alive) {
         if (kind != MCX_DETECTOR && pass) fate = MCX_FATE_MISSED;  // fate = what the last component said
         if (!pass) {
           alive = false;
@@ -1354,8 +1496,9 @@ cudaError_t launch_trace(const DInstrument* d_inst, int features, int n_mats, co
                           : launch_one<F, false, false>(d_inst, n_mats, A, stream, g_n_sm);
   switch (features) {
     case 0: MCX_DISPATCH_GATED(0)
-    case F_SOLIDS: MCX_DISPATCH_GATED(F_SOLIDS)
+    case F_SOLIDS | F_PRIM: MCX_DISPATCH_GATED(F_SOLIDS | F_PRIM)
     case F_SOLIDS | F_MESH: MCX_DISPATCH(F_SOLIDS | F_MESH)
+    case F_SOLIDS | F_MESH | F_PRIM: MCX_DISPATCH(F_SOLIDS | F_MESH | F_PRIM)
     case F_VOXELS: MCX_DISPATCH(F_VOXELS)
     case F_OPTICS: MCX_DISPATCH_GATED(F_OPTICS)
     default: MCX_DISPATCH_GATED(F_ALL)
