@@ -5,10 +5,13 @@ binding roofline").
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config k] [--instruments 0,1,2,3,4] [--impl reference]
 
 A step = one pass of the whole hot path over one batch of synthetic rays: mcx_trace(n_rays) + mcx_tally_read.
-The headline line is BASELINE.json configs[1] (polychromatic energy-dispersive instrument, 1e8 rays); the other four
-instruments are measured the same way and reported under "instruments" in the same JSON line (north_star: "all five
-configs ... each reported in rays/s with its achieved fraction of the binding roofline").
-states the algorithmic work model used for the roofline fractions.
+The headline line is BASELINE.json configs[1] (polychromatic energy-dispersive instrument, 1e8 rays: the config the
+task names for the N=1 line); every instrument, the headline included, is measured the same way and reported under
+"instruments" in the same JSON line with its own roofline (the binding one of several candidates, each against a peak
+measured in this run), e2e and cpu_baseline (north_star: "all five configs ... each reported in rays/s with its
+achieved fraction of the binding roofline").  DESIGN.md "Measurement" states the algorithmic work model.
+The CPU baselines (the oracle on one core and on all cores, as independent processes over disjoint ray windows,
+PAPER.md:77) run first, before CUDA is initialised, so that the worker processes can be forked.
 """
 from __future__ import annotations
 
@@ -40,9 +43,9 @@ OPS_SOLIDS_ENTRY, OPS_PRIMITIVE_TEST, OPS_SEGMENT, OPS_MU, OPS_EXP = 35, 45, 10,
 OPS_VOXEL_ENTRY, OPS_VOXEL_STEP = 100, 6
 OPS_TRI_TEST, OPS_BVH_NODE = 45, 14
 NOMINAL_FP64_LANES_PER_SM, N_SM = 64, 148
-# DRAM bytes per ray of trace_kernel (dram__bytes_read.sum + dram__bytes_write.sum of one launch of 2^26 rays / 2^26) from
-# the ncu --set full captures summarised in profiles/r01d_README.md (c0, c2: whole run / n_rays; their tallies stay in L2).
-NCU_DRAM_BYTES_PER_RAY = {"c0_minimal": 0.001, "c1_polychromatic": 10.5, "c2_beamline": 0.01, "c3_mesh": 17.3, "c4_edxct": 28.6}
+# roofline.traffic (DRAM bytes of the dominant kernel) needs a profiler and is therefore null in this line; the ncu
+# captures of the same command are summarised under profiles/ (TRAFFIC_NOTE names the file).
+TRAFFIC_NOTE = "not measurable inside bench.py (needs ncu); see profiles/r02_README.md for dram__bytes of this command"
 
 
 def reached_per_component(n_rays, absorbed):
@@ -98,6 +101,26 @@ def algorithmic_bytes(inst, n_rays, counters, work_per_ray):
     return b
 
 
+def mesh_l2(inst, n_rays, counters, work_per_ray):
+    """Mesh instruments (L2 sector traffic binds the BVH walk).  Algorithmic 32-byte L2 sectors
+    per trace: per surface crossing a root-to-leaf path of the balanced BVH2 (both 32-byte children of every node on
+    the path) plus the 72-byte fp64 triangle (3 sectors).  Returns (sectors, bytes of BVH + triangles) or None."""
+    reach = reached_per_component(n_rays, counters["absorbed"])
+    sectors, footprint = 0.0, 0
+    for c, cd in enumerate(inst["components"]):
+        if cd["kind"] != "solids":
+            continue
+        meshes = [s for s in cd["solids"] if s["shape"] == "mesh"]
+        if not meshes:
+            continue
+        depth = float(np.mean([np.ceil(np.log2(max(len(s["tris"]), 2))) for s in meshes]))
+        sectors += reach[c] * work_per_ray["tri_hits"] * (2.0 * depth + 3.0)
+        for s in meshes:
+            d = int(np.ceil(np.log2(max(len(s["tris"]), 2))))
+            footprint += (2 << d) * 32 + (1 << d) * 72
+    return (sectors, footprint) if footprint else None
+
+
 # ---------------------------------------------------------------------------------------------------------------
 def oracle_work_per_ray(inst, n=20000):
     """Unit counts per ray from a small oracle sample (the oracle counts voxel steps, primitive tests, elementary
@@ -130,6 +153,51 @@ def time_oracle(inst, budget_s=15.0, first=0):
     O.trace(oi, first=first, n=n_big, mesh_accel=accel)
     dt = time.perf_counter() - t0
     return n_big / dt, n_big, dt
+
+
+def _oracle_worker(oi, first, n, accel, barrier, q):
+    from oracle import oracle as O
+    barrier.wait()
+    t0 = time.time()
+    O.trace(oi, first=first, n=n, mesh_accel=accel)
+    q.put((t0, time.time()))
+
+
+def cpu_baseline(inst, budget_s=4.0):
+    """The oracle as it stands on the host cores of this box: one thread over a bounded prefix of the workload's ray
+    indices, then os.cpu_count() independent processes over disjoint windows of the same length (the paper's own
+    scatter-gather scheme), all started together; rate = rays of all windows / (last end - first start).
+    Must run before CUDA is initialised (the workers are forked)."""
+    import multiprocessing as mp
+    from oracle import oracle as O
+    has_mesh = any(s["shape"] == "mesh" for c in inst["components"] if c["kind"] == "solids" for s in c["solids"])
+    accel = 1 if has_mesh else 0
+    rate1, n1, dt1 = time_oracle(inst, budget_s=budget_s)
+    cores = os.cpu_count() or 1
+    n_w = int(max(1000, rate1 * 0.75 * budget_s))   # windows may lie beyond n_rays: ray indices are just counters
+    ctx = mp.get_context("fork")
+    oi = O.Instrument(inst)
+    barrier, q = ctx.Barrier(cores), ctx.Queue()
+    procs = [ctx.Process(target=_oracle_worker, args=(oi, w * n_w, n_w, accel, barrier, q)) for w in range(cores)]
+    for p_ in procs:
+        p_.start()
+    spans = [q.get(timeout=600) for _ in procs]
+    for p_ in procs:
+        p_.join(timeout=60)
+    span = max(e for _, e in spans) - min(b for b, _ in spans)
+    rate_all = cores * n_w / span
+    cpu_model = "unknown"
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                cpu_model = line.split(":", 1)[1].strip()
+                break
+    except OSError:
+        pass
+    return {"value": rate_all, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{cores} processes x {n_w} consecutive ray indices of {inst['name']} ({span:.1f} s wall)",
+            "one_core": {"value": rate1, "cores": 1, "sample": f"first {n1} ray indices ({dt1:.1f} s)"},
+            "cpu_model": cpu_model}
 
 
 class ClockSampler(threading.Thread):
@@ -198,10 +266,12 @@ def measured_peaks():
 EXEC_MODE = "auto"   # lane scheduling (mcx_instrument_set_exec); --exec overrides for experiments
 
 
-def bench_instrument(M, torch, inst, n_rays, first, steps, warmup, device, dfma_peak, peaks, with_e2e=True, local_rank=0):
-    """Times `steps` steps of mcx_trace + mcx_tally_read for one instrument on the current stream.  Returns a dict."""
+def bench_instrument(M, torch, inst, n_rays, first, steps, warmup, device, probes, peaks, with_e2e=True, local_rank=0):
+    """Times `steps` steps of mcx_trace + mcx_tally_read for one instrument on the current stream.  Returns a dict.
+    probes: dict(dfma=lane-ops/s, l2=callable(bytes)->sectors/s, tally=callable(records)->records/s)."""
     g = M.Instrument(inst, device=device)
     g.set_exec(EXEC_MODE)
+    g.set_timing(True)
     det = g.dets[-1]
     nb = det["nx"] * det["ny"] * det["nE"]
     last = len(g.dets) - 1
@@ -214,6 +284,7 @@ def bench_instrument(M, torch, inst, n_rays, first, steps, warmup, device, dfma_
         g.tally(last, out)
     torch.cuda.synchronize(device)
     g.reset()
+    g.timing()                                          # forget the warm-up launches
     launches0 = g.launch_count()
     marks = []
     sampler = ClockSampler(physical_gpu_index(local_rank))
@@ -229,6 +300,7 @@ def bench_instrument(M, torch, inst, n_rays, first, steps, warmup, device, dfma_
         marks.append((e0, e1, e2))
     torch.cuda.synchronize(device)
     clocks = sampler.result()
+    split = g.timing()                                  # CUDA events inside the library, around sort and trace_kernel
     launches = g.launch_count() - launches0
     t_trace = [a.elapsed_time(b) for a, b, _ in marks]
     t_step = [a.elapsed_time(c) for a, _, c in marks]
@@ -236,43 +308,56 @@ def bench_instrument(M, torch, inst, n_rays, first, steps, warmup, device, dfma_
     traced = int(counters["absorbed"].sum()) + counters["detected"] + counters["missed"] + counters["degenerate"]
     assert traced == steps * n_rays, "ray accounting does not add up"
     per_trace = {k: (v / steps if not isinstance(v, np.ndarray) else v / steps) for k, v in counters.items()}
-    res = {"n_rays": n_rays, "ms_per_step": float(np.mean(t_step)), "ms_trace_kernel": float(np.mean(t_trace)),
-           "ms_tally_read": float(np.mean(t_step) - np.mean(t_trace)), "ms_step_min": float(np.min(t_step)),
+    ms_sort, ms_kernel = split["sort_ms"] / steps, split["trace_ms"] / steps
+    res = {"n_rays": n_rays, "ms_per_step": float(np.mean(t_step)), "ms_step_min": float(np.min(t_step)),
+           "kernel_ms": {"sort_kernels": ms_sort, "trace_kernel": ms_kernel,
+                         "tally_read_kernel": float(np.mean(t_step) - np.mean(t_trace)),
+                         "trace_kernel_launches_per_step": split["launches"] / steps,
+                         "how": "CUDA events on the launching stream: around every sort / trace_kernel launch inside the "
+                                "library (mcx_instrument_set_timing), around mcx_tally_read in bench.py"},
            "rays_per_s": n_rays / (np.mean(t_step) * 1e-3), "launches": launches, "clocks": clocks,
            "detected_fraction": counters["detected"] / traced, "tally_bytes": 32 * nb}
-    # roofline of the dominant kernel (trace_kernel), DESIGN.md "Measurement"
+    # rooflines of the dominant kernel (trace_kernel): every candidate is algorithmic work per
+    # launch / trace_kernel's own device time / a peak measured in this run; the binding one is the largest fraction
     work = oracle_work_per_ray(inst)
     ops = algorithmic_ops(inst, n_rays, per_trace, work)
     byt = algorithmic_bytes(inst, n_rays, per_trace, work)
-    sec = np.mean(t_trace) * 1e-3
-    alu_frac = ops / sec / dfma_peak
+    sec = ms_kernel * 1e-3
     hbm_peak = (peaks or {}).get("hbm_gbs", 6650.0)
-    hbm_frac = byt / sec / 1e9 / hbm_peak
+    cand = {"alu": {"achieved": ops / sec / 1e12, "peak": probes["dfma"] / 1e12, "unit": "Tlane-op/s (fp64)",
+                    "frac": ops / sec / probes["dfma"], "per_ray": ops / n_rays,
+                    "peak_source": "mcx_probe_dfma, measured in this run",
+                    "note": "fp64 lane-operations the METHOD needs (work model at the top of bench.py); the voxel walk does "
+                            "its 6 per voxel step as integer carries and skips most steps (DESIGN.md 5.3)"},
+            "hbm": {"achieved": byt / sec / 1e9, "peak": hbm_peak, "unit": "GB/s", "frac": byt / sec / 1e9 / hbm_peak,
+                    "per_ray": byt / n_rays, "peak_source": "MEASURED_PEAKS.json" if peaks else "fallback 6650 GB/s"}}
+    n_rec = 1 << (int(nb).bit_length() - 1)
+    tally_peak = probes["tally"](n_rec)
+    det_rate = res["detected_fraction"] * n_rays / sec
+    cand["tally"] = {"achieved": det_rate, "peak": tally_peak, "unit": "records/s", "frac": det_rate / tally_peak,
+                     "per_ray": res["detected_fraction"],
+                     "peak_source": f"mcx_probe_tally, {n_rec} random 32-byte records, measured in this run"}
+    ml2 = mesh_l2(inst, n_rays, per_trace, work)
+    if ml2 is not None:
+        sectors, footprint = ml2
+        table = 1 << int(np.ceil(np.log2(footprint)))
+        l2_peak = probes["l2"](table)
+        cand["l2"] = {"achieved": sectors / sec * 32 / 1e9, "peak": l2_peak * 32 / 1e9, "unit": "GB/s of 32-byte sectors",
+                      "frac": sectors / sec / l2_peak, "per_ray": 32 * sectors / n_rays,
+                      "peak_source": f"mcx_probe_l2, random sectors of a {table >> 20} MiB table (BVH + triangles = "
+                                     f"{footprint / 2**20:.1f} MiB), measured in this run",
+                      "note": "sectors the per-ray walk needs; warps that walk one beam share them (DESIGN.md 5.1)"}
+    bound = max(cand, key=lambda k: cand[k]["frac"])
     res["work_per_ray"] = work
-    bpr = NCU_DRAM_BYTES_PER_RAY.get(inst["name"])
-    traffic = None if bpr is None else bpr * n_rays      # bytes per step (all launches of the step)
-    traffic_src = None if bpr is None else f"ncu dram bytes {bpr} B/ray (profiles/r01d_README.md) x n_rays"
-    res["roofline"] = {"bound": "alu", "achieved": ops / sec / 1e12, "peak": dfma_peak / 1e12, "unit": "Tlane-op/s (fp64)",
-                       "frac": alu_frac, "traffic": traffic, "traffic_source": traffic_src, "kernel": "trace_kernel",
-                       "ops_per_ray": ops / n_rays, "peak_source": "mcx_probe_dfma, measured in this run",
-                       "hbm": {"achieved": byt / sec / 1e9, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_frac,
-                               "bytes_per_ray": byt / n_rays,
-                               "peak_source": "MEASURED_PEAKS.json" if peaks else "fallback 6650 GB/s"}}
-    if with_e2e:
-        # the second candidate roofline: random tally-record updates at this detector's footprint
-        n_rec = 1 << (int(nb).bit_length() - 1)
-        g.close()
-        g = None
-        torch.cuda.empty_cache()
-        tally_peak = max(M.probe_tally(n_rec, N_SM * 8, 128, device=str(device)) for _ in range(2))
-        det_rate = res["detected_fraction"] * n_rays / sec
-        res["roofline"]["tally"] = {"achieved": det_rate, "peak": tally_peak, "unit": "records/s", "frac": det_rate / tally_peak,
-                                    "peak_source": f"mcx_probe_tally, {n_rec} random 32-byte records, measured in this run"}
-        res["e2e"] = bench_e2e(M, torch, inst, n_rays, first, max(2, min(steps, 3)), device)
-    if g is not None:
-        g.close()
+    res["roofline"] = {"bound": bound, "achieved": cand[bound]["achieved"], "peak": cand[bound]["peak"],
+                       "unit": cand[bound]["unit"], "frac": cand[bound]["frac"], "traffic": None,
+                       "traffic_note": TRAFFIC_NOTE, "kernel": "trace_kernel", "kernel_ms": ms_kernel,
+                       "candidates": cand}
+    g.close()
     del flush, out
     torch.cuda.empty_cache()
+    if with_e2e:
+        res["e2e"] = bench_e2e(M, torch, inst, n_rays, first, 2, device)
     return res
 
 
@@ -343,6 +428,27 @@ def run_reference(args):
     return 0
 
 
+def make_probes(M, device):
+    """Peaks measured in this run (memoised per footprint): FP64 pipe, random L2 sectors, random tally records."""
+    dev = str(device)
+    memo_l2, memo_tally = {}, {}
+
+    def l2(table_bytes):
+        if table_bytes not in memo_l2:
+            memo_l2[table_bytes] = max(M.probe_l2(table_bytes, N_SM * 8, 256, device=dev) for _ in range(2))
+        return memo_l2[table_bytes]
+
+    def tally(n_rec):
+        if n_rec not in memo_tally:
+            memo_tally[n_rec] = max(M.probe_tally(n_rec, N_SM * 8, 128, device=dev) for _ in range(2))
+        return memo_tally[n_rec]
+
+    # 8 independent DFMA chains per thread, 148 x 8 blocks of 256: the rate the chip holds at its clock under this load
+    dfma = max(M.probe_dfma(N_SM * 8, 1 << 15, device=dev) for _ in range(3))
+    return {"dfma": dfma, "l2": l2, "tally": tally,
+            "latency_ns": {"unloaded_32MiB": M.probe_latency(32 << 20, 1, 32, 4096, device=dev) * 1e9}}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -353,7 +459,7 @@ def main():
     ap.add_argument("--rays", type=float, default=None, help="override n_rays of the headline config")
     ap.add_argument("--instruments", default="0,2,3,4", help="other configs to report under 'instruments' ('' = none)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--sweep", action="store_true", help="configs[4] throughput sweep 1e6..1e10 rays")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the configs[4] throughput sweep 1e6..1e10 rays")
     ap.add_argument("--exec", default="auto", choices=["auto", "direct", "sorted"], help="lane scheduling (row a13)")
     args = ap.parse_args()
     global EXEC_MODE
@@ -362,15 +468,25 @@ def main():
     if args.impl == "reference":
         return run_reference(args)
 
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    import workloads as W
+    ks = [args.config] + ([int(x) for x in args.instruments.split(",") if x != "" and int(x) != args.config]
+                          if (rank == 0 and world == 1) else [])
+    insts = {k: make_instrument(W, k, args.rays if k == args.config else None) for k in ks}
+
+    # CPU baselines first: the oracle's worker processes are forked, which must happen before CUDA is initialised
+    cpu = {}
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        for k in ks:
+            cpu[k] = cpu_baseline(insts[k])
+
     import torch
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the mcx hot path has no CPU fallback")
     import paper_2410_08747_b200 as M
-    from paper_2410_08747_b200.shard import ray_range
-    import workloads as W
+    from paper_2410_08747_b200.shard import ray_range, reduce_tallies
     M.lib()
-    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     device = torch.device(f"cuda:{local_rank}")
     torch.cuda.set_device(device)
     dist = None
@@ -378,56 +494,76 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=device)
     peaks = measured_peaks()
+    probes = make_probes(M, device)
 
-    # FP64 pipe peak at the clock the chip holds (8 independent DFMA chains per thread, 148 x 8 blocks of 256)
-    dfma_peak = max(M.probe_dfma(N_SM * 8, 1 << 15, device=str(device)) for _ in range(3))
-
-    inst = make_instrument(W, args.config, args.rays)
+    inst = insts[args.config]
     n_rays = inst["n_rays"]
     first, _ = ray_range(rank, world, n_rays, "weak")   # every rank traces n_rays of its own index window
     if dist is not None:
         dist.barrier()
     torch.cuda.synchronize(device)
-    head = bench_instrument(M, torch, inst, n_rays, first, args.steps, args.warmup, device, dfma_peak, peaks,
+    head = bench_instrument(M, torch, inst, n_rays, first, args.steps, args.warmup, device, probes, peaks,
                             with_e2e=True, local_rank=local_rank)
     torch.cuda.synchronize(device)
     ms = head["ms_per_step"]
     e2e_ms = head["e2e"]["ms_per_step"]
+    reduce_info = None
     if dist is not None:
         t = torch.tensor([ms, e2e_ms], dtype=torch.float64, device=device)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms, e2e_ms = float(t[0]), float(t[1])
         dist.barrier()
+        # the paper's gather/add of the monitor arrays: one sum-reduce of (N, p, p2) to rank 0 over
+        # NCCL, after the timed path and reported on its own
+        g = M.Instrument(inst, device=device)
+        g.trace(min(n_rays, 1 << 22), first=first)
+        tl = list(g.tally(len(g.dets) - 1))
+        torch.cuda.synchronize(device)
+        dist.barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        reduce_tallies(tl, dst=0)
+        e1.record()
+        torch.cuda.synchronize(device)
+        tr = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=device)
+        dist.all_reduce(tr, op=dist.ReduceOp.MAX)
+        reduce_info = {"ms": float(tr[0]), "bytes_per_rank": int(sum(x.numel() * x.element_size() for x in tl)),
+                       "what": "ncclReduce (sum) of N, p, p2 of the last detector to rank 0; not part of the timed step"}
+        g.close()
     value = world * n_rays / (ms * 1e-3)
 
-    others = {}
-    if rank == 0 and world == 1 and args.instruments:
-        for k in [int(x) for x in args.instruments.split(",") if x != ""]:
-            if k == args.config:
-                continue
-            ik = make_instrument(W, k)
-            r = bench_instrument(M, torch, ik, ik["n_rays"], 0, args.steps, args.warmup, device, dfma_peak, peaks, with_e2e=False)
-            others[f"c{k}_{ik['name']}"] = slim(r)
+    instruments = {}
+    if rank == 0 and world == 1:
+        head_entry = slim(head)
+        if args.config in cpu:
+            head_entry["cpu_baseline"] = cpu[args.config]
+        instruments[f"c{args.config}_{inst['name']}"] = head_entry
+        for k in ks[1:]:
+            ik = insts[k]
+            r = bench_instrument(M, torch, ik, ik["n_rays"], 0, args.steps, args.warmup, device, probes, peaks, with_e2e=True)
+            e = slim(r)
+            if k in cpu:
+                e["cpu_baseline"] = cpu[k]
+            instruments[f"c{k}_{ik['name']}"] = e
             if k == 0:                                  # 1e6 rays is launch-latency sized: also the asymptote
-                r = bench_instrument(M, torch, ik, 100_000_000, 0, args.steps, args.warmup, device, dfma_peak, peaks, with_e2e=False)
-                others["c0_minimal_1e8_rays"] = slim(r)
-            del ik
-    if rank == 0 and world == 1 and args.sweep:
-        i4 = make_instrument(W, 4)
-        for n in (10**6, 10**7, 10**8, 10**9, 10**10):
-            r = bench_instrument(M, torch, i4, n, 0, max(1, args.steps if n < 10**10 else 1), 3 if n < 10**9 else 1, device,
-                                 dfma_peak, peaks, with_e2e=False)
-            others[f"c4_sweep_{n:.0e}"] = slim(r)
+                r = bench_instrument(M, torch, ik, 100_000_000, 0, args.steps, args.warmup, device, probes, peaks, with_e2e=True)
+                e = slim(r)
+                if k in cpu:
+                    e["cpu_baseline"] = cpu[k]
+                instruments["c0_minimal_1e8_rays"] = e
+        if 4 in insts and not args.no_sweep:            # configs[4]: "also run a throughput sweep at 1e6-1e10 rays"
+            sweep = {}
+            for n in (10**6, 10**7, 10**8, 10**9, 10**10):
+                r = bench_instrument(M, torch, insts[4], n, 0, args.steps if n < 10**9 else 1, 3 if n < 10**9 else 1, device,
+                                     probes, peaks, with_e2e=False)
+                sweep[f"{n:.0e}"] = {"rays_per_s": r["rays_per_s"], "ms_per_step": r["ms_per_step"],
+                                     "kernel_ms": {k_: v for k_, v in r["kernel_ms"].items() if k_ != "how"}}
+            instruments["c4_sweep"] = sweep
 
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
         return 0
-    cpu = None
-    if world == 1 and not args.no_cpu_baseline:
-        rate, n_s, dt = time_oracle(inst, budget_s=15.0)
-        cpu = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
-               "sample": f"first {n_s} ray indices of {inst['name']} ({dt:.1f} s, one thread of {os.cpu_count()} host cores)"}
     roof = dict(head["roofline"])
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
@@ -441,13 +577,16 @@ def main():
                     "h2d_bytes_per_step": head["e2e"]["h2d_bytes_per_step"], "d2h_bytes_per_step": head["e2e"]["d2h_bytes_per_step"],
                     "ms_per_step": e2e_ms, "what": "mcx_instrument_create (host tables) + mcx_trace + mcx_tally_read_host (pinned)"},
             "gpu_launches": head["launches"], "clocks": head["clocks"], "roofline": roof,
-            "kernel_ms": {"trace_kernel": head["ms_trace_kernel"], "tally_read_kernel": head["ms_tally_read"]},
-            "dfma_peak_measured_tlaneops": dfma_peak / 1e12,
-            "dfma_peak_nominal_tlaneops": N_SM * NOMINAL_FP64_LANES_PER_SM * 1.965e9 / 1e12}
-    if cpu is not None:
-        line["cpu_baseline"] = cpu
-    if others:
-        line["instruments"] = others
+            "kernel_ms": head["kernel_ms"],
+            "peaks_measured_in_this_run": {"fp64_tlaneops": probes["dfma"] / 1e12,
+                                           "fp64_nominal_tlaneops": N_SM * NOMINAL_FP64_LANES_PER_SM * 1.965e9 / 1e12,
+                                           "dependent_load_latency_ns": probes["latency_ns"]}}
+    if args.config in cpu:
+        line["cpu_baseline"] = cpu[args.config]
+    if reduce_info is not None:
+        line["tally_reduce"] = reduce_info
+    if instruments:
+        line["instruments"] = instruments
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
@@ -455,13 +594,10 @@ def main():
 
 
 def slim(r):
-    keep = ("n_rays", "rays_per_s", "ms_per_step", "ms_trace_kernel", "ms_tally_read", "launches", "detected_fraction",
-            "tally_bytes", "clocks")
-    out = {k: r[k] for k in keep}
-    rf = r["roofline"]
-    out["roofline"] = {"bound": rf["bound"], "frac": rf["frac"], "achieved": rf["achieved"], "peak": rf["peak"], "unit": rf["unit"],
-                       "ops_per_ray": rf["ops_per_ray"], "hbm_frac": rf["hbm"]["frac"], "hbm_gbs": rf["hbm"]["achieved"],
-                       "bytes_per_ray": rf["hbm"]["bytes_per_ray"]}
+    keep = ("n_rays", "rays_per_s", "ms_per_step", "kernel_ms", "launches", "detected_fraction", "tally_bytes", "clocks",
+            "roofline", "e2e")
+    out = {k: r[k] for k in keep if k in r}
+    out["kernel_ms"] = {k: v for k, v in r["kernel_ms"].items() if k != "how"}
     return out
 
 

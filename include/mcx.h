@@ -220,9 +220,19 @@ mcx_status mcx_instrument_set_exec(mcx_instrument* inst, int mode);
  *                   buffer of a 2^26 chunk, 256 MiB, whatever is set here);
  *   sort_grid_bits  bits per axis of the bucket grid of MCX_EXEC_SORTED, 1..11 (default: by chunk length, at most 9
  *                   for instruments of analytic solids only, else 10);
- *   absorber_gate   1 = on (default), 2 = off. */
+ *   absorber_gate   1 = on (default), 2 = off;
+ *   tally_mode      how a detected ray reaches its tally record (step 14), an mcx_tally_mode:
+ *                   MCX_TALLY_GLOBAL  three reductions (u64 count, two fp64 sums) per detected ray into its record;
+ *                   MCX_TALLY_WARP    warp-aggregated: lanes of a warp in the same bin are summed first, one leader
+ *                                     per distinct bin issues the reductions;
+ *                   MCX_TALLY_BLOCK   warp-aggregated into a block-private shared-memory cache of tally records
+ *                                     (2048 direct-mapped slots; chains without solids or voxels only, MCX_TALLY_WARP
+ *                                     elsewhere), flushed to the records once per block and launch;
+ *                   MCX_TALLY_AUTO (0 here = keep) is the library's choice from measurement.
+ *                   N is the same integer in every mode; p and p2 differ in summation order only. */
+typedef enum { MCX_TALLY_AUTO = 0, MCX_TALLY_GLOBAL = 1, MCX_TALLY_WARP = 2, MCX_TALLY_BLOCK = 3 } mcx_tally_mode;
 typedef struct mcx_tuning {
-  int32_t chunk_log2, sort_grid_bits, absorber_gate, reserved;
+  int32_t chunk_log2, sort_grid_bits, absorber_gate, tally_mode;
 } mcx_tuning;
 mcx_status mcx_instrument_set_tuning(mcx_instrument* inst, const mcx_tuning* tuning);
 
@@ -261,6 +271,14 @@ mcx_status mcx_trace_dump(mcx_instrument* inst, uint64_t first_ray, uint64_t n_r
 
 /* Number of kernel launches this handle has enqueued so far (create, trace, read, reset). */
 uint64_t mcx_launch_count(const mcx_instrument* inst);
+
+/* Device-time split of the traces, for the measurement of SURVEY.md 8(d).  With timing on (on != 0), every chunk of a
+ * trace records CUDA events on the launching stream before its ray sort, between the sort and trace_kernel, and after
+ * trace_kernel (at most 4096 chunks between two reads; later ones go untimed).  mcx_timing_read waits for the last of
+ * them and gives the sums since the previous read: milliseconds in the sort kernels, milliseconds in trace_kernel, and
+ * the number of trace_kernel launches timed (all HOST pointers, each may be NULL); then it forgets them. */
+mcx_status mcx_instrument_set_timing(mcx_instrument* inst, int on);
+mcx_status mcx_timing_read(mcx_instrument* inst, double* sort_ms, double* trace_ms, int64_t* n_trace_launches);
 
 /* Sustained-FP64 probe used for the ALU roofline: enqueues a kernel in which every thread of a
  * (n_blocks x 256) grid runs n_iters x 8 dependent-chain-free DFMAs; `sink` is DEVICE [n_blocks*256] doubles.

@@ -22,11 +22,12 @@ DIR_MODE = {"target": 0, "gauss": 1}
 ENERGY_MODE = {"mono": 0, "uniform": 1, "spectrum": 2}
 SHAPE = {"box": 0, "cyl": 1, "sphere": 2, "mesh": 3}
 EXEC_MODE = {"auto": 0, "direct": 1, "sorted": 2}
+TALLY_MODE = {"auto": 0, "global": 1, "warp": 2, "block": 3}
 FATE_DETECTED, FATE_MISSED, FATE_DEGENERATE = -1, -2, -3
 
 EXPORTS = ["mcx_instrument_workspace_size", "mcx_instrument_create", "mcx_trace", "mcx_trace_range", "mcx_tally_read",
            "mcx_tally_read_host", "mcx_instrument_set_exec", "mcx_instrument_set_tuning", "mcx_upload_bytes", "mcx_tally_reset",
-           "mcx_counters_read", "mcx_trace_status", "mcx_trace_dump", "mcx_launch_count", "mcx_probe_dfma", "mcx_probe_tally",
+           "mcx_counters_read", "mcx_trace_status", "mcx_trace_dump", "mcx_launch_count", "mcx_instrument_set_timing", "mcx_timing_read", "mcx_probe_dfma", "mcx_probe_tally",
            "mcx_probe_l2", "mcx_probe_latency", "mcx_instrument_destroy", "mcx_last_error"]
 MCX_ERR_CAPACITY = 6
 
@@ -95,7 +96,7 @@ class McxComponent(C.Structure):
 
 
 class McxTuning(C.Structure):
-    _fields_ = [("chunk_log2", C.c_int32), ("sort_grid_bits", C.c_int32), ("absorber_gate", C.c_int32), ("reserved", C.c_int32)]
+    _fields_ = [("chunk_log2", C.c_int32), ("sort_grid_bits", C.c_int32), ("absorber_gate", C.c_int32), ("tally_mode", C.c_int32)]
 
 
 FATE_DTYPE = np.dtype([("fate", np.int32), ("reserved", np.int32), ("bin", np.int64), ("p", np.float64)])
@@ -130,6 +131,10 @@ def lib(strict=False):
     L.mcx_probe_l2.restype = C.c_int
     L.mcx_probe_latency.argtypes = [vp, C.c_uint64, vp, C.c_int, C.c_int, C.c_int64, vp]
     L.mcx_probe_latency.restype = C.c_int
+    L.mcx_instrument_set_timing.argtypes = [vp, C.c_int]
+    L.mcx_instrument_set_timing.restype = C.c_int
+    L.mcx_timing_read.argtypes = [vp, _dp, _dp, C.POINTER(C.c_int64)]
+    L.mcx_timing_read.restype = C.c_int
     L.mcx_upload_bytes.argtypes = [vp]
     L.mcx_upload_bytes.restype = C.c_uint64
     L.mcx_tally_reset.argtypes = [vp, vp]
@@ -323,15 +328,25 @@ class Instrument:
         """mcx_instrument_set_exec: "auto" | "direct" | "sorted" (lane scheduling, row a13)."""
         _check(self.L.mcx_instrument_set_exec(self.handle, EXEC_MODE[mode]), self.L)
 
-    def set_tuning(self, chunk_log2=0, sort_grid_bits=0, absorber_gate=0):
-        """mcx_instrument_set_tuning; 0 = keep the library's choice."""
-        t = McxTuning(int(chunk_log2), int(sort_grid_bits), int(absorber_gate), 0)
+    def set_tuning(self, chunk_log2=0, sort_grid_bits=0, absorber_gate=0, tally_mode="auto"):
+        """mcx_instrument_set_tuning; 0 / "auto" = keep the library's choice."""
+        t = McxTuning(int(chunk_log2), int(sort_grid_bits), int(absorber_gate), TALLY_MODE[tally_mode])
         _check(self.L.mcx_instrument_set_tuning(self.handle, C.byref(t)), self.L)
 
     def status(self):
         """mcx_trace_status: synchronises the current stream; raises McxError (MCX_ERR_CAPACITY / MCX_ERR_CUDA) if a
         trace since the last reset went wrong."""
         _check(self.L.mcx_trace_status(self.handle, self._stream()), self.L)
+
+    def set_timing(self, on=True):
+        """mcx_instrument_set_timing: CUDA events around the ray sort and trace_kernel of every chunk."""
+        _check(self.L.mcx_instrument_set_timing(self.handle, int(bool(on))), self.L)
+
+    def timing(self):
+        """mcx_timing_read -> dict(sort_ms, trace_ms, launches) summed since the last read; waits for the last event."""
+        a, b, n = C.c_double(), C.c_double(), C.c_int64()
+        _check(self.L.mcx_timing_read(self.handle, C.byref(a), C.byref(b), C.byref(n)), self.L)
+        return {"sort_ms": a.value, "trace_ms": b.value, "launches": int(n.value)}
 
     def upload_bytes(self):
         """host -> device bytes moved to build this instrument (tables by create + the voxel volume)."""

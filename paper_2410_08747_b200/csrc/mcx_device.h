@@ -159,6 +159,8 @@ struct TraceArgs {
   unsigned int* gate_known;  // the absorber gate an earlier launch on this instrument settled on, plus 1 (0 = not yet)
   unsigned int* host_flag;   // mapped pinned host word: receives epoch + 1 when a ray overflowed its scratch capacity
   unsigned int epoch;        // number of mcx_tally_reset calls on the handle so far
+  int tally_mode;            // mcx_tally_mode (never MCX_TALLY_AUTO here)
+  int tally_cache_log2;      // MCX_TALLY_BLOCK: log2 of the slots of the block-private cache (32 bytes each); 0 = none
 };
 
 // sizes of the sort workspace

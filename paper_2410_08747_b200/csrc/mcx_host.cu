@@ -34,10 +34,18 @@ struct mcx_instrument {
   uint64_t chunk_rays = 0;  // rays per sorted chunk (<= kChunkCapacity, the order buffer in the workspace)
   int sort_grid_bits = 0;   // 0 = by chunk length (sort_bits)
   bool gate_enabled = true;
+  int tally_mode = MCX_TALLY_AUTO;
   // MCX_ERR_CAPACITY: a mapped pinned host word the trace kernel writes (epoch + 1) when a ray overflows its scratch
   unsigned int* host_flag = nullptr;
   unsigned int epoch = 0;   // resets so far: an overflow of an earlier epoch is forgotten
-  ~mcx_instrument() { if (host_flag) cudaFreeHost(host_flag); }
+  // mcx_instrument_set_timing: events around the sort and trace_kernel of every chunk (three per chunk, reused)
+  bool timing = false;
+  std::vector<cudaEvent_t> events;  // pool, 3 per timed chunk
+  size_t events_used = 0;
+  ~mcx_instrument() {
+    if (host_flag) cudaFreeHost(host_flag);
+    for (cudaEvent_t e : events) cudaEventDestroy(e);
+  }
 };
 
 namespace {
@@ -692,6 +700,17 @@ bool use_sorted(const mcx_instrument* H) {
   return H->sort_pays;
 }
 
+constexpr size_t kMaxTimedChunks = 4096;
+constexpr int kTallyCacheLog2 = 11;  // MCX_TALLY_BLOCK: 2048 slots of 32 bytes per block
+
+// Step 14 update path (include/mcx.h, mcx_tally_mode).  AUTO: see DESIGN.md 5.5 for the measurements behind it.
+int tally_mode_of(const mcx_instrument* H) {
+  int mode = H->tally_mode;
+  if (mode == MCX_TALLY_AUTO) mode = MCX_TALLY_GLOBAL;
+  if (mode == MCX_TALLY_BLOCK && (H->features & (F_SOLIDS | F_VOXELS))) mode = MCX_TALLY_WARP;  // no room beside their scratch
+  return mode;
+}
+
 // Traces rays [first, first + n) chunk by chunk; dump == nullptr tallies.
 mcx_status run_trace(mcx_instrument* H, uint64_t first, uint64_t n, uint64_t seed, mcx_ray_fate* dump, cudaStream_t stream) {
   const bool sorted = use_sorted(H);
@@ -707,10 +726,23 @@ mcx_status run_trace(mcx_instrument* H, uint64_t first, uint64_t n, uint64_t see
     A.gate_max = H->gate_enabled ? H->gate_max : 0;
     A.host_flag = H->host_flag;
     A.epoch = H->epoch;
+    A.tally_mode = tally_mode_of(H);
+    A.tally_cache_log2 = A.tally_mode == MCX_TALLY_BLOCK ? kTallyCacheLog2 : 0;
     A.order = nullptr;
     A.dump = dump ? dump + base : nullptr;
     A.ticket = (unsigned int*)(ws + H->off_ticket);
     A.gate_known = (unsigned int*)(ws + H->off_gate);
+    cudaEvent_t* tev = nullptr;  // mcx_instrument_set_timing: before the sort, after it, after trace_kernel
+    if (H->timing && !dump && H->events_used + 3 <= kMaxTimedChunks * 3) {
+      while (H->events.size() < H->events_used + 3) {
+        cudaEvent_t ev;
+        if (cudaEventCreate(&ev) != cudaSuccess) return cuda_fail(cudaGetLastError(), "event create");
+        H->events.push_back(ev);
+      }
+      tev = H->events.data() + H->events_used;
+      H->events_used += 3;
+      cudaEventRecord(tev[0], stream);
+    }
     if (sorted && m >= kSortMinRays) {
       const int g = sort_bits(m, H->features, H->sort_grid_bits);
       unsigned int* cnt = (unsigned int*)(ws + H->off_sort_cnt);
@@ -721,8 +753,10 @@ mcx_status run_trace(mcx_instrument* H, uint64_t first, uint64_t n, uint64_t see
       H->launches += 3;
       A.order = (const uint32_t*)(ws + H->off_order);
     }
+    if (tev) cudaEventRecord(tev[1], stream);
     const cudaError_t e = launch_trace((const DInstrument*)ws, H->features, H->n_mats, A, stream);
     if (e != cudaSuccess) return cuda_fail(e, "trace launch");
+    if (tev) cudaEventRecord(tev[2], stream);
     H->launches++;
   }
   return MCX_OK;
@@ -835,13 +869,44 @@ mcx_status mcx_instrument_set_tuning(mcx_instrument* inst, const mcx_tuning* t) 
     return fail(MCX_ERR_INVALID_ARG, "chunk_log2 %d outside %d..%d", t->chunk_log2, kChunkLog2Min, kChunkLog2Max);
   if (t->sort_grid_bits < 0 || t->sort_grid_bits > MCX_SORT_MAX_G) return fail(MCX_ERR_INVALID_ARG, "sort_grid_bits %d outside 1..%d", t->sort_grid_bits, MCX_SORT_MAX_G);
   if (t->absorber_gate < 0 || t->absorber_gate > 2) return fail(MCX_ERR_INVALID_ARG, "absorber_gate must be 0, 1 or 2");
+  if (t->tally_mode < 0 || t->tally_mode > MCX_TALLY_BLOCK) return fail(MCX_ERR_INVALID_ARG, "tally_mode must be an mcx_tally_mode");
   if (t->chunk_log2) inst->chunk_rays = (uint64_t)1 << t->chunk_log2;
   if (t->sort_grid_bits) inst->sort_grid_bits = t->sort_grid_bits;
   if (t->absorber_gate) inst->gate_enabled = t->absorber_gate == 1;
+  if (t->tally_mode) inst->tally_mode = t->tally_mode;
   return MCX_OK;
 }
 
 uint64_t mcx_launch_count(const mcx_instrument* inst) { return inst ? inst->launches : 0; }
+
+mcx_status mcx_instrument_set_timing(mcx_instrument* inst, int on) {
+  if (!inst) return fail(MCX_ERR_INVALID_ARG, "inst is null");
+  inst->timing = on != 0;
+  return MCX_OK;
+}
+
+mcx_status mcx_timing_read(mcx_instrument* inst, double* sort_ms, double* trace_ms, int64_t* n_trace_launches) {
+  if (!inst) return fail(MCX_ERR_INVALID_ARG, "inst is null");
+  double s_ms = 0.0, t_ms = 0.0;
+  const size_t n = inst->events_used / 3;
+  if (n > 0) {
+    cudaError_t e = cudaEventSynchronize(inst->events[3 * n - 1]);
+    if (e != cudaSuccess) return cuda_fail(e, "event synchronize");
+    for (size_t k = 0; k < n; ++k) {
+      float a = 0.0f, b = 0.0f;
+      e = cudaEventElapsedTime(&a, inst->events[3 * k], inst->events[3 * k + 1]);
+      if (e == cudaSuccess) e = cudaEventElapsedTime(&b, inst->events[3 * k + 1], inst->events[3 * k + 2]);
+      if (e != cudaSuccess) return cuda_fail(e, "event elapsed time");
+      s_ms += a;
+      t_ms += b;
+    }
+  }
+  inst->events_used = 0;
+  if (sort_ms) *sort_ms = s_ms;
+  if (trace_ms) *trace_ms = t_ms;
+  if (n_trace_launches) *n_trace_launches = (int64_t)n;
+  return MCX_OK;
+}
 
 mcx_status mcx_probe_dfma(double* sink, int n_blocks, int64_t n_iters, void* cuda_stream) {
   if (!sink || n_blocks < 1 || n_iters < 0) return fail(MCX_ERR_INVALID_ARG, "bad probe arguments");

@@ -1084,6 +1084,97 @@ __global__ void __launch_bounds__(256) sort_scatter_kernel(uint64_t first, uint3
 }
 
 // ------------------------------------------------------------------------------------------------------------
+// Step 14, the tally update (row a12; monitor arrays updated atomically).  Three ways, chosen per
+// launch (TraceArgs::tally_mode, mcx_tuning.tally_mode; DESIGN.md 5.5 has the measurements that pick the default):
+//   TALLY_GLOBAL   every detected ray issues its own three reductions (u64 count, two fp64 sums) into its 32-byte record;
+//   TALLY_WARP     warp-aggregated: the lanes of a warp that hit the same bin are found with match.any, their weights
+//                  are summed with a shuffle butterfly, and one leader per distinct bin issues the three reductions;
+//   TALLY_BLOCK    as TALLY_WARP, but the leader adds into a block-private cache in shared memory (a direct-mapped
+//                  table of 2^k records keyed by detector and bin, claimed with a compare-and-swap); bins whose slot is
+//                  taken by another bin go to global memory as before.  The block flushes its cache with one set of
+//                  reductions per occupied slot when it has no work left: the "privatised per block, then reduced"
+//                  scheme north_star names, for detectors whose illuminated bins fit (c0: 32 x 32 pixels).
+// All three add the same integers; the fp64 sums differ in summation order only.
+// ------------------------------------------------------------------------------------------------------------
+struct TallyCache {
+  unsigned long long* key;  // [2^log2] 0 = empty, else ((detector + 1) << 48) | bin; then N, P, P2 arrays of the same length
+  int log2;                 // 0 = no cache
+};
+
+__device__ __forceinline__ void tally_global(TallyBin* rec, unsigned long long cnt, double sp, double sp2) {
+  atomicAdd(&rec->N, cnt);
+  atomicAdd(&rec->P, sp);
+  atomicAdd(&rec->P2, sp2);
+}
+
+// The aggregating paths (TALLY_WARP, TALLY_BLOCK).  Must be called by all 32 lanes; `on` = this lane has a ray to tally
+// into bin `bin` of detector `det` with weight p.  Kept out of line: the default path (tally_add below) must not pay
+// registers for it (the optics kernel sits at the edge of two resident blocks).
+__device__ __noinline__ void tally_add_aggregated(TallyBin* const* tallies, int mode, unsigned long long* cache_key, int cache_log2,
+                                                  unsigned det, bool on, long long bin, double p) {
+  const unsigned full = 0xffffffffu;
+  const int lane = threadIdx.x & 31;
+  const unsigned m = __ballot_sync(full, on);
+  if (m == 0u) return;
+  unsigned grp = 0u;
+  if (on) grp = __match_any_sync(m, (unsigned long long)bin);
+  const bool lead = on && (__ffs(grp) - 1) == lane;
+  const unsigned cnt = (unsigned)__popc(grp);
+  double sp = p, sp2 = p * p;
+  // groups of more than one lane (rare unless a warp's rays share pixel AND energy bin): butterfly sums, group by group
+  for (unsigned todo = __ballot_sync(full, lead && cnt > 1u); todo; todo &= todo - 1u) {
+    const int l = __ffs(todo) - 1;
+    const unsigned g = __shfl_sync(full, grp, l);
+    const bool in = (g >> lane) & 1u;
+    double a = in ? p : 0.0, b = in ? p * p : 0.0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      a += __shfl_xor_sync(full, a, o);
+      b += __shfl_xor_sync(full, b, o);
+    }
+    if (lane == l) { sp = a; sp2 = b; }
+  }
+  if (!lead) return;
+  if (mode == MCX_TALLY_BLOCK && cache_log2 > 0) {
+    const unsigned long long k = ((unsigned long long)(det + 1u) << 48) | (unsigned long long)bin;
+    const unsigned h = (unsigned)((k * 0x9E3779B97F4A7C15ull) >> (64 - cache_log2));
+    const unsigned long long prev = atomicCAS(&cache_key[h], 0ull, k);
+    if (prev == 0ull || prev == k) {
+      const size_t n = (size_t)1 << cache_log2;
+      atomicAdd(&cache_key[n + h], (unsigned long long)cnt);
+      atomicAdd(reinterpret_cast<double*>(&cache_key[2 * n + h]), sp);
+      atomicAdd(reinterpret_cast<double*>(&cache_key[3 * n + h]), sp2);
+      return;
+    }
+  }
+  tally_global(tallies[det] + bin, (unsigned long long)cnt, sp, sp2);
+}
+
+// Step 14 for one warp and one detector (all 32 lanes call it).
+__device__ __forceinline__ void tally_add(const DInstrument& I, int mode, const TallyCache& tc, unsigned det, bool on, long long bin,
+                                          double p) {
+  if (mode == MCX_TALLY_GLOBAL) {
+    if (on) tally_global(I.tallies[det] + bin, 1ull, p, p * p);
+  } else {
+    tally_add_aggregated(I.tallies, mode, tc.key, tc.log2, det, on, bin, p);
+  }
+}
+
+// the block's cache goes to global memory: one set of reductions per occupied slot (all threads of the block)
+__device__ __forceinline__ void tally_flush(const DInstrument& I, const TallyCache& tc) {
+  if (tc.log2 == 0) return;
+  const int n = 1 << tc.log2;
+  for (int h = threadIdx.x; h < n; h += kBlock) {
+    const unsigned long long k = tc.key[h];
+    if (k == 0ull) continue;
+    const unsigned det = (unsigned)(k >> 48) - 1u;
+    const unsigned long long bin = k & 0xFFFFFFFFFFFFull;
+    tally_global(I.tallies[det] + bin, tc.key[n + h], __longlong_as_double((long long)tc.key[2 * n + h]),
+                 __longlong_as_double((long long)tc.key[3 * n + h]));
+  }
+}
+
+// ------------------------------------------------------------------------------------------------------------
 // The megakernel.  FEAT selects which component kinds are compiled in; DUMP writes per-ray fates instead of
 // tallying; GATE compiles in the absorber gate.  Shared memory: the instrument image, per-block ray-accounting and
 // scheduling counters, (GATE) per-warp rings of survivors, the solids of every group, per-thread interval end
@@ -1096,7 +1187,8 @@ constexpr int kSmemSolids = 32;    // solids staged in shared memory (all groups
 
 // resident blocks per SM the register budget is held to: the voxel walk hides its byte loads with warps
 constexpr int min_blocks(int feat) {
-  return feat == F_VOXELS || feat == (F_SOLIDS | F_PRIM) || feat == (F_SOLIDS | F_MESH) || feat == (F_SOLIDS | F_MESH | F_PRIM) ? 3 : 1;
+  return feat == F_VOXELS || feat == (F_SOLIDS | F_PRIM) || feat == (F_SOLIDS | F_MESH) || feat == (F_SOLIDS | F_MESH | F_PRIM) ? 3
+         : feat == F_OPTICS ? 2 : 1;
 }
 
 template <int FEAT, bool DUMP, bool GATE>
@@ -1145,6 +1237,14 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
     }
   }
   double* len_s = reinterpret_cast<double*>(s_extra) + threadIdx.x;  // per-thread path length per material (voxel walk)
+  TallyCache tcache{nullptr, 0};
+  const int tally_mode = A.tally_mode;
+  if (!DUMP && !(FEAT & (F_SOLIDS | F_VOXELS)) && A.tally_cache_log2 > 0) {  // block-private tally cache (light chains only)
+    tcache.key = reinterpret_cast<unsigned long long*>(s_extra);
+    tcache.log2 = A.tally_cache_log2;
+    for (int k = threadIdx.x; k < (4 << tcache.log2); k += kBlock) tcache.key[k] = 0ull;
+    // (the barrier after the first ticket fetch below orders these stores before any update)
+  }
   const int lane = threadIdx.x & 31;
   const uint64_t first = A.first, n = A.n, seed = A.seed;
   const uint32_t* __restrict__ order = A.order;
@@ -1189,7 +1289,7 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
     for (int c = 1; c < c_end; ++c) {
       const DComponent& C = I.comps[c];
       const int kind = C.kind;  // warp-uniform
-      bool pass = true;
+      bool pass = true, tally_now = false;
       if ((FEAT & F_SOLIDS) && kind == MCX_SOLIDS) {  // whole warp: the mesh walk is warp-cooperative
         const int rc = trace_solids<(FEAT & F_MESH) != 0, (FEAT & F_PRIM) != 0>(I, C, ray, ep, tri_queue, alive, order != nullptr);
         if (alive && rc != 1) {
@@ -1215,17 +1315,13 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
           if (b >= 0) {
             bin = b;
             fate = MCX_FATE_DETECTED;
-            if (!DUMP) {
-              TallyBin* rec = I.tallies[C.u.detector.index] + b;
-              atomicAdd(&rec->N, 1ull);
-              atomicAdd(&rec->P, ray.p);
-              atomicAdd(&rec->P2, ray.p * ray.p);
-            }
+            tally_now = true;
           } else {
             fate = MCX_FATE_MISSED;  // monitors do not absorb: the ray goes on
           }
         }
       }
+      if (!DUMP && kind == MCX_DETECTOR) tally_add(I, tally_mode, tcache, (unsigned)C.u.detector.index, tally_now, bin, ray.p);  // whole warp
       if (alive) {
         if (kind != MCX_DETECTOR && pass) fate = MCX_FATE_MISSED;  // fate = what the last component said
         if (!pass) {
@@ -1351,6 +1447,7 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
   }
   if (!DUMP) {
     __syncthreads();
+    tally_flush(I, tcache);
     if (threadIdx.x < MCX_MAX_COMPONENTS + 4) {
       const unsigned v = s_cnt[threadIdx.x];
       if (v) {
@@ -1438,7 +1535,8 @@ template <int FEAT, bool DUMP, bool GATE>
 cudaError_t launch_one(const DInstrument* d_inst, int n_mats, const TraceArgs& A, cudaStream_t stream, int n_sm) {
   const size_t smem = kSmemBase + (GATE ? kRingBytes : 0) + ((FEAT & F_SOLIDS) ? kSmemSolids * sizeof(DSolid) + (size_t)A.cap_endpoints * kBlock * 9 : 0) +
                       ((FEAT & F_MESH) ? (size_t)kTriQueue * kBlock * sizeof(unsigned) : 0) +
-                      ((FEAT & F_VOXELS) ? (size_t)(n_mats + VC_COUNT) * kBlock * sizeof(double) : 0);
+                      ((FEAT & F_VOXELS) ? (size_t)(n_mats + VC_COUNT) * kBlock * sizeof(double) : 0) +
+                      ((!DUMP && !(FEAT & (F_SOLIDS | F_VOXELS)) && A.tally_cache_log2 > 0) ? ((size_t)32 << A.tally_cache_log2) : 0);
   static std::atomic<unsigned long long> configured{0ull};  // bit d: the opt-in below was made on device d
   int blocks_per_sm = 1, dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
