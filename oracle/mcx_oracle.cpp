@@ -21,11 +21,15 @@
 // DEGENERATE return), icosphere vs analytic sphere (levels 5 and 6), grid accelerator == brute force, no degenerate
 // ray in 1e6 through closed meshes, voxel closed forms and the paper's fixed-step marching as a
 // convergence cross-check, ellipse focal property, bilinear exactness, Darwin closed forms, detector binning, the
-// fate rule of chains with several monitors against plane geometry written out in numpy.
+// fate rule of chains with several monitors against plane geometry written out in numpy; compound refractive lens:
+// thin-lens deflection 2 N delta x / R, thick-stack focal length R / (2 N delta) + L / 6, plane-parallel slab
+// displacement by Snell's law, on-axis transmission exp(-mu N d), parabolic thickness profile, reversibility;
+// Darwin-Prins: g = kappa = 0 limit, closed form at eta = 0, numpy complex arithmetic; wavelength bins: lambda = hc / E.
 // Whole-config tallies of c1..c4 have no closed form: "parity unpinned" beyond those part-wise pins
 // (SURVEY.md 8(c) last row).
 #include <algorithm>
 #include <cmath>
+#include <complex>
 #include <cstdint>
 #include <cstring>
 #include <limits>
@@ -41,7 +45,8 @@ const double kHC_keV_A = 12.398419843;  // h*c in keV*Angstrom (SURVEY 8(c) conv
 // Interface structs (the oracle's own; the CUDA library has a different, unrelated ABI in include/mcx.h)
 // ---------------------------------------------------------------------------------------------------
 enum Kind { K_SOURCE = 0, K_SLIT_RECT = 1, K_SLIT_CIRC = 2, K_SOLIDS = 3, K_VOXELS = 4, K_MIRROR = 5,
-            K_CRYSTAL = 6, K_DETECTOR = 7 };
+            K_CRYSTAL = 6, K_DETECTOR = 7, K_LENS = 8 };
+enum DetMode { DET_ENERGY = 0, DET_WAVELENGTH = 1 };  // what the third detector axis bins (step 14 / 14b)
 enum PosMode { POS_POINT = 0, POS_DISK = 1, POS_GAUSS = 2 };
 enum DirMode { DIR_TARGET = 0, DIR_GAUSS = 1 };
 enum EMode { E_MONO = 0, E_UNIFORM = 1, E_SPECTRUM = 2 };
@@ -97,6 +102,16 @@ struct OrcComponent {
   // detector (step 14)
   double det_xmin, det_xmax, det_ymin, det_ymax, det_Emin, det_Emax;
   int64_t det_nx, det_ny, det_nE;
+  // ---- SURVEY.md 8(f) rows ----
+  int64_t det_mode;       // DetMode (step 14b): DET_WAVELENGTH bins lambda = hc / E [Angstrom] over [det_Emin, det_Emax]
+  // Darwin-Prins crystal (step 13b): absorption ratios g = Im(chi_0) / |chi_h|', kappa = Im(chi_h) / Re(chi_h); 0, 0 = Darwin
+  double xtal_g, xtal_kappa;
+  // compound refractive lens (step 16)
+  double lens_R, lens_d, lens_pitch, lens_ra;  // apex radius of curvature, web thickness, lens-to-lens pitch, aperture radius
+  int64_t lens_N, lens_material;               // number of double-sided lenses; material index of mu(E)
+  int64_t lens_nd;                             // points of the delta(E) table (refractive index n = 1 - delta)
+  const double* lens_dE;                       // keV, strictly increasing
+  const double* lens_delta;                    // > 0, log-log interpolated like mu(E) (step 7)
 };
 
 struct OrcRayFate {
@@ -459,6 +474,7 @@ struct Prepared {
   std::vector<std::vector<MeshPrep>> meshes;     // per component, per solid
   std::vector<MirrorPrep> mirrors;               // per component
   std::vector<int> det_index;                    // per component: detector ordinal or -1
+  std::vector<MuTable> lens_delta;               // per component: delta(E) of a lens as ln-tables
   bool use_grid;
 };
 
@@ -474,6 +490,7 @@ void prepare(Prepared* P, const OrcComponent* comps, int n_comps, const OrcMater
     }
   }
   P->cdf.resize(n_comps); P->meshes.resize(n_comps); P->mirrors.resize(n_comps); P->det_index.assign(n_comps, -1);
+  P->lens_delta.resize(n_comps);
   int ndet = 0;
   for (int c = 0; c < n_comps; ++c) {
     const OrcComponent& k = comps[c];
@@ -494,6 +511,14 @@ void prepare(Prepared* P, const OrcComponent* comps, int n_comps, const OrcMater
     }
     if (k.kind == K_MIRROR) P->mirrors[c] = mirror_prep(k.mir_p, k.mir_q, k.mir_theta);
     if (k.kind == K_DETECTOR) P->det_index[c] = ndet++;
+    if (k.kind == K_LENS) {
+      MuTable& t = P->lens_delta[c];
+      for (int64_t j = 0; j < k.lens_nd; ++j) {
+        t.E.push_back(k.lens_dE[j]);
+        t.lnE.push_back(std::log(k.lens_dE[j]));
+        t.lnMu.push_back(std::log(k.lens_delta[j]));
+      }
+    }
   }
 }
 
@@ -505,6 +530,20 @@ double darwin_R(double eta) {
   if (ae <= 1.0) return 1.0;
   const double s = ae + std::sqrt(ae * ae - 1.0);
   return 1.0 / (s * s);
+}
+
+// Step 13b (reading in DESIGN.md): Darwin-Prins curve of a thick ABSORBING crystal in symmetric
+// Bragg geometry (Zachariasen 1945, eq. 3.192 in reduced form): with the complex deviation parameter
+//   eta_c = (eta + i g) / (1 + i kappa),   g = Im(chi_0) / Re(chi_h) >= 0,  kappa = Im(chi_h) / Re(chi_h),
+// the reflectivity is R = |eta_c - s|^2, s = the square root of eta_c^2 - 1 for which |eta_c - s| <= 1.  Because
+// (eta_c - s)(eta_c + s) = 1 this is R = 1 / |eta_c + s|^2 with s the root whose inner product with eta_c is
+// non-negative: no cancellation.  g = kappa = 0 is the Darwin curve of step 13 (and is evaluated by darwin_R).
+double darwin_prins_R(double eta, double g, double kappa) {
+  if (g == 0.0 && kappa == 0.0) return darwin_R(eta);
+  const std::complex<double> ec = std::complex<double>(eta, g) / std::complex<double>(1.0, kappa);
+  std::complex<double> s = std::sqrt(ec * ec - 1.0);
+  if (ec.real() * s.real() + ec.imag() * s.imag() < 0.0) s = -s;
+  return 1.0 / std::norm(ec + s);
 }
 
 // Step 12: bilinear R(theta, E) on a uniform grid; theta above range is handled by the caller.
@@ -762,10 +801,67 @@ bool crystal(const OrcComponent& k, Ray* ray) {
   const double thetaB = std::asin(s);
   const double wD = k.xtal_zeta * std::tan(thetaB);
   const double eta = (theta - thetaB - k.xtal_delta0) / (0.5 * wD);
-  ray->p *= darwin_R(eta);
+  ray->p *= darwin_prins_R(eta, k.xtal_g, k.xtal_kappa);
   const V3 dr{d.x, -d.y, d.z};
   ray->r = to_lab_pos(k.R, k.T, V3{h.x, 0.0, h.z});
   ray->d = rotT(k.R, dr);
+  return true;
+}
+
+// Step 16 ("a stack of sixteen double-sided parabolic beryllium lenses",
+// where problem 2 spends its time).  Lens frame: z = axis of the stack, origin at its centre.  Lens i = 0..N-1 is centred
+// at z_i = (i - (N-1)/2) pitch and is material between two paraboloids of revolution, apex radius R, web thickness d:
+//   front surface  z = z_i - d/2 - rho^2 / (2R)   (the ray enters the material),
+//   back surface   z = z_i + d/2 + rho^2 / (2R)   (the ray leaves it),        rho^2 = x^2 + y^2.
+// The ray meets the 2N surfaces in order.  At each: intersection (the root of the quadratic that tends to the plane
+// intersection as R -> inf, in its cancellation-free form), aperture test rho <= r_a (outside: absorbed by the holder),
+// Snell's law in vector form with n = 1 - delta(E) inside the material.  With m = n_before / n_after, c = d.nrm > 0
+// (nrm = unit normal along +z) and c_t = sqrt(1 - m^2 (1 - c^2)):  d' = m d + (c_t - m c) nrm, where
+// c_t - m c = (1 - m)(1 + m) / (c_t + m c) and 1 - m is formed from delta directly (entering: -delta / (1 - delta),
+// leaving: delta), so the deflection, of relative size delta ~ 1e-6, carries no cancellation.  Total reflection or a
+// ray running backwards: absorbed.  Beer-Lambert with mu(E) of the lens material over the summed path inside the N lenses.
+bool lens(const Prepared& P, int c, Ray* ray) {
+  const OrcComponent& k = P.comps[c];
+  V3 o = to_local_pos(k.R, k.T, ray->r);
+  V3 d = rot(k.R, ray->d);
+  const double delta = mu_of_E(P.lens_delta[c], ray->E);  // the same log-log interpolation as mu(E), step 7
+  const double n_in = 1.0 - delta;
+  double path = 0.0;
+  for (int64_t surf = 0; surf < 2 * k.lens_N; ++surf) {
+    const int64_t i = surf / 2;
+    const bool entering = (surf % 2) == 0;
+    const double zc = ((double)i - 0.5 * (double)(k.lens_N - 1)) * k.lens_pitch;
+    const double sgn = entering ? -1.0 : 1.0;
+    const double z0 = zc + sgn * 0.5 * k.lens_d;
+    // F(r) = z - z0 - sgn rho^2 / (2R) = 0 along o + t d:  a t^2 + b t + cc = 0
+    const double a = -sgn * (d.x * d.x + d.y * d.y) / (2.0 * k.lens_R);
+    const double b = d.z - sgn * (o.x * d.x + o.y * d.y) / k.lens_R;
+    const double cc = o.z - z0 - sgn * (o.x * o.x + o.y * o.y) / (2.0 * k.lens_R);
+    if (!(b > 0.0)) return false;
+    const double disc = b * b - 4.0 * a * cc;
+    if (!(disc >= 0.0)) return false;
+    const double t = -2.0 * cc / (b + std::sqrt(disc));
+    if (t < 0.0) return false;
+    const V3 h = o + t * d;
+    if (h.x * h.x + h.y * h.y > k.lens_ra * k.lens_ra) return false;
+    if (!entering) path += t;  // d is unit: t is the length of the chord inside lens i
+    // unit normal along +z: grad F = (-sgn x / R, -sgn y / R, 1)
+    const V3 gr{-sgn * h.x / k.lens_R, -sgn * h.y / k.lens_R, 1.0};
+    const V3 nrm = (1.0 / std::sqrt(dot(gr, gr))) * gr;
+    const double cs = dot(d, nrm);
+    if (!(cs > 0.0)) return false;
+    const double m = entering ? 1.0 / n_in : n_in;
+    const double one_minus_m = entering ? -delta / n_in : delta;
+    const double under = 1.0 - m * m * (1.0 - cs * cs);
+    if (!(under > 0.0)) return false;  // total reflection
+    const double ct = std::sqrt(under);
+    const double coef = one_minus_m * (1.0 + m) / (ct + m * cs);
+    d = m * d + coef * nrm;
+    o = h;
+  }
+  ray->p *= std::exp(-mu_of_E(P.mats[k.lens_material], ray->E) * path);
+  ray->r = to_lab_pos(k.R, k.T, o);
+  ray->d = rotT(k.R, d);
   return true;
 }
 
@@ -775,7 +871,9 @@ int64_t detector_bin(const OrcComponent& k, const Ray& ray) {
   if (!plane_hit(k, ray, &h, &d)) return -1;
   const double fx = (h.x - k.det_xmin) / (k.det_xmax - k.det_xmin) * (double)k.det_nx;
   const double fy = (h.y - k.det_ymin) / (k.det_ymax - k.det_ymin) * (double)k.det_ny;
-  const double fe = (ray.E - k.det_Emin) / (k.det_Emax - k.det_Emin) * (double)k.det_nE;
+  // step 14b: an L_monitor bins the wavelength lambda = hc / E [Angstrom] instead of the energy
+  const double q = k.det_mode == DET_WAVELENGTH ? kHC_keV_A / ray.E : ray.E;
+  const double fe = (q - k.det_Emin) / (k.det_Emax - k.det_Emin) * (double)k.det_nE;
   const double ix = std::floor(fx), iy = std::floor(fy), ie = std::floor(fe);
   if (!(ix >= 0.0 && ix < (double)k.det_nx)) return -1;
   if (!(iy >= 0.0 && iy < (double)k.det_ny)) return -1;
@@ -816,6 +914,7 @@ int orc_trace(const OrcComponent* comps, int n_comps, const OrcMaterial* mats, i
         case K_VOXELS: voxels(P, c, &ray, &w); break;
         case K_MIRROR: alive = mirror(P, c, &ray); break;
         case K_CRYSTAL: alive = crystal(k, &ray); break;
+        case K_LENS: alive = lens(P, c, &ray); break;
         case K_DETECTOR: {
           const int64_t b = detector_bin(k, ray);
           if (b >= 0) {
@@ -918,6 +1017,7 @@ int orc_apply(const OrcComponent* comp, const OrcMaterial* mats, int n_mats, dou
     case K_VOXELS: voxels(P, 1, &ray, &w); break;
     case K_MIRROR: rc = mirror(P, 1, &ray) ? 1 : 0; break;
     case K_CRYSTAL: rc = crystal(two[1], &ray) ? 1 : 0; break;
+    case K_LENS: rc = lens(P, 1, &ray) ? 1 : 0; break;
     case K_DETECTOR: { const int64_t b = detector_bin(two[1], ray); if (bin) *bin = b; break; }
     default: rc = -100;
   }
@@ -927,6 +1027,7 @@ int orc_apply(const OrcComponent* comp, const OrcMaterial* mats, int n_mats, dou
 }
 
 double orc_darwin(double eta) { return darwin_R(eta); }
+double orc_darwin_prins(double eta, double g, double kappa) { return darwin_prins_R(eta, g, kappa); }
 double orc_bilinear(const OrcComponent* comp, double theta, double E) { return bilinear_R(*comp, theta, E); }
 // mirror constants out[8] = a, b, Z0, Y0, nZ, nY, tZ, tY
 void orc_mirror_prep(double p, double q, double theta, double* out) {

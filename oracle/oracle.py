@@ -16,7 +16,9 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "mcx_oracle.cpp")
 _LIB = os.path.join(_HERE, "liboracle_mcx.so")
 
-KIND = {"source": 0, "slit_rect": 1, "slit_circ": 2, "solids": 3, "voxels": 4, "mirror": 5, "crystal": 6, "detector": 7}
+KIND = {"source": 0, "slit_rect": 1, "slit_circ": 2, "solids": 3, "voxels": 4, "mirror": 5, "crystal": 6, "detector": 7,
+        "lens": 8}
+DET_MODE = {"energy": 0, "wavelength": 1}
 POS = {"point": 0, "disk": 1, "gauss": 2}
 DIR = {"target": 0, "gauss": 1}
 EMODE = {"mono": 0, "uniform": 1, "spectrum": 2}
@@ -58,7 +60,11 @@ class OrcComponent(C.Structure):
                 ("xtal_zeta", C.c_double), ("xtal_delta0", C.c_double),
                 ("det_xmin", C.c_double), ("det_xmax", C.c_double), ("det_ymin", C.c_double), ("det_ymax", C.c_double),
                 ("det_Emin", C.c_double), ("det_Emax", C.c_double),
-                ("det_nx", C.c_int64), ("det_ny", C.c_int64), ("det_nE", C.c_int64)]
+                ("det_nx", C.c_int64), ("det_ny", C.c_int64), ("det_nE", C.c_int64),
+                ("det_mode", C.c_int64), ("xtal_g", C.c_double), ("xtal_kappa", C.c_double),
+                ("lens_R", C.c_double), ("lens_d", C.c_double), ("lens_pitch", C.c_double), ("lens_ra", C.c_double),
+                ("lens_N", C.c_int64), ("lens_material", C.c_int64), ("lens_nd", C.c_int64), ("lens_dE", _dp),
+                ("lens_delta", _dp)]
 
 
 class OrcRayFate(C.Structure):
@@ -89,6 +95,8 @@ def lib():
         L.orc_mu.argtypes = [_dp, _dp, C.c_int64, C.c_double]
         L.orc_darwin.restype = C.c_double
         L.orc_darwin.argtypes = [C.c_double]
+        L.orc_darwin_prins.restype = C.c_double
+        L.orc_darwin_prins.argtypes = [C.c_double, C.c_double, C.c_double]
         L.orc_bilinear.restype = C.c_double
         L.orc_bilinear.argtypes = [C.POINTER(OrcComponent), C.c_double, C.c_double]
         L.orc_draw2.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint32, _dp, _dp]
@@ -173,10 +181,19 @@ def marshal_component(cd, keep):
     elif k == "crystal":
         c.xtal_length, c.xtal_width, c.xtal_d = cd["length"], cd["width"], cd["d_hkl"]
         c.xtal_zeta, c.xtal_delta0 = cd["zeta"], cd["delta0"]
+        c.xtal_g, c.xtal_kappa = cd.get("g", 0.0), cd.get("kappa", 0.0)
+    elif k == "lens":
+        c.lens_R, c.lens_d, c.lens_pitch, c.lens_ra = cd["radius"], cd["web"], cd["pitch"], cd["aperture"]
+        c.lens_N, c.lens_material = cd["n_lenses"], cd["material"]
+        dE = np.ascontiguousarray(cd["delta_table"]["E"], dtype=np.float64)
+        dl = np.ascontiguousarray(cd["delta_table"]["delta"], dtype=np.float64)
+        keep += [dE, dl]
+        c.lens_nd, c.lens_dE, c.lens_delta = len(dE), _ptr(dE), _ptr(dl)
     elif k == "detector":
         c.det_xmin, c.det_xmax, c.det_ymin, c.det_ymax = cd["xmin"], cd["xmax"], cd["ymin"], cd["ymax"]
         c.det_Emin, c.det_Emax = cd["Emin"], cd["Emax"]
         c.det_nx, c.det_ny, c.det_nE = cd["nx"], cd["ny"], cd["nE"]
+        c.det_mode = DET_MODE[cd.get("mode", "energy")]
     else:
         raise ValueError(k)
     return c
@@ -322,6 +339,10 @@ def darwin(eta):
     return lib().orc_darwin(float(eta))
 
 
+def darwin_prins(eta, g, kappa):
+    return lib().orc_darwin_prins(float(eta), float(g), float(kappa))
+
+
 def bilinear(mirror_comp, theta, E):
     keep = []
     c = marshal_component(mirror_comp, keep)
@@ -332,3 +353,39 @@ def mirror_prep(p, q, theta):
     out = (C.c_double * 8)()
     lib().orc_mirror_prep(C.c_double(p), C.c_double(q), C.c_double(theta), out)
     return dict(zip(("a", "b", "Z0", "Y0", "nZ", "nY", "tZ", "tY"), out[:]))
+
+
+def cnr(N, P, P2, ny, nx, nE, region_mat, region_ref, Emin, Emax, E_fit_min):
+    """Contrast-to-noise ratio of PAPER.md:257 Eq. (1), CNR = |I_mat - I_ref| / sqrt(sigma_mat^2 + sigma_ref^2), per
+    energy bin of one detector's tallies (arrays of ny*nx*nE, bin = (iy*nx + ix)*nE + iE), and its least-squares line
+    above E_fit_min ("A least-squares-fit was used to fit the CNR's for energies above the 80 keV").
+    Plain definition, numpy.  Readings: a region is a pixel rectangle (x0, x1, y0, y1), half-open; I = mean
+    over the region's pixels of the bin's weight sum P; the noise of a region is "the summed squared standard deviations
+    of the means": sigma_region^2 = sum_pixels sigma_bin^2 / n_pixels^2, with the McXtrace error estimate of a monitor
+    bin, sigma_bin^2 = N/(N-1) |P2 - (P/N)^2| for N > 1 and sigma_bin = P for N <= 1 (sqrt(N) for unit weights).
+    Returns (cnr[nE], intercept, slope); cnr = 0 where the noise is 0; the fit uses the bins whose centre energy is
+    >= E_fit_min (intercept = slope = 0 with fewer than two such bins)."""
+    N = np.asarray(N, dtype=np.float64).reshape(ny, nx, nE)
+    P = np.asarray(P, dtype=np.float64).reshape(ny, nx, nE)
+    P2 = np.asarray(P2, dtype=np.float64).reshape(ny, nx, nE)
+    Ns = np.where(N > 1, N, 2.0)
+    var = np.where(N > 1, Ns / (Ns - 1.0) * np.abs(P2 - (P / Ns) ** 2), P * P)
+
+    def region(r):
+        x0, x1, y0, y1 = r
+        n = (x1 - x0) * (y1 - y0)
+        return P[y0:y1, x0:x1, :].sum(axis=(0, 1)) / n, var[y0:y1, x0:x1, :].sum(axis=(0, 1)) / (n * n)
+
+    Im, vm = region(region_mat)
+    Ir, vr = region(region_ref)
+    noise = np.sqrt(vm + vr)
+    out = np.where(noise > 0, np.abs(Im - Ir) / np.where(noise > 0, noise, 1.0), 0.0)
+    Ec = Emin + (np.arange(nE) + 0.5) * (Emax - Emin) / nE
+    sel = Ec >= E_fit_min
+    a = b = 0.0
+    if sel.sum() >= 2:
+        x, y = Ec[sel], out[sel]
+        xm, ym = x.mean(), y.mean()
+        b = float(((x - xm) * (y - ym)).sum() / ((x - xm) ** 2).sum())
+        a = float(ym - b * xm)
+    return out, a, b

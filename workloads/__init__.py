@@ -95,16 +95,29 @@ def mirror_elliptic(p, q, theta, length, width, table, R=None, T=(0, 0, 0)):
     return d
 
 
-def crystal_bragg(length, width, d_hkl, zeta, delta0=0.0, R=None, T=(0, 0, 0)):
+def crystal_bragg(length, width, d_hkl, zeta, delta0=0.0, g=0.0, kappa=0.0, R=None, T=(0, 0, 0)):
+    """g, kappa: absorption ratios of the Darwin-Prins curve (0, 0 = the non-absorbing Darwin curve)."""
     d = {"kind": "crystal", "length": float(length), "width": float(width), "d_hkl": float(d_hkl),
-         "zeta": float(zeta), "delta0": float(delta0)}
+         "zeta": float(zeta), "delta0": float(delta0), "g": float(g), "kappa": float(kappa)}
     d.update(_pose(R, T))
     return d
 
 
-def detector(xmin, xmax, ymin, ymax, nx, ny, Emin, Emax, nE, R=None, T=(0, 0, 0)):
+def lens_parab(radius, web, pitch, aperture, n_lenses, material, delta_table, R=None, T=(0, 0, 0)):
+    """Stack of n_lenses double-sided parabolic lenses along the local z axis, centred on the component origin
+    (PAPER.md:134, 138).  radius: apex radius of curvature; web: thickness on the axis; pitch: lens-to-lens distance;
+    aperture: radius of the circular opening; delta_table: {"E": array, "delta": array}, n = 1 - delta(E)."""
+    d = {"kind": "lens", "radius": float(radius), "web": float(web), "pitch": float(pitch), "aperture": float(aperture),
+         "n_lenses": int(n_lenses), "material": int(material), "delta_table": delta_table}
+    d.update(_pose(R, T))
+    return d
+
+
+def detector(xmin, xmax, ymin, ymax, nx, ny, Emin, Emax, nE, R=None, T=(0, 0, 0), mode="energy"):
+    """mode "energy": the third axis bins E [keV] over [Emin, Emax); mode "wavelength" (an L_monitor): it
+    bins lambda = hc / E [Angstrom] over [Emin, Emax) read as wavelengths."""
     d = {"kind": "detector", "xmin": float(xmin), "xmax": float(xmax), "ymin": float(ymin), "ymax": float(ymax),
-         "nx": int(nx), "ny": int(ny), "Emin": float(Emin), "Emax": float(Emax), "nE": int(nE)}
+         "nx": int(nx), "ny": int(ny), "Emin": float(Emin), "Emax": float(Emax), "nE": int(nE), "mode": mode}
     d.update(_pose(R, T))
     return d
 
