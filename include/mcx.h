@@ -54,7 +54,7 @@ typedef enum {
                               every other ray. */
 } mcx_status;
 
-enum { MCX_MAX_COMPONENTS = 16, MCX_MAX_DETECTORS = 4, MCX_MAX_MATERIALS = 32, MCX_MAX_SOLIDS = 16 };
+enum { MCX_MAX_COMPONENTS = 16, MCX_MAX_DETECTORS = 8, MCX_MAX_MATERIALS = 32, MCX_MAX_SOLIDS = 16, MCX_MAX_LENSES = 256 };
 
 typedef enum {
   MCX_SOURCE = 0,          /* step 3 (point / flat / Gaussian emitters) */
@@ -64,13 +64,16 @@ typedef enum {
   MCX_VOXELS = 4,          /* step 11: uint8 material-ID volume, exact traversal */
   MCX_MIRROR_ELLIPTIC = 5, /* step 12 (optics category) */
   MCX_CRYSTAL_BRAGG = 6,   /* step 13 */
-  MCX_DETECTOR = 7         /* step 14: PSD / E / EPSD monitors */
+  MCX_DETECTOR = 7,        /* step 14: PSD / E / EPSD / L monitors */
+  MCX_LENS_PARAB = 8       /* step 16: compound refractive lens, a stack of double-sided parabolic lenses (PAPER.md:134,
+                              138, 153: where the paper's focusing instrument spends its time) */
 } mcx_kind;
 
 typedef enum { MCX_POS_POINT = 0, MCX_POS_DISK = 1, MCX_POS_GAUSS = 2 } mcx_pos_mode;
 typedef enum { MCX_DIR_TARGET = 0, MCX_DIR_GAUSS = 1 } mcx_dir_mode;
 typedef enum { MCX_E_MONO = 0, MCX_E_UNIFORM = 1, MCX_E_SPECTRUM = 2 } mcx_energy_mode;
 typedef enum { MCX_BOX = 0, MCX_CYLINDER = 1, MCX_SPHERE = 2, MCX_MESH = 3 } mcx_shape;
+typedef enum { MCX_DET_ENERGY = 0, MCX_DET_WAVELENGTH = 1 } mcx_det_mode;
 
 /* Fate of a ray (mcx_ray_fate.fate): >= 0 means "absorbed by the component with that chain index". */
 enum { MCX_FATE_DETECTED = -1, MCX_FATE_MISSED = -2, MCX_FATE_DEGENERATE = -3 };
@@ -146,11 +149,33 @@ typedef struct mcx_crystal_params {
   double d_hkl;             /* Angstrom */
   double zeta;              /* relative Darwin width: w_D = zeta tan(theta_B) */
   double delta0;            /* refraction offset of the curve centre, radians */
+  double g, kappa;          /* step 13b, Darwin-Prins curve of an absorbing crystal: g = Im(chi_0) / Re(chi_h) >= 0,
+                               kappa = Im(chi_h) / Re(chi_h); eta_c = (eta + i g) / (1 + i kappa), R = |eta_c - sqrt(eta_c^2 - 1)|^2
+                               on the branch with R <= 1.  0, 0: the non-absorbing Darwin curve of step 13 */
 } mcx_crystal_params;
+
+/* Step 16.  Lens frame: z = axis of the stack, origin at its centre.  Lens i = 0..n_lenses-1 is centred at
+ * z_i = (i - (n_lenses-1)/2) pitch; it is material between the paraboloids z = z_i -+ (web/2 + rho^2 / (2 radius)).  At each
+ * of the 2 n_lenses surfaces, in order: intersection, aperture test rho <= aperture (outside: absorbed), Snell's law with
+ * n = 1 - delta(E) (total reflection or a ray running backwards: absorbed).  Beer-Lambert with mu(E) of `material` over
+ * the summed chords inside the lenses.  Needs web/2 + aperture^2 / (2 radius) <= pitch/2 (the lenses do not overlap). */
+typedef struct mcx_lens_params {
+  double radius;            /* apex radius of curvature of the paraboloids */
+  double web;               /* thickness of a lens on the axis */
+  double pitch;             /* lens-to-lens distance */
+  double aperture;          /* radius of the circular opening */
+  int64_t n_lenses;         /* <= MCX_MAX_LENSES */
+  int64_t material;         /* index into the materials array: mu(E) of the lens material */
+  int64_t n_delta;          /* points of the delta(E) table, >= 2 */
+  const double* delta_energy_keV; /* HOST [n_delta], strictly increasing */
+  const double* delta;      /* HOST [n_delta], > 0; log-log interpolated like mu(E) (step 7) */
+} mcx_lens_params;
 
 typedef struct mcx_detector_params {
   double xmin, xmax, ymin, ymax, emin, emax; /* half-open bins */
   int64_t nx, ny, ne;
+  int64_t mode;             /* mcx_det_mode.  MCX_DET_WAVELENGTH (an L_monitor): the third axis bins
+                               lambda = hc / E in Angstrom over [emin, emax) read as wavelengths (step 14b) */
 } mcx_detector_params;
 
 typedef struct mcx_component {
@@ -165,6 +190,7 @@ typedef struct mcx_component {
     mcx_mirror_params mirror;
     mcx_crystal_params crystal;
     mcx_detector_params detector;
+    mcx_lens_params lens;
   } u;
 } mcx_component;
 
@@ -251,6 +277,26 @@ mcx_status mcx_tally_read_host(mcx_instrument* inst, int detector, uint64_t* N, 
 /* Bytes mcx_instrument_create copied from the host to the device for this handle (instrument image and tables; the
  * voxel volume is the caller's own upload). */
 uint64_t mcx_upload_bytes(const mcx_instrument* inst);
+
+/* Moves component `component` (a slit, voxel volume, mirror, crystal, lens or detector; not the source, not a solids
+ * group, whose solids carry their own poses) to a new pose for the traces enqueued after this call: the line-by-line scan
+ * of PAPER.md:190 ("550 lines per projection") translates the sample between traces.  Tallies are kept (read and reset
+ * them per line as needed).  The pose is read before the call returns.  A voxel volume keeps the memory layout chosen at
+ * create (fastest axis = the one most aligned with source -> volume); a pose that would change that choice is refused
+ * with MCX_ERR_UNSUPPORTED. */
+mcx_status mcx_instrument_set_pose(mcx_instrument* inst, int component, const mcx_pose* pose, void* cuda_stream);
+
+/* Contrast-to-noise ratio of PAPER.md:257 Eq. (1) per energy bin of one detector's finalised tallies, and its
+ * least-squares line above e_fit_min.  N, p, p2: DEVICE [ny*nx*ne] as written by mcx_tally_read.
+ * region_mat, region_ref: HOST int32[4] = pixel rectangles x0, x1, y0, y1 (half-open, inside the detector, non-empty).
+ * I_region = mean over its pixels of p; sigma_region^2 = sum over its pixels of sigma_bin^2 / n_pixels^2 with
+ * sigma_bin^2 = N/(N-1) |p2 - (p/N)^2| for N > 1 and sigma_bin = p for N <= 1;
+ * cnr_out[e] = |I_mat - I_ref| / sqrt(sigma_mat^2 + sigma_ref^2) (0 where the noise is 0): DEVICE [ne].
+ * fit_out: DEVICE [2] = intercept, slope of the least-squares line through (bin-centre energy, cnr) over the bins with
+ * centre >= e_fit_min (0, 0 with fewer than two such bins); emin, emax: the detector's energy range.  Asynchronous. */
+mcx_status mcx_cnr(const uint64_t* N, const double* p, const double* p2, int64_t nx, int64_t ny, int64_t ne,
+                   const int32_t* region_mat, const int32_t* region_ref, double emin, double emax, double e_fit_min,
+                   double* cnr_out, double* fit_out, void* cuda_stream);
 
 /* Zeroes all tallies and counters. */
 mcx_status mcx_tally_reset(mcx_instrument* inst, void* cuda_stream);

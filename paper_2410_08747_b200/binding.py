@@ -16,7 +16,9 @@ from . import build as _build
 MCX_OK = 0
 STATUS_NAMES = {0: "MCX_OK", 1: "MCX_ERR_INVALID_ARG", 2: "MCX_ERR_UNSUPPORTED", 3: "MCX_ERR_RANGE", 4: "MCX_ERR_WORKSPACE",
                 5: "MCX_ERR_CUDA", 6: "MCX_ERR_CAPACITY"}
-KIND = {"source": 0, "slit_rect": 1, "slit_circ": 2, "solids": 3, "voxels": 4, "mirror": 5, "crystal": 6, "detector": 7}
+KIND = {"source": 0, "slit_rect": 1, "slit_circ": 2, "solids": 3, "voxels": 4, "mirror": 5, "crystal": 6, "detector": 7,
+        "lens": 8}
+DET_MODE = {"energy": 0, "wavelength": 1}
 POS_MODE = {"point": 0, "disk": 1, "gauss": 2}
 DIR_MODE = {"target": 0, "gauss": 1}
 ENERGY_MODE = {"mono": 0, "uniform": 1, "spectrum": 2}
@@ -27,7 +29,7 @@ FATE_DETECTED, FATE_MISSED, FATE_DEGENERATE = -1, -2, -3
 
 EXPORTS = ["mcx_instrument_workspace_size", "mcx_instrument_create", "mcx_trace", "mcx_trace_range", "mcx_tally_read",
            "mcx_tally_read_host", "mcx_instrument_set_exec", "mcx_instrument_set_tuning", "mcx_upload_bytes", "mcx_tally_reset",
-           "mcx_counters_read", "mcx_trace_status", "mcx_trace_dump", "mcx_launch_count", "mcx_instrument_set_timing", "mcx_timing_read", "mcx_probe_dfma", "mcx_probe_tally",
+           "mcx_counters_read", "mcx_trace_status", "mcx_trace_dump", "mcx_launch_count", "mcx_instrument_set_timing", "mcx_timing_read", "mcx_instrument_set_pose", "mcx_cnr", "mcx_probe_dfma", "mcx_probe_tally",
            "mcx_probe_l2", "mcx_probe_latency", "mcx_instrument_destroy", "mcx_last_error"]
 MCX_ERR_CAPACITY = 6
 
@@ -77,18 +79,25 @@ class McxMirrorParams(C.Structure):
 
 class McxCrystalParams(C.Structure):
     _fields_ = [("length", C.c_double), ("width", C.c_double), ("d_hkl", C.c_double), ("zeta", C.c_double),
-                ("delta0", C.c_double)]
+                ("delta0", C.c_double), ("g", C.c_double), ("kappa", C.c_double)]
+
+
+class McxLensParams(C.Structure):
+    _fields_ = [("radius", C.c_double), ("web", C.c_double), ("pitch", C.c_double), ("aperture", C.c_double),
+                ("n_lenses", C.c_int64), ("material", C.c_int64), ("n_delta", C.c_int64), ("delta_energy_keV", _dp),
+                ("delta", _dp)]
 
 
 class McxDetectorParams(C.Structure):
     _fields_ = [("xmin", C.c_double), ("xmax", C.c_double), ("ymin", C.c_double), ("ymax", C.c_double),
-                ("emin", C.c_double), ("emax", C.c_double), ("nx", C.c_int64), ("ny", C.c_int64), ("ne", C.c_int64)]
+                ("emin", C.c_double), ("emax", C.c_double), ("nx", C.c_int64), ("ny", C.c_int64), ("ne", C.c_int64),
+                ("mode", C.c_int64)]
 
 
 class McxParamsUnion(C.Union):
     _fields_ = [("source", McxSourceParams), ("slit", McxSlitParams), ("solids", McxSolidsParams),
                 ("voxels", McxVoxelsParams), ("mirror", McxMirrorParams), ("crystal", McxCrystalParams),
-                ("detector", McxDetectorParams)]
+                ("detector", McxDetectorParams), ("lens", McxLensParams)]
 
 
 class McxComponent(C.Structure):
@@ -135,6 +144,11 @@ def lib(strict=False):
     L.mcx_instrument_set_timing.restype = C.c_int
     L.mcx_timing_read.argtypes = [vp, _dp, _dp, C.POINTER(C.c_int64)]
     L.mcx_timing_read.restype = C.c_int
+    L.mcx_instrument_set_pose.argtypes = [vp, C.c_int, C.POINTER(McxPose), vp]
+    L.mcx_instrument_set_pose.restype = C.c_int
+    L.mcx_cnr.argtypes = [vp, vp, vp, C.c_int64, C.c_int64, C.c_int64, C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.c_double,
+                          C.c_double, C.c_double, vp, vp, vp]
+    L.mcx_cnr.restype = C.c_int
     L.mcx_upload_bytes.argtypes = [vp]
     L.mcx_upload_bytes.restype = C.c_uint64
     L.mcx_tally_reset.argtypes = [vp, vp]
@@ -234,10 +248,20 @@ def marshal(inst, keep, device_voxels):
         elif k == "crystal":
             x = c.u.crystal
             x.length, x.width, x.d_hkl, x.zeta, x.delta0 = cd["length"], cd["width"], cd["d_hkl"], cd["zeta"], cd["delta0"]
+            x.g, x.kappa = cd.get("g", 0.0), cd.get("kappa", 0.0)
+        elif k == "lens":
+            l = c.u.lens
+            l.radius, l.web, l.pitch, l.aperture = cd["radius"], cd["web"], cd["pitch"], cd["aperture"]
+            l.n_lenses, l.material = cd["n_lenses"], cd["material"]
+            dE = np.ascontiguousarray(cd["delta_table"]["E"], dtype=np.float64)
+            dl = np.ascontiguousarray(cd["delta_table"]["delta"], dtype=np.float64)
+            keep += [dE, dl]
+            l.n_delta, l.delta_energy_keV, l.delta = len(dE), _ptr(dE), _ptr(dl)
         elif k == "detector":
             d = c.u.detector
             d.xmin, d.xmax, d.ymin, d.ymax = cd["xmin"], cd["xmax"], cd["ymin"], cd["ymax"]
             d.emin, d.emax, d.nx, d.ny, d.ne = cd["Emin"], cd["Emax"], cd["nx"], cd["ny"], cd["nE"]
+            d.mode = DET_MODE[cd.get("mode", "energy")]
         else:
             raise ValueError(f"unknown component kind {k!r}")
     mats = (McxMaterial * max(1, len(inst["materials"])))()
@@ -347,6 +371,24 @@ class Instrument:
         a, b, n = C.c_double(), C.c_double(), C.c_int64()
         _check(self.L.mcx_timing_read(self.handle, C.byref(a), C.byref(b), C.byref(n)), self.L)
         return {"sort_ms": a.value, "trace_ms": b.value, "launches": int(n.value)}
+
+    def set_pose(self, component, R=None, T=(0.0, 0.0, 0.0)):
+        """mcx_instrument_set_pose: new pose (rotation rows R, origin T) of a component for the traces enqueued next."""
+        pose = McxPose()
+        _set_pose(pose, {"R": np.eye(3) if R is None else R, "T": T})
+        _check(self.L.mcx_instrument_set_pose(self.handle, int(component), C.byref(pose), self._stream()), self.L)
+
+    def cnr(self, detector, region_mat, region_ref, e_fit_min, tallies=None):
+        """mcx_cnr on the tallies of `detector` (read with mcx_tally_read unless given): (cnr[nE], fit[2]) device tensors."""
+        torch = self.torch
+        d = self.dets[detector]
+        N, P, P2 = self.tally(detector) if tallies is None else tallies
+        out = torch.empty(d["nE"], dtype=torch.float64, device=self.device)
+        fit = torch.empty(2, dtype=torch.float64, device=self.device)
+        rm, rr = (C.c_int32 * 4)(*region_mat), (C.c_int32 * 4)(*region_ref)
+        _check(self.L.mcx_cnr(N.data_ptr(), P.data_ptr(), P2.data_ptr(), d["nx"], d["ny"], d["nE"], rm, rr, d["Emin"], d["Emax"],
+                              float(e_fit_min), out.data_ptr(), fit.data_ptr(), self._stream()), self.L)
+        return out, fit
 
     def upload_bytes(self):
         """host -> device bytes moved to build this instrument (tables by create + the voxel volume)."""

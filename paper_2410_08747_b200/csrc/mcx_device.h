@@ -99,6 +99,15 @@ struct DMirror {
 
 struct DCrystal {
   double half_length, half_width, d_hkl, zeta, delta0;
+  double g, kappa;  // step 13b (Darwin-Prins); 0, 0 = Darwin
+};
+
+// Step 16: a stack of double-sided parabolic lenses.  delta(E) is kept as the same ln-tables as mu(E).
+struct DLens {
+  double inv_R, half_inv_R;  // 1 / R, 1 / (2 R)
+  double half_web, pitch, ra2;
+  int n_lenses, material;
+  DMaterial delta;
 };
 
 struct DDetector {
@@ -106,6 +115,7 @@ struct DDetector {
   double sx, sy, se;  // bins per unit: nx / (xmax - xmin), ...
   int nx, ny, ne, index;
   uint64_t n_bins;
+  int mode, pad;  // mcx_det_mode
 };
 
 struct DComponent {
@@ -120,6 +130,7 @@ struct DComponent {
     DMirror mirror;
     DCrystal crystal;
     DDetector detector;
+    DLens lens;
   } u;
 };
 
@@ -145,7 +156,7 @@ static_assert(sizeof(DInstrument) % 16 == 0, "copied to shared memory as int4");
 static_assert(sizeof(TallyBin) == 32, "one tally record per 32-byte sector");
 
 // feature bits: select the kernel instantiation (code for absent component kinds is compiled out)
-enum { F_SOLIDS = 1, F_MESH = 2, F_VOXELS = 4, F_OPTICS = 8, F_PRIM = 16, F_ALL = 31 };  // F_SOLIDS: a solids group; F_PRIM / F_MESH: what it holds
+enum { F_SOLIDS = 1, F_MESH = 2, F_VOXELS = 4, F_OPTICS = 8, F_PRIM = 16, F_LENS = 32, F_ALL = 63 };  // F_SOLIDS: a solids group; F_PRIM / F_MESH: what it holds
 
 // One trace launch: rays first + offset(q) for positions q in [0, n); offset(q) = order[q] if order != null, else q.
 struct TraceArgs {
@@ -174,6 +185,9 @@ cudaError_t launch_tally_read(const TallyBin* bins, uint64_t n_bins, unsigned lo
                               cudaStream_t stream);
 cudaError_t launch_voxel_relayout(const uint8_t* src, uint8_t* dst, int nx, int ny, int nz, int fast, int a1, int a2,
                                   int pitch, int run_dir, int n_mats, cudaStream_t stream);
+cudaError_t launch_cnr(const unsigned long long* N, const double* p, const double* p2, int nx, int ny, int ne, const int* region_mat,
+                       const int* region_ref, double emin, double emax, double e_fit_min, double* cnr_out, double* fit_out,
+                       cudaStream_t stream);
 cudaError_t launch_probe_dfma(double* sink, int n_blocks, long long n_iters, cudaStream_t stream);
 cudaError_t launch_probe_tally(void* table, unsigned long long n_records, int n_blocks, long long n_iters, cudaStream_t stream);
 cudaError_t launch_probe_l2(const void* table, unsigned long long n_bytes, uint32_t* sink, int n_blocks, long long n_iters,

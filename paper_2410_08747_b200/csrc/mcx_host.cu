@@ -26,7 +26,9 @@ struct mcx_instrument {
   int cap_endpoints = 16;               // interval endpoints per ray and solids group (shared memory of the trace kernel)
   int gate_max = 0;                     // leading slits / mirrors / crystals of the chain (TraceArgs::gate_max)
   bool sort_pays = false;               // AUTO lane scheduling: detector-tile order
-  uint64_t det_bins[MCX_MAX_DETECTORS] = {0, 0, 0, 0};
+  uint64_t det_bins[MCX_MAX_DETECTORS] = {};
+  mcx_pose source_pose;                 // for mcx_instrument_set_pose on a voxel volume (layout check)
+  mcx_voxels_params voxel_params[MCX_MAX_COMPONENTS];  // sizes of the voxel components (same purpose)
   uint64_t launches = 0;
   // lane scheduling (row a13)
   int exec_mode = MCX_EXEC_AUTO;
@@ -263,6 +265,10 @@ mcx_status make_plan(const mcx_component* comps, int n_comps, const mcx_material
         }
         break;
       case MCX_SLIT_RECT: case MCX_SLIT_CIRC: case MCX_CRYSTAL_BRAGG: break;
+      case MCX_LENS_PARAB:
+        if (C.u.lens.n_delta < 2) return fail(MCX_ERR_INVALID_ARG, "component %d: the delta(E) table needs >= 2 points", c);
+        P->off_table[c] = A.reserve((size_t)C.u.lens.n_delta * 4 * sizeof(double));
+        break;
       case MCX_SOLIDS: {
         const mcx_solids_params& G = C.u.solids;
         if (G.n_solids < 0 || G.n_solids > MCX_MAX_SOLIDS) return fail(MCX_ERR_UNSUPPORTED, "component %d: more than %d solids", c, MCX_MAX_SOLIDS);
@@ -636,6 +642,44 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
         if (!(X.d_hkl > 0.0) || !(X.zeta > 0.0)) MCX_BAIL(MCX_ERR_INVALID_ARG, "component %d: d_hkl and zeta must be positive", c);
         D.u.crystal.half_length = 0.5 * X.length; D.u.crystal.half_width = 0.5 * X.width;
         D.u.crystal.d_hkl = X.d_hkl; D.u.crystal.zeta = X.zeta; D.u.crystal.delta0 = X.delta0;
+        if (!(X.g >= 0.0) || !std::isfinite(X.kappa)) MCX_BAIL(MCX_ERR_INVALID_ARG, "component %d: g must be >= 0 and kappa finite", c);
+        D.u.crystal.g = X.g; D.u.crystal.kappa = X.kappa;
+        break;
+      }
+      case MCX_LENS_PARAB: {
+        features |= F_LENS;
+        const mcx_lens_params& L = C.u.lens;
+        DLens& d = D.u.lens;
+        if (!(L.radius > 0.0) || !(L.web >= 0.0) || !(L.pitch > 0.0) || !(L.aperture > 0.0))
+          MCX_BAIL(MCX_ERR_INVALID_ARG, "component %d: radius, pitch, aperture must be positive, web non-negative", c);
+        if (L.n_lenses < 1 || L.n_lenses > MCX_MAX_LENSES) MCX_BAIL(MCX_ERR_UNSUPPORTED, "component %d: 1..%d lenses", c, MCX_MAX_LENSES);
+        if (L.material < 0 || L.material >= n_materials) MCX_BAIL(MCX_ERR_INVALID_ARG, "component %d: lens material out of range", c);
+        if (0.5 * L.web + L.aperture * L.aperture / (2.0 * L.radius) > 0.5 * L.pitch * (1.0 + 1e-12))
+          MCX_BAIL(MCX_ERR_INVALID_ARG, "component %d: lenses overlap (web/2 + aperture^2 / (2 radius) > pitch/2)", c);
+        if (!L.delta_energy_keV || !L.delta) MCX_BAIL(MCX_ERR_INVALID_ARG, "component %d: null delta table", c);
+        d.inv_R = 1.0 / L.radius; d.half_inv_R = 1.0 / (2.0 * L.radius);
+        d.half_web = 0.5 * L.web; d.pitch = L.pitch; d.ra2 = L.aperture * L.aperture;
+        d.n_lenses = (int)L.n_lenses; d.material = (int)L.material;
+        const size_t n = (size_t)L.n_delta;
+        double* E = (double*)host_ptr(P.off_table[c]);
+        double* lnE = E + n;
+        double* lnD = lnE + n;
+        double* slope = lnD + n;
+        for (size_t j = 0; j < n; ++j) {
+          if (!(L.delta_energy_keV[j] > 0.0) || !(L.delta[j] > 0.0)) MCX_BAIL(MCX_ERR_RANGE, "component %d: non-positive delta table entry %zu", c, j);
+          if (j > 0 && !(L.delta_energy_keV[j] > L.delta_energy_keV[j - 1])) MCX_BAIL(MCX_ERR_RANGE, "component %d: delta energies not increasing at %zu", c, j);
+          E[j] = L.delta_energy_keV[j];
+          lnE[j] = std::log(L.delta_energy_keV[j]);
+          lnD[j] = std::log(L.delta[j]);
+        }
+        for (size_t j = 0; j + 1 < n; ++j) slope[j] = (lnD[j + 1] - lnD[j]) / (lnE[j + 1] - lnE[j]);
+        slope[n - 1] = 0.0;
+        d.delta.n = (int)n;
+        d.delta.E = (const double*)dev_ptr(P.off_table[c]);
+        d.delta.lnE = d.delta.E + n;
+        d.delta.lnMu = d.delta.lnE + n;
+        d.delta.slope = d.delta.lnMu + n;
+        d.delta.inv_dlnE = (double)(n - 1) / (lnE[n - 1] - lnE[0]);
         break;
       }
       case MCX_DETECTOR: {
@@ -643,6 +687,8 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
         if (!(T.xmax > T.xmin) || !(T.ymax > T.ymin) || !(T.emax > T.emin)) MCX_BAIL(MCX_ERR_RANGE, "component %d: empty detector range", c);
         DDetector& d = D.u.detector;
         d.xmin = T.xmin; d.xmax = T.xmax; d.ymin = T.ymin; d.ymax = T.ymax; d.emin = T.emin; d.emax = T.emax;
+        if (T.mode != MCX_DET_ENERGY && T.mode != MCX_DET_WAVELENGTH) MCX_BAIL(MCX_ERR_INVALID_ARG, "component %d: bad detector mode", c);
+        d.mode = (int)T.mode;
         d.nx = (int)T.nx; d.ny = (int)T.ny; d.ne = (int)T.ne; d.index = n_dets;
         d.sx = (double)T.nx / (T.xmax - T.xmin); d.sy = (double)T.ny / (T.ymax - T.ymin); d.se = (double)T.ne / (T.emax - T.emin);
         d.n_bins = (uint64_t)T.nx * T.ny * T.ne;
@@ -660,6 +706,9 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
   I.counters = (unsigned long long*)dev_ptr(P.off_counters);
   H->n_dets = n_dets;
   H->features = features;
+  H->source_pose = components[0].pose;
+  for (int c = 0; c < n_components; ++c)
+    if (components[c].kind == MCX_VOXELS) H->voxel_params[c] = components[c].u.voxels;
   H->cap_endpoints = cap_endpoints;
   for (int c = 1; c + 1 < n_components; ++c) {
       const int k = components[c].kind;
@@ -826,6 +875,52 @@ mcx_status mcx_tally_read_host(mcx_instrument* inst, int detector, uint64_t* N, 
   if (e == cudaSuccess) e = cudaMemcpyAsync(p2, dP2, n_bins * sizeof(double), cudaMemcpyDeviceToHost, stream);
   if (e != cudaSuccess) return cuda_fail(e, "tally copy to the host");
   return st;
+}
+
+mcx_status mcx_instrument_set_pose(mcx_instrument* inst, int component, const mcx_pose* pose, void* cuda_stream) {
+  if (!inst || !pose) return fail(MCX_ERR_INVALID_ARG, "null argument");
+  if (component < 1 || component >= inst->n_comps) return fail(MCX_ERR_INVALID_ARG, "component %d out of range (1..%d)", component, inst->n_comps - 1);
+  if (!pose_ok(*pose)) return fail(MCX_ERR_INVALID_ARG, "pose is not finite");
+  DComponent& D = inst->host_image.comps[component];
+  if (D.kind == MCX_SOLIDS) return fail(MCX_ERR_UNSUPPORTED, "component %d is a solids group: its solids carry their own poses", component);
+  if (D.kind == MCX_VOXELS) {  // the traversal layout was chosen at create from the old pose
+    mcx_component src, vox;
+    std::memset(&src, 0, sizeof(src));
+    std::memset(&vox, 0, sizeof(vox));
+    src.pose = inst->source_pose;
+    vox.pose = *pose;
+    vox.u.voxels = inst->voxel_params[component];
+    int fast, a1, a2, run_dir;
+    voxel_axes(src, vox, &fast, &a1, &a2, &run_dir);
+    if (fast != D.u.voxels.fast || run_dir != D.u.voxels.run_dir)
+      return fail(MCX_ERR_UNSUPPORTED, "component %d: the new pose would change the voxel layout (fast axis %d -> %d); create a new instrument",
+                  component, D.u.voxels.fast, fast);
+  }
+  mcx_status st = check_sticky();
+  if (st != MCX_OK) return st;
+  copy_pose(&D.pose, *pose);
+  // host_image outlives the copy: pageable memory is staged before cudaMemcpyAsync returns
+  const size_t off = (size_t)((const unsigned char*)&D.pose - (const unsigned char*)&inst->host_image);
+  const cudaError_t e = cudaMemcpyAsync(inst->workspace + off, &D.pose, sizeof(DPose), cudaMemcpyHostToDevice, (cudaStream_t)cuda_stream);
+  if (e != cudaSuccess) return cuda_fail(e, "pose upload");
+  return MCX_OK;
+}
+
+mcx_status mcx_cnr(const uint64_t* N, const double* p, const double* p2, int64_t nx, int64_t ny, int64_t ne, const int32_t* region_mat,
+                   const int32_t* region_ref, double emin, double emax, double e_fit_min, double* cnr_out, double* fit_out,
+                   void* cuda_stream) {
+  if (!N || !p || !p2 || !region_mat || !region_ref || !cnr_out || !fit_out) return fail(MCX_ERR_INVALID_ARG, "null argument");
+  if (nx < 1 || ny < 1 || ne < 1 || nx > (1 << 20) || ny > (1 << 20) || ne > (1 << 20)) return fail(MCX_ERR_INVALID_ARG, "bad detector shape");
+  if (!(emax > emin)) return fail(MCX_ERR_RANGE, "empty energy range");
+  for (const int32_t* r : {region_mat, region_ref})
+    if (r[0] < 0 || r[1] > nx || r[0] >= r[1] || r[2] < 0 || r[3] > ny || r[2] >= r[3])
+      return fail(MCX_ERR_INVALID_ARG, "region (%d, %d, %d, %d) is empty or outside the %lld x %lld detector", r[0], r[1], r[2], r[3], (long long)nx, (long long)ny);
+  mcx_status st = check_sticky();
+  if (st != MCX_OK) return st;
+  const cudaError_t e = launch_cnr((const unsigned long long*)N, p, p2, (int)nx, (int)ny, (int)ne, region_mat, region_ref, emin, emax,
+                                   e_fit_min, cnr_out, fit_out, (cudaStream_t)cuda_stream);
+  if (e != cudaSuccess) return cuda_fail(e, "cnr launch");
+  return MCX_OK;
 }
 
 uint64_t mcx_upload_bytes(const mcx_instrument* inst) { return inst ? (uint64_t)inst->upload_bytes : 0; }

@@ -158,7 +158,9 @@ __device__ __forceinline__ long long detector_bin(const DComponent& C, const Ray
   // oracle's order of operations by 2 ulp, i.e. only for a ray within 1e-15 of a bin edge
   const double fx = floor((h.x - D.xmin) * D.sx);
   const double fy = floor((h.y - D.ymin) * D.sy);
-  const double fe = floor((ray.E - D.emin) * D.se);
+  // step 14b: an L_monitor bins lambda = hc / E [Angstrom]
+  const double q = D.mode == MCX_DET_WAVELENGTH ? 12.398419843 / ray.E : ray.E;
+  const double fe = floor((q - D.emin) * D.se);
   if (!(fx >= 0.0 && fx < (double)D.nx)) return -1;
   if (!(fy >= 0.0 && fy < (double)D.ny)) return -1;
   if (!(fe >= 0.0 && fe < (double)D.ne)) return -1;
@@ -967,6 +969,82 @@ __device__ __forceinline__ bool trace_mirror(const DComponent& C, Ray& ray) {
   return false;
 }
 
+// Step 13b: Darwin-Prins curve of an absorbing crystal.  eta_c = (eta + i g) / (1 + i kappa); R = 1 / |eta_c + s|^2 with s
+// the square root of eta_c^2 - 1 whose inner product with eta_c is non-negative (then |eta_c + s| >= 1: no cancellation).
+__device__ __forceinline__ double darwin_prins(double eta, double g, double kappa) {
+  // (eta + i g) / (1 + i kappa) by the plain formula: |kappa| is small, nothing over- or underflows
+  const double den = 1.0 + kappa * kappa;
+  const double er = (eta + g * kappa) / den, ei = (g - eta * kappa) / den;
+  // w = eta_c^2 - 1
+  const double wr = er * er - ei * ei - 1.0, wi = 2.0 * er * ei;
+  // principal square root of w: sr = sqrt((|w| + wr) / 2) without cancellation, si = wi / (2 sr) (or the mirrored form)
+  const double mod = hypot(wr, wi);
+  double sr, si;
+  if (mod == 0.0) {
+    sr = 0.0; si = 0.0;
+  } else if (wr >= 0.0) {
+    sr = sqrt(0.5 * (mod + wr));
+    si = wi / (2.0 * sr);
+  } else {
+    const double t = sqrt(0.5 * (mod - wr));
+    sr = fabs(wi) / (2.0 * t);
+    si = wi < 0.0 ? -t : t;
+  }
+  if (er * sr + ei * si < 0.0) { sr = -sr; si = -si; }
+  const double ar = er + sr, ai = ei + si;
+  return 1.0 / (ar * ar + ai * ai);
+}
+
+// Step 16: compound refractive lens, DLens.  The ray meets the 2 N paraboloids in order; at each:
+// the root of the intersection quadratic that tends to the plane intersection as R -> inf, in its cancellation-free form;
+// aperture test; Snell's law in vector form, d' = m d + (c_t - m c) nrm with c_t - m c = (1 - m)(1 + m) / (c_t + m c) and
+// 1 - m formed from delta directly, so the deflection (relative size delta ~ 1e-6) carries no cancellation.
+__device__ __forceinline__ bool trace_lens(const DInstrument& I, const DComponent& C, Ray& ray) {
+  const DLens& L = C.u.lens;
+  Vec3 o = to_local(C.pose, ray.r);
+  Vec3 d = rotate(C.pose.R, ray.d);
+  const double lnE = log(ray.E);
+  const double delta = mu_of(L.delta, ray.E, lnE);
+  const double n_in = 1.0 - delta;
+  const double m_in = 1.0 / n_in, omm_in = -delta / n_in;  // entering: m = 1 / n, 1 - m = -delta / n
+  double path = 0.0;
+  const int n_surf = 2 * L.n_lenses;
+  const double mid = 0.5 * (double)(L.n_lenses - 1);
+  for (int surf = 0; surf < n_surf; ++surf) {
+    const bool entering = (surf & 1) == 0;
+    const double zc = ((double)(surf >> 1) - mid) * L.pitch;
+    const double sgn = entering ? -1.0 : 1.0;
+    const double z0 = zc + sgn * L.half_web;
+    const double a = -sgn * (d.x * d.x + d.y * d.y) * L.half_inv_R;
+    const double b = d.z - sgn * (o.x * d.x + o.y * d.y) * L.inv_R;
+    const double cc = o.z - z0 - sgn * (o.x * o.x + o.y * o.y) * L.half_inv_R;
+    if (!(b > 0.0)) return false;
+    const double disc = b * b - 4.0 * a * cc;
+    if (!(disc >= 0.0)) return false;
+    const double t = -2.0 * cc / (b + sqrt(disc));
+    if (t < 0.0) return false;
+    const Vec3 h = o + t * d;
+    if (h.x * h.x + h.y * h.y > L.ra2) return false;
+    if (!entering) path += t;
+    const Vec3 gr{-sgn * h.x * L.inv_R, -sgn * h.y * L.inv_R, 1.0};
+    const Vec3 nrm = (1.0 / sqrt(dot(gr, gr))) * gr;
+    const double cs = dot(d, nrm);
+    if (!(cs > 0.0)) return false;
+    const double m = entering ? m_in : n_in;
+    const double one_minus_m = entering ? omm_in : delta;
+    const double under = 1.0 - m * m * (1.0 - cs * cs);
+    if (!(under > 0.0)) return false;  // total reflection
+    const double ct = sqrt(under);
+    const double coef = one_minus_m * (1.0 + m) / (ct + m * cs);
+    d = m * d + coef * nrm;
+    o = h;
+  }
+  ray.p *= exp(-mu_of(I.mats[L.material], ray.E, lnE) * path);
+  ray.r = to_lab(C.pose, o);
+  ray.d = rotate_back(C.pose.R, d);
+  return true;
+}
+
 // Step 13: symmetric Bragg reflection off a thick non-absorbing crystal (Darwin curve).
 __device__ __forceinline__ bool trace_crystal(const DComponent& C, Ray& ray) {
   const DCrystal& X = C.u.crystal;
@@ -983,10 +1061,15 @@ __device__ __forceinline__ bool trace_crystal(const DComponent& C, Ray& ray) {
   if (!(s < 1.0)) return false;
   const double theta_b = asin(s);
   const double w_d = X.zeta * tan(theta_b);
-  const double eta = fabs((theta - theta_b - X.delta0) / (0.5 * w_d));
-  if (eta > 1.0) {
-    const double g = eta + sqrt(eta * eta - 1.0);
-    ray.p *= 1.0 / (g * g);
+  const double eta_s = (theta - theta_b - X.delta0) / (0.5 * w_d);
+  if (X.g != 0.0 || X.kappa != 0.0) {
+    ray.p *= darwin_prins(eta_s, X.g, X.kappa);
+  } else {
+    const double eta = fabs(eta_s);
+    if (eta > 1.0) {
+      const double g = eta + sqrt(eta * eta - 1.0);
+      ray.p *= 1.0 / (g * g);
+    }
   }
   ray.r = to_lab(C.pose, Vec3{hp.x, 0.0, hp.z});
   ray.d = rotate_back(C.pose.R, Vec3{d.x, -d.y, d.z});
@@ -1188,7 +1271,7 @@ constexpr int kSmemSolids = 32;    // solids staged in shared memory (all groups
 // resident blocks per SM the register budget is held to: the voxel walk hides its byte loads with warps
 constexpr int min_blocks(int feat) {
   return feat == F_VOXELS || feat == (F_SOLIDS | F_PRIM) || feat == (F_SOLIDS | F_MESH) || feat == (F_SOLIDS | F_MESH | F_PRIM) ? 3
-         : feat == F_OPTICS ? 2 : 1;
+         : (feat == F_OPTICS || feat == F_LENS) ? 2 : 1;
 }
 
 template <int FEAT, bool DUMP, bool GATE>
@@ -1239,7 +1322,7 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
   double* len_s = reinterpret_cast<double*>(s_extra) + threadIdx.x;  // per-thread path length per material (voxel walk)
   TallyCache tcache{nullptr, 0};
   const int tally_mode = A.tally_mode;
-  if (!DUMP && !(FEAT & (F_SOLIDS | F_VOXELS)) && A.tally_cache_log2 > 0) {  // block-private tally cache (light chains only)
+  if (!DUMP && !(FEAT & (F_SOLIDS | F_VOXELS)) && A.tally_cache_log2 > 0) {  // block-private tally cache (chains without solids or voxels)
     tcache.key = reinterpret_cast<unsigned long long*>(s_extra);
     tcache.log2 = A.tally_cache_log2;
     for (int k = threadIdx.x; k < (4 << tcache.log2); k += kBlock) tcache.key[k] = 0ull;
@@ -1310,6 +1393,8 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
           pass = trace_mirror(C, ray);
         } else if ((FEAT & F_OPTICS) && kind == MCX_CRYSTAL_BRAGG) {
           pass = trace_crystal(C, ray);
+        } else if ((FEAT & F_LENS) && kind == MCX_LENS_PARAB) {
+          pass = trace_lens(I, C, ray);
         } else if (kind == MCX_DETECTOR) {
           const long long b = detector_bin(C, ray);
           if (b >= 0) {
@@ -1599,6 +1684,7 @@ cudaError_t launch_trace(const DInstrument* d_inst, int features, int n_mats, co
     case F_SOLIDS | F_MESH | F_PRIM: MCX_DISPATCH(F_SOLIDS | F_MESH | F_PRIM)
     case F_VOXELS: MCX_DISPATCH(F_VOXELS)
     case F_OPTICS: MCX_DISPATCH_GATED(F_OPTICS)
+    case F_LENS: MCX_DISPATCH_GATED(F_LENS)
     default: MCX_DISPATCH_GATED(F_ALL)
   }
 #undef MCX_DISPATCH
@@ -1712,6 +1798,88 @@ cudaError_t launch_probe_latency(void* table, unsigned long long n_bytes, uint32
   const unsigned long long n_sectors = n_bytes / 32;
   probe_chain_init_kernel<<<1024, 256, 0, stream>>>(reinterpret_cast<unsigned long long*>(table), n_sectors);
   probe_latency_kernel<<<n_blocks, n_threads, 0, stream>>>(reinterpret_cast<const unsigned long long*>(table), n_sectors, sink, n_iters);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Contrast-to-noise ratio of PAPER.md:257 Eq. (1) (include/mcx.h, mcx_cnr).  One block per energy bin sums, over the pixels
+// of the two regions, the bin's weight sums and its McXtrace error estimates (fixed-order tree: deterministic); one more
+// block fits the least-squares line through the bins above e_fit_min.
+// ------------------------------------------------------------------------------------------------------------
+struct CnrRegions {
+  int mat[4], ref[4];  // x0, x1, y0, y1
+};
+
+__device__ __forceinline__ double block_sum(double v, double* s_red) {
+  __syncthreads();
+  s_red[threadIdx.x] = v;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if ((int)threadIdx.x < o) s_red[threadIdx.x] += s_red[threadIdx.x + o];
+    __syncthreads();
+  }
+  return s_red[0];
+}
+
+__global__ void __launch_bounds__(256) cnr_kernel(const unsigned long long* __restrict__ N, const double* __restrict__ P,
+                                                  const double* __restrict__ P2, int nx, int ne, CnrRegions R,
+                                                  double* __restrict__ cnr_out) {
+  __shared__ double s_red[256];
+  const int e = blockIdx.x;
+  double mean[2], var[2];
+#pragma unroll
+  for (int r = 0; r < 2; ++r) {
+    const int* q = r == 0 ? R.mat : R.ref;
+    const int w = q[1] - q[0], n_pix = w * (q[3] - q[2]);
+    double sp = 0.0, sv = 0.0;
+    for (int k = threadIdx.x; k < n_pix; k += 256) {
+      const int ix = q[0] + k % w, iy = q[2] + k / w;
+      const size_t b = ((size_t)iy * nx + ix) * ne + e;
+      const double n = (double)N[b], p = P[b];
+      sp += p;
+      sv += n > 1.0 ? n / (n - 1.0) * fabs(P2[b] - (p / n) * (p / n)) : p * p;
+    }
+    mean[r] = block_sum(sp, s_red) / (double)n_pix;
+    var[r] = block_sum(sv, s_red) / ((double)n_pix * (double)n_pix);
+  }
+  if (threadIdx.x == 0) {
+    const double noise = sqrt(var[0] + var[1]);
+    cnr_out[e] = noise > 0.0 ? fabs(mean[0] - mean[1]) / noise : 0.0;
+  }
+}
+
+__global__ void __launch_bounds__(256) cnr_fit_kernel(const double* __restrict__ cnr, int ne, double emin, double emax, double e_fit_min,
+                                                      double* __restrict__ fit_out) {
+  __shared__ double s_red[256];
+  const double de = (emax - emin) / (double)ne;
+  double cnt = 0.0, sx = 0.0, sy = 0.0;
+  for (int e = threadIdx.x; e < ne; e += 256) {
+    const double x = emin + ((double)e + 0.5) * de;
+    if (x >= e_fit_min) { cnt += 1.0; sx += x; sy += cnr[e]; }
+  }
+  const double n = block_sum(cnt, s_red);
+  const double xm = block_sum(sx, s_red) / fmax(n, 1.0), ym = block_sum(sy, s_red) / fmax(n, 1.0);
+  double sxy = 0.0, sxx = 0.0;
+  for (int e = threadIdx.x; e < ne; e += 256) {
+    const double x = emin + ((double)e + 0.5) * de;
+    if (x >= e_fit_min) { sxy += (x - xm) * (cnr[e] - ym); sxx += (x - xm) * (x - xm); }
+  }
+  const double txy = block_sum(sxy, s_red), txx = block_sum(sxx, s_red);
+  if (threadIdx.x == 0) {
+    const double slope = (n >= 2.0 && txx > 0.0) ? txy / txx : 0.0;
+    fit_out[0] = n >= 2.0 ? ym - slope * xm : 0.0;
+    fit_out[1] = slope;
+  }
+}
+
+cudaError_t launch_cnr(const unsigned long long* N, const double* p, const double* p2, int nx, int ny, int ne, const int* region_mat,
+                       const int* region_ref, double emin, double emax, double e_fit_min, double* cnr_out, double* fit_out,
+                       cudaStream_t stream) {
+  (void)ny;
+  CnrRegions R;
+  for (int k = 0; k < 4; ++k) { R.mat[k] = region_mat[k]; R.ref[k] = region_ref[k]; }
+  cnr_kernel<<<ne, 256, 0, stream>>>(N, p, p2, nx, ne, R, cnr_out);
+  cnr_fit_kernel<<<1, 256, 0, stream>>>(cnr_out, ne, emin, emax, e_fit_min, fit_out);
   return cudaGetLastError();
 }
 

@@ -459,5 +459,98 @@ def config4(n_rays=1_000_000_000, small=False, n_vox=None):
     return instrument("c4_edxct", comps, mats, n_rays)
 
 
+def delta_table(rng, n=200, Emin=15.0, Emax=35.0, A=3.41e-4):
+    """Refractive-index decrement delta(E) = A / E^2 (free-electron form; A = 3.41e-4 keV^2 is beryllium, delta = 6.27e-7 at
+    23.32 keV) with a smooth seeded ripple of 0.5 %, n points uniform in ln E."""
+    E = np.exp(np.linspace(np.log(Emin), np.log(Emax), n))
+    E[0], E[-1] = Emin, Emax
+    phase, period = rng.uniform(0, 2 * np.pi), rng.uniform(0.15, 0.4)
+    delta = A / E ** 2 * (1.0 + 0.005 * np.sin(phase + np.log(E) / period))
+    return {"E": np.ascontiguousarray(E), "delta": np.ascontiguousarray(delta)}
+
+
+def config5(n_rays=100_000_000, small=False):
+    """The paper's basic instrument (problem 1): Source_pt, a point source with a flat spectrum of
+    5 +- 1 keV, cropped to the 20 mm x 20 mm L_monitor 1 m away, which histograms the wavelength."""
+    nL = 32 if small else 128
+    comps = [
+        source("point", "target", "uniform", target_w=20e-3, target_h=20e-3, target_dist=1.0, E0=5.0, dE_rel=0.2),
+        detector(-10e-3, 10e-3, -10e-3, 10e-3, 1, 1, 2.0, 3.2, nL, T=(0, 0, 1.0), mode="wavelength"),
+    ]
+    return instrument("c5_basic_lmonitor", comps, [None], n_rays)
+
+
+def config6(n_rays=200_000_000, small=False):
+    """The paper's focusing instrument (problem 2, Table 1): undulator-like Gaussian source cropped to
+    a 1 mm x 1 mm window at the lens 31.5 m away, a stack of sixteen double-sided parabolic Be lenses (R = 200 um), a
+    0.1 mm circular slit 14 m behind the lens centre, then a PSD_monitor and an E_monitor."""
+    rng = np.random.default_rng(WORKLOAD_SEED0 + 6)
+    p, q = 31.5, 14.0
+    be = mu_table(rng, n=400, Emin=15.0, Emax=35.0, a_range=(18.0, 22.0))     # ~ 40 / m at 23 keV, like Be
+    dtab = delta_table(rng)
+    npx, nE = (64, 32) if small else (256, 128)
+    comps = [
+        source("gauss", "target", "uniform", sigma_x=48.2e-6, sigma_y=9.5e-6, target_w=1e-3, target_h=1e-3, target_dist=p,
+               E0=23.32, dE_rel=1.0 / 23.32),
+        lens_parab(200e-6, 50e-6, 1.3e-3, 0.5e-3, 16, 1, dtab, T=(0, 0, p)),
+        slit_circ(0.05e-3, T=(0, 0, p + q)),
+        detector(-0.1e-3, 0.1e-3, -0.1e-3, 0.1e-3, npx, npx, 0.0, 50.0, 1, T=(0, 0, p + q + 1e-3)),          # PSD_monitor
+        detector(-0.1e-3, 0.1e-3, -0.1e-3, 0.1e-3, 1, 1, 22.0, 24.7, nE, T=(0, 0, p + q + 2e-3)),            # E_monitor
+    ]
+    return instrument("c6_focusing_crl", comps, [None, be], n_rays)
+
+
+EDXCT_N_DET, EDXCT_PIX, EDXCT_DIST = 5, 0.8e-3, 2.5
+
+
+def edxct_line_detectors(n_pix, nE, Emin=20.0, Emax=160.0, pix=EDXCT_PIX, dist=EDXCT_DIST):
+    """Five 1 x n_pix line detectors stacked vertically on a circle of radius `dist` about the source, each tilted so
+    that the line from the source to its centre is perpendicular to its plane (Fig. 3)."""
+    half = 0.5 * n_pix * pix
+    step = 2.0 * np.arctan(half / dist)
+    out = []
+    for k in range(EDXCT_N_DET):
+        al = (k - (EDXCT_N_DET - 1) / 2) * step
+        zax = np.array([0.0, np.sin(al), np.cos(al)])
+        yax = np.array([0.0, np.cos(al), -np.sin(al)])
+        xax = np.array([1.0, 0.0, 0.0])
+        out.append(detector(-0.5 * pix, 0.5 * pix, -half, half, 1, n_pix, Emin, Emax, nE, R=np.array([xax, yax, zax]),
+                            T=dist * zax))
+    return out
+
+
+def config7(n_rays=10_000_000, small=False, water=True):
+    """The paper's EDXCT in-line instrument (problem 3, Table 2, Fig. 3): polychromatic fan beam, a
+    voxel sample (a solid block of water, 1 mm voxels, 550 (scan) x 400 (up) x 300 (beam) mm; small: 10 mm voxels with the
+    seeded ellipsoid phantom painted in), five tilted 1 x 128 line detectors of 0.8 mm pixels and 128 energy bins over
+    20-160 keV.  One trace = one line; extra["scan"] gives the sample's x positions of the 550 lines of a projection."""
+    rng = np.random.default_rng(WORKLOAD_SEED0 + 7)
+    spec = bremsstrahlung_spectrum(rng, 1500, 20.0, 160.0, 160.0)
+    n_mat = 1 if (water and not small) else 15
+    mats = [None] + [mu_table(rng, Emin=20.0, Emax=160.0, a_range=(25.0, 45.0) if m == 0 else (5.0, 300.0)) for m in range(n_mat)]
+    if small:
+        h, shape = 10e-3, (30, 40, 55)                                  # (nz, ny, nx)
+        cube = ellipsoid_phantom(rng, n=64, h=0.512 / 64)
+        ids = np.ascontiguousarray(cube[:30, 12:52, 4:59])
+        ids[ids == 0] = 1                                               # water between the objects
+        n_pix, nE = 32, 16
+        pix = EDXCT_PIX * 4
+    else:
+        h, shape = 1e-3, (300, 400, 550)
+        ids = np.ones(shape, dtype=np.uint8)
+        n_pix, nE = 128, 128
+        pix = EDXCT_PIX
+    nz, ny, nx = shape
+    corner = (-0.5 * nx * h, -0.5 * ny * h, 1.8 - 0.5 * nz * h)
+    dets = edxct_line_detectors(n_pix, nE, pix=pix)
+    fan_h = 2.0 * EDXCT_DIST * np.tan(0.5 * EDXCT_N_DET * 2.0 * np.arctan(0.5 * n_pix * pix / EDXCT_DIST)) * 1.01
+    comps = [source("point", "target", "spectrum", target_w=pix, target_h=fan_h, target_dist=EDXCT_DIST, spec_Emin=20.0,
+                    spec_Emax=160.0, spectrum=spec),
+             voxels(ids, h, T=corner)] + dets
+    n_lines = nx if not small else 11
+    scan = [(corner[0] + (line - (n_lines - 1) / 2) * (h if not small else 5 * h), corner[1], corner[2]) for line in range(n_lines)]
+    return instrument("c7_edxct_lines", comps, mats, n_rays, scan=scan, sample_component=1)
+
+
 def config(k, **kw):
-    return (config0, config1, config2, config3, config4)[k](**kw)
+    return (config0, config1, config2, config3, config4, config5, config6, config7)[k](**kw)
