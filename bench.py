@@ -37,7 +37,8 @@ FLUSH_BYTES = 256 << 20          # > the 126 MB L2
 # evaluation (sqrt, div ~ 12; exp ~ 25; log, asin ~ 35; sincos ~ 45; tan ~ 50).  Philox is integer work (not counted).
 # ---------------------------------------------------------------------------------------------------------------
 OPS_SOURCE = {("disk", "target", "mono"): 120, ("gauss", "target", "spectrum"): 250, ("point", "target", "spectrum"): 150,
-              ("gauss", "gauss", "uniform"): 330}
+              ("gauss", "gauss", "uniform"): 330, ("point", "target", "uniform"): 50, ("gauss", "target", "uniform"): 160}
+OPS_LENS_ENTRY, OPS_LENS_SURFACE = 35 + 35 + 25, 110   # log E + delta(E) + final exp; quadratic, 3 sqrt, 3 div, Snell per surface
 OPS_SLIT, OPS_DETECTOR, OPS_MIRROR, OPS_CRYSTAL = 35, 80, 250, 180
 OPS_SOLIDS_ENTRY, OPS_PRIMITIVE_TEST, OPS_SEGMENT, OPS_MU, OPS_EXP = 35, 45, 10, 35, 25
 OPS_VOXEL_ENTRY, OPS_VOXEL_STEP = 100, 6
@@ -74,6 +75,8 @@ def algorithmic_ops(inst, n_rays, counters, work_per_ray):
             ops += r * OPS_MIRROR
         elif k == "crystal":
             ops += r * OPS_CRYSTAL
+        elif k == "lens":
+            ops += r * (OPS_LENS_ENTRY + 2 * cd["n_lenses"] * OPS_LENS_SURFACE)
         elif k == "solids":
             n_prim = sum(1 for s in cd["solids"] if s["shape"] != "mesh")
             n_mesh = len(cd["solids"]) - n_prim
@@ -271,7 +274,7 @@ def bench_instrument(M, torch, inst, n_rays, first, steps, warmup, device, probe
     probes: dict(dfma=lane-ops/s, l2=callable(bytes)->sectors/s, tally=callable(records)->records/s)."""
     g = M.Instrument(inst, device=device)
     g.set_exec(EXEC_MODE)
-    g.set_timing(True)
+    tuning = g.get_tuning()
     det = g.dets[-1]
     nb = det["nx"] * det["ny"] * det["nE"]
     last = len(g.dets) - 1
@@ -284,7 +287,6 @@ def bench_instrument(M, torch, inst, n_rays, first, steps, warmup, device, probe
         g.tally(last, out)
     torch.cuda.synchronize(device)
     g.reset()
-    g.timing()                                          # forget the warm-up launches
     launches0 = g.launch_count()
     marks = []
     sampler = ClockSampler(physical_gpu_index(local_rank))
@@ -300,7 +302,6 @@ def bench_instrument(M, torch, inst, n_rays, first, steps, warmup, device, probe
         marks.append((e0, e1, e2))
     torch.cuda.synchronize(device)
     clocks = sampler.result()
-    split = g.timing()                                  # CUDA events inside the library, around sort and trace_kernel
     launches = g.launch_count() - launches0
     t_trace = [a.elapsed_time(b) for a, b, _ in marks]
     t_step = [a.elapsed_time(c) for a, _, c in marks]
@@ -308,6 +309,14 @@ def bench_instrument(M, torch, inst, n_rays, first, steps, warmup, device, probe
     traced = int(counters["absorbed"].sum()) + counters["detected"] + counters["missed"] + counters["degenerate"]
     assert traced == steps * n_rays, "ray accounting does not add up"
     per_trace = {k: (v / steps if not isinstance(v, np.ndarray) else v / steps) for k, v in counters.items()}
+    # the same steps once more with the library's own events around every sort / trace_kernel launch (kept out of the
+    # steps timed above: three event records per chunk are visible in a 60 us step)
+    g.set_timing(True)
+    for _ in range(steps):
+        flush.zero_()
+        g.trace(n_rays, first=first)
+        g.tally(last, out)
+    split = g.timing()
     ms_sort, ms_kernel = split["sort_ms"] / steps, split["trace_ms"] / steps
     res = {"n_rays": n_rays, "ms_per_step": float(np.mean(t_step)), "ms_step_min": float(np.min(t_step)),
            "kernel_ms": {"sort_kernels": ms_sort, "trace_kernel": ms_kernel,
@@ -347,8 +356,12 @@ def bench_instrument(M, torch, inst, n_rays, first, steps, warmup, device, probe
                       "peak_source": f"mcx_probe_l2, random sectors of a {table >> 20} MiB table (BVH + triangles = "
                                      f"{footprint / 2**20:.1f} MiB), measured in this run",
                       "note": "sectors the per-ray walk needs; warps that walk one beam share them (DESIGN.md 5.1)"}
-    bound = max(cand, key=lambda k: cand[k]["frac"])
+    if tuning["tally_mode"] == "block":
+        cand["tally"]["bypassed"] = ("block-private shared-memory tallies (mcx_tally_mode MCX_TALLY_BLOCK): the records in "
+                                     "L2 see one flush per block, so this roof does not bind; frac > 1 is the gain over it")
+    bound = max((k for k in cand if "bypassed" not in cand[k]), key=lambda k: cand[k]["frac"])
     res["work_per_ray"] = work
+    res["tuning"] = tuning
     res["roofline"] = {"bound": bound, "achieved": cand[bound]["achieved"], "peak": cand[bound]["peak"],
                        "unit": cand[bound]["unit"], "frac": cand[bound]["frac"], "traffic": None,
                        "traffic_note": TRAFFIC_NOTE, "kernel": "trace_kernel", "kernel_ms": ms_kernel,
@@ -359,6 +372,40 @@ def bench_instrument(M, torch, inst, n_rays, first, steps, warmup, device, probe
     if with_e2e:
         res["e2e"] = bench_e2e(M, torch, inst, n_rays, first, 2, device)
     return res
+
+
+def bench_scan(M, torch, inst, device, steps=1):
+    """One projection of the paper's line scanner (550 lines of 1e7 rays): per line the sample is
+    moved (mcx_instrument_set_pose), the line's rays are traced, all detectors are read into that line's slice of the
+    sinogram stack and the tallies are reset.  CUDA events around the whole projection."""
+    g = M.Instrument(inst, device=device)
+    scan, comp, n = inst["scan"], inst["sample_component"], inst["n_rays"]
+    nb = [d["nx"] * d["ny"] * d["nE"] for d in g.dets]
+    stack = [(torch.empty((len(scan), b), dtype=torch.int64, device=device), torch.empty((len(scan), b), dtype=torch.float64, device=device),
+              torch.empty((len(scan), b), dtype=torch.float64, device=device)) for b in nb]
+    times = []
+    for it in range(steps + 1):
+        launches0 = g.launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for line, T in enumerate(scan):
+            g.set_pose(comp, T=T)
+            g.trace(n, first=line * n)
+            for d in range(len(nb)):
+                g.tally(d, (stack[d][0][line], stack[d][1][line], stack[d][2][line]))
+            g.reset()
+        e1.record()
+        torch.cuda.synchronize(device)
+        if it > 0:                                      # first projection = warm-up
+            times.append(e0.elapsed_time(e1))
+        launches = g.launch_count() - launches0
+    detected = int(sum(int(s_[0].sum()) for s_ in stack))
+    g.close()
+    ms = float(np.mean(times))
+    return {"lines": len(scan), "rays_per_line": n, "ms_per_projection": ms, "rays_per_s": len(scan) * n / (ms * 1e-3),
+            "launches_per_projection": launches, "detected_per_projection": detected,
+            "paper": "~1500 h single thread, ~50 h on 32 cores, < 4 h on an H100 per projection (PAPER.md:274; other hardware, "
+                     "other sample physics: context only)"}
 
 
 def bench_e2e(M, torch, inst, n_rays, first, steps, device):
@@ -457,7 +504,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs[k] of the headline line")
     ap.add_argument("--rays", type=float, default=None, help="override n_rays of the headline config")
-    ap.add_argument("--instruments", default="0,2,3,4", help="other configs to report under 'instruments' ('' = none)")
+    ap.add_argument("--instruments", default="0,2,3,4,5,6,7",
+                    help="other configs to report under 'instruments' ('' = none); 5-7 are the paper's own three instruments")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-sweep", action="store_true", help="skip the configs[4] throughput sweep 1e6..1e10 rays")
     ap.add_argument("--exec", default="auto", choices=["auto", "direct", "sorted"], help="lane scheduling (row a13)")
@@ -551,6 +599,8 @@ def main():
                 if k in cpu:
                     e["cpu_baseline"] = cpu[k]
                 instruments["c0_minimal_1e8_rays"] = e
+        if 7 in insts:
+            instruments["c7_projection_scan"] = bench_scan(M, torch, insts[7], device)
         if 4 in insts and not args.no_sweep:            # configs[4]: "also run a throughput sweep at 1e6-1e10 rays"
             sweep = {}
             for n in (10**6, 10**7, 10**8, 10**9, 10**10):
@@ -595,7 +645,7 @@ def main():
 
 def slim(r):
     keep = ("n_rays", "rays_per_s", "ms_per_step", "kernel_ms", "launches", "detected_fraction", "tally_bytes", "clocks",
-            "roofline", "e2e")
+            "roofline", "e2e", "tuning")
     out = {k: r[k] for k in keep if k in r}
     out["kernel_ms"] = {k: v for k, v in r["kernel_ms"].items() if k != "how"}
     return out

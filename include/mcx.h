@@ -253,14 +253,19 @@ mcx_status mcx_instrument_set_exec(mcx_instrument* inst, int mode);
  *                                     per distinct bin issues the reductions;
  *                   MCX_TALLY_BLOCK   warp-aggregated into a block-private shared-memory cache of tally records
  *                                     (2048 direct-mapped slots; chains without solids or voxels only, MCX_TALLY_WARP
- *                                     elsewhere), flushed to the records once per block and launch;
- *                   MCX_TALLY_AUTO (0 here = keep) is the library's choice from measurement.
+ *                                     elsewhere), flushed to the records once per block and launch; only detectors
+ *                                     whose bins fit (together at most 1024, smallest first) go through the cache;
+ *                   MCX_TALLY_AUTO (0 here = keep) is the library's choice from measurement:
+ *                   MCX_TALLY_BLOCK where some detector fits the cache, MCX_TALLY_GLOBAL otherwise.
  *                   N is the same integer in every mode; p and p2 differ in summation order only. */
 typedef enum { MCX_TALLY_AUTO = 0, MCX_TALLY_GLOBAL = 1, MCX_TALLY_WARP = 2, MCX_TALLY_BLOCK = 3 } mcx_tally_mode;
 typedef struct mcx_tuning {
   int32_t chunk_log2, sort_grid_bits, absorber_gate, tally_mode;
 } mcx_tuning;
 mcx_status mcx_instrument_set_tuning(mcx_instrument* inst, const mcx_tuning* tuning);
+/* The settings in effect: chunk_log2; sort_grid_bits (0 = chosen per chunk length); absorber_gate 1 / 2; tally_mode =
+ * the mode the next trace will use (never MCX_TALLY_AUTO). */
+mcx_status mcx_instrument_get_tuning(const mcx_instrument* inst, mcx_tuning* tuning_out);
 
 /* Finalises detector `detector` (ordinal among MCX_DETECTOR components): writes N (ray counts), p (sum of
  * weights) and p2 (sum of squared weights) for all bins, bin = (iy * nx + ix) * ne + ie.

@@ -29,7 +29,7 @@ FATE_DETECTED, FATE_MISSED, FATE_DEGENERATE = -1, -2, -3
 
 EXPORTS = ["mcx_instrument_workspace_size", "mcx_instrument_create", "mcx_trace", "mcx_trace_range", "mcx_tally_read",
            "mcx_tally_read_host", "mcx_instrument_set_exec", "mcx_instrument_set_tuning", "mcx_upload_bytes", "mcx_tally_reset",
-           "mcx_counters_read", "mcx_trace_status", "mcx_trace_dump", "mcx_launch_count", "mcx_instrument_set_timing", "mcx_timing_read", "mcx_instrument_set_pose", "mcx_cnr", "mcx_probe_dfma", "mcx_probe_tally",
+           "mcx_counters_read", "mcx_trace_status", "mcx_trace_dump", "mcx_launch_count", "mcx_instrument_set_timing", "mcx_timing_read", "mcx_instrument_get_tuning", "mcx_instrument_set_pose", "mcx_cnr", "mcx_probe_dfma", "mcx_probe_tally",
            "mcx_probe_l2", "mcx_probe_latency", "mcx_instrument_destroy", "mcx_last_error"]
 MCX_ERR_CAPACITY = 6
 
@@ -134,6 +134,8 @@ def lib(strict=False):
     L.mcx_instrument_set_exec.restype = C.c_int
     L.mcx_instrument_set_tuning.argtypes = [vp, C.POINTER(McxTuning)]
     L.mcx_instrument_set_tuning.restype = C.c_int
+    L.mcx_instrument_get_tuning.argtypes = [vp, C.POINTER(McxTuning)]
+    L.mcx_instrument_get_tuning.restype = C.c_int
     L.mcx_trace_status.argtypes = [vp, vp]
     L.mcx_trace_status.restype = C.c_int
     L.mcx_probe_l2.argtypes = [vp, C.c_uint64, vp, C.c_int, C.c_int64, vp]
@@ -356,6 +358,14 @@ class Instrument:
         """mcx_instrument_set_tuning; 0 / "auto" = keep the library's choice."""
         t = McxTuning(int(chunk_log2), int(sort_grid_bits), int(absorber_gate), TALLY_MODE[tally_mode])
         _check(self.L.mcx_instrument_set_tuning(self.handle, C.byref(t)), self.L)
+
+    def get_tuning(self):
+        """mcx_instrument_get_tuning -> dict of the settings in effect (tally_mode by name)."""
+        t = McxTuning()
+        _check(self.L.mcx_instrument_get_tuning(self.handle, C.byref(t)), self.L)
+        names = {v: k for k, v in TALLY_MODE.items()}
+        return {"chunk_log2": t.chunk_log2, "sort_grid_bits": t.sort_grid_bits, "absorber_gate": t.absorber_gate,
+                "tally_mode": names[t.tally_mode]}
 
     def status(self):
         """mcx_trace_status: synchronises the current stream; raises McxError (MCX_ERR_CAPACITY / MCX_ERR_CUDA) if a

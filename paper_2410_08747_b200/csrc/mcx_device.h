@@ -172,6 +172,7 @@ struct TraceArgs {
   unsigned int epoch;        // number of mcx_tally_reset calls on the handle so far
   int tally_mode;            // mcx_tally_mode (never MCX_TALLY_AUTO here)
   int tally_cache_log2;      // MCX_TALLY_BLOCK: log2 of the slots of the block-private cache (32 bytes each); 0 = none
+  unsigned tally_cache_dets; // MCX_TALLY_BLOCK: bit d = detector d's updates go through the cache (its bins fit in it)
 };
 
 // sizes of the sort workspace

@@ -752,10 +752,31 @@ bool use_sorted(const mcx_instrument* H) {
 constexpr size_t kMaxTimedChunks = 4096;
 constexpr int kTallyCacheLog2 = 11;  // MCX_TALLY_BLOCK: 2048 slots of 32 bytes per block
 
-// Step 14 update path (include/mcx.h, mcx_tally_mode).  AUTO: see DESIGN.md 5.5 for the measurements behind it.
+// MCX_TALLY_BLOCK: the detectors whose bins all fit in half the cache go through it (smallest first, while they fit
+// together); a detector with more bins would only evict those and takes the global path.
+unsigned tally_cache_dets(const mcx_instrument* H) {
+  unsigned mask = 0u;
+  uint64_t used = 0;
+  const uint64_t room = ((uint64_t)1 << kTallyCacheLog2) / 2;
+  for (;;) {
+    int best = -1;
+    for (int d = 0; d < H->n_dets; ++d)
+      if (!((mask >> d) & 1u) && (best < 0 || H->det_bins[d] < H->det_bins[best])) best = d;
+    if (best < 0 || used + H->det_bins[best] > room) break;
+    mask |= 1u << best;
+    used += H->det_bins[best];
+  }
+  return mask;
+}
+
+// Step 14 update path (include/mcx.h, mcx_tally_mode).  AUTO (measured): per-ray reductions into the
+// records, except where a detector has so few bins that every block can keep a private copy of all of them in shared
+// memory (an L_monitor or E_monitor: all rays into ~100 bins; there same-address reductions serialise in
+// L2 and the private copy is 11x faster); warp aggregation alone never paid.
 int tally_mode_of(const mcx_instrument* H) {
   int mode = H->tally_mode;
-  if (mode == MCX_TALLY_AUTO) mode = MCX_TALLY_GLOBAL;
+  if (mode == MCX_TALLY_AUTO)
+    mode = (!(H->features & (F_SOLIDS | F_VOXELS)) && tally_cache_dets(H) != 0u) ? MCX_TALLY_BLOCK : MCX_TALLY_GLOBAL;
   if (mode == MCX_TALLY_BLOCK && (H->features & (F_SOLIDS | F_VOXELS))) mode = MCX_TALLY_WARP;  // no room beside their scratch
   return mode;
 }
@@ -777,6 +798,7 @@ mcx_status run_trace(mcx_instrument* H, uint64_t first, uint64_t n, uint64_t see
     A.epoch = H->epoch;
     A.tally_mode = tally_mode_of(H);
     A.tally_cache_log2 = A.tally_mode == MCX_TALLY_BLOCK ? kTallyCacheLog2 : 0;
+    A.tally_cache_dets = tally_cache_dets(H);
     A.order = nullptr;
     A.dump = dump ? dump + base : nullptr;
     A.ticket = (unsigned int*)(ws + H->off_ticket);
@@ -969,6 +991,17 @@ mcx_status mcx_instrument_set_tuning(mcx_instrument* inst, const mcx_tuning* t) 
   if (t->sort_grid_bits) inst->sort_grid_bits = t->sort_grid_bits;
   if (t->absorber_gate) inst->gate_enabled = t->absorber_gate == 1;
   if (t->tally_mode) inst->tally_mode = t->tally_mode;
+  return MCX_OK;
+}
+
+mcx_status mcx_instrument_get_tuning(const mcx_instrument* inst, mcx_tuning* t) {
+  if (!inst || !t) return fail(MCX_ERR_INVALID_ARG, "null argument");
+  int log2 = 0;
+  while (((uint64_t)1 << log2) < inst->chunk_rays) ++log2;
+  t->chunk_log2 = log2;
+  t->sort_grid_bits = inst->sort_grid_bits;
+  t->absorber_gate = inst->gate_enabled ? 1 : 2;
+  t->tally_mode = tally_mode_of(inst);
   return MCX_OK;
 }
 

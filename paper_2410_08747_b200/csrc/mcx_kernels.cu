@@ -1182,6 +1182,7 @@ __global__ void __launch_bounds__(256) sort_scatter_kernel(uint64_t first, uint3
 struct TallyCache {
   unsigned long long* key;  // [2^log2] 0 = empty, else ((detector + 1) << 48) | bin; then N, P, P2 arrays of the same length
   int log2;                 // 0 = no cache
+  unsigned dets;            // bit d: detector d goes through the cache (its bins fit; TraceArgs::tally_cache_dets)
 };
 
 __device__ __forceinline__ void tally_global(TallyBin* rec, unsigned long long cnt, double sp, double sp2) {
@@ -1218,7 +1219,7 @@ __device__ __noinline__ void tally_add_aggregated(TallyBin* const* tallies, int 
     if (lane == l) { sp = a; sp2 = b; }
   }
   if (!lead) return;
-  if (mode == MCX_TALLY_BLOCK && cache_log2 > 0) {
+  if (cache_log2 > 0) {
     const unsigned long long k = ((unsigned long long)(det + 1u) << 48) | (unsigned long long)bin;
     const unsigned h = (unsigned)((k * 0x9E3779B97F4A7C15ull) >> (64 - cache_log2));
     const unsigned long long prev = atomicCAS(&cache_key[h], 0ull, k);
@@ -1239,7 +1240,7 @@ __device__ __forceinline__ void tally_add(const DInstrument& I, int mode, const 
   if (mode == MCX_TALLY_GLOBAL) {
     if (on) tally_global(I.tallies[det] + bin, 1ull, p, p * p);
   } else {
-    tally_add_aggregated(I.tallies, mode, tc.key, tc.log2, det, on, bin, p);
+    tally_add_aggregated(I.tallies, mode, tc.key, (mode == MCX_TALLY_BLOCK && ((tc.dets >> det) & 1u)) ? tc.log2 : 0, det, on, bin, p);
   }
 }
 
@@ -1320,7 +1321,7 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
     }
   }
   double* len_s = reinterpret_cast<double*>(s_extra) + threadIdx.x;  // per-thread path length per material (voxel walk)
-  TallyCache tcache{nullptr, 0};
+  TallyCache tcache{nullptr, 0, A.tally_cache_dets};
   const int tally_mode = A.tally_mode;
   if (!DUMP && !(FEAT & (F_SOLIDS | F_VOXELS)) && A.tally_cache_log2 > 0) {  // block-private tally cache (chains without solids or voxels)
     tcache.key = reinterpret_cast<unsigned long long*>(s_extra);
