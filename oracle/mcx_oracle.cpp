@@ -24,7 +24,10 @@
 // fate rule of chains with several monitors against plane geometry written out in numpy; compound refractive lens:
 // thin-lens deflection 2 N delta x / R, thick-stack focal length R / (2 N delta) + L / 6, plane-parallel slab
 // displacement by Snell's law, on-axis transmission exp(-mu N d), parabolic thickness profile, reversibility;
-// Darwin-Prins: g = kappa = 0 limit, closed form at eta = 0, numpy complex arithmetic; wavelength bins: lambda = hc / E.
+// Darwin-Prins: g = kappa = 0 limit, closed form at eta = 0, numpy complex arithmetic; wavelength bins: lambda = hc / E;
+// scattering (step 17): K = 0 and mu_s = 0 reduce to steps 10 / 11 bit for bit, Thomson inverse CDF and moments, unit
+// orthogonal frames, exp(-mu_s L) unscattered fraction, event depth = -ln(u) / mu_s replayed from the draws, weight 1 in a
+// purely scattering medium, a fine-step marching of the same draws (the paper's own stepping) on a small volume.
 // Whole-config tallies of c1..c4 have no closed form: "parity unpinned" beyond those part-wise pins
 // (SURVEY.md 8(c) last row).
 #include <algorithm>
@@ -59,8 +62,9 @@ extern "C" {
 
 struct OrcMaterial {  // n == 0: vacuum, mu == 0 (step 7)
   int64_t n;
-  const double* E;   // keV, strictly increasing
-  const double* mu;  // 1/m
+  const double* E;     // keV, strictly increasing
+  const double* mu;    // 1/m, total attenuation
+  const double* mu_s;  // 1/m, the part of mu that scatters (step 17); null = none
 };
 
 struct OrcSolid {
@@ -112,6 +116,8 @@ struct OrcComponent {
   int64_t lens_nd;                             // points of the delta(E) table (refractive index n = 1 - delta)
   const double* lens_dE;                       // keV, strictly increasing
   const double* lens_delta;                    // > 0, log-log interpolated like mu(E) (step 7)
+  // scattering in samples (step 17): at most this many direction changes per ray in this component; 0 = attenuation only
+  int64_t scatter_order;
 };
 
 struct OrcRayFate {
@@ -194,6 +200,7 @@ V3 to_lab_pos(const double R[9], const double T[3], V3 r) { return rotT(R, r) + 
 // ---------------------------------------------------------------------------------------------------
 struct MuTable {
   std::vector<double> E, lnE, lnMu;
+  std::vector<double> lnMuS;  // ln of the scattering part (step 17); empty = the material does not scatter
 };
 
 double mu_of_E(const MuTable& m, double E) {
@@ -206,6 +213,14 @@ double mu_of_E(const MuTable& m, double E) {
   const double lnE = std::log(E);
   const double slope = (m.lnMu[j + 1] - m.lnMu[j]) / (m.lnE[j + 1] - m.lnE[j]);
   return std::exp(m.lnMu[j] + (lnE - m.lnE[j]) * slope);
+}
+
+// Step 17: the scattering part of mu(E), the same log-log interpolation on the same grid; 0 without a table.
+double mu_s_of_E(const MuTable& m, double E) {
+  if (m.lnMuS.empty()) return 0.0;
+  MuTable t;
+  t.E = m.E; t.lnE = m.lnE; t.lnMu = m.lnMuS;
+  return mu_of_E(t, E);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -487,6 +502,7 @@ void prepare(Prepared* P, const OrcComponent* comps, int n_comps, const OrcMater
       t.E.push_back(mats[m].E[j]);
       t.lnE.push_back(std::log(mats[m].E[j]));
       t.lnMu.push_back(std::log(mats[m].mu[j]));
+      if (mats[m].mu_s) t.lnMuS.push_back(std::log(mats[m].mu_s[j]));
     }
   }
   P->cdf.resize(n_comps); P->meshes.resize(n_comps); P->mirrors.resize(n_comps); P->det_index.assign(n_comps, -1);
@@ -637,15 +653,91 @@ bool slit(const OrcComponent& k, const Ray& ray) {
   return h.x * h.x + h.y * h.y <= k.slit_radius * k.slit_radius;
 }
 
-// Steps 8-10.  Returns 1 = continue, 0 = degenerate.
-int solids(const Prepared& P, int c, Ray* ray, Work* w) {
+struct Seg { double ta, tb; int material; };  // a stretch of the ray inside one material
+
+// Step 17 (a step updates "the ray's attenuation (Monte Carlo weight) and direction
+// (wavevector)"; reading in DESIGN.md).  Elastic scattering with the Thomson angular distribution
+// dsigma/dOmega ~ 1 + cos^2(theta): cos(theta) by inversion of its distribution function
+// F(x) = 1/2 + (3/8)(x + x^3/3), i.e. the real root of x^3 + 3x - (8u - 4) = 0, x = w - 1/w with
+// w = cbrt(q + sqrt(q^2 + 1)), q = 4u - 2 (Cardano); azimuth phi = 2 pi u'.  The new direction is
+// cos(theta) d + sin(theta) (cos(phi) e1 + sin(phi) e2), e1 = (d x a) / |d x a| with a the coordinate axis along which
+// |d| is smallest (ties: the lowest axis), e2 = d x e1; normalised once more.
+V3 cross(V3 a, V3 b) { return {a.y * b.z - a.z * b.y, a.z * b.x - a.x * b.z, a.x * b.y - a.y * b.x}; }
+
+V3 scatter_direction(V3 d, double u_mu, double u_phi) {
+  const double q = 4.0 * u_mu - 2.0;
+  const double w = std::cbrt(q + std::sqrt(q * q + 1.0));
+  const double ct = w - 1.0 / w;
+  const double st = std::sqrt(std::max(0.0, 1.0 - ct * ct));
+  const double phi = 2.0 * kPi * u_phi;
+  V3 a{1.0, 0.0, 0.0};
+  double m = std::fabs(d.x);
+  if (std::fabs(d.y) < m) { a = {0.0, 1.0, 0.0}; m = std::fabs(d.y); }
+  if (std::fabs(d.z) < m) { a = {0.0, 0.0, 1.0}; }
+  V3 e1 = cross(d, a);
+  e1 = (1.0 / std::sqrt(dot(e1, e1))) * e1;
+  const V3 e2 = cross(d, e1);
+  const V3 v = ct * d + st * (std::cos(phi) * e1 + std::sin(phi) * e2);
+  return (1.0 / std::sqrt(dot(v, v))) * v;
+}
+
+// Step 17: the walk of one ray through a sample with up to K direction changes.  `segments(o, d, &segs)` gives the
+// stretches of the half-line o + t d, t >= 0, inside materials, in order (1 = ok, 0 = degenerate).  Leg k < K draws
+// (u_f, u_mu) from slot 2k and u_phi from slot 2k + 1 of this component (step 1): the scattering optical depth to the next
+// event is -ln(u_f); walking the stretches, the event lies where the running sum of mu_s * length reaches it.  Up to
+// there, and on a leg that leaves the sample without an event, the weight is attenuated by what does not scatter,
+// mu - mu_s; once the K events are used up a further scattering counts as a loss and the full mu attenuates.  K = 0 or
+// mu_s = 0 is Beer-Lambert as in steps 10 and 11.  *o, *d: the ray, updated at every event; *tau: the optical depth of
+// the weight, accumulated over all legs.
+template <class SegFn>
+int scatter_walk(const Prepared& P, int c, int64_t K, uint64_t seed, uint64_t i, double E, V3* o, V3* d, SegFn segments,
+                 double* tau, int* n_events) {
+  std::vector<Seg> segs;
+  int64_t k = 0;
+  for (;;) {
+    segs.clear();
+    if (!segments(*o, *d, &segs)) return 0;
+    double tau_s = kInf, u_mu = 0.0;
+    if (k < K) {
+      double u_f;
+      draw2(seed, i, (uint32_t)(2 * k), (uint32_t)c, &u_f, &u_mu);
+      tau_s = -std::log(u_f);
+    }
+    double cum = 0.0;
+    bool event = false;
+    for (const Seg& sg : segs) {
+      const double len = sg.tb - sg.ta;
+      const double mt = mu_of_E(P.mats[sg.material], E);
+      const double ms = k < K ? mu_s_of_E(P.mats[sg.material], E) : 0.0;
+      if (k < K && ms > 0.0 && cum + ms * len >= tau_s) {
+        const double l = (tau_s - cum) / ms;
+        *tau += (mt - ms) * l;
+        double u_phi, unused;
+        draw2(seed, i, (uint32_t)(2 * k + 1), (uint32_t)c, &u_phi, &unused);
+        *o = *o + (sg.ta + l) * (*d);
+        *d = scatter_direction(*d, u_mu, u_phi);
+        ++k;
+        event = true;
+        break;
+      }
+      cum += ms * len;
+      *tau += (mt - ms) * len;
+    }
+    if (!event) break;
+  }
+  *n_events = (int)k;
+  return 1;
+}
+
+// Steps 8-10 up to the elementary segments of the half-line r + t d, t >= 0, and their owners.  1 = ok, 0 = degenerate.
+int solid_segments(const Prepared& P, int c, V3 r, V3 dl, Work* w, std::vector<Seg>* segs) {
   const OrcComponent& k = P.comps[c];
   std::vector<Interval> iv;
   std::vector<Hit> hits;
   for (int64_t s = 0; s < k.n_solids; ++s) {
     const OrcSolid& S = k.solids[s];
-    const V3 o = to_local_pos(S.R, S.T, ray->r);
-    const V3 d = rot(S.R, ray->d);
+    const V3 o = to_local_pos(S.R, S.T, r);
+    const V3 d = rot(S.R, dl);
     double a, b;
     bool hit = false;
     w->solid_tests++;
@@ -670,7 +762,6 @@ int solids(const Prepared& P, int c, Ray* ray, Work* w) {
   std::vector<double> ts;
   for (const Interval& x : cl) { ts.push_back(x.a); ts.push_back(x.b); }
   std::sort(ts.begin(), ts.end());
-  double tau = 0.0;
   for (size_t m = 0; m + 1 < ts.size(); ++m) {
     const double ta = ts[m], tb = ts[m + 1];
     if (!(tb > ta)) continue;
@@ -683,8 +774,29 @@ int solids(const Prepared& P, int c, Ray* ray, Work* w) {
       }
     if (owner < 0) continue;  // vacuum gap
     w->segments++;
-    tau += mu_of_E(P.mats[k.solids[owner].material], ray->E) * (tb - ta);
+    segs->push_back({ta, tb, k.solids[owner].material});
   }
+  return 1;
+}
+
+// Steps 8-10 (and 17 where the group scatters).  Returns 1 = continue, 0 = degenerate.
+int solids(const Prepared& P, int c, Ray* ray, Work* w, uint64_t seed, uint64_t i) {
+  const OrcComponent& k = P.comps[c];
+  if (k.scatter_order > 0) {
+    double tau = 0.0;
+    int n_events = 0;
+    V3 o = ray->r, d = ray->d;
+    auto segments = [&](V3 oo, V3 dd, std::vector<Seg>* segs) { return solid_segments(P, c, oo, dd, w, segs); };
+    if (!scatter_walk(P, c, k.scatter_order, seed, i, ray->E, &o, &d, segments, &tau, &n_events)) return 0;
+    ray->p *= std::exp(-tau);
+    if (n_events > 0) { ray->r = o; ray->d = d; }
+    return 1;
+  }
+  std::vector<Seg> segs;
+  if (!solid_segments(P, c, ray->r, ray->d, w, &segs)) return 0;
+  if (segs.empty()) return 1;
+  double tau = 0.0;
+  for (const Seg& sg : segs) tau += mu_of_E(P.mats[sg.material], ray->E) * (sg.tb - sg.ta);
   ray->p *= std::exp(-tau);
   return 1;
 }
@@ -736,6 +848,64 @@ void voxels(const Prepared& P, int c, Ray* ray, Work* w) {
     if (idx[a] < 0 || idx[a] >= n[a]) break;
   }
   ray->p *= std::exp(-tau);
+}
+
+// Step 11 as a list: the voxels the half-line o + t d, t >= 0, crosses (volume frame), one stretch per voxel visited
+// with positive length, in the order and with the face parameters of voxels() above.
+int voxel_segments(const OrcComponent& k, V3 ol, V3 dl, Work* w, std::vector<Seg>* segs) {
+  const double o[3] = {ol.x, ol.y, ol.z}, d[3] = {dl.x, dl.y, dl.z};
+  const int64_t n[3] = {k.vnx, k.vny, k.vnz};
+  const double h = k.vox_h;
+  double t0 = -kInf, t1 = kInf;
+  for (int a = 0; a < 3; ++a)
+    if (!slab_axis(o[a], d[a], 0.0, (double)n[a] * h, &t0, &t1)) return 1;
+  if (t0 < 0.0) t0 = 0.0;
+  if (!(t0 < t1)) return 1;
+  int64_t idx[3];
+  int step[3];
+  for (int a = 0; a < 3; ++a) {
+    const double q = o[a] + t0 * d[a];
+    int64_t v = (int64_t)std::floor(q / h);
+    idx[a] = std::min(n[a] - 1, std::max((int64_t)0, v));
+    step[a] = d[a] > 0.0 ? 1 : (d[a] < 0.0 ? -1 : 0);
+  }
+  auto next_face = [&](int a) {
+    if (step[a] == 0) return kInf;
+    const double face = (double)(idx[a] + (step[a] > 0 ? 1 : 0)) * h;
+    return (face - o[a]) / d[a];
+  };
+  double tcur = t0;
+  while (true) {
+    const double tx = next_face(0), ty = next_face(1), tz = next_face(2);
+    int a = 0;
+    double tn = tx;
+    if (ty < tn) { tn = ty; a = 1; }
+    if (tz < tn) { tn = tz; a = 2; }
+    const bool last = !(tn < t1);
+    if (last) tn = t1;
+    const uint8_t id = k.vox_ids[(idx[2] * n[1] + idx[1]) * n[0] + idx[0]];
+    w->voxel_steps++;
+    if (tn > tcur) { segs->push_back({tcur, tn, (int)id}); tcur = tn; }
+    if (last) break;
+    idx[a] += step[a];
+    if (idx[a] < 0 || idx[a] >= n[a]) break;
+  }
+  return 1;
+}
+
+// Steps 11 + 17: a voxel volume that scatters (scatter_order > 0).  The walk runs in the volume's frame.
+void voxels_scatter(const Prepared& P, int c, Ray* ray, Work* w, uint64_t seed, uint64_t i) {
+  const OrcComponent& k = P.comps[c];
+  V3 o = to_local_pos(k.R, k.T, ray->r), d = rot(k.R, ray->d);
+  double tau = 0.0;
+  int n_events = 0;
+  auto segments = [&](V3 oo, V3 dd, std::vector<Seg>* segs) { return voxel_segments(k, oo, dd, w, segs); };
+  scatter_walk(P, c, k.scatter_order, seed, i, ray->E, &o, &d, segments, &tau, &n_events);
+  ray->p *= std::exp(-tau);
+  if (n_events > 0) {
+    ray->r = to_lab_pos(k.R, k.T, o);
+    ray->d = rotT(k.R, d);
+  }
 }
 
 // Step 12.  Returns true if reflected.
@@ -909,9 +1079,12 @@ int orc_trace(const OrcComponent* comps, int n_comps, const OrcMaterial* mats, i
       switch (k.kind) {
         case K_SLIT_RECT: case K_SLIT_CIRC: alive = slit(k, ray); break;
         case K_SOLIDS:
-          if (!solids(P, c, &ray, &w)) { fate = F_DEGENERATE; alive = false; }
+          if (!solids(P, c, &ray, &w, seed, i)) { fate = F_DEGENERATE; alive = false; }
           break;
-        case K_VOXELS: voxels(P, c, &ray, &w); break;
+        case K_VOXELS:
+          if (k.scatter_order > 0) voxels_scatter(P, c, &ray, &w, seed, i);
+          else voxels(P, c, &ray, &w);
+          break;
         case K_MIRROR: alive = mirror(P, c, &ray); break;
         case K_CRYSTAL: alive = crystal(k, &ray); break;
         case K_LENS: alive = lens(P, c, &ray); break;
@@ -999,7 +1172,14 @@ int64_t orc_mesh_hits(const OrcSolid* solid, const double* o, const double* d, i
 
 // apply one non-source component to a given ray state: io[8] = r, d, E, p (lab frame).
 // Returns 1 = continues, 0 = absorbed, -3 = degenerate.  For a detector, *bin receives the bin (or -1).
+// (a scattering sample draws from the stream of ray index `ray_index` under `seed`, as component 1)
+int orc_apply_seeded(const OrcComponent* comp, const OrcMaterial* mats, int n_mats, double* io, int64_t* bin, int mesh_accel,
+                     uint64_t seed, uint64_t ray_index);
 int orc_apply(const OrcComponent* comp, const OrcMaterial* mats, int n_mats, double* io, int64_t* bin, int mesh_accel) {
+  return orc_apply_seeded(comp, mats, n_mats, io, bin, mesh_accel, 1, 0);
+}
+int orc_apply_seeded(const OrcComponent* comp, const OrcMaterial* mats, int n_mats, double* io, int64_t* bin, int mesh_accel,
+                     uint64_t seed, uint64_t ray_index) {
   // the component is placed at chain index 1 behind a dummy slot so Prepared indexing matches
   OrcComponent two[2];
   std::memset(&two[0], 0, sizeof(OrcComponent));
@@ -1013,8 +1193,11 @@ int orc_apply(const OrcComponent* comp, const OrcMaterial* mats, int n_mats, dou
   if (bin) *bin = -1;
   switch (comp->kind) {
     case K_SLIT_RECT: case K_SLIT_CIRC: rc = slit(two[1], ray) ? 1 : 0; break;
-    case K_SOLIDS: rc = solids(P, 1, &ray, &w) ? 1 : -3; break;
-    case K_VOXELS: voxels(P, 1, &ray, &w); break;
+    case K_SOLIDS: rc = solids(P, 1, &ray, &w, seed, ray_index) ? 1 : -3; break;
+    case K_VOXELS:
+      if (comp->scatter_order > 0) voxels_scatter(P, 1, &ray, &w, seed, ray_index);
+      else voxels(P, 1, &ray, &w);
+      break;
     case K_MIRROR: rc = mirror(P, 1, &ray) ? 1 : 0; break;
     case K_CRYSTAL: rc = crystal(two[1], &ray) ? 1 : 0; break;
     case K_LENS: rc = lens(P, 1, &ray) ? 1 : 0; break;
@@ -1026,6 +1209,10 @@ int orc_apply(const OrcComponent* comp, const OrcMaterial* mats, int n_mats, dou
   return rc;
 }
 
+void orc_scatter_direction(const double* d, double u_mu, double u_phi, double* out) {
+  const V3 v = scatter_direction(V3{d[0], d[1], d[2]}, u_mu, u_phi);
+  out[0] = v.x; out[1] = v.y; out[2] = v.z;
+}
 double orc_darwin(double eta) { return darwin_R(eta); }
 double orc_darwin_prins(double eta, double g, double kappa) { return darwin_prins_R(eta, g, kappa); }
 double orc_bilinear(const OrcComponent* comp, double theta, double E) { return bilinear_R(*comp, theta, E); }

@@ -29,7 +29,7 @@ _dp = C.POINTER(C.c_double)
 
 
 class OrcMaterial(C.Structure):
-    _fields_ = [("n", C.c_int64), ("E", _dp), ("mu", _dp)]
+    _fields_ = [("n", C.c_int64), ("E", _dp), ("mu", _dp), ("mu_s", _dp)]
 
 
 class OrcSolid(C.Structure):
@@ -64,7 +64,7 @@ class OrcComponent(C.Structure):
                 ("det_mode", C.c_int64), ("xtal_g", C.c_double), ("xtal_kappa", C.c_double),
                 ("lens_R", C.c_double), ("lens_d", C.c_double), ("lens_pitch", C.c_double), ("lens_ra", C.c_double),
                 ("lens_N", C.c_int64), ("lens_material", C.c_int64), ("lens_nd", C.c_int64), ("lens_dE", _dp),
-                ("lens_delta", _dp)]
+                ("lens_delta", _dp), ("scatter_order", C.c_int64)]
 
 
 class OrcRayFate(C.Structure):
@@ -164,12 +164,14 @@ def marshal_component(cd, keep):
         arr = (OrcSolid * len(cd["solids"]))(*[marshal_solid(s, keep) for s in cd["solids"]])
         keep.append(arr)
         c.n_solids, c.solids = len(cd["solids"]), arr
+        c.scatter_order = cd.get("scatter_order", 0)
     elif k == "voxels":
         ids = np.ascontiguousarray(cd["ids"], dtype=np.uint8)
         keep.append(ids)
         c.vox_h = cd["h"]
         c.vnz, c.vny, c.vnx = ids.shape
         c.vox_ids = _ptr(ids, C.POINTER(C.c_uint8))
+        c.scatter_order = cd.get("scatter_order", 0)
     elif k == "mirror":
         c.mir_p, c.mir_q, c.mir_theta = cd["p"], cd["q"], cd["theta"]
         c.mir_length, c.mir_width = cd["length"], cd["width"]
@@ -209,6 +211,10 @@ def marshal_materials(mats, keep):
         mu = np.ascontiguousarray(md["mu"], dtype=np.float64)
         keep += [E, mu]
         arr[m].n, arr[m].E, arr[m].mu = len(E), _ptr(E), _ptr(mu)
+        if md.get("mu_s") is not None:
+            mus = np.ascontiguousarray(md["mu_s"], dtype=np.float64)
+            keep.append(mus)
+            arr[m].mu_s = _ptr(mus)
     return arr
 
 
@@ -324,15 +330,24 @@ def mesh_hits(solid, o, d, use_grid=False, cap=4096):
     return t[:n].copy(), orient[:n].copy(), int(nt.value)
 
 
-def apply(comp, ray8, materials=(None,), mesh_accel=0):
-    """Apply one non-source component to a ray state (r, d, E, p).  Returns (rc, state, bin)."""
+def apply(comp, ray8, materials=(None,), mesh_accel=0, seed=1, ray_index=0):
+    """Apply one non-source component to a ray state (r, d, E, p).  Returns (rc, state, bin).  A scattering sample draws
+    from the Philox stream of (seed, ray_index) as component 1."""
     keep = []
     c = marshal_component(comp, keep)
     mats = marshal_materials(list(materials), keep)
     io = (C.c_double * 8)(*ray8)
     b = C.c_int64(-1)
-    rc = lib().orc_apply(C.byref(c), mats, C.c_int(len(materials)), io, C.byref(b), C.c_int(mesh_accel))
+    rc = lib().orc_apply_seeded(C.byref(c), mats, C.c_int(len(materials)), io, C.byref(b), C.c_int(mesh_accel),
+                                C.c_uint64(seed), C.c_uint64(ray_index))
     return rc, np.array(io[:]), int(b.value)
+
+
+def scatter_direction(d, u_mu, u_phi):
+    dd = (C.c_double * 3)(*d)
+    out = (C.c_double * 3)()
+    lib().orc_scatter_direction(dd, C.c_double(u_mu), C.c_double(u_phi), out)
+    return np.array(out[:])
 
 
 def darwin(eta):

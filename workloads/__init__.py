@@ -75,15 +75,17 @@ def solid_mesh(verts, tris, material, priority, R=None, T=(0, 0, 0)):
     return d
 
 
-def solids(solid_list):
-    d = {"kind": "solids", "solids": list(solid_list)}
+def solids(solid_list, scatter_order=0):
+    """scatter_order: at most this many direction changes per ray in the group (materials with a "mu_s" table scatter)."""
+    d = {"kind": "solids", "solids": list(solid_list), "scatter_order": int(scatter_order)}
     d.update(_pose())
     return d
 
 
-def voxels(ids, h, R=None, T=(0, 0, 0)):
-    """ids: uint8 [nz][ny][nx] (x fastest); T = lab position of the corner of voxel (0,0,0)."""
-    d = {"kind": "voxels", "ids": np.ascontiguousarray(ids, dtype=np.uint8), "h": float(h)}
+def voxels(ids, h, R=None, T=(0, 0, 0), scatter_order=0):
+    """ids: uint8 [nz][ny][nx] (x fastest); T = lab position of the corner of voxel (0,0,0); scatter_order: at most this
+    many direction changes per ray in the volume (materials with a "mu_s" table scatter)."""
+    d = {"kind": "voxels", "ids": np.ascontiguousarray(ids, dtype=np.uint8), "h": float(h), "scatter_order": int(scatter_order)}
     d.update(_pose(R, T))
     return d
 
@@ -188,6 +190,18 @@ def mu_table(rng, n=1000, Emin=10.0, Emax=150.0, a_range=(20.0, 400.0)):
     for Ee, J in zip(edges, jumps):
         mu = np.where(E > Ee, mu * J, mu)
     return {"E": np.ascontiguousarray(E), "mu": np.ascontiguousarray(mu)}
+
+
+def with_scattering(rng, table, frac_range=(0.2, 0.9)):
+    """Adds the scattering part mu_s(E) = f(E) mu(E) to a mu table: the fraction rises smoothly with energy from about
+    frac_range[0] to frac_range[1] (photo-absorption dominates at low energy, scattering at high), seeded midpoint."""
+    E = table["E"]
+    x = (np.log(E) - np.log(E[0])) / (np.log(E[-1]) - np.log(E[0]))
+    mid, width = rng.uniform(0.3, 0.6), rng.uniform(0.1, 0.2)
+    f = frac_range[0] + (frac_range[1] - frac_range[0]) / (1.0 + np.exp(-(x - mid) / width))
+    out = dict(table)
+    out["mu_s"] = np.ascontiguousarray(f * table["mu"])
+    return out
 
 
 def reflectivity_table(rng, n_theta=200, n_E=500, theta_max=8e-3, Emin=5.0, Emax=25.0):
