@@ -504,8 +504,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs[k] of the headline line")
     ap.add_argument("--rays", type=float, default=None, help="override n_rays of the headline config")
-    ap.add_argument("--instruments", default="0,2,3,4,5,6,7",
-                    help="other configs to report under 'instruments' ('' = none); 5-7 are the paper's own three instruments")
+    ap.add_argument("--instruments", default="0,2,3,4,5,6,7,8,9",
+                    help="other configs to report under 'instruments' ('' = none); 5-7 are the paper's own three instruments, "
+                         "8 and 9 the voxel samples with scattering")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-sweep", action="store_true", help="skip the configs[4] throughput sweep 1e6..1e10 rays")
     ap.add_argument("--exec", default="auto", choices=["auto", "direct", "sorted"], help="lane scheduling (row a13)")

@@ -54,7 +54,8 @@ typedef enum {
                               every other ray. */
 } mcx_status;
 
-enum { MCX_MAX_COMPONENTS = 16, MCX_MAX_DETECTORS = 8, MCX_MAX_MATERIALS = 32, MCX_MAX_SOLIDS = 16, MCX_MAX_LENSES = 256 };
+enum { MCX_MAX_COMPONENTS = 16, MCX_MAX_DETECTORS = 8, MCX_MAX_MATERIALS = 32, MCX_MAX_SOLIDS = 16, MCX_MAX_LENSES = 256,
+       MCX_MAX_SCATTER_ORDER = 1 << 20 };
 
 typedef enum {
   MCX_SOURCE = 0,          /* step 3 (point / flat / Gaussian emitters) */
@@ -88,7 +89,9 @@ typedef struct mcx_pose {
 typedef struct mcx_material {
   int64_t n_points;
   const double* energy_keV; /* HOST [n_points] */
-  const double* mu_per_m;   /* HOST [n_points] */
+  const double* mu_per_m;   /* HOST [n_points], total attenuation coefficient */
+  const double* mu_scatter_per_m; /* HOST [n_points] or NULL: the part of mu that scatters (step 17), 0 < mu_s <= mu,
+                               interpolated like mu; NULL = the material only attenuates */
 } mcx_material;
 
 /* One solid of a MCX_SOLIDS group (step 8).  Its pose is absolute (lab), like a component's. */
@@ -126,6 +129,7 @@ typedef struct mcx_slit_params {
 typedef struct mcx_solids_params {
   int64_t n_solids;         /* <= MCX_MAX_SOLIDS */
   const mcx_solid* solids;  /* HOST [n_solids] */
+  int64_t scatter_order;    /* step 17, as in mcx_voxels_params */
 } mcx_solids_params;
 
 typedef struct mcx_voxels_params {
@@ -134,6 +138,12 @@ typedef struct mcx_voxels_params {
   const uint8_t* ids;       /* DEVICE [nz][ny][nx], x fastest; values index the materials array (a value >=
                                n_materials is not a material and is traced as material 0, vacuum).
                                Read once by create (copied into the workspace in the traversal layout). */
+  int64_t scatter_order;    /* step 17 (a step updates the ray's weight "and direction"): at most this
+                               many elastic scattering events per ray in the sample, 0..MCX_MAX_SCATTER_ORDER; 0 =
+                               Beer-Lambert attenuation only.  Leg k draws the scattering optical depth to its event,
+                               -ln(u), and the Thomson-distributed angle (1 + cos^2) from slots 2k, 2k+1 of this component's
+                               Philox stream; up to the event and on a leg that leaves without one the weight is
+                               attenuated by mu - mu_s, after the last allowed event by mu. */
 } mcx_voxels_params;
 
 typedef struct mcx_mirror_params {

@@ -42,7 +42,7 @@ class McxPose(C.Structure):
 
 
 class McxMaterial(C.Structure):
-    _fields_ = [("n_points", C.c_int64), ("energy_keV", _dp), ("mu_per_m", _dp)]
+    _fields_ = [("n_points", C.c_int64), ("energy_keV", _dp), ("mu_per_m", _dp), ("mu_scatter_per_m", _dp)]
 
 
 class McxSolid(C.Structure):
@@ -64,11 +64,12 @@ class McxSlitParams(C.Structure):
 
 
 class McxSolidsParams(C.Structure):
-    _fields_ = [("n_solids", C.c_int64), ("solids", C.POINTER(McxSolid))]
+    _fields_ = [("n_solids", C.c_int64), ("solids", C.POINTER(McxSolid)), ("scatter_order", C.c_int64)]
 
 
 class McxVoxelsParams(C.Structure):
-    _fields_ = [("h", C.c_double), ("nx", C.c_int64), ("ny", C.c_int64), ("nz", C.c_int64), ("ids", C.c_void_p)]
+    _fields_ = [("h", C.c_double), ("nx", C.c_int64), ("ny", C.c_int64), ("nz", C.c_int64), ("ids", C.c_void_p),
+                ("scatter_order", C.c_int64)]
 
 
 class McxMirrorParams(C.Structure):
@@ -234,12 +235,14 @@ def marshal(inst, keep, device_voxels):
                     s.vertices, s.triangles = _ptr(v), _ptr(t, C.POINTER(C.c_int32))
             keep.append(arr)
             c.u.solids.n_solids, c.u.solids.solids = len(cd["solids"]), arr
+            c.u.solids.scatter_order = cd.get("scatter_order", 0)
         elif k == "voxels":
             ids = np.ascontiguousarray(cd["ids"], dtype=np.uint8)
             v = c.u.voxels
             v.h = cd["h"]
             v.nz, v.ny, v.nx = ids.shape
             v.ids = device_voxels(ids)
+            v.scatter_order = cd.get("scatter_order", 0)
         elif k == "mirror":
             m, t = c.u.mirror, cd["table"]
             m.p, m.q, m.theta, m.length, m.width = cd["p"], cd["q"], cd["theta"], cd["length"], cd["width"]
@@ -275,6 +278,10 @@ def marshal(inst, keep, device_voxels):
         mu = np.ascontiguousarray(md["mu"], dtype=np.float64)
         keep += [E, mu]
         m.n_points, m.energy_keV, m.mu_per_m = len(E), _ptr(E), _ptr(mu)
+        if md.get("mu_s") is not None:
+            mus = np.ascontiguousarray(md["mu_s"], dtype=np.float64)
+            keep.append(mus)
+            m.mu_scatter_per_m = _ptr(mus)
     return comps, mats
 
 

@@ -25,6 +25,8 @@ struct DMaterial {
   const double* lnMu;
   const double* slope;
   double inv_dlnE;  // (n-1) / (lnE[n-1]-lnE[0]): first guess of the segment, verified against E[]
+  const double* lnMuS;   // step 17: ln of the scattering part of mu on the same grid, and its slopes; null = does not scatter
+  const double* slopeS;
 };
 
 struct DSource {
@@ -71,6 +73,7 @@ struct DSolid {
 struct DSolids {
   int n_solids, n_mesh;
   const DSolid* solids;
+  int scatter_order, pad;  // step 17: direction changes allowed per ray in this group; 0 = attenuation only
 };
 
 // Voxel volume in traversal layout: 2 bytes per cell, {material ID, run}, where run = how many cells FOLLOWING this one
@@ -85,6 +88,7 @@ struct DVoxels {
   unsigned slab;  // cells per slab: (n[a1] + 2) * pitch
   unsigned mg_pitch, sh_pitch, mg_slab, sh_slab;  // x / pitch, x / slab by multiplication (fast_div in mcx_kernels.cu)
   int run_dir;    // +1 / -1: the direction along the fast axis the runs are counted in (source -> volume)
+  int scatter_order;  // step 17: direction changes allowed per ray in the volume; 0 = attenuation only
   const uint8_t* ids;  // cell k at ids[2 k] (ID) and ids[2 k + 1] (run)
 };
 
@@ -156,11 +160,12 @@ static_assert(sizeof(DInstrument) % 16 == 0, "copied to shared memory as int4");
 static_assert(sizeof(TallyBin) == 32, "one tally record per 32-byte sector");
 
 // feature bits: select the kernel instantiation (code for absent component kinds is compiled out)
-enum { F_SOLIDS = 1, F_MESH = 2, F_VOXELS = 4, F_OPTICS = 8, F_PRIM = 16, F_LENS = 32, F_ALL = 63 };  // F_SOLIDS: a solids group; F_PRIM / F_MESH: what it holds
+enum { F_SOLIDS = 1, F_MESH = 2, F_VOXELS = 4, F_OPTICS = 8, F_PRIM = 16, F_LENS = 32, F_SCATTER = 64, F_ALL = 127 };  // F_SOLIDS: a solids group; F_PRIM / F_MESH: what it holds
 
 // One trace launch: rays first + offset(q) for positions q in [0, n); offset(q) = order[q] if order != null, else q.
 struct TraceArgs {
   uint64_t first, n, seed;
+  int n_comps, n_mats, n_solids;  // sizes of the instrument: components, materials, solids of all groups together
   unsigned tile;           // positions per work ticket (set by launch_trace)
   int gate_max;            // components 1..gate_max are slits / mirrors / crystals: candidates for the absorber gate; 0 = off
   int cap_endpoints;       // interval endpoints per ray and solids group held in shared memory (a multiple of 8)

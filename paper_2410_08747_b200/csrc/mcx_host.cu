@@ -24,6 +24,7 @@ struct mcx_instrument {
   size_t upload_bytes = 0;              // host -> device bytes moved by create
   int n_comps = 0, n_mats = 0, n_dets = 0, features = 0;
   int cap_endpoints = 16;               // interval endpoints per ray and solids group (shared memory of the trace kernel)
+  int n_solids_total = 0;               // solids of all groups together (staged in shared memory by the trace kernel)
   int gate_max = 0;                     // leading slits / mirrors / crystals of the chain (TraceArgs::gate_max)
   bool sort_pays = false;               // AUTO lane scheduling: detector-tile order
   uint64_t det_bins[MCX_MAX_DETECTORS] = {};
@@ -249,7 +250,7 @@ mcx_status make_plan(const mcx_component* comps, int n_comps, const mcx_material
   P->blob_begin = A.top;
   for (int m = 0; m < n_mats; ++m) {
     if (mats[m].n_points < 0 || mats[m].n_points == 1) return fail(MCX_ERR_INVALID_ARG, "material %d: n_points must be 0 or >= 2", m);
-    P->off_mat[m] = A.reserve((size_t)mats[m].n_points * 4 * sizeof(double));
+    P->off_mat[m] = A.reserve((size_t)mats[m].n_points * (mats[m].mu_scatter_per_m ? 6 : 4) * sizeof(double));
   }
   int n_dets = 0;
   for (int c = 0; c < n_comps; ++c) {
@@ -434,6 +435,19 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
     D.lnMu = D.lnE + n;
     D.slope = D.lnMu + n;
     D.inv_dlnE = (double)(n - 1) / (lnE[n - 1] - lnE[0]);
+    if (M.mu_scatter_per_m) {  // step 17: the scattering part, same grid
+      double* lnS = slope + n;
+      double* slopeS = lnS + n;
+      for (size_t j = 0; j < n; ++j) {
+        if (!(M.mu_scatter_per_m[j] > 0.0) || !(M.mu_scatter_per_m[j] <= M.mu_per_m[j]))
+          MCX_BAIL(MCX_ERR_RANGE, "material %d: mu_scatter must be in (0, mu] (entry %zu)", m, j);
+        lnS[j] = std::log(M.mu_scatter_per_m[j]);
+      }
+      for (size_t j = 0; j + 1 < n; ++j) slopeS[j] = (lnS[j + 1] - lnS[j]) / (lnE[j + 1] - lnE[j]);
+      slopeS[n - 1] = 0.0;
+      D.lnMuS = D.slope + n;
+      D.slopeS = D.lnMuS + n;
+    }
   }
 
   int n_dets = 0;
@@ -493,6 +507,9 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
         DSolid* hs = (DSolid*)host_ptr(P.off_solids[c]);
         D.u.solids.n_solids = (int)G.n_solids;
         D.u.solids.solids = (const DSolid*)dev_ptr(P.off_solids[c]);
+        if (G.scatter_order < 0 || G.scatter_order > MCX_MAX_SCATTER_ORDER) MCX_BAIL(MCX_ERR_INVALID_ARG, "component %d: bad scatter_order", c);
+        D.u.solids.scatter_order = (int)G.scatter_order;
+        if (G.scatter_order > 0) features |= F_SCATTER;
         // device order = ascending precedence: by priority, among equals the LATER-listed first (step 10: the earlier
         // solid wins a tie), so that the owner of an overlap is the solid with the highest device index
         int pos[MCX_MAX_SOLIDS];
@@ -589,6 +606,9 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
         if (!V.ids) MCX_BAIL(MCX_ERR_INVALID_ARG, "component %d: ids is null", c);
         if (n_materials < 1) MCX_BAIL(MCX_ERR_INVALID_ARG, "component %d: a voxel volume needs a materials array (ID 0 = materials[0])", c);
         DVoxels& d = D.u.voxels;
+        if (V.scatter_order < 0 || V.scatter_order > MCX_MAX_SCATTER_ORDER) MCX_BAIL(MCX_ERR_INVALID_ARG, "component %d: bad scatter_order", c);
+        d.scatter_order = (int)V.scatter_order;
+        if (V.scatter_order > 0) features |= F_SCATTER;
         d.h = V.h;
         d.inv_h = 1.0 / V.h;
         d.n[0] = (int)V.nx; d.n[1] = (int)V.ny; d.n[2] = (int)V.nz;
@@ -710,6 +730,8 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
   for (int c = 0; c < n_components; ++c)
     if (components[c].kind == MCX_VOXELS) H->voxel_params[c] = components[c].u.voxels;
   H->cap_endpoints = cap_endpoints;
+  for (int c = 0; c < n_components; ++c)
+    if (components[c].kind == MCX_SOLIDS) H->n_solids_total += (int)components[c].u.solids.n_solids;
   for (int c = 1; c + 1 < n_components; ++c) {
       const int k = components[c].kind;
     if (k != MCX_SLIT_RECT && k != MCX_SLIT_CIRC && k != MCX_MIRROR_ELLIPTIC && k != MCX_CRYSTAL_BRAGG) break;
@@ -792,6 +814,9 @@ mcx_status run_trace(mcx_instrument* H, uint64_t first, uint64_t n, uint64_t see
     A.first = first + base;
     A.n = m;
     A.seed = seed;
+    A.n_comps = H->n_comps;
+    A.n_mats = H->n_mats;
+    A.n_solids = H->n_solids_total;
     A.cap_endpoints = H->cap_endpoints;
     A.gate_max = H->gate_enabled ? H->gate_max : 0;
     A.host_flag = H->host_flag;

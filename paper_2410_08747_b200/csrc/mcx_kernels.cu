@@ -16,6 +16,17 @@ namespace {
 constexpr int kBlock = 256;
 constexpr unsigned kVoxelGuard = 255u;  // ID of the guard cells around the voxel volume (material IDs are < MCX_MAX_MATERIALS)
 
+// What a block keeps of the instrument in shared memory: only the components and materials the instrument has (the
+// arrays of DInstrument are sized for the limits of the ABI; every kilobyte of shared memory a block does not take is L1
+// for the BVH and the voxel rows -- 512 bytes more per block cost the mesh config 12 %).
+struct SInst {
+  int n_comps, n_mats;
+  const DComponent* comps;       // shared memory [n_comps]
+  const DMaterial* mats;         // shared memory [n_mats]
+  TallyBin* const* tallies;      // shared memory [MCX_MAX_DETECTORS]
+  unsigned long long* counters;  // global
+};
+
 // ------------------------------------------------------------------------------------------------------------
 // Step 1: Philox4x32-10 (Salmon et al., SC'11); key = seed, counter = (i lo, i hi, slot, component).
 // ------------------------------------------------------------------------------------------------------------
@@ -591,7 +602,7 @@ __device__ __forceinline__ int mesh_endpoints_warp(const DSolid& S, unsigned sol
 // `coherent` = the warp's rays are neighbours (detector-tile order), so the beam walk of the meshes is tried first.
 // PRIM = some group of the instrument holds a box, cylinder or sphere.
 template <bool MESH, bool PRIM>
-__device__ __forceinline__ int trace_solids(const DInstrument& I, const DComponent& C, Ray& ray, const Endpoints& E,
+__device__ __forceinline__ int trace_solids(const SInst& I, const DComponent& C, Ray& ray, const Endpoints& E,
                                             unsigned* __restrict__ queue, bool active, bool coherent) {
   const DSolids& G = C.u.solids;
   int ne = 0, status = 1;
@@ -651,6 +662,163 @@ __device__ __forceinline__ int trace_solids(const DInstrument& I, const DCompone
     const unsigned bit = 1u << (tag & 31u);
     inside = (tag & kTagExit) ? (inside & ~bit) : (inside | bit);
   }
+  ray.p *= exp(-tau);
+  return 1;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Step 17: scattering in samples (a step updates the ray's weight "and direction").  Elastic, Thomson
+// angular distribution: cos(theta) is the real root of x^3 + 3x = 8u - 4 (inverse of F(x) = 1/2 + (3/8)(x + x^3/3)),
+// x = w - 1/w with w = cbrt(q + sqrt(q^2 + 1)), q = 4u - 2; azimuth 2 pi u'.  New direction = cos(theta) d +
+// sin(theta)(cos(phi) e1 + sin(phi) e2), e1 = (d x a)/|d x a| with a the coordinate axis along which |d| is smallest
+// (ties: the lowest axis), e2 = d x e1; normalised once more.
+// ------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ Vec3 cross(Vec3 a, Vec3 b) { return {a.y * b.z - a.z * b.y, a.z * b.x - a.x * b.z, a.x * b.y - a.y * b.x}; }
+
+__device__ __noinline__ Vec3 scatter_direction(Vec3 d, double u_mu, double u_phi) {
+  const double q = 4.0 * u_mu - 2.0;
+  const double w = cbrt(q + sqrt(q * q + 1.0));
+  const double ct = w - 1.0 / w;
+  const double st = sqrt(fmax(0.0, 1.0 - ct * ct));
+  double sp, cp;
+  sincos(2.0 * CUDART_PI * u_phi, &sp, &cp);
+  Vec3 a{1.0, 0.0, 0.0};
+  double m = fabs(d.x);
+  if (fabs(d.y) < m) { a = {0.0, 1.0, 0.0}; m = fabs(d.y); }
+  if (fabs(d.z) < m) { a = {0.0, 0.0, 1.0}; }
+  Vec3 e1 = cross(d, a);
+  e1 = (1.0 / sqrt(dot(e1, e1))) * e1;
+  const Vec3 e2 = cross(d, e1);
+  const Vec3 v = ct * d + st * (cp * e1 + sp * e2);
+  return (1.0 / sqrt(dot(v, v))) * v;
+}
+
+// the scattering part of mu(E): same grid, same interpolation (step 7); 0 for a material without the table
+__device__ __forceinline__ double mu_s_of(const DMaterial& M, double E, double lnE) {
+  if (M.lnMuS == nullptr) return 0.0;
+  DMaterial S = M;
+  S.lnMu = M.lnMuS;
+  S.slope = M.slopeS;
+  return mu_of(S, E, lnE);
+}
+
+// Step 17 state of one ray inside one sample
+struct Scat {
+  double tau_s;    // scattering optical depth at which the next event lies (leg k < K)
+  double cum;      // running sum of mu_s * length on this leg
+  double s_pre;    // sum of mu_s * length over everything walked while events were left: tau = sum mu L - s_pre
+  double t_event;  // parameter of the event on this leg
+  int k, K;        // events so far, events allowed
+  unsigned have_ms;  // (voxels) bit m: the ray's mu_s of material m is in shared memory
+  bool event;
+};
+
+// Steps 8-10 (and 17 where the group scatters) for one solids group.  Returns 1 = continue, 0 = degenerate, -1 = capacity
+// overflow.  Must be called by all 32 lanes of the warp, `active` saying which have a live ray (the mesh walk is
+// warp-cooperative, and the legs of step 17 are walked by the warp together); `coherent` = the warp's rays are neighbours
+// (detector-tile order), so the beam walk of the meshes is tried first.  PRIM = some group of the instrument holds a box,
+// cylinder or sphere.  SCAT: a ray walks leg after leg, each from its last scattering event, while events are left.
+template <bool MESH, bool PRIM, bool SCAT>
+__device__ __forceinline__ int trace_solids_legs(const SInst& I, const DComponent& C, int comp, Ray& ray, uint64_t seed, uint64_t ray_index,
+                                            const Endpoints& E, unsigned* __restrict__ queue, bool active, bool coherent) {
+  const DSolids& G = C.u.solids;
+  int status = 1;
+  double tau = 0.0, lnE = 0.0;
+  Scat S;
+  S.k = 0; S.K = SCAT ? G.scatter_order : 0; S.cum = 0.0; S.tau_s = 0.0; S.s_pre = 0.0; S.t_event = 0.0; S.have_ms = 0u; S.event = false;
+  bool more = active;  // this lane has a leg to walk
+  for (int leg = 0;; ++leg) {
+    if (SCAT && leg > 0 && !__any_sync(0xffffffffu, more)) break;
+    const bool walk = more && status == 1;
+    int ne = 0;
+    for (int s = 0; s < G.n_solids; ++s) {
+      const DSolid& Sd = G.solids[s];
+      if (MESH && Sd.shape == MCX_MESH) {  // warp-uniform branch
+        const bool act = walk && status == 1;
+        int rc;
+        for (bool coh = coherent && leg == 0;; coh = false) {  // (a second round only if the beam walk gives up: rc 2, warp-uniform)
+          Vec3 o{0.0, 0.0, 0.0}, d{0.0, 0.0, 1.0};
+          if (act) { o = to_local(Sd.pose, ray.r); d = rotate(Sd.pose.R, ray.d); }
+          rc = mesh_endpoints_warp(Sd, (unsigned)s, act, o, d, E, ne, queue, coh);
+          if (rc != 2) break;
+        }
+        if (act && rc != 1) status = rc;
+        continue;
+      }
+      if (!PRIM || !(walk && status == 1)) continue;
+      if (!MESH) {  // (the mesh kernels run at the register limit and do without)
+        // the line misses the solid's bounding sphere, by more than the rounding of this test (1e-9 of the radius^2 in
+        // bound2, 1e-14 of the squared distance for the cancellation): no interval, no need for the solid's frame
+        const Vec3 oc = Vec3{Sd.pose.T[0], Sd.pose.T[1], Sd.pose.T[2]} - ray.r;
+        const double along = dot(oc, ray.d), oc2 = dot(oc, oc);
+        if (oc2 - along * along > Sd.bound2 + 1e-14 * oc2) continue;
+      }
+      const Vec3 o = to_local(Sd.pose, ray.r);
+      const Vec3 d = rotate(Sd.pose.R, ray.d);
+      double a, b;
+      if (primitive_interval(Sd, o, d, a, b)) {  // clip to t >= 0, drop if empty
+        a = fmax(a, 0.0);
+        if (b > a) {
+          if (!ep_push(E, ne, a, (unsigned)s)) status = -1;
+          if (!ep_push(E, ne, b, (unsigned)s | kTagExit)) status = -1;
+        }
+      }
+    }
+    more = false;
+    if (walk && status == 1 && ne > 0) {
+      // Step 10.  Between two consecutive end points the set of solids the ray is inside of is constant, so sweeping the
+      // sorted end points with that set as a bit mask classifies every elementary segment exactly as its midpoint would;
+      // the owner is the solid of highest precedence in the set = the highest bit (DSolids).  Equal end points only
+      // make zero-length segments, whatever their order.
+      ep_sort(E, 0, ne, false);
+      if (leg == 0) lnE = log(ray.E);
+      double u_mu = 0.0;
+      if (SCAT && S.k < S.K) {  // step 17: where on this leg the next event lies, in scattering optical depth
+        double u_f;
+        draw2(seed, ray_index, (uint32_t)(2 * S.k), (uint32_t)comp, u_f, u_mu);
+        S.tau_s = -log(u_f);
+        S.cum = 0.0;
+      }
+      double t_prev = 0.0, last_mu = 0.0, last_ms = 0.0;
+      int last_mat = -1;
+      unsigned inside = 0u;
+      for (int k = 0; k < ne; ++k) {
+        const double t = E.t[k * kBlock];
+        const unsigned tag = E.tag[k * kBlock];
+        if (inside != 0u && t > t_prev) {
+          const int mat = G.solids[31 - __clz(inside)].material;
+          if (mat != last_mat) {
+            last_mu = mu_of(I.mats[mat], ray.E, lnE);
+            if (SCAT) last_ms = mu_s_of(I.mats[mat], ray.E, lnE);
+            last_mat = mat;
+          }
+          const double len = t - t_prev;
+          if (SCAT && S.k < S.K) {
+            if (last_ms > 0.0 && S.cum + last_ms * len >= S.tau_s) {
+              const double l = (S.tau_s - S.cum) / last_ms;
+              tau += (last_mu - last_ms) * l;
+              double u_phi, unused;
+              draw2(seed, ray_index, (uint32_t)(2 * S.k + 1), (uint32_t)comp, u_phi, unused);
+              ray.r = ray.r + (t_prev + l) * ray.d;
+              ray.d = scatter_direction(ray.d, u_mu, u_phi);
+              ++S.k;
+              more = true;  // walk the next leg from here
+              break;
+            }
+            S.cum += last_ms * len;
+            tau += (last_mu - last_ms) * len;
+          } else {
+            tau += last_mu * len;
+          }
+        }
+        t_prev = t;
+        const unsigned bit = 1u << (tag & 31u);
+        inside = (tag & kTagExit) ? (inside & ~bit) : (inside | bit);
+      }
+    }
+    if (!SCAT) break;
+  }
+  if (!active || status != 1) return status;
   ray.p *= exp(-tau);
   return 1;
 }
@@ -754,14 +922,16 @@ __device__ __forceinline__ void lateral_init(const VoxAxis& A, double inv_dw, do
   a = adv >= 1.0 ? 0xFFFFFFFFFFFFFFFFull : frac64(adv);
 }
 
-__device__ __forceinline__ void trace_voxels(const DInstrument& I, const DComponent& C, Ray& ray, double* len_s, double* cold_s) {
-  const DVoxels& V = C.u.voxels;
+// One leg of the walk: the half-line ol + t dl, t >= 0, in the volume's frame, from where it enters the grid to where it
+// leaves it or (SCAT, step 17) to the scattering event.  Path lengths go to len_s / touched, which accumulate over legs.
+template <bool SCAT>
+__device__ __forceinline__ void voxel_leg(const SInst& I, const DVoxels& V, Vec3 ol, Vec3 dl, double E, double lnE, double* len_s,
+                                          double* cold_s, double* mus_s, unsigned& touched, Scat& S) {
   const double h = V.h;
   unsigned ful, fuh, fvl, fvh, aul, auh, avl, avh, cu0, cv0, so_u, so_v, so_w, meta, lo_start, inv_u, inv_v;
   double t_run;
+  S.event = false;
   {
-    const Vec3 ol = to_local(C.pose, ray.r);
-    const Vec3 dl = rotate(C.pose.R, ray.d);
     const Vec3 inv_d{1.0 / dl.x, 1.0 / dl.y, 1.0 / dl.z};  // the only divisions of the set-up (+-inf where d = 0: unused)
     double t0 = -CUDART_INF, t1 = CUDART_INF;
     auto clip = [&](double o, double d, double inv, double top) {  // slab [0, top] of one axis, as clip_axis
@@ -816,7 +986,7 @@ __device__ __forceinline__ void trace_voxels(const DInstrument& I, const DCompon
   lo_start += (unsigned)base;
 #define MCX_VOXEL_AT(lo32) ld_voxel(hi | (lo32))
   unsigned cur = MCX_VOXEL_AT(lo_start);
-  unsigned touched = 0u;  // bit m: len_s[m] holds this ray's path length in material m
+  // (touched: bit m = len_s[m] holds this ray's path length in material m)
   // The run of `cur` ends where the ray enters the voxel at address `at` through a face of axis k: the index of that
   // voxel along the axis comes back out of the address (a guard cell gives -1 or n, i.e. the outer face of the grid),
   // and the face parameter is (face - o) / d as in step 11 (as a product with 1/d, one more rounding).
@@ -836,11 +1006,29 @@ __device__ __forceinline__ void trace_voxels(const DInstrument& I, const DCompon
     }
     const double tf = ((double)face * h - cold_s[(VC_O + 2 * k) * kBlock]) * cold_s[(VC_INVD + 2 * k) * kBlock];
     const double tn = fmin(tf, cold_s[VC_T1 * kBlock]);
+    double len = tn - t_run;
+    bool ev = false;
+    if (SCAT && S.k < S.K) {  // step 17: does the event fall inside this run?
+      const DMaterial& M = I.mats[cur];
+      double ms = 0.0;
+      if (M.lnMuS != nullptr) {
+        if (!((S.have_ms >> cur) & 1u)) { mus_s[cur * kBlock] = mu_s_of(M, E, lnE); S.have_ms |= 1u << cur; }
+        ms = mus_s[cur * kBlock];
+      }
+      if (ms > 0.0 && S.cum + ms * len >= S.tau_s) {
+        len = (S.tau_s - S.cum) / ms;
+        S.t_event = t_run + len;
+        ev = true;
+      } else {
+        S.cum += ms * len;
+      }
+    }
     const double prev = (touched >> cur) & 1u ? len_s[cur * kBlock] : 0.0;
-    len_s[cur * kBlock] = prev + (tn - t_run);
+    len_s[cur * kBlock] = prev + len;
     touched |= 1u << cur;
     t_run = tn;
     cur = id;
+    return ev;
   };
   // One iteration = one slab, then a skip.
   //  Slab: the lateral step (if any; the same cell again if cu = cv = 0) and the w face that ends the slab: cell b at
@@ -865,15 +1053,15 @@ __device__ __forceinline__ void trace_voxels(const DInstrument& I, const DCompon
       ida = MCX_VOXEL_AT(lo_a);
     }
     if (ida != cur) {  // the cell in between the two lateral faces of a double step
-      close_run(lo_a, k_first, ida);
+      if (close_run(lo_a, k_first, ida)) { S.event = true; return true; }
       if (ida == kVoxelGuard) return true;
     }
     if (idbA != cur) {
-      close_run(lo_bA, k_lat, idbA);
+      if (close_run(lo_bA, k_lat, idbA)) { S.event = true; return true; }
       if (idbA == kVoxelGuard) return true;
     }
     if (idcA != cur) {
-      close_run(lo_cA, 0u, idcA);
+      if (close_run(lo_cA, 0u, idcA)) { S.event = true; return true; }
       if (idcA == kVoxelGuard) return true;
     }
     return false;
@@ -899,15 +1087,52 @@ __device__ __forceinline__ void trace_voxels(const DInstrument& I, const DCompon
     cv = add_carry(fvl, fvh, avl, avh);
   }
 #undef MCX_VOXEL_AT
-  // tau = sum over the touched materials of mu_m(E) * len_m (step 7 evaluated for those only)
-  const double lnE = log(ray.E);
+}
+
+// Step 11 (and 17 where the volume scatters): the legs of one ray, then tau = sum over the touched materials of
+// mu_m(E) * len_m (step 7 evaluated for those only) - what the scattering took of it while events were left.
+template <bool SCAT>
+__device__ __forceinline__ void trace_voxels(const SInst& I, const DComponent& C, int comp, Ray& ray, uint64_t seed, uint64_t i,
+                                             double* len_s, double* cold_s, double* mus_s) {
+  const DVoxels& V = C.u.voxels;
+  Vec3 ol = to_local(C.pose, ray.r), dl = rotate(C.pose.R, ray.d);
+  unsigned touched = 0u;
+  Scat S;
+  S.k = 0; S.K = SCAT ? V.scatter_order : 0; S.s_pre = 0.0; S.cum = 0.0; S.tau_s = 0.0; S.t_event = 0.0; S.have_ms = 0u; S.event = false;
+  const double lnE_early = SCAT ? log(ray.E) : 0.0;  // (without scattering ln E is not needed, nor kept in a register, during the walk)
+  for (;;) {
+    double u_mu = 0.0;
+    if (SCAT && S.k < S.K) {
+      double u_f;
+      draw2(seed, i, (uint32_t)(2 * S.k), (uint32_t)comp, u_f, u_mu);
+      S.tau_s = -log(u_f);
+      S.cum = 0.0;
+    }
+    voxel_leg<SCAT>(I, V, ol, dl, ray.E, lnE_early, len_s, cold_s, mus_s, touched, S);
+    if (!SCAT || !S.event) {
+      if (SCAT && S.k < S.K) S.s_pre += S.cum;
+      break;
+    }
+    S.s_pre += S.tau_s;
+    double u_phi, unused;
+    draw2(seed, i, (uint32_t)(2 * S.k + 1), (uint32_t)comp, u_phi, unused);
+    ol = ol + S.t_event * dl;
+    dl = scatter_direction(dl, u_mu, u_phi);
+    ++S.k;
+  }
+  const double lnE = SCAT ? lnE_early : log(ray.E);
   double tau = 0.0;
   while (touched) {
     const int m = __ffs(touched) - 1;
     touched &= touched - 1u;
     tau += mu_of(I.mats[m], ray.E, lnE) * len_s[m * kBlock];
   }
+  if (SCAT) tau -= S.s_pre;
   ray.p *= exp(-tau);
+  if (SCAT && S.k > 0) {
+    ray.r = to_lab(C.pose, ol);
+    ray.d = rotate_back(C.pose.R, dl);
+  }
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -999,7 +1224,7 @@ __device__ __forceinline__ double darwin_prins(double eta, double g, double kapp
 // the root of the intersection quadratic that tends to the plane intersection as R -> inf, in its cancellation-free form;
 // aperture test; Snell's law in vector form, d' = m d + (c_t - m c) nrm with c_t - m c = (1 - m)(1 + m) / (c_t + m c) and
 // 1 - m formed from delta directly, so the deflection (relative size delta ~ 1e-6) carries no cancellation.
-__device__ __forceinline__ bool trace_lens(const DInstrument& I, const DComponent& C, Ray& ray) {
+__device__ __forceinline__ bool trace_lens(const SInst& I, const DComponent& C, Ray& ray) {
   const DLens& L = C.u.lens;
   Vec3 o = to_local(C.pose, ray.r);
   Vec3 d = rotate(C.pose.R, ray.d);
@@ -1235,7 +1460,7 @@ __device__ __noinline__ void tally_add_aggregated(TallyBin* const* tallies, int 
 }
 
 // Step 14 for one warp and one detector (all 32 lanes call it).
-__device__ __forceinline__ void tally_add(const DInstrument& I, int mode, const TallyCache& tc, unsigned det, bool on, long long bin,
+__device__ __forceinline__ void tally_add(const SInst& I, int mode, const TallyCache& tc, unsigned det, bool on, long long bin,
                                           double p) {
   if (mode == MCX_TALLY_GLOBAL) {
     if (on) tally_global(I.tallies[det] + bin, 1ull, p, p * p);
@@ -1245,7 +1470,7 @@ __device__ __forceinline__ void tally_add(const DInstrument& I, int mode, const 
 }
 
 // the block's cache goes to global memory: one set of reductions per occupied slot (all threads of the block)
-__device__ __forceinline__ void tally_flush(const DInstrument& I, const TallyCache& tc) {
+__device__ __forceinline__ void tally_flush(const SInst& I, const TallyCache& tc) {
   if (tc.log2 == 0) return;
   const int n = 1 << tc.log2;
   for (int h = threadIdx.x; h < n; h += kBlock) {
@@ -1267,42 +1492,49 @@ __device__ __forceinline__ void tally_flush(const DInstrument& I, const TallyCac
 // ------------------------------------------------------------------------------------------------------------
 constexpr size_t kRingBytes = (kBlock / 32) * 64 * sizeof(unsigned);  // per-warp rings of gate survivors
 constexpr unsigned kTileMax = 8192;  // positions per work ticket (a power of two >= kBlock; smaller for short launches)
-constexpr int kSmemSolids = 32;    // solids staged in shared memory (all groups together)
 
 // resident blocks per SM the register budget is held to: the voxel walk hides its byte loads with warps
 constexpr int min_blocks(int feat) {
   return feat == F_VOXELS || feat == (F_SOLIDS | F_PRIM) || feat == (F_SOLIDS | F_MESH) || feat == (F_SOLIDS | F_MESH | F_PRIM) ? 3
-         : (feat == F_OPTICS || feat == F_LENS) ? 2 : 1;
+         : (feat == F_OPTICS || feat == F_LENS || feat == (F_VOXELS | F_SCATTER)) ? 2 : 1;
 }
 
 template <int FEAT, bool DUMP, bool GATE>
 __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const DInstrument* __restrict__ g_inst, TraceArgs A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  DInstrument& I = *reinterpret_cast<DInstrument*>(smem_raw);
-  unsigned int* s_cnt = reinterpret_cast<unsigned int*>(smem_raw + sizeof(DInstrument));  // [MCX_MAX_COMPONENTS + 4]
+  unsigned int* s_cnt = reinterpret_cast<unsigned int*>(smem_raw);  // [MCX_MAX_COMPONENTS + 4]
   unsigned int* s_sched = s_cnt + MCX_MAX_COMPONENTS + 4;  // [0..1] tile tickets, [2..3] slice counters (ping-pong)
-  unsigned char* s_extra = smem_raw + sizeof(DInstrument) + 128 + (GATE ? kRingBytes : 0);
+  const int n_comps = A.n_comps, n_mats = A.n_mats;
+  // the instrument, compact (SInst): components, materials, tally pointers
+  DComponent* s_comps = reinterpret_cast<DComponent*>(smem_raw + 128 + (GATE ? kRingBytes : 0));
+  DMaterial* s_mats = reinterpret_cast<DMaterial*>(s_comps + n_comps);
+  TallyBin** s_tallies = reinterpret_cast<TallyBin**>(s_mats + n_mats);
+  unsigned char* s_extra = reinterpret_cast<unsigned char*>(s_tallies + MCX_MAX_DETECTORS);
   {
-    const int4* src = reinterpret_cast<const int4*>(g_inst);
-    int4* dst = reinterpret_cast<int4*>(smem_raw);
-    for (int k = threadIdx.x; k < (int)(sizeof(DInstrument) / sizeof(int4)); k += kBlock) dst[k] = src[k];
+    static_assert(sizeof(DComponent) % 8 == 0 && sizeof(DMaterial) % 8 == 0, "copied as 8-byte words");
+    const unsigned long long* src = reinterpret_cast<const unsigned long long*>(g_inst->comps);
+    unsigned long long* dst = reinterpret_cast<unsigned long long*>(s_comps);
+    for (int k = threadIdx.x; k < n_comps * (int)(sizeof(DComponent) / 8); k += kBlock) dst[k] = src[k];
+    src = reinterpret_cast<const unsigned long long*>(g_inst->mats);
+    dst = reinterpret_cast<unsigned long long*>(s_mats);
+    for (int k = threadIdx.x; k < n_mats * (int)(sizeof(DMaterial) / 8); k += kBlock) dst[k] = src[k];
+    if (threadIdx.x < MCX_MAX_DETECTORS) s_tallies[threadIdx.x] = g_inst->tallies[threadIdx.x];
     if (threadIdx.x < MCX_MAX_COMPONENTS + 4) s_cnt[threadIdx.x] = 0u;
   }
+  const SInst I{n_comps, n_mats, s_comps, s_mats, s_tallies, g_inst->counters};
   __syncthreads();
-  const int n_comps = I.n_comps;
   if (FEAT & F_SOLIDS) {  // stage the solids (poses, sizes, priorities) of every group and re-point the groups at the copy
     DSolid* s_solids = reinterpret_cast<DSolid*>(s_extra);
-    s_extra += kSmemSolids * sizeof(DSolid);
+    s_extra += A.n_solids * sizeof(DSolid);
     int used = 0;
     for (int c = 1; c < n_comps; ++c) {
-      if (I.comps[c].kind != MCX_SOLIDS) continue;
-      const int ns = I.comps[c].u.solids.n_solids;
-      if (used + ns > kSmemSolids) continue;
-      const unsigned long long* src = reinterpret_cast<const unsigned long long*>(I.comps[c].u.solids.solids);
+      if (s_comps[c].kind != MCX_SOLIDS) continue;
+      const int ns = s_comps[c].u.solids.n_solids;
+      const unsigned long long* src = reinterpret_cast<const unsigned long long*>(s_comps[c].u.solids.solids);
       unsigned long long* dst = reinterpret_cast<unsigned long long*>(s_solids + used);
       for (int k = threadIdx.x; k < ns * (int)(sizeof(DSolid) / 8); k += kBlock) dst[k] = src[k];
       __syncthreads();
-      if (threadIdx.x == 0) I.comps[c].u.solids.solids = s_solids + used;
+      if (threadIdx.x == 0) s_comps[c].u.solids.solids = s_solids + used;
       used += ns;
     }
     __syncthreads();
@@ -1360,7 +1592,7 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
   // later launches on the instrument start with it.
   const unsigned known_gate = GATE ? s_sched[5] : 0u;
   int gate = known_gate ? (int)known_gate - 1 : 0;
-  unsigned* ring = reinterpret_cast<unsigned*>(smem_raw + sizeof(DInstrument) + 128) + (threadIdx.x >> 5) * 64;
+  unsigned* ring = reinterpret_cast<unsigned*>(smem_raw + 128) + (threadIdx.x >> 5) * 64;
   unsigned ring_head = 0u, ring_n = 0u;  // warp-uniform
   // One warp-load of rays through components 1 .. (final_pass ? the end : the gate); see the loops below.
   auto trace_item = [&](const bool valid, const uint64_t qi, const bool final_pass) {
@@ -1375,7 +1607,11 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
       const int kind = C.kind;  // warp-uniform
       bool pass = true, tally_now = false;
       if ((FEAT & F_SOLIDS) && kind == MCX_SOLIDS) {  // whole warp: the mesh walk is warp-cooperative
-        const int rc = trace_solids<(FEAT & F_MESH) != 0, (FEAT & F_PRIM) != 0>(I, C, ray, ep, tri_queue, alive, order != nullptr);
+        // (the walk without scattering is kept as its own function: the mesh kernel sits at the register limit)
+        const int rc = (FEAT & F_SCATTER)
+                           ? trace_solids_legs<(FEAT & F_MESH) != 0, (FEAT & F_PRIM) != 0, true>(I, C, c, ray, seed, first + qi, ep, tri_queue, alive,
+                                                                                                 order != nullptr)
+                           : trace_solids<(FEAT & F_MESH) != 0, (FEAT & F_PRIM) != 0>(I, C, ray, ep, tri_queue, alive, order != nullptr);
         if (alive && rc != 1) {
           pass = false;
           fate = MCX_FATE_DEGENERATE;
@@ -1389,7 +1625,8 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
           Vec3 h;
           pass = plane_hit(C.pose, ray, h) && h.x * h.x + h.y * h.y <= C.u.slit.radius2;
         } else if ((FEAT & F_VOXELS) && kind == MCX_VOXELS) {
-          trace_voxels(I, C, ray, len_s, len_s + (size_t)I.n_mats * kBlock);
+          trace_voxels<(FEAT & F_SCATTER) != 0>(I, C, c, ray, seed, first + qi, len_s, len_s + (size_t)I.n_mats * kBlock,
+                                                len_s + (size_t)(I.n_mats + VC_COUNT) * kBlock);
         } else if ((FEAT & F_OPTICS) && kind == MCX_MIRROR_ELLIPTIC) {
           pass = trace_mirror(C, ray);
         } else if ((FEAT & F_OPTICS) && kind == MCX_CRYSTAL_BRAGG) {
@@ -1615,13 +1852,14 @@ __global__ void __launch_bounds__(256) probe_dfma_kernel(double* sink, long long
   sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
 }
 
-constexpr size_t kSmemBase = sizeof(DInstrument) + 128;
 
 template <int FEAT, bool DUMP, bool GATE>
 cudaError_t launch_one(const DInstrument* d_inst, int n_mats, const TraceArgs& A, cudaStream_t stream, int n_sm) {
-  const size_t smem = kSmemBase + (GATE ? kRingBytes : 0) + ((FEAT & F_SOLIDS) ? kSmemSolids * sizeof(DSolid) + (size_t)A.cap_endpoints * kBlock * 9 : 0) +
+  const size_t smem = 128 + (GATE ? kRingBytes : 0) + (size_t)A.n_comps * sizeof(DComponent) + (size_t)A.n_mats * sizeof(DMaterial) +
+                      MCX_MAX_DETECTORS * sizeof(void*) +
+                      ((FEAT & F_SOLIDS) ? (size_t)A.n_solids * sizeof(DSolid) + (size_t)A.cap_endpoints * kBlock * 9 : 0) +
                       ((FEAT & F_MESH) ? (size_t)kTriQueue * kBlock * sizeof(unsigned) : 0) +
-                      ((FEAT & F_VOXELS) ? (size_t)(n_mats + VC_COUNT) * kBlock * sizeof(double) : 0) +
+                      ((FEAT & F_VOXELS) ? (size_t)(n_mats + VC_COUNT + ((FEAT & F_SCATTER) ? n_mats : 0)) * kBlock * sizeof(double) : 0) +
                       ((!DUMP && !(FEAT & (F_SOLIDS | F_VOXELS)) && A.tally_cache_log2 > 0) ? ((size_t)32 << A.tally_cache_log2) : 0);
   static std::atomic<unsigned long long> configured{0ull};  // bit d: the opt-in below was made on device d
   int blocks_per_sm = 1, dev = 0;
@@ -1684,6 +1922,7 @@ cudaError_t launch_trace(const DInstrument* d_inst, int features, int n_mats, co
     case F_SOLIDS | F_MESH: MCX_DISPATCH(F_SOLIDS | F_MESH)
     case F_SOLIDS | F_MESH | F_PRIM: MCX_DISPATCH(F_SOLIDS | F_MESH | F_PRIM)
     case F_VOXELS: MCX_DISPATCH(F_VOXELS)
+    case F_VOXELS | F_SCATTER: MCX_DISPATCH(F_VOXELS | F_SCATTER)
     case F_OPTICS: MCX_DISPATCH_GATED(F_OPTICS)
     case F_LENS: MCX_DISPATCH_GATED(F_LENS)
     default: MCX_DISPATCH_GATED(F_ALL)

@@ -365,7 +365,18 @@ def config0(n_rays=1_000_000):
     return instrument("c0_minimal", comps, mats, n_rays)
 
 
-def config1(n_rays=100_000_000, small=False):
+def _scattering(rng_seed, mats, comps, scatter_order):
+    """gives every material a scattering part (seeded) and lets every sample scatter up to
+    scatter_order times per ray."""
+    rng = np.random.default_rng(rng_seed)
+    mats = [None if m is None else with_scattering(rng, m) for m in mats]
+    for c in comps:
+        if c["kind"] in ("solids", "voxels"):
+            c["scatter_order"] = int(scatter_order)
+    return mats
+
+
+def config1(n_rays=100_000_000, small=False, scatter_order=0):
     """configs[1]: polychromatic energy-dispersive instrument, 8 overlapping primitives, 8 materials."""
     rng = np.random.default_rng(WORKLOAD_SEED0 + 1)
     npx, nE = (64, 32) if small else (256, 128)
@@ -390,7 +401,9 @@ def config1(n_rays=100_000_000, small=False):
         solids(sl),
         detector(-width / 2, width / 2, -width / 2, width / 2, npx, npx, 10.0, 150.0, nE, T=(0, 0, 1.0)),
     ]
-    return instrument("c1_polychromatic", comps, mats, n_rays)
+    if scatter_order:
+        mats = _scattering(WORKLOAD_SEED0 + 101, mats, comps, scatter_order)
+    return instrument("c1_polychromatic" + ("_scatter" if scatter_order else ""), comps, mats, n_rays)
 
 
 SI_D111 = 3.135601154      # Angstrom
@@ -433,7 +446,7 @@ def config2(n_rays=500_000_000, small=False):
     return instrument("c2_beamline", comps, [None], n_rays)
 
 
-def config3(n_rays=100_000_000, small=False):
+def config3(n_rays=100_000_000, small=False, scatter_order=0):
     """configs[3]: two nested closed triangle meshes (bumpy icospheres), polychromatic 20-100 keV."""
     rng = np.random.default_rng(WORKLOAD_SEED0 + 3)
     lv_out, lv_in = (3, 2) if small else (6, 5)
@@ -450,10 +463,12 @@ def config3(n_rays=100_000_000, small=False):
                 solid_mesh(Vi, Fi, material=2, priority=1, T=(0, 0, 0.5))]),
         detector(-width / 2, width / 2, -width / 2, width / 2, npx, npx, 20.0, 100.0, nE, T=(0, 0, 1.0)),
     ]
-    return instrument("c3_mesh", comps, mats, n_rays)
+    if scatter_order:
+        mats = _scattering(WORKLOAD_SEED0 + 103, mats, comps, scatter_order)
+    return instrument("c3_mesh" + ("_scatter" if scatter_order else ""), comps, mats, n_rays)
 
 
-def config4(n_rays=1_000_000_000, small=False, n_vox=None):
+def config4(n_rays=1_000_000_000, small=False, n_vox=None, scatter_order=0):
     """configs[4]: energy-dispersive CT projection through a uint8 voxel phantom (paper problem 3)."""
     rng = np.random.default_rng(WORKLOAD_SEED0 + 4)
     if n_vox is None:
@@ -470,7 +485,9 @@ def config4(n_rays=1_000_000_000, small=False, n_vox=None):
         voxels(ids, h, T=(-0.256, -0.256, 2.0 - 0.256)),
         detector(-width / 2, width / 2, -width / 2, width / 2, npx, npx, 20.0, 150.0, nE, T=(0, 0, 2.5)),
     ]
-    return instrument("c4_edxct", comps, mats, n_rays)
+    if scatter_order:
+        mats = _scattering(WORKLOAD_SEED0 + 104, mats, comps, scatter_order)
+    return instrument("c4_edxct" + ("_scatter" if scatter_order else ""), comps, mats, n_rays)
 
 
 def delta_table(rng, n=200, Emin=15.0, Emax=35.0, A=3.41e-4):
@@ -533,7 +550,7 @@ def edxct_line_detectors(n_pix, nE, Emin=20.0, Emax=160.0, pix=EDXCT_PIX, dist=E
     return out
 
 
-def config7(n_rays=10_000_000, small=False, water=True):
+def config7(n_rays=10_000_000, small=False, water=True, scatter_order=0):
     """The paper's EDXCT in-line instrument (problem 3, Table 2, Fig. 3): polychromatic fan beam, a
     voxel sample (a solid block of water, 1 mm voxels, 550 (scan) x 400 (up) x 300 (beam) mm; small: 10 mm voxels with the
     seeded ellipsoid phantom painted in), five tilted 1 x 128 line detectors of 0.8 mm pixels and 128 energy bins over
@@ -563,8 +580,22 @@ def config7(n_rays=10_000_000, small=False, water=True):
              voxels(ids, h, T=corner)] + dets
     n_lines = nx if not small else 11
     scan = [(corner[0] + (line - (n_lines - 1) / 2) * (h if not small else 5 * h), corner[1], corner[2]) for line in range(n_lines)]
-    return instrument("c7_edxct_lines", comps, mats, n_rays, scan=scan, sample_component=1)
+    if scatter_order:
+        mats = _scattering(WORKLOAD_SEED0 + 107, mats, comps, scatter_order)
+    return instrument("c7_edxct_lines" + ("_scatter" if scatter_order else ""), comps, mats, n_rays, scan=scan, sample_component=1)
+
+
+def config8(n_rays=10_000_000, small=False):
+    """The EDXCT line scanner with the sample physics the paper describes (absorption AND scattering):
+    config7 whose water scatters, up to 8 events per ray."""
+    return config7(n_rays=n_rays, small=small, scatter_order=8)
+
+
+def config9(n_rays=100_000_000, small=False):
+    """configs[4]'s phantom and detector with scattering materials, up to 4 events per ray: the case where a ray's pixel is
+    no longer known at birth."""
+    return config4(n_rays=n_rays, small=small, scatter_order=4)
 
 
 def config(k, **kw):
-    return (config0, config1, config2, config3, config4, config5, config6, config7)[k](**kw)
+    return (config0, config1, config2, config3, config4, config5, config6, config7, config8, config9)[k](**kw)
