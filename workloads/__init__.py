@@ -591,7 +591,7 @@ def config8(n_rays=10_000_000, small=False):
     return config7(n_rays=n_rays, small=small, scatter_order=8)
 
 
-def config9(n_rays=100_000_000, small=False):
+def config9(n_rays=10_000_000, small=False):
     """configs[4]'s phantom and detector with scattering materials, up to 4 events per ray: the case where a ray's pixel is
     no longer known at birth."""
     return config4(n_rays=n_rays, small=small, scatter_order=4)
