@@ -1505,40 +1505,10 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
   unsigned int* s_cnt = reinterpret_cast<unsigned int*>(smem_raw);  // [MCX_MAX_COMPONENTS + 4]
   unsigned int* s_sched = s_cnt + MCX_MAX_COMPONENTS + 4;  // [0..1] tile tickets, [2..3] slice counters (ping-pong)
   const int n_comps = A.n_comps, n_mats = A.n_mats;
-  // the instrument, compact (SInst): components, materials, tally pointers
-  DComponent* s_comps = reinterpret_cast<DComponent*>(smem_raw + 128 + (GATE ? kRingBytes : 0));
-  DMaterial* s_mats = reinterpret_cast<DMaterial*>(s_comps + n_comps);
-  TallyBin** s_tallies = reinterpret_cast<TallyBin**>(s_mats + n_mats);
-  unsigned char* s_extra = reinterpret_cast<unsigned char*>(s_tallies + MCX_MAX_DETECTORS);
-  {
-    static_assert(sizeof(DComponent) % 8 == 0 && sizeof(DMaterial) % 8 == 0, "copied as 8-byte words");
-    const unsigned long long* src = reinterpret_cast<const unsigned long long*>(g_inst->comps);
-    unsigned long long* dst = reinterpret_cast<unsigned long long*>(s_comps);
-    for (int k = threadIdx.x; k < n_comps * (int)(sizeof(DComponent) / 8); k += kBlock) dst[k] = src[k];
-    src = reinterpret_cast<const unsigned long long*>(g_inst->mats);
-    dst = reinterpret_cast<unsigned long long*>(s_mats);
-    for (int k = threadIdx.x; k < n_mats * (int)(sizeof(DMaterial) / 8); k += kBlock) dst[k] = src[k];
-    if (threadIdx.x < MCX_MAX_DETECTORS) s_tallies[threadIdx.x] = g_inst->tallies[threadIdx.x];
-    if (threadIdx.x < MCX_MAX_COMPONENTS + 4) s_cnt[threadIdx.x] = 0u;
-  }
-  const SInst I{n_comps, n_mats, s_comps, s_mats, s_tallies, g_inst->counters};
-  __syncthreads();
-  if (FEAT & F_SOLIDS) {  // stage the solids (poses, sizes, priorities) of every group and re-point the groups at the copy
-    DSolid* s_solids = reinterpret_cast<DSolid*>(s_extra);
-    s_extra += A.n_solids * sizeof(DSolid);
-    int used = 0;
-    for (int c = 1; c < n_comps; ++c) {
-      if (s_comps[c].kind != MCX_SOLIDS) continue;
-      const int ns = s_comps[c].u.solids.n_solids;
-      const unsigned long long* src = reinterpret_cast<const unsigned long long*>(s_comps[c].u.solids.solids);
-      unsigned long long* dst = reinterpret_cast<unsigned long long*>(s_solids + used);
-      for (int k = threadIdx.x; k < ns * (int)(sizeof(DSolid) / 8); k += kBlock) dst[k] = src[k];
-      __syncthreads();
-      if (threadIdx.x == 0) s_comps[c].u.solids.solids = s_solids + used;
-      used += ns;
-    }
-    __syncthreads();
-  }
+  // Layout: counters (128 bytes), gate rings, then the per-thread scratch at offsets that do not depend on the instrument
+  // (interval end points, triangle queue | voxel path lengths | tally cache), then the instrument itself, compact (SInst:
+  // components, materials, tally pointers, solids).
+  unsigned char* s_extra = smem_raw + 128 + (GATE ? kRingBytes : 0);
   Endpoints ep{nullptr, nullptr, 0};
   unsigned* tri_queue = nullptr;
   if (FEAT & F_SOLIDS) {  // per-thread interval end points (and, with meshes, the candidate-triangle queue)
@@ -1553,13 +1523,46 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
     }
   }
   double* len_s = reinterpret_cast<double*>(s_extra) + threadIdx.x;  // per-thread path length per material (voxel walk)
+  if (FEAT & F_VOXELS) s_extra += (size_t)(n_mats + VC_COUNT + ((FEAT & F_SCATTER) ? n_mats : 0)) * kBlock * sizeof(double);
   TallyCache tcache{nullptr, 0, A.tally_cache_dets};
   const int tally_mode = A.tally_mode;
   if (!DUMP && !(FEAT & (F_SOLIDS | F_VOXELS)) && A.tally_cache_log2 > 0) {  // block-private tally cache (chains without solids or voxels)
     tcache.key = reinterpret_cast<unsigned long long*>(s_extra);
     tcache.log2 = A.tally_cache_log2;
+    s_extra += (size_t)32 << tcache.log2;
     for (int k = threadIdx.x; k < (4 << tcache.log2); k += kBlock) tcache.key[k] = 0ull;
     // (the barrier after the first ticket fetch below orders these stores before any update)
+  }
+  DComponent* s_comps = reinterpret_cast<DComponent*>(s_extra);
+  DMaterial* s_mats = reinterpret_cast<DMaterial*>(s_comps + n_comps);
+  TallyBin** s_tallies = reinterpret_cast<TallyBin**>(s_mats + n_mats);
+  {
+    static_assert(sizeof(DComponent) % 8 == 0 && sizeof(DMaterial) % 8 == 0, "copied as 8-byte words");
+    const unsigned long long* src = reinterpret_cast<const unsigned long long*>(g_inst->comps);
+    unsigned long long* dst = reinterpret_cast<unsigned long long*>(s_comps);
+    for (int k = threadIdx.x; k < n_comps * (int)(sizeof(DComponent) / 8); k += kBlock) dst[k] = src[k];
+    src = reinterpret_cast<const unsigned long long*>(g_inst->mats);
+    dst = reinterpret_cast<unsigned long long*>(s_mats);
+    for (int k = threadIdx.x; k < n_mats * (int)(sizeof(DMaterial) / 8); k += kBlock) dst[k] = src[k];
+    if (threadIdx.x < MCX_MAX_DETECTORS) s_tallies[threadIdx.x] = g_inst->tallies[threadIdx.x];
+    if (threadIdx.x < MCX_MAX_COMPONENTS + 4) s_cnt[threadIdx.x] = 0u;
+  }
+  const SInst I{n_comps, n_mats, s_comps, s_mats, s_tallies, g_inst->counters};
+  __syncthreads();
+  if (FEAT & F_SOLIDS) {  // stage the solids (poses, sizes, priorities) of every group and re-point the groups at the copy
+    DSolid* s_solids = reinterpret_cast<DSolid*>(s_tallies + MCX_MAX_DETECTORS);
+    int used = 0;
+    for (int c = 1; c < n_comps; ++c) {
+      if (s_comps[c].kind != MCX_SOLIDS) continue;
+      const int ns = s_comps[c].u.solids.n_solids;
+      const unsigned long long* src = reinterpret_cast<const unsigned long long*>(s_comps[c].u.solids.solids);
+      unsigned long long* dst = reinterpret_cast<unsigned long long*>(s_solids + used);
+      for (int k = threadIdx.x; k < ns * (int)(sizeof(DSolid) / 8); k += kBlock) dst[k] = src[k];
+      __syncthreads();
+      if (threadIdx.x == 0) s_comps[c].u.solids.solids = s_solids + used;
+      used += ns;
+    }
+    __syncthreads();
   }
   const int lane = threadIdx.x & 31;
   const uint64_t first = A.first, n = A.n, seed = A.seed;
