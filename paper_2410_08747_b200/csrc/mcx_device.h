@@ -14,6 +14,7 @@ namespace mcx {
 struct DPose {
   double R[9];
   double T[3];
+  int identity, pad;  // R is exactly the identity matrix
 };
 
 // mu(E) of one material as ln-tables (step 7); slope[j] = (lnMu[j+1]-lnMu[j]) / (lnE[j+1]-lnE[j]).

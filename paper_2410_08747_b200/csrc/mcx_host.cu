@@ -90,6 +90,10 @@ bool pose_ok(const mcx_pose& P) {
 void copy_pose(DPose* d, const mcx_pose& s) {
   std::memcpy(d->R, s.rot, sizeof(d->R));
   std::memcpy(d->T, s.origin, sizeof(d->T));
+  d->identity = 1;
+  for (int k = 0; k < 9; ++k)
+    if (s.rot[k] != ((k % 4 == 0) ? 1.0 : 0.0)) d->identity = 0;
+  d->pad = 0;
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -948,7 +952,7 @@ mcx_status mcx_instrument_set_pose(mcx_instrument* inst, int component, const mc
   copy_pose(&D.pose, *pose);
   // host_image outlives the copy: pageable memory is staged before cudaMemcpyAsync returns
   const size_t off = (size_t)((const unsigned char*)&D.pose - (const unsigned char*)&inst->host_image);
-  const cudaError_t e = cudaMemcpyAsync(inst->workspace + off, &D.pose, sizeof(DPose), cudaMemcpyHostToDevice, (cudaStream_t)cuda_stream);
+  const cudaError_t e = cudaMemcpyAsync(inst->workspace + off, &D.pose, sizeof(DPose), cudaMemcpyHostToDevice, (cudaStream_t)cuda_stream);  // (rotation, origin and the identity flag)
   if (e != cudaSuccess) return cuda_fail(e, "pose upload");
   return MCX_OK;
 }

@@ -78,14 +78,20 @@ __device__ __forceinline__ Vec3 operator*(double s, Vec3 a) { return {s * a.x, s
 __device__ __forceinline__ double dot(Vec3 a, Vec3 b) { return a.x * b.x + a.y * b.y + a.z * b.z; }
 
 // Step 4: into a component frame and back
-__device__ __forceinline__ Vec3 rotate(const double* R, Vec3 v) {
+// (a pose whose rotation is the identity -- most components of an in-line instrument -- skips the nine products: x * 1 +
+// y * 0 + z * 0 is x exactly)
+__device__ __forceinline__ Vec3 rotate(const DPose& P, Vec3 v) {
+  if (P.identity) return v;
+  const double* R = P.R;
   return {R[0] * v.x + R[1] * v.y + R[2] * v.z, R[3] * v.x + R[4] * v.y + R[5] * v.z, R[6] * v.x + R[7] * v.y + R[8] * v.z};
 }
-__device__ __forceinline__ Vec3 rotate_back(const double* R, Vec3 v) {
+__device__ __forceinline__ Vec3 rotate_back(const DPose& P, Vec3 v) {
+  if (P.identity) return v;
+  const double* R = P.R;
   return {R[0] * v.x + R[3] * v.y + R[6] * v.z, R[1] * v.x + R[4] * v.y + R[7] * v.z, R[2] * v.x + R[5] * v.y + R[8] * v.z};
 }
-__device__ __forceinline__ Vec3 to_local(const DPose& P, Vec3 r) { return rotate(P.R, r - Vec3{P.T[0], P.T[1], P.T[2]}); }
-__device__ __forceinline__ Vec3 to_lab(const DPose& P, Vec3 r) { return rotate_back(P.R, r) + Vec3{P.T[0], P.T[1], P.T[2]}; }
+__device__ __forceinline__ Vec3 to_local(const DPose& P, Vec3 r) { return rotate(P, r - Vec3{P.T[0], P.T[1], P.T[2]}); }
+__device__ __forceinline__ Vec3 to_lab(const DPose& P, Vec3 r) { return rotate_back(P, r) + Vec3{P.T[0], P.T[1], P.T[2]}; }
 
 struct Ray {
   Vec3 r, d;
@@ -144,7 +150,7 @@ __device__ __forceinline__ void sample_source(const DComponent& C, uint64_t seed
     E = S.spec_emin + ((double)lo + (v01 - c0) / (c1 - c0)) * S.spec_bin_w;
   }
   ray.r = to_lab(C.pose, r);
-  ray.d = rotate_back(C.pose.R, d);
+  ray.d = rotate_back(C.pose, d);
   ray.E = E;
   ray.p = 1.0;
 }
@@ -152,7 +158,7 @@ __device__ __forceinline__ void sample_source(const DComponent& C, uint64_t seed
 // Step 5: intersection with the plane z' = 0 of a component frame
 __device__ __forceinline__ bool plane_hit(const DPose& P, const Ray& ray, Vec3& hit) {
   const Vec3 o = to_local(P, ray.r);
-  const Vec3 d = rotate(P.R, ray.d);
+  const Vec3 d = rotate(P, ray.d);
   if (!(d.z > 0.0)) return false;
   const double t = -o.z / d.z;
   if (t < 0.0) return false;
@@ -613,7 +619,7 @@ __device__ __forceinline__ int trace_solids(const SInst& I, const DComponent& C,
       int rc;
       for (bool coh = coherent;; coh = false) {  // (a second round only if the beam walk gives up: rc 2, warp-uniform)
         Vec3 o{0.0, 0.0, 0.0}, d{0.0, 0.0, 1.0};
-        if (act) { o = to_local(S.pose, ray.r); d = rotate(S.pose.R, ray.d); }
+        if (act) { o = to_local(S.pose, ray.r); d = rotate(S.pose, ray.d); }
         rc = mesh_endpoints_warp(S, (unsigned)s, act, o, d, E, ne, queue, coh);
         if (rc != 2) break;
       }
@@ -629,7 +635,7 @@ __device__ __forceinline__ int trace_solids(const SInst& I, const DComponent& C,
       if (oc2 - along * along > S.bound2 + 1e-14 * oc2) continue;
     }
     const Vec3 o = to_local(S.pose, ray.r);
-    const Vec3 d = rotate(S.pose.R, ray.d);
+    const Vec3 d = rotate(S.pose, ray.d);
     double a, b;
     if (primitive_interval(S, o, d, a, b)) {  // clip to t >= 0, drop if empty
       a = fmax(a, 0.0);
@@ -738,7 +744,7 @@ __device__ __forceinline__ int trace_solids_legs(const SInst& I, const DComponen
         int rc;
         for (bool coh = coherent && leg == 0;; coh = false) {  // (a second round only if the beam walk gives up: rc 2, warp-uniform)
           Vec3 o{0.0, 0.0, 0.0}, d{0.0, 0.0, 1.0};
-          if (act) { o = to_local(Sd.pose, ray.r); d = rotate(Sd.pose.R, ray.d); }
+          if (act) { o = to_local(Sd.pose, ray.r); d = rotate(Sd.pose, ray.d); }
           rc = mesh_endpoints_warp(Sd, (unsigned)s, act, o, d, E, ne, queue, coh);
           if (rc != 2) break;
         }
@@ -754,7 +760,7 @@ __device__ __forceinline__ int trace_solids_legs(const SInst& I, const DComponen
         if (oc2 - along * along > Sd.bound2 + 1e-14 * oc2) continue;
       }
       const Vec3 o = to_local(Sd.pose, ray.r);
-      const Vec3 d = rotate(Sd.pose.R, ray.d);
+      const Vec3 d = rotate(Sd.pose, ray.d);
       double a, b;
       if (primitive_interval(Sd, o, d, a, b)) {  // clip to t >= 0, drop if empty
         a = fmax(a, 0.0);
@@ -1095,7 +1101,7 @@ template <bool SCAT>
 __device__ __forceinline__ void trace_voxels(const SInst& I, const DComponent& C, int comp, Ray& ray, uint64_t seed, uint64_t i,
                                              double* len_s, double* cold_s, double* mus_s) {
   const DVoxels& V = C.u.voxels;
-  Vec3 ol = to_local(C.pose, ray.r), dl = rotate(C.pose.R, ray.d);
+  Vec3 ol = to_local(C.pose, ray.r), dl = rotate(C.pose, ray.d);
   unsigned touched = 0u;
   Scat S;
   S.k = 0; S.K = SCAT ? V.scatter_order : 0; S.s_pre = 0.0; S.cum = 0.0; S.tau_s = 0.0; S.t_event = 0.0; S.have_ms = 0u; S.event = false;
@@ -1131,7 +1137,7 @@ __device__ __forceinline__ void trace_voxels(const SInst& I, const DComponent& C
   ray.p *= exp(-tau);
   if (SCAT && S.k > 0) {
     ray.r = to_lab(C.pose, ol);
-    ray.d = rotate_back(C.pose.R, dl);
+    ray.d = rotate_back(C.pose, dl);
   }
 }
 
@@ -1156,7 +1162,7 @@ __device__ __forceinline__ double reflectivity(const DMirror& M, double theta, d
 __device__ __forceinline__ bool trace_mirror(const DComponent& C, Ray& ray) {
   const DMirror& M = C.u.mirror;
   const Vec3 o = to_local(C.pose, ray.r);
-  const Vec3 d = rotate(C.pose.R, ray.d);
+  const Vec3 d = rotate(C.pose, ray.d);
   // into the ellipse's principal frame (Z, Y)
   const double oZ = M.Z0 + o.z * M.tZ + o.y * M.nZ, oY = M.Y0 + o.z * M.tY + o.y * M.nY;
   const double dZ = d.z * M.tZ + d.y * M.nZ, dY = d.z * M.tY + d.y * M.nY;
@@ -1188,7 +1194,7 @@ __device__ __forceinline__ bool trace_mirror(const DComponent& C, Ray& ray) {
     ray.p *= reflectivity(M, theta, ray.E);
     const Vec3 dr = d - (2.0 * dn) * nrm;
     ray.r = to_lab(C.pose, hp);
-    ray.d = rotate_back(C.pose.R, dr);
+    ray.d = rotate_back(C.pose, dr);
     return true;
   }
   return false;
@@ -1227,7 +1233,7 @@ __device__ __forceinline__ double darwin_prins(double eta, double g, double kapp
 __device__ __forceinline__ bool trace_lens(const SInst& I, const DComponent& C, Ray& ray) {
   const DLens& L = C.u.lens;
   Vec3 o = to_local(C.pose, ray.r);
-  Vec3 d = rotate(C.pose.R, ray.d);
+  Vec3 d = rotate(C.pose, ray.d);
   const double lnE = log(ray.E);
   const double delta = mu_of(L.delta, ray.E, lnE);
   const double n_in = 1.0 - delta;
@@ -1269,7 +1275,7 @@ __device__ __forceinline__ bool trace_lens(const SInst& I, const DComponent& C, 
   }
   ray.p *= exp(-mu_of(I.mats[L.material], ray.E, lnE) * path);
   ray.r = to_lab(C.pose, o);
-  ray.d = rotate_back(C.pose.R, d);
+  ray.d = rotate_back(C.pose, d);
   return true;
 }
 
@@ -1277,7 +1283,7 @@ __device__ __forceinline__ bool trace_lens(const SInst& I, const DComponent& C, 
 __device__ __forceinline__ bool trace_crystal(const DComponent& C, Ray& ray) {
   const DCrystal& X = C.u.crystal;
   const Vec3 o = to_local(C.pose, ray.r);
-  const Vec3 d = rotate(C.pose.R, ray.d);
+  const Vec3 d = rotate(C.pose, ray.d);
   if (!(d.y < 0.0)) return false;
   const double t = -o.y / d.y;
   if (!(t > 0.0)) return false;
@@ -1300,7 +1306,7 @@ __device__ __forceinline__ bool trace_crystal(const DComponent& C, Ray& ray) {
     }
   }
   ray.r = to_lab(C.pose, Vec3{hp.x, 0.0, hp.z});
-  ray.d = rotate_back(C.pose.R, Vec3{d.x, -d.y, d.z});
+  ray.d = rotate_back(C.pose, Vec3{d.x, -d.y, d.z});
   return true;
 }
 
