@@ -359,6 +359,19 @@ def bench_instrument(M, torch, inst, n_rays, first, steps, warmup, device, probe
     if tuning["tally_mode"] == "block":
         cand["tally"]["bypassed"] = ("block-private shared-memory tallies (mcx_tally_mode MCX_TALLY_BLOCK): the records in "
                                      "L2 see one flush per block, so this roof does not bind; frac > 1 is the gain over it")
+    vox = [c for c in inst["components"] if c["kind"] == "voxels" and c.get("scatter_order", 0) > 0]
+    if vox:
+        # after its first scattering event a ray walks voxel by voxel in a direction of its own: one 32-byte sector of
+        # the volume per voxel visited, at random as far as the memory system is concerned
+        sectors = float(n_rays) * work["voxel_steps"]
+        footprint = 2 * sum(int(np.prod(c["ids"].shape)) for c in vox)          # cells of {ID, run}
+        table = 1 << int(np.ceil(np.log2(footprint)))
+        l2_peak = probes["l2"](table)
+        cand["l2"] = {"achieved": sectors / sec * 32 / 1e9, "peak": l2_peak * 32 / 1e9, "unit": "GB/s of 32-byte sectors",
+                      "frac": sectors / sec / l2_peak, "per_ray": 32 * sectors / n_rays,
+                      "peak_source": f"mcx_probe_l2, random sectors of a {table >> 20} MiB table (voxel cells = "
+                                     f"{footprint / 2**20:.0f} MiB), measured in this run",
+                      "note": "one sector per voxel visited on the legs of scattered rays"}
     bound = max((k for k in cand if "bypassed" not in cand[k]), key=lambda k: cand[k]["frac"])
     res["work_per_ray"] = work
     res["tuning"] = tuning
