@@ -928,16 +928,31 @@ __device__ __forceinline__ void lateral_init(const VoxAxis& A, double inv_dw, do
   a = adv >= 1.0 ? 0xFFFFFFFFFFFFFFFFull : frac64(adv);
 }
 
-// One leg of the walk: the half-line ol + t dl, t >= 0, in the volume's frame, from where it enters the grid to where it
-// leaves it or (SCAT, step 17) to the scattering event.  Path lengths go to len_s / touched, which accumulate over legs.
+// The walk of one ray through the volume, leg by leg: a leg is the half-line ol + t dl, t >= 0, in the volume's frame,
+// from where it enters the grid to where it leaves it or (SCAT, step 17) to the scattering event.  setup() starts a leg,
+// step() does one slab and a skip and says when the leg is over.  Path lengths go to len_s / touched, which accumulate
+// over the legs.  (Everything is inlined; the members live in registers.)
+#define MCX_VOXEL_AT(lo32) ld_voxel(hi | (lo32))
 template <bool SCAT>
-__device__ __forceinline__ void voxel_leg(const SInst& I, const DVoxels& V, Vec3 ol, Vec3 dl, double E, double lnE, double* len_s,
-                                          double* cold_s, double* mus_s, unsigned& touched, Scat& S) {
-  const double h = V.h;
-  unsigned ful, fuh, fvl, fvh, aul, auh, avl, avh, cu0, cv0, so_u, so_v, so_w, meta, lo_start, inv_u, inv_v;
+struct VoxWalk {
+  const SInst& I;
+  const DVoxels& V;
+  double E, lnE;
+  double* len_s;
+  double* cold_s;
+  double* mus_s;
+  unsigned& touched;
+  Scat& S;
+  unsigned ful, fuh, fvl, fvh, aul, auh, avl, avh, so_u, so_v, so_w, meta, inv_u, inv_v;
+  unsigned cur, w_crossed, cu, cv, lo;
+  unsigned long long base, hi;
   double t_run;
-  S.event = false;
-  {
+
+  // false: the half-line misses the grid
+  __device__ __forceinline__ bool setup(Vec3 ol, Vec3 dl) {
+    const double h = V.h;
+    unsigned cu0, cv0, lo_start;
+    S.event = false;
     const Vec3 inv_d{1.0 / dl.x, 1.0 / dl.y, 1.0 / dl.z};  // the only divisions of the set-up (+-inf where d = 0: unused)
     double t0 = -CUDART_INF, t1 = CUDART_INF;
     auto clip = [&](double o, double d, double inv, double top) {  // slab [0, top] of one axis, as clip_axis
@@ -947,11 +962,11 @@ __device__ __forceinline__ void voxel_leg(const SInst& I, const DVoxels& V, Vec3
       t1 = fmin(t1, fmax(ta, tb));
       return true;
     };
-    if (!clip(ol.x, dl.x, inv_d.x, (double)V.n[0] * h)) return;
-    if (!clip(ol.y, dl.y, inv_d.y, (double)V.n[1] * h)) return;
-    if (!clip(ol.z, dl.z, inv_d.z, (double)V.n[2] * h)) return;
+    if (!clip(ol.x, dl.x, inv_d.x, (double)V.n[0] * h)) return false;
+    if (!clip(ol.y, dl.y, inv_d.y, (double)V.n[1] * h)) return false;
+    if (!clip(ol.z, dl.z, inv_d.z, (double)V.n[2] * h)) return false;
     if (t0 < 0.0) t0 = 0.0;
-    if (!(t0 < t1)) return;
+    if (!(t0 < t1)) return false;
     // the ray's dominant axis w and the two lateral axes u < v
     int gw = 0;
     {
@@ -984,21 +999,23 @@ __device__ __forceinline__ void voxel_leg(const SInst& I, const DVoxels& V, Vec3
     }
     lo_start = (unsigned)(W.idx + 1) * W.stride + (unsigned)(U.idx + 1) * U.stride + (unsigned)(X.idx + 1) * X.stride;
     t_run = t0;
+    // The volume does not straddle a 4 GiB address boundary (mcx_instrument_create places it so): the walk keeps the
+    // low address word only and a step is one 32-bit add.
+    base = (unsigned long long)V.ids;
+    hi = base & 0xFFFFFFFF00000000ull;
+    lo_start += (unsigned)base;
+    cur = MCX_VOXEL_AT(lo_start);
+    w_crossed = 0u;
+    cu = cu0; cv = cv0; lo = lo_start;
+    return true;
   }
-  // The volume does not straddle a 4 GiB address boundary (mcx_instrument_create places it so): the walk keeps the
-  // low address word only and a step is one 32-bit add.
-  const unsigned long long base = (unsigned long long)V.ids;
-  const unsigned long long hi = base & 0xFFFFFFFF00000000ull;
-  lo_start += (unsigned)base;
-#define MCX_VOXEL_AT(lo32) ld_voxel(hi | (lo32))
-  unsigned cur = MCX_VOXEL_AT(lo_start);
   // (touched: bit m = len_s[m] holds this ray's path length in material m)
   // The run of `cur` ends where the ray enters the voxel at address `at` through a face of axis k: the index of that
   // voxel along the axis comes back out of the address (a guard cell gives -1 or n, i.e. the outer face of the grid),
   // and the face parameter is (face - o) / d as in step 11 (as a product with 1/d, one more rounding).
   // (For w faces, most of them, the index is simply counted: w_crossed faces lie behind the current slab.)
-  unsigned w_crossed = 0u;
-  auto close_run = [&](unsigned at, unsigned k, unsigned id) {
+  __device__ __forceinline__ bool close_run(unsigned at, unsigned k, unsigned id) {
+    const double h = V.h;
     int face;
     if (k == 0u) {
       const double wf = cold_s[VC_WFACE * kBlock];
@@ -1035,7 +1052,7 @@ __device__ __forceinline__ void voxel_leg(const SInst& I, const DVoxels& V, Vec3
     t_run = tn;
     cur = id;
     return ev;
-  };
+  }
   // One iteration = one slab, then a skip.
   //  Slab: the lateral step (if any; the same cell again if cu = cv = 0) and the w face that ends the slab: cell b at
   //  lo_b, then cell c at lo_c.  If both lateral faces are crossed in one slab (rare) lo_b is the diagonal neighbour
@@ -1045,7 +1062,7 @@ __device__ __forceinline__ void voxel_leg(const SInst& I, const DVoxels& V, Vec3
   //  s additions of a leave the fraction below 1: s <= (2^64 - 1 - f) / a, taken conservatively from the high words
   //  as mulhi(~f_hi, inv) with inv <= 2^32 / (a_hi + 1).  Then f += s a exactly and the address moves s cells on.
   //  inv = 0 (no skipping) unless the ray runs along the fast axis in the direction the runs were counted in.
-  auto settle_slab = [&](unsigned cuA, unsigned cvA, unsigned lo_bA, unsigned lo_cA, unsigned idbA, unsigned idcA) {
+  __device__ __forceinline__ bool settle_slab(unsigned cuA, unsigned cvA, unsigned lo_bA, unsigned lo_cA, unsigned idbA, unsigned idcA) {
     unsigned k_lat = cuA ? 1u : 2u, k_first = 0u, lo_a = 0u, ida = cur;
     if (cuA & cvA) {
       // The face crossed first is the one with more of the slab left after it: f / a, f the fraction after this
@@ -1071,15 +1088,15 @@ __device__ __forceinline__ void voxel_leg(const SInst& I, const DVoxels& V, Vec3
       if (idcA == kVoxelGuard) return true;
     }
     return false;
-  };
-  unsigned cu = cu0, cv = cv0, lo = lo_start;
-  for (;;) {
+  }
+  // one slab and a skip; true = the leg is over (the ray left the grid, or S.event)
+  __device__ __forceinline__ bool step() {
     const unsigned lo_b = lo + cu * so_u + cv * so_v, lo_c = lo_b + so_w;
     const unsigned idb = MCX_VOXEL_AT(lo_b);
     const unsigned cell_c = ld_cell(hi | lo_c);
     const unsigned idc = cell_c & 0xffu;
     if (idb != cur || idc != cur || (cu & cv) != 0u) {
-      if (settle_slab(cu, cv, lo_b, lo_c, idb, idc)) break;
+      if (settle_slab(cu, cv, lo_b, lo_c, idb, idc)) return true;
     }
     const unsigned s = min(min(cell_c >> 8, __umulhi(~fuh, inv_u)), __umulhi(~fvh, inv_v));
     lo = lo_c + s * so_w;
@@ -1091,40 +1108,74 @@ __device__ __forceinline__ void voxel_leg(const SInst& I, const DVoxels& V, Vec3
     }
     cu = add_carry(ful, fuh, aul, auh);
     cv = add_carry(fvl, fvh, avl, avh);
+    return false;
   }
+};
 #undef MCX_VOXEL_AT
-}
+
 
 // Step 11 (and 17 where the volume scatters): the legs of one ray, then tau = sum over the touched materials of
 // mu_m(E) * len_m (step 7 evaluated for those only) - what the scattering took of it while events were left.
 template <bool SCAT>
 __device__ __forceinline__ void trace_voxels(const SInst& I, const DComponent& C, int comp, Ray& ray, uint64_t seed, uint64_t i,
-                                             double* len_s, double* cold_s, double* mus_s) {
+                                             double* len_s, double* cold_s, double* mus_s, unsigned lanes) {
   const DVoxels& V = C.u.voxels;
   Vec3 ol = to_local(C.pose, ray.r), dl = rotate(C.pose, ray.d);
   unsigned touched = 0u;
   Scat S;
   S.k = 0; S.K = SCAT ? V.scatter_order : 0; S.s_pre = 0.0; S.cum = 0.0; S.tau_s = 0.0; S.t_event = 0.0; S.have_ms = 0u; S.event = false;
   const double lnE_early = SCAT ? log(ray.E) : 0.0;  // (without scattering ln E is not needed, nor kept in a register, during the walk)
-  for (;;) {
+  VoxWalk<SCAT> walk{I, V, ray.E, lnE_early, len_s, cold_s, mus_s, touched, S};
+  if (!SCAT) {
+    if (walk.setup(ol, dl))
+      while (!walk.step()) {}
+  } else {
+    // The lanes of the warp that are in this volume (`lanes`) stay in ONE loop, whose iteration is warp-uniformly either
+    // one slab for the lanes that are walking, or -- when nobody walks any more, or kBatch lanes are waiting -- the end of
+    // a leg (the scattering event) and the set-up of the next one for all the lanes whose leg is over.  So the long
+    // set-up and event code runs with many lanes at a time, and a lane whose leg ends early waits for company instead of
+    // stalling 31 walkers.  (Left to themselves, lanes that re-enter a walk loop after an event never rejoin those
+    // still in it: a first version with a loop per leg and no barrier ran with 1.4 of 32 lanes active.)
+    enum { kPending, kWalking, kDone };
+    constexpr int kBatch = 8;
+    int state = kPending;
+    bool first_leg = true;
     double u_mu = 0.0;
-    if (SCAT && S.k < S.K) {
-      double u_f;
-      draw2(seed, i, (uint32_t)(2 * S.k), (uint32_t)comp, u_f, u_mu);
-      S.tau_s = -log(u_f);
-      S.cum = 0.0;
+    for (;;) {
+      const unsigned pending = __ballot_sync(lanes, state == kPending), walking = __ballot_sync(lanes, state == kWalking);
+      if ((pending | walking) == 0u) break;
+      if (walking == 0u || __popc(pending) >= kBatch) {
+        if (state == kPending) {
+          bool go_on = true;
+          if (!first_leg) {  // how the last leg ended
+            if (!S.event) {
+              if (S.k < S.K) S.s_pre += S.cum;
+              state = kDone;
+              go_on = false;
+            } else {
+              S.s_pre += S.tau_s;
+              double u_phi, unused;
+              draw2(seed, i, (uint32_t)(2 * S.k + 1), (uint32_t)comp, u_phi, unused);
+              ol = ol + S.t_event * dl;
+              dl = scatter_direction(dl, u_mu, u_phi);
+              ++S.k;
+            }
+          }
+          if (go_on) {
+            first_leg = false;
+            if (S.k < S.K) {
+              double u_f;
+              draw2(seed, i, (uint32_t)(2 * S.k), (uint32_t)comp, u_f, u_mu);
+              S.tau_s = -log(u_f);
+              S.cum = 0.0;
+            }
+            if (walk.setup(ol, dl)) state = kWalking;  // (a half-line that misses the grid: leg over at once, no event)
+          }
+        }
+      } else if (state == kWalking) {
+        if (walk.step()) state = kPending;
+      }
     }
-    voxel_leg<SCAT>(I, V, ol, dl, ray.E, lnE_early, len_s, cold_s, mus_s, touched, S);
-    if (!SCAT || !S.event) {
-      if (SCAT && S.k < S.K) S.s_pre += S.cum;
-      break;
-    }
-    S.s_pre += S.tau_s;
-    double u_phi, unused;
-    draw2(seed, i, (uint32_t)(2 * S.k + 1), (uint32_t)comp, u_phi, unused);
-    ol = ol + S.t_event * dl;
-    dl = scatter_direction(dl, u_mu, u_phi);
-    ++S.k;
   }
   const double lnE = SCAT ? lnE_early : log(ray.E);
   double tau = 0.0;
@@ -1618,6 +1669,7 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
       const DComponent& C = I.comps[c];
       const int kind = C.kind;  // warp-uniform
       bool pass = true, tally_now = false;
+      const unsigned lanes_alive = (FEAT & F_SCATTER) ? __ballot_sync(0xffffffffu, alive) : 0u;  // (the legs of step 17 are walked by the warp)
       if ((FEAT & F_SOLIDS) && kind == MCX_SOLIDS) {  // whole warp: the mesh walk is warp-cooperative
         // (the walk without scattering is kept as its own function: the mesh kernel sits at the register limit)
         const int rc = (FEAT & F_SCATTER)
@@ -1638,7 +1690,7 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
           pass = plane_hit(C.pose, ray, h) && h.x * h.x + h.y * h.y <= C.u.slit.radius2;
         } else if ((FEAT & F_VOXELS) && kind == MCX_VOXELS) {
           trace_voxels<(FEAT & F_SCATTER) != 0>(I, C, c, ray, seed, first + qi, len_s, len_s + (size_t)I.n_mats * kBlock,
-                                                len_s + (size_t)(I.n_mats + VC_COUNT) * kBlock);
+                                                len_s + (size_t)(I.n_mats + VC_COUNT) * kBlock, lanes_alive);
         } else if ((FEAT & F_OPTICS) && kind == MCX_MIRROR_ELLIPTIC) {
           pass = trace_mirror(C, ray);
         } else if ((FEAT & F_OPTICS) && kind == MCX_CRYSTAL_BRAGG) {
