@@ -1553,9 +1553,10 @@ __device__ __forceinline__ void tally_flush(const SInst& I, const TallyCache& tc
 constexpr size_t kRingBytes = (kBlock / 32) * 64 * sizeof(unsigned);  // per-warp rings of gate survivors
 constexpr unsigned kTileMax = 8192;  // positions per work ticket (a power of two >= kBlock; smaller for short launches)
 
-// resident blocks per SM the register budget is held to: the voxel walk hides its byte loads with warps
+// resident blocks per SM the register budget is held to: the voxel walk and the primitives hide their loads with warps
+// (3 x 80 registers; with 2 blocks c4 loses 14 %, c1 18 %), the mesh kernels spill at 80 and run 12 % faster with 2 x 128
 constexpr int min_blocks(int feat) {
-  return feat == F_VOXELS || feat == (F_SOLIDS | F_PRIM) || feat == (F_SOLIDS | F_MESH) || feat == (F_SOLIDS | F_MESH | F_PRIM) ? 3
+  return (feat == F_VOXELS || feat == (F_SOLIDS | F_PRIM)) ? 3 : (feat == (F_SOLIDS | F_MESH | F_PRIM) || feat == (F_SOLIDS | F_MESH)) ? 2
          : (feat == F_OPTICS || feat == F_LENS || feat == (F_VOXELS | F_SCATTER)) ? 2 : 1;
 }
 
