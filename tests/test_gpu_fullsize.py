@@ -93,3 +93,20 @@ def test_c3_full_size(M, O, W):
 
 def test_c4_full_size(M, O, W):
     full_size(M, O, W, 4, window=20_000)
+
+
+def test_c5_basic_instrument_full_size(M, O, W):
+    full_size(M, O, W, 5)
+
+
+def test_c6_focusing_instrument_full_size(M, O, W):
+    full_size(M, O, W, 6)
+
+
+def test_c7_line_scanner_full_size(M, O, W):
+    full_size(M, O, W, 7, window=20_000)
+
+
+def test_c8_c9_scattering_full_size(M, O, W):
+    full_size(M, O, W, 8, window=4_000)
+    full_size(M, O, W, 9, window=8_000)
