@@ -78,7 +78,8 @@ struct DSolids {
 };
 
 // Voxel volume in traversal layout: 2 bytes per cell, {material ID, run}, where run = how many cells FOLLOWING this one
-// along the fast axis in the beam's direction (run_dir) hold the same ID (capped at 255).  Cells are addressed as
+// along the fast axis in the beam's direction (run_dir) hold the same ID (capped at 255).  In a scattering volume
+// (scatter_order > 0) the second byte is instead the radius of the cube of equal IDs around the cell (mcx_kernels.cu).  Cells are addressed as
 // ((i[a2]+1) * (n[a1]+2) + i[a1]+1) * pitch + i[fast]+1, with a one-cell guard border of ID kVoxelGuard all around.
 struct DVoxels {
   double h, inv_h;
@@ -195,6 +196,7 @@ cudaError_t launch_voxel_relayout(const uint8_t* src, uint8_t* dst, int nx, int 
 cudaError_t launch_cnr(const unsigned long long* N, const double* p, const double* p2, int nx, int ny, int ne, const int* region_mat,
                        const int* region_ref, double emin, double emax, double e_fit_min, double* cnr_out, double* fit_out,
                        cudaStream_t stream);
+cudaError_t launch_voxel_radius(uint8_t* cells, uint8_t* scratch, int d0, int d1, int d2, cudaStream_t stream);
 cudaError_t launch_probe_dfma(double* sink, int n_blocks, long long n_iters, cudaStream_t stream);
 cudaError_t launch_probe_tally(void* table, unsigned long long n_records, int n_blocks, long long n_iters, cudaStream_t stream);
 cudaError_t launch_probe_l2(const void* table, unsigned long long n_bytes, uint32_t* sink, int n_blocks, long long n_iters,

@@ -188,6 +188,7 @@ struct Plan {
   size_t off_inst = 0;
   size_t blob_begin = 0, blob_end = 0;  // tables, built on the host
   size_t off_voxels[MCX_MAX_COMPONENTS];
+  size_t off_vox_scratch[MCX_MAX_COMPONENTS];
   size_t off_tally[MCX_MAX_DETECTORS];
   size_t off_counters = 0;
   size_t zero_begin = 0, zero_end = 0;
@@ -314,6 +315,8 @@ mcx_status make_plan(const mcx_component* comps, int n_comps, const mcx_material
         return fail(MCX_ERR_UNSUPPORTED, "component %d: voxel volume above 2^31 cells (the walk uses 32-bit byte offsets, 2 bytes per cell)", c);
       // twice the size: create shifts the volume past a 4 GiB address boundary if it would straddle one
       P->off_voxels[c] = A.reserve(2 * voxel_bytes(n[f], n[a1], n[a2]) + 4 * voxel_pad(n[f], n[a1]));
+      // a scattering volume: two scratch arrays of one byte per cell for the radius transform at create
+      if (V.scatter_order > 0) P->off_vox_scratch[c] = A.reserve(voxel_bytes(n[f], n[a1], n[a2]));
     }
   P->zero_begin = A.top;
   int d = 0;
@@ -632,6 +635,12 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
                                                     d.a1, d.a2, d.pitch, d.run_dir, n_materials, stream);
         if (e != cudaSuccess) { const mcx_status s_ = cuda_fail(e, "voxel relayout"); delete H; return s_; }
         H->launches += 2;
+        if (V.scatter_order > 0) {  // radii in place of runs (step 17)
+          const cudaError_t e2 = launch_voxel_radius((uint8_t*)d.ids, (uint8_t*)dev_ptr(P.off_vox_scratch[c]), d.pitch, d.n[d.a1] + 2,
+                                                     d.n[d.a2] + 2, stream);
+          if (e2 != cudaSuccess) { const mcx_status s_ = cuda_fail(e2, "voxel radius transform"); delete H; return s_; }
+          H->launches += 34;
+        }
         break;
       }
       case MCX_MIRROR_ELLIPTIC: {

@@ -51,3 +51,19 @@ def test_purely_scattering_block_keeps_the_weight(M, O, W):
     assert np.all(np.abs(gd["p"] - 1.0) < 1e-12)
     o = O.trace(inst, n=50_000, dump=True)
     assert_dump_parity(gd, o["dump"], strict=False)
+
+
+def test_scattering_and_plain_volumes_in_one_instrument(M, O, W):
+    # the all-features kernel walks both: the scattering volume by its cube radii, the plain one by its runs
+    rng = np.random.default_rng(8)
+    mats = [None] + [W.with_scattering(rng, W.mu_table(rng, Emin=10.0, Emax=60.0, a_range=(20.0, 120.0))) for _ in range(3)]
+    ids_a = rng.integers(1, 4, size=(10, 12, 14), dtype=np.uint8)
+    ids_a[2:8, 3:9, 2:12] = 2
+    ids_b = rng.integers(0, 4, size=(9, 9, 9), dtype=np.uint8)
+    comps = [W.source("gauss", "target", "uniform", sigma_x=1e-4, sigma_y=1e-4, target_w=0.03, target_h=0.03, target_dist=1.0, E0=30.0,
+                      dE_rel=0.5),
+             W.voxels(ids_a, 2e-3, R=W.random_rotation(rng), T=(-0.01, -0.012, 0.4), scatter_order=3),
+             W.solids([W.solid_sphere(0.006, 1, 0, T=(0.001, 0.0, 0.55))]),
+             W.voxels(ids_b, 3e-3, T=(-0.0135, -0.0135, 0.7)),
+             W.detector(-0.2, 0.2, -0.2, 0.2, 20, 20, 10.0, 50.0, 4, T=(0, 0, 1.0))]
+    check(M, O, W, W.instrument("two_volumes", comps, mats, 40_000), 40_003)
