@@ -372,6 +372,11 @@ def bench_instrument(M, torch, inst, n_rays, first, steps, warmup, device, probe
                       "peak_source": f"mcx_probe_l2, random sectors of a {table >> 20} MiB table (voxel cells = "
                                      f"{footprint / 2**20:.0f} MiB), measured in this run",
                       "note": "one sector per voxel visited on the legs of scattered rays"}
+    for k, c in cand.items():
+        # a roof the kernel goes past cannot bind it: the kernel does less of that resource's work than the per-ray model
+        # counts (a warp's beam walk reads a BVH sector once for 32 rays; cube-radius skipping does not visit every voxel)
+        if c["frac"] > 1.0 and "bypassed" not in c:
+            c["bypassed"] = "frac > 1: the kernel needs less of this than the per-ray model counts (DESIGN.md 5.1, 5.4); not binding"
     bound = max((k for k in cand if "bypassed" not in cand[k]), key=lambda k: cand[k]["frac"])
     res["work_per_ray"] = work
     res["tuning"] = tuning
