@@ -29,6 +29,7 @@ if ROOT not in sys.path:
 import numpy as np
 
 METRIC, UNIT = "rays_per_second", "rays/s"
+L2_NOTE = "CUDA arm: L2 flushed between timed steps (256 MiB memset, untimed); reference arm: host cores only"
 FLUSH_BYTES = 256 << 20          # > the 126 MB L2
 
 # ---------------------------------------------------------------------------------------------------------------
@@ -483,10 +484,14 @@ def run_reference(args):
     t = float(np.mean(ts))
     v = n_step / t
     sample = f"{n_step} consecutive ray indices of {inst['name']} per step (of {inst['n_rays']})"
+    det_last = [c for c in inst["components"] if c["kind"] == "detector"][-1]
+    nb_last = det_last["nx"] * det_last["ny"] * det_last["nE"]
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"configs[{args.config}] {inst['name']}", "n_rays": inst["n_rays"], "rays_per_step": n_step},
+            "config": {"workload": f"configs[{args.config}] {inst['name']}", "n_rays_per_gpu": inst["n_rays"],
+                       "detector_bins": int(nb_last), "seed": inst["seed"], "l2": L2_NOTE},
+            "sampling": {"rays_per_step": n_step, "what": "each step traces a bounded window of the workload's ray indices"},
             "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
             "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
     print(json.dumps(line))
@@ -638,9 +643,8 @@ def main():
             "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic",
             "config": {"workload": f"configs[{args.config}] {inst['name']}", "n_rays_per_gpu": n_rays,
-                       "detector_bins": head["tally_bytes"] // 32, "seed": inst["seed"],
-                       "step": "mcx_trace + mcx_tally_read", "l2": "flushed between steps (256 MiB memset, untimed); "
-                       "steps timed one by one with CUDA events on the launching stream",
+                       "detector_bins": head["tally_bytes"] // 32, "seed": inst["seed"], "l2": L2_NOTE},
+            "timing": {"step": "mcx_trace + mcx_tally_read", "how": "steps timed one by one with CUDA events on the launching stream",
                        "parallelism": f"ray-index shards x{world}, no data-path collective"},
             "e2e": {"value": world * n_rays / (e2e_ms * 1e-3), "unit": UNIT,
                     "h2d_bytes_per_step": head["e2e"]["h2d_bytes_per_step"], "d2h_bytes_per_step": head["e2e"]["d2h_bytes_per_step"],
