@@ -1948,7 +1948,9 @@ __global__ void __launch_bounds__(256) voxel_radius_pass_kernel(const uint8_t* _
   const long long total = (long long)d0 * d1 * d2, stride = (long long)gridDim.x * blockDim.x;
   for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < total; k += stride) {
     unsigned r = rin[k];
-    if (r != 0u) {  // (a cell with r > 0 is not on the border of the arrays: all 26 neighbours exist)
+    // (a value changes once, from the cap to the cell's distance d in pass d: only cells still at the cap have work; and
+    // a cell with r > 0 is not on the border of the arrays: all 26 neighbours exist)
+    if (r == (unsigned)kVoxelRadiusMax) {
       unsigned m = 255u;
       for (int dz = -1; dz <= 1; ++dz)
         for (int dy = -1; dy <= 1; ++dy)
