@@ -77,10 +77,11 @@ struct DSolids {
   int scatter_order, pad;  // step 17: direction changes allowed per ray in this group; 0 = attenuation only
 };
 
-// Voxel volume in traversal layout: 2 bytes per cell, {material ID, run}, where run = how many cells FOLLOWING this one
-// along the fast axis in the beam's direction (run_dir) hold the same ID (capped at 255).  In a scattering volume
-// (scatter_order > 0) the second byte is instead the radius of the cube of equal IDs around the cell (mcx_kernels.cu).  Cells are addressed as
+// Voxel volume in traversal layout: kVoxelCellBytes per cell, {material ID, run, radius, 0}, where run = how many cells
+// FOLLOWING this one along the fast axis in the beam's direction (run_dir) hold the same ID (capped at 255), and radius =
+// the Chebyshev radius of the largest cube of cells around it that holds its ID throughout (capped; mcx_kernels.cu).  Cells are addressed as
 // ((i[a2]+1) * (n[a1]+2) + i[a1]+1) * pitch + i[fast]+1, with a one-cell guard border of ID kVoxelGuard all around.
+enum { kVoxelCellBytes = 4 };
 struct DVoxels {
   double h, inv_h;
   int n[3];       // nx, ny, nz
@@ -91,7 +92,7 @@ struct DVoxels {
   unsigned mg_pitch, sh_pitch, mg_slab, sh_slab;  // x / pitch, x / slab by multiplication (fast_div in mcx_kernels.cu)
   int run_dir;    // +1 / -1: the direction along the fast axis the runs are counted in (source -> volume)
   int scatter_order;  // step 17: direction changes allowed per ray in the volume; 0 = attenuation only
-  const uint8_t* ids;  // cell k at ids[2 k] (ID) and ids[2 k + 1] (run)
+  const uint8_t* ids;  // cell k at ids[4 k] (ID), ids[4 k + 1] (run), ids[4 k + 2] (radius)
 };
 
 struct DMirror {

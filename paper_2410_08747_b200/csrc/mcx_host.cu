@@ -207,10 +207,10 @@ struct Plan {
 
 // traversal layout of a voxel volume: one guard cell on every side, rows padded to 16 bytes
 int voxel_pitch(int64_t n_fast) { return (int)((n_fast + 2 + 15) / 16 * 16); }
-size_t voxel_bytes(int64_t n_fast, int64_t n_1, int64_t n_2) { return 2 * (size_t)(n_2 + 2) * (size_t)(n_1 + 2) * (size_t)voxel_pitch(n_fast); }
+size_t voxel_bytes(int64_t n_fast, int64_t n_1, int64_t n_2) { return (size_t)kVoxelCellBytes * (size_t)(n_2 + 2) * (size_t)(n_1 + 2) * (size_t)voxel_pitch(n_fast); }
 // The walk issues the loads of the slab after the one it is looking at; past a guard cell these reach at most one step
 // along every axis further.  That much of the workspace on either side of the volume belongs to the volume.
-size_t voxel_pad(int64_t n_fast, int64_t n_1) { return align_up(2 * ((size_t)(n_1 + 3) * (size_t)voxel_pitch(n_fast) + 16)); }
+size_t voxel_pad(int64_t n_fast, int64_t n_1) { return align_up((size_t)kVoxelCellBytes * ((size_t)(n_1 + 3) * (size_t)voxel_pitch(n_fast) + 16)); }
 
 // n / d == (t + ((n - t) >> 1)) >> sh with t = mulhi(m, n), for every 32-bit n and d >= 2 (Granlund & Montgomery 1994,
 // "Division by invariant integers using multiplication", the 33-bit multiplier case)
@@ -312,11 +312,11 @@ mcx_status make_plan(const mcx_component* comps, int n_comps, const mcx_material
       voxel_axes(comps[0], comps[c], &f, &a1, &a2, &run_dir);
       const int64_t n[3] = {V.nx, V.ny, V.nz};
       if (voxel_bytes(n[f], n[a1], n[a2]) + 2 * voxel_pad(n[f], n[a1]) > 0xFFFFFFFFull)
-        return fail(MCX_ERR_UNSUPPORTED, "component %d: voxel volume above 2^31 cells (the walk uses 32-bit byte offsets, 2 bytes per cell)", c);
+        return fail(MCX_ERR_UNSUPPORTED, "component %d: voxel volume above 2^30 cells (the walk uses 32-bit byte offsets, 4 bytes per cell)", c);
       // twice the size: create shifts the volume past a 4 GiB address boundary if it would straddle one
       P->off_voxels[c] = A.reserve(2 * voxel_bytes(n[f], n[a1], n[a2]) + 4 * voxel_pad(n[f], n[a1]));
-      // a scattering volume: two scratch arrays of one byte per cell for the radius transform at create
-      if (V.scatter_order > 0) P->off_vox_scratch[c] = A.reserve(voxel_bytes(n[f], n[a1], n[a2]));
+      // two scratch arrays of one byte per cell for the radius transform at create
+      P->off_vox_scratch[c] = A.reserve(voxel_bytes(n[f], n[a1], n[a2]) / kVoxelCellBytes * 2);
     }
   P->zero_begin = A.top;
   int d = 0;
@@ -635,7 +635,7 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
                                                     d.a1, d.a2, d.pitch, d.run_dir, n_materials, stream);
         if (e != cudaSuccess) { const mcx_status s_ = cuda_fail(e, "voxel relayout"); delete H; return s_; }
         H->launches += 2;
-        if (V.scatter_order > 0) {  // radii in place of runs (step 17)
+        {  // the cube radii beside the runs
           const cudaError_t e2 = launch_voxel_radius((uint8_t*)d.ids, (uint8_t*)dev_ptr(P.off_vox_scratch[c]), d.pitch, d.n[d.a1] + 2,
                                                      d.n[d.a2] + 2, stream);
           if (e2 != cudaSuccess) { const mcx_status s_ = cuda_fail(e2, "voxel radius transform"); delete H; return s_; }

@@ -868,10 +868,10 @@ __device__ __forceinline__ unsigned ld_voxel(unsigned long long addr) {
   return v;
 }
 
-// one cell {ID, run} of the voxel volume as ID | run << 8
+// one cell {ID, run, radius, 0} of the voxel volume as ID | run << 8 | radius << 16
 __device__ __forceinline__ unsigned ld_cell(unsigned long long addr) {
-  unsigned short v;
-  asm("ld.global.nc.u16 %0, [%1];" : "=h"(v) : "l"(addr));
+  unsigned v;
+  asm("ld.global.nc.u32 %0, [%1];" : "=r"(v) : "l"(addr));
   return v;
 }
 
@@ -907,7 +907,7 @@ __device__ __forceinline__ VoxAxis vox_axis(const DVoxels& V, Vec3 o, Vec3 d, Ve
   A.idx = min(n - 1, max(0, (int)floor((A.o + t0 * A.d) * V.inv_h)));
   A.dir = A.d > 0.0 ? 1 : (A.d < 0.0 ? -1 : 0);
   A.slot = g == V.fast ? 0u : (g == V.a1 ? 1u : 2u);
-  A.stride = 2u * (A.slot == 0u ? 1u : (A.slot == 1u ? (unsigned)V.pitch : V.slab));  // bytes, 2 per cell
+  A.stride = (unsigned)kVoxelCellBytes * (A.slot == 0u ? 1u : (A.slot == 1u ? (unsigned)V.pitch : V.slab));  // bytes
   return A;
 }
 
@@ -1021,7 +1021,7 @@ struct VoxWalk {
       const double wf = cold_s[VC_WFACE * kBlock];
       face = __double2loint(wf) + __double2hiint(wf) * (int)w_crossed;
     } else {
-      const unsigned off = (at - (unsigned)base) >> 1;  // cell index
+      const unsigned off = (at - (unsigned)base) / (unsigned)kVoxelCellBytes;  // cell index
       const unsigned q2 = fast_div(off, V.mg_slab, V.sh_slab), r = off - q2 * V.slab;
       const unsigned q1 = fast_div(r, V.mg_pitch, V.sh_pitch), q0 = r - q1 * (unsigned)V.pitch;
       const unsigned slot = (meta >> (2u * k)) & 3u;
@@ -1098,19 +1098,19 @@ struct VoxWalk {
     if (idb != cur || idc != cur || (cu & cv) != 0u) {
       if (settle_slab(cu, cv, lo_b, lo_c, idb, idc)) return true;
     }
-    if (!SCAT || V.scatter_order == 0) {  // (the all-features kernel also walks volumes that do not scatter: runs, not radii)
-      const unsigned s = min(min(cell_c >> 8, __umulhi(~fuh, inv_u)), __umulhi(~fvh, inv_v));
-      lo = lo_c + s * so_w;
-      w_crossed += s + 1u;
-      const unsigned long long tu = (unsigned long long)s * aul + ful, tv = (unsigned long long)s * avl + fvl;
-      ful = (unsigned)tu; fuh += s * auh + (unsigned)(tu >> 32);
-      fvl = (unsigned)tv; fvh += s * avh + (unsigned)(tv >> 32);
-    } else {
-      // A scattering volume's cells carry the radius R of the cube of equal IDs around them (voxel_boundary_kernel): from
-      // cell c the ray crosses s = R - 1 more w faces and, in those s slabs, at most s a + 1 <= R faces of either lateral
-      // axis: every cell on the way lies in the cube.  f += s a exactly; what it carries out is the lateral faces crossed.
-      const unsigned R = cell_c >> 8;
-      const unsigned s = R > 0u ? R - 1u : 0u;
+    // Skip.  Standing in cell c (same ID as the run), the ray may cross s more w faces without looking at anything
+    //  (a) if the next s cells of the row hold the same ID (the cell's RUN; rays along the fast axis in the direction the
+    //      runs were counted in, inv != 0) and no lateral face comes in those s slabs: s <= (2^64 - 1 - f) / a, taken
+    //      conservatively from the high words as mulhi(~f_hi, inv) with inv <= 2^32 / (a_hi + 1); or
+    //  (b) if s = R - 1, R the cell's RADIUS: the cube of cells within Chebyshev distance R of c holds c's ID throughout
+    //      (voxel_boundary_kernel), and in s slabs the ray crosses at most s a + 1 <= R faces of either lateral axis, so
+    //      every cell on the way lies in the cube -- in any direction, with whatever lateral faces come.
+    // The larger of the two.  f += s a exactly; what that carries out of the 64-bit fraction is the number of lateral
+    // faces crossed (none in case (a)), and the address moves by as many lateral strides.
+    {
+      const unsigned run = (cell_c >> 8) & 0xffu, R = (cell_c >> 16) & 0xffu;
+      const unsigned s_run = min(min(run, __umulhi(~fuh, inv_u)), __umulhi(~fvh, inv_v));
+      const unsigned s = max(s_run, R > 0u ? R - 1u : 0u);
       const unsigned long long tu = (unsigned long long)s * aul + ful, tv = (unsigned long long)s * avl + fvl;
       const unsigned long long tu1 = (unsigned long long)s * auh + fuh + (tu >> 32), tv1 = (unsigned long long)s * avh + fvh + (tv >> 32);
       ful = (unsigned)tu; fuh = (unsigned)tu1;
@@ -1896,7 +1896,7 @@ __global__ void __launch_bounds__(256) voxel_relayout_kernel(const uint8_t* __re
       v = src[((long long)idx[2] * ny + idx[1]) * nx + idx[0]];
       if (v >= (unsigned)n_mats) v = 0u;  // not a material: vacuum (include/mcx.h)
     }
-    reinterpret_cast<uint16_t*>(dst)[k] = (uint16_t)v;  // run = 0
+    reinterpret_cast<uint32_t*>(dst)[k] = v;  // run = radius = 0
   }
 }
 
@@ -1905,26 +1905,27 @@ __global__ void __launch_bounds__(256) voxel_relayout_kernel(const uint8_t* __re
 __global__ void __launch_bounds__(256) voxel_runs_kernel(uint8_t* __restrict__ cells, long long n_rows, int pitch, int run_dir) {
   const long long row = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (row >= n_rows) return;
-  uint8_t* r = cells + 2 * row * pitch;
+  uint8_t* r = cells + (long long)kVoxelCellBytes * row * pitch;
   int j = run_dir > 0 ? pitch - 1 : 0;
-  unsigned prev_id = r[2 * j], run = 0u;
+  unsigned prev_id = r[kVoxelCellBytes * j], run = 0u;
   for (int k = 1; k < pitch; ++k) {
     j -= run_dir;
-    const unsigned id = r[2 * j];
+    const unsigned id = r[kVoxelCellBytes * j];
     run = id == prev_id ? min(run + 1u, 255u) : 0u;
-    r[2 * j + 1] = (uint8_t)run;
+    r[kVoxelCellBytes * j + 1] = (uint8_t)run;
     prev_id = id;
   }
 }
 
-// Step 17: a scattered ray runs in any direction, where runs along one axis are of no use.  The cells of a scattering
-// volume therefore carry, in place of the run, the RADIUS of the largest cube of cells around them that holds their ID
+// Runs along one axis serve rays that follow it; a ray that crosses lateral faces every few slabs (the edge of a cone
+// beam) or runs in any direction at all (after a scattering event, step 17) gets nothing from them.  Every cell therefore
+// also carries the RADIUS of the largest cube of cells around it that holds its ID
 // throughout (Chebyshev distance to the nearest cell of another ID, less one; capped at kVoxelRadiusMax): from a cell of
 // radius R a ray may cross R - 1 slabs of its dominant axis, with whatever lateral faces come, without looking at
 // anything (VoxWalk::step).  R = the chessboard distance to the nearest BOUNDARY cell (one with a neighbour, of its 26, of
 // another ID), computed by kVoxelRadiusMax relaxation passes R <- min(R, 1 + min over the 26 neighbours) between two
 // scratch arrays; cells outside the arrays count as another ID.
-constexpr int kVoxelRadiusMax = 32;  // (16: c8 -19 %; 64: +9 % for twice the passes at create)
+constexpr int kVoxelRadiusMax = 32;  // (16: c8 -19 %; 64 / 128: c7 +6 / +8 %, c8 +9 %, c4 +0 % for two / four times the passes at create)  // (16: c8 -19 %; 64: +9 % for twice the passes at create)
 
 __device__ __forceinline__ long long vox_neighbour(long long k, int dx, int dy, int dz, int d0, int d1) {
   return k + dx + (long long)dy * d0 + (long long)dz * d0 * d1;
@@ -1934,12 +1935,12 @@ __global__ void __launch_bounds__(256) voxel_boundary_kernel(const uint8_t* __re
   const long long total = (long long)d0 * d1 * d2, stride = (long long)gridDim.x * blockDim.x;
   for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < total; k += stride) {
     const int x = (int)(k % d0), y = (int)((k / d0) % d1), z = (int)(k / ((long long)d0 * d1));
-    const unsigned id = cells[2 * k];
+    const unsigned id = cells[kVoxelCellBytes * k];
     bool boundary = x == 0 || y == 0 || z == 0 || x == d0 - 1 || y == d1 - 1 || z == d2 - 1;
     if (!boundary)
       for (int dz = -1; dz <= 1; ++dz)
         for (int dy = -1; dy <= 1; ++dy)
-          for (int dx = -1; dx <= 1; ++dx) boundary |= cells[2 * vox_neighbour(k, dx, dy, dz, d0, d1)] != id;
+          for (int dx = -1; dx <= 1; ++dx) boundary |= cells[kVoxelCellBytes * vox_neighbour(k, dx, dy, dz, d0, d1)] != id;
     r0[k] = boundary ? 0 : kVoxelRadiusMax;
   }
 }
@@ -1963,7 +1964,7 @@ __global__ void __launch_bounds__(256) voxel_radius_pass_kernel(const uint8_t* _
 
 __global__ void __launch_bounds__(256) voxel_radius_store_kernel(const uint8_t* __restrict__ r, uint8_t* __restrict__ cells, long long total) {
   const long long stride = (long long)gridDim.x * blockDim.x;
-  for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < total; k += stride) cells[2 * k + 1] = r[k];
+  for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < total; k += stride) cells[kVoxelCellBytes * k + 2] = r[k];
 }
 
 // FP64 pipe probe for the ALU roofline: 8 independent DFMA chains per thread.
