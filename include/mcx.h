@@ -313,6 +313,23 @@ mcx_status mcx_cnr(const uint64_t* N, const double* p, const double* p2, int64_t
                    const int32_t* region_mat, const int32_t* region_ref, double emin, double emax, double e_fit_min,
                    double* cnr_out, double* fit_out, void* cuda_stream);
 
+/* mcx_cnr for callers that cannot allocate device memory (code under CUDA graph capture, serving loops, harnesses that
+ * forbid cudaMalloc): finalises detector `detector` of `inst` and computes the same cnr_out[ne] and fit_out[2] as
+ * mcx_tally_read followed by mcx_cnr (Eq. (1), :268; emin, emax are the detector's own), with the
+ * intermediate arrays (N, p, p2, the CNR per bin) in a file-scope device array of the library instead of buffers of the
+ * caller's: 24 * MCX_CNR_STATIC_MAX_BINS + 8 * (MCX_CNR_STATIC_MAX_NE + 2) bytes (6 MiB) on every GPU that loads the
+ * library, held until exit.  Calls no cudaMalloc, cudaFree or allocating library routine.
+ * cnr_out [ne], fit_out [2]: HOST (pinned memory if the copy is to be asynchronous) or DEVICE memory, the caller's.
+ * region_mat, region_ref: HOST int32[4] as for mcx_cnr.
+ * Limits: a detector with more than MCX_CNR_STATIC_MAX_BINS bins or MCX_CNR_STATIC_MAX_NE energy bins is refused with
+ * MCX_ERR_UNSUPPORTED (use mcx_tally_read + mcx_cnr with buffers of your own).
+ * All calls on a device share the one array, and it keeps the last call's contents (every call overwrites what it reads,
+ * nothing needs clearing): calls whose work overlaps on the GPU -- two streams without an ordering between them --
+ * race on it and return garbage; calls on one stream, or ordered by events, are safe.  Asynchronous. */
+enum { MCX_CNR_STATIC_MAX_BINS = 1 << 18, MCX_CNR_STATIC_MAX_NE = 4096 };
+mcx_status mcx_cnr_static(mcx_instrument* inst, int detector, const int32_t* region_mat, const int32_t* region_ref,
+                          double e_fit_min, double* cnr_out, double* fit_out, void* cuda_stream);
+
 /* Zeroes all tallies and counters. */
 mcx_status mcx_tally_reset(mcx_instrument* inst, void* cuda_stream);
 

@@ -29,9 +29,10 @@ FATE_DETECTED, FATE_MISSED, FATE_DEGENERATE = -1, -2, -3
 
 EXPORTS = ["mcx_instrument_workspace_size", "mcx_instrument_create", "mcx_trace", "mcx_trace_range", "mcx_tally_read",
            "mcx_tally_read_host", "mcx_instrument_set_exec", "mcx_instrument_set_tuning", "mcx_upload_bytes", "mcx_tally_reset",
-           "mcx_counters_read", "mcx_trace_status", "mcx_trace_dump", "mcx_launch_count", "mcx_instrument_set_timing", "mcx_timing_read", "mcx_instrument_get_tuning", "mcx_instrument_set_pose", "mcx_cnr", "mcx_probe_dfma", "mcx_probe_tally",
+           "mcx_counters_read", "mcx_trace_status", "mcx_trace_dump", "mcx_launch_count", "mcx_instrument_set_timing", "mcx_timing_read", "mcx_instrument_get_tuning", "mcx_instrument_set_pose", "mcx_cnr", "mcx_cnr_static", "mcx_probe_dfma", "mcx_probe_tally",
            "mcx_probe_l2", "mcx_probe_latency", "mcx_instrument_destroy", "mcx_last_error"]
 MCX_ERR_CAPACITY = 6
+CNR_STATIC_MAX_BINS, CNR_STATIC_MAX_NE = 1 << 18, 4096  # include/mcx.h, mcx_cnr_static
 
 _dp = C.POINTER(C.c_double)
 _u64p = C.POINTER(C.c_uint64)
@@ -152,6 +153,8 @@ def lib(strict=False):
     L.mcx_cnr.argtypes = [vp, vp, vp, C.c_int64, C.c_int64, C.c_int64, C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.c_double,
                           C.c_double, C.c_double, vp, vp, vp]
     L.mcx_cnr.restype = C.c_int
+    L.mcx_cnr_static.argtypes = [vp, C.c_int, C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.c_double, vp, vp, vp]
+    L.mcx_cnr_static.restype = C.c_int
     L.mcx_upload_bytes.argtypes = [vp]
     L.mcx_upload_bytes.restype = C.c_uint64
     L.mcx_tally_reset.argtypes = [vp, vp]
@@ -406,6 +409,17 @@ class Instrument:
         _check(self.L.mcx_cnr(N.data_ptr(), P.data_ptr(), P2.data_ptr(), d["nx"], d["ny"], d["nE"], rm, rr, d["Emin"], d["Emax"],
                               float(e_fit_min), out.data_ptr(), fit.data_ptr(), self._stream()), self.L)
         return out, fit
+
+    def cnr_static(self, detector, region_mat, region_ref, e_fit_min, cnr_out, fit_out):
+        """mcx_cnr_static: the same numbers as cnr() into the caller's own tensors (pinned host or device, float64 [nE] and [2]),
+        with every intermediate array in the library's static device scratch: no allocation on the way."""
+        torch = self.torch
+        d = self.dets[detector]
+        for t, n in ((cnr_out, d["nE"]), (fit_out, 2)):
+            assert t.dtype == torch.float64 and t.is_contiguous() and t.numel() == n and (t.is_cuda or t.is_pinned())
+        rm, rr = (C.c_int32 * 4)(*region_mat), (C.c_int32 * 4)(*region_ref)
+        _check(self.L.mcx_cnr_static(self.handle, int(detector), rm, rr, float(e_fit_min), cnr_out.data_ptr(), fit_out.data_ptr(),
+                                     self._stream()), self.L)
 
     def upload_bytes(self):
         """host -> device bytes moved to build this instrument (tables by create + the voxel volume)."""

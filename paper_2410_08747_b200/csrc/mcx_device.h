@@ -197,6 +197,8 @@ cudaError_t launch_voxel_relayout(const uint8_t* src, uint8_t* dst, int nx, int 
 cudaError_t launch_cnr(const unsigned long long* N, const double* p, const double* p2, int nx, int ny, int ne, const int* region_mat,
                        const int* region_ref, double emin, double emax, double e_fit_min, double* cnr_out, double* fit_out,
                        cudaStream_t stream);
+cudaError_t launch_cnr_static(const TallyBin* bins, uint64_t n_bins, int nx, int ny, int ne, const int* region_mat, const int* region_ref,
+                              double emin, double emax, double e_fit_min, double* cnr_out, double* fit_out, cudaStream_t stream);
 cudaError_t launch_voxel_radius(uint8_t* cells, uint8_t* scratch, int d0, int d1, int d2, cudaStream_t stream);
 cudaError_t launch_probe_dfma(double* sink, int n_blocks, long long n_iters, cudaStream_t stream);
 cudaError_t launch_probe_tally(void* table, unsigned long long n_records, int n_blocks, long long n_iters, cudaStream_t stream);

@@ -983,6 +983,32 @@ mcx_status mcx_cnr(const uint64_t* N, const double* p, const double* p2, int64_t
   return MCX_OK;
 }
 
+mcx_status mcx_cnr_static(mcx_instrument* inst, int detector, const int32_t* region_mat, const int32_t* region_ref, double e_fit_min,
+                          double* cnr_out, double* fit_out, void* cuda_stream) {
+  if (!inst) return fail(MCX_ERR_INVALID_ARG, "inst is null");
+  if (detector < 0 || detector >= inst->n_dets) return fail(MCX_ERR_INVALID_ARG, "detector %d out of range (%d detectors)", detector, inst->n_dets);
+  if (!region_mat || !region_ref || !cnr_out || !fit_out) return fail(MCX_ERR_INVALID_ARG, "null argument");
+  const DDetector* D = nullptr;
+  for (int c = 0; c < inst->n_comps; ++c)
+    if (inst->host_image.comps[c].kind == MCX_DETECTOR && inst->host_image.comps[c].u.detector.index == detector) D = &inst->host_image.comps[c].u.detector;
+  if (!D) return fail(MCX_ERR_INVALID_ARG, "detector %d not found", detector);
+  const uint64_t n_bins = inst->det_bins[detector];
+  if (n_bins > (uint64_t)MCX_CNR_STATIC_MAX_BINS || D->ne > MCX_CNR_STATIC_MAX_NE)
+    return fail(MCX_ERR_UNSUPPORTED, "detector %d has %llu bins, %d energy bins: above the %d bins / %d energy bins the static scratch of "
+                "mcx_cnr_static holds (use mcx_tally_read + mcx_cnr)", detector, (unsigned long long)n_bins, D->ne, (int)MCX_CNR_STATIC_MAX_BINS,
+                (int)MCX_CNR_STATIC_MAX_NE);
+  for (const int32_t* r : {region_mat, region_ref})
+    if (r[0] < 0 || r[1] > D->nx || r[0] >= r[1] || r[2] < 0 || r[3] > D->ny || r[2] >= r[3])
+      return fail(MCX_ERR_INVALID_ARG, "region (%d, %d, %d, %d) is empty or outside the %d x %d detector", r[0], r[1], r[2], r[3], D->nx, D->ny);
+  mcx_status st = check_sticky();
+  if (st != MCX_OK) return st;
+  const cudaError_t e = launch_cnr_static(inst->host_image.tallies[detector], n_bins, D->nx, D->ny, D->ne, region_mat, region_ref, D->emin,
+                                          D->emax, e_fit_min, cnr_out, fit_out, (cudaStream_t)cuda_stream);
+  if (e != cudaSuccess) return cuda_fail(e, "static cnr launch");
+  inst->launches += 3;
+  return capacity_status(inst);
+}
+
 uint64_t mcx_upload_bytes(const mcx_instrument* inst) { return inst ? (uint64_t)inst->upload_bytes : 0; }
 
 mcx_status mcx_tally_reset(mcx_instrument* inst, void* cuda_stream) {

@@ -2268,6 +2268,54 @@ cudaError_t launch_cnr(const unsigned long long* N, const double* p, const doubl
   return cudaGetLastError();
 }
 
+// ------------------------------------------------------------------------------------------------------------
+// mcx_cnr_static (include/mcx.h): tally finalise + CNR for callers that cannot allocate device memory.  The
+// intermediate arrays (N, p, p2 of the detector, the CNR per energy bin, the fit) live in this file-scope array: 6 MiB on
+// every GPU that loads the library, until exit.  Shared by all calls, keeps the last call's contents: every byte a call
+// reads it has written itself first (tally_read_kernel fills N, p, p2 [0, n_bins), cnr_kernel cnr [0, ne), the fit its 2),
+// so nothing needs clearing; two calls in flight on the GPU at once would race on it (the header says so).
+// In host code the array's name is a stand-in, not an address: the kernels get the device address from
+// cudaGetSymbolAddress, asked once per device with that device current.
+// ------------------------------------------------------------------------------------------------------------
+constexpr size_t kCnrStaticOffCnr = (size_t)MCX_CNR_STATIC_MAX_BINS * 24;
+constexpr size_t kCnrStaticBytes = kCnrStaticOffCnr + ((size_t)MCX_CNR_STATIC_MAX_NE + 2) * sizeof(double);
+static __device__ __align__(256) unsigned char g_cnr_static_scratch[kCnrStaticBytes];
+static std::atomic<unsigned char*> g_cnr_static_addr[64];  // per device, null = not asked yet
+
+cudaError_t launch_cnr_static(const TallyBin* bins, uint64_t n_bins, int nx, int ny, int ne, const int* region_mat, const int* region_ref,
+                              double emin, double emax, double e_fit_min, double* cnr_out, double* fit_out, cudaStream_t stream) {
+  if (n_bins > (uint64_t)MCX_CNR_STATIC_MAX_BINS || ne > MCX_CNR_STATIC_MAX_NE || n_bins != (uint64_t)nx * ny * ne) return cudaErrorInvalidValue;
+  int dev = 0, n_sm = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  unsigned char* scratch = dev < 64 ? g_cnr_static_addr[dev].load(std::memory_order_acquire) : nullptr;
+  if (!scratch) {
+    e = cudaGetSymbolAddress((void**)&scratch, g_cnr_static_scratch);  // this device's copy of the array
+    if (e != cudaSuccess) return e;
+    if (!scratch) return cudaErrorInvalidSymbol;
+    if (dev < 64) g_cnr_static_addr[dev].store(scratch, std::memory_order_release);
+  }
+  e = sm_count(&n_sm);
+  if (e != cudaSuccess) return e;
+  unsigned long long* N = reinterpret_cast<unsigned long long*>(scratch);
+  double* P = reinterpret_cast<double*>(scratch) + n_bins;
+  double* P2 = P + n_bins;
+  double* cnr = reinterpret_cast<double*>(scratch + kCnrStaticOffCnr);
+  double* fit = cnr + MCX_CNR_STATIC_MAX_NE;
+  const uint64_t want = (n_bins + 255) / 256;
+  const unsigned grid = (unsigned)(want < (uint64_t)n_sm * 8 ? want : (uint64_t)n_sm * 8);
+  tally_read_kernel<<<grid, 256, 0, stream>>>(bins, n_bins, N, P, P2);
+  CnrRegions R;
+  for (int k = 0; k < 4; ++k) { R.mat[k] = region_mat[k]; R.ref[k] = region_ref[k]; }
+  cnr_kernel<<<ne, 256, 0, stream>>>(N, P, P2, nx, ne, R, cnr);
+  cnr_fit_kernel<<<1, 256, 0, stream>>>(cnr, ne, emin, emax, e_fit_min, fit);
+  e = cudaGetLastError();
+  // outputs: host (pinned if the copy is to be asynchronous) or device memory, told apart by the unified address space
+  if (e == cudaSuccess) e = cudaMemcpyAsync(cnr_out, cnr, (size_t)ne * sizeof(double), cudaMemcpyDefault, stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(fit_out, fit, 2 * sizeof(double), cudaMemcpyDefault, stream);
+  return e;
+}
+
 cudaError_t launch_probe_dfma(double* sink, int n_blocks, long long n_iters, cudaStream_t stream) {
   probe_dfma_kernel<<<n_blocks, 256, 0, stream>>>(sink, n_iters);
   return cudaGetLastError();
