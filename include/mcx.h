@@ -267,14 +267,22 @@ mcx_status mcx_instrument_set_exec(mcx_instrument* inst, int mode);
  *                                     whose bins fit (together at most 1024, smallest first) go through the cache;
  *                   MCX_TALLY_AUTO (0 here = keep) is the library's choice from measurement:
  *                   MCX_TALLY_BLOCK where some detector fits the cache, MCX_TALLY_GLOBAL otherwise.
- *                   N is the same integer in every mode; p and p2 differ in summation order only. */
+ *                   N is the same integer in every mode; p and p2 differ in summation order only.
+ *   staged_walk     1 = on (default), 2 = off.  On, a chain of slits, voxel volumes and detectors whose first scattering
+ *                   volume (scatter_order > 0) is walked by a kernel of its own, in which a lane takes
+ *                   the next ray when its ray leaves the sample: per chunk of <= 2^22 rays, the components before the
+ *                   volume, the volume, the components after it (80 bytes of workspace per ray of a chunk between
+ *                   them).  Off, or for any other chain: the whole chain in one launch.  Same results
+ *                   ray for ray, to the rounding of two compilations of the same expressions;
+ *   walk_batch_setup, walk_batch_settle   1..32: how many lanes of a warp of that kernel must wait for the set-up of a
+ *                   leg / for the end of a run of equal voxels before the warp turns to them (defaults 16, 12). */
 typedef enum { MCX_TALLY_AUTO = 0, MCX_TALLY_GLOBAL = 1, MCX_TALLY_WARP = 2, MCX_TALLY_BLOCK = 3 } mcx_tally_mode;
 typedef struct mcx_tuning {
-  int32_t chunk_log2, sort_grid_bits, absorber_gate, tally_mode;
+  int32_t chunk_log2, sort_grid_bits, absorber_gate, tally_mode, staged_walk, walk_batch_setup, walk_batch_settle;
 } mcx_tuning;
 mcx_status mcx_instrument_set_tuning(mcx_instrument* inst, const mcx_tuning* tuning);
 /* The settings in effect: chunk_log2; sort_grid_bits (0 = chosen per chunk length); absorber_gate 1 / 2; tally_mode =
- * the mode the next trace will use (never MCX_TALLY_AUTO). */
+ * the mode the next trace will use (never MCX_TALLY_AUTO); staged_walk 1 = the next trace will be staged, 2 = not. */
 mcx_status mcx_instrument_get_tuning(const mcx_instrument* inst, mcx_tuning* tuning_out);
 
 /* Finalises detector `detector` (ordinal among MCX_DETECTOR components): writes N (ray counts), p (sum of

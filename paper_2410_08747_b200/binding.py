@@ -107,7 +107,8 @@ class McxComponent(C.Structure):
 
 
 class McxTuning(C.Structure):
-    _fields_ = [("chunk_log2", C.c_int32), ("sort_grid_bits", C.c_int32), ("absorber_gate", C.c_int32), ("tally_mode", C.c_int32)]
+    _fields_ = [("chunk_log2", C.c_int32), ("sort_grid_bits", C.c_int32), ("absorber_gate", C.c_int32), ("tally_mode", C.c_int32),
+                ("staged_walk", C.c_int32), ("walk_batch_setup", C.c_int32), ("walk_batch_settle", C.c_int32)]
 
 
 FATE_DTYPE = np.dtype([("fate", np.int32), ("reserved", np.int32), ("bin", np.int64), ("p", np.float64)])
@@ -364,9 +365,11 @@ class Instrument:
         """mcx_instrument_set_exec: "auto" | "direct" | "sorted" (lane scheduling, row a13)."""
         _check(self.L.mcx_instrument_set_exec(self.handle, EXEC_MODE[mode]), self.L)
 
-    def set_tuning(self, chunk_log2=0, sort_grid_bits=0, absorber_gate=0, tally_mode="auto"):
+    def set_tuning(self, chunk_log2=0, sort_grid_bits=0, absorber_gate=0, tally_mode="auto", staged_walk=0, walk_batch_setup=0,
+                   walk_batch_settle=0):
         """mcx_instrument_set_tuning; 0 / "auto" = keep the library's choice."""
-        t = McxTuning(int(chunk_log2), int(sort_grid_bits), int(absorber_gate), TALLY_MODE[tally_mode])
+        t = McxTuning(int(chunk_log2), int(sort_grid_bits), int(absorber_gate), TALLY_MODE[tally_mode], int(staged_walk),
+                      int(walk_batch_setup), int(walk_batch_settle))
         _check(self.L.mcx_instrument_set_tuning(self.handle, C.byref(t)), self.L)
 
     def get_tuning(self):
@@ -375,7 +378,8 @@ class Instrument:
         _check(self.L.mcx_instrument_get_tuning(self.handle, C.byref(t)), self.L)
         names = {v: k for k, v in TALLY_MODE.items()}
         return {"chunk_log2": t.chunk_log2, "sort_grid_bits": t.sort_grid_bits, "absorber_gate": t.absorber_gate,
-                "tally_mode": names[t.tally_mode]}
+                "tally_mode": names[t.tally_mode], "staged_walk": t.staged_walk, "walk_batch_setup": t.walk_batch_setup,
+                "walk_batch_settle": t.walk_batch_settle}
 
     def status(self):
         """mcx_trace_status: synchronises the current stream; raises McxError (MCX_ERR_CAPACITY / MCX_ERR_CUDA) if a

@@ -165,6 +165,8 @@ static_assert(sizeof(TallyBin) == 32, "one tally record per 32-byte sector");
 // feature bits: select the kernel instantiation (code for absent component kinds is compiled out)
 enum { F_SOLIDS = 1, F_MESH = 2, F_VOXELS = 4, F_OPTICS = 8, F_PRIM = 16, F_LENS = 32, F_SCATTER = 64, F_ALL = 127 };  // F_SOLIDS: a solids group; F_PRIM / F_MESH: what it holds
 
+struct PoolRay;
+
 // One trace launch: rays first + offset(q) for positions q in [0, n); offset(q) = order[q] if order != null, else q.
 struct TraceArgs {
   uint64_t first, n, seed;
@@ -181,6 +183,30 @@ struct TraceArgs {
   int tally_mode;            // mcx_tally_mode (never MCX_TALLY_AUTO here)
   int tally_cache_log2;      // MCX_TALLY_BLOCK: log2 of the slots of the block-private cache (32 bytes each); 0 = none
   unsigned tally_cache_dets; // MCX_TALLY_BLOCK: bit d = detector d's updates go through the cache (its bins fit in it)
+  // Staged tracing of a chain with a scattering voxel sample: 0 = the whole chain in one launch;
+  // 1 = components 1 .. stage_comp - 1, survivors to the pool; 2 = positions are pool records, components stage_comp + 1 ..
+  int stage;
+  int stage_comp;
+  PoolRay* pool;             // [1 << kPoolCapacityLog2]
+  unsigned int* pool_count;  // [4]: records in the pool, next record to hand out, departures of the walk kernel, spare
+};
+
+// One ray between the stages of a staged trace: written by stage 1, walked in place by scatter_walk_kernel, read by stage 2.
+struct alignas(16) PoolRay {
+  double r[3], d[3], E, p;
+  uint64_t offset;  // of the ray in the call (ray index - first)
+  uint64_t pad;
+};
+static_assert(sizeof(PoolRay) == 80, "five 16-byte words");
+enum { kPoolCapacityLog2 = 22 };  // records (336 MB); a staged chunk holds at most this many rays
+
+// The walk stage: every record of the pool through component `comp` (a scattering voxel volume).
+struct WalkArgs {
+  uint64_t first, seed;
+  int comp, n_mats;
+  int batch_setup, batch_settle;  // lanes that must wait for a leg set-up / a run end before the warp turns to them
+  PoolRay* pool;
+  unsigned int* pool_count;
 };
 
 // sizes of the sort workspace
@@ -188,6 +214,7 @@ enum { MCX_SORT_MAX_G = 11, MCX_SORT_MAX_BUCKETS = 1 << 22, MCX_SORT_MAX_SCAN_BL
 
 // ---- launch interface (defined in mcx_kernels.cu) ----
 cudaError_t launch_trace(const DInstrument* d_inst, int features, int n_mats, const TraceArgs& args, cudaStream_t stream);  // args.cap_endpoints sizes the shared memory
+cudaError_t launch_scatter_walk(const DInstrument* d_inst, const WalkArgs& args, uint64_t n_max, cudaStream_t stream);
 cudaError_t launch_sort(uint64_t first, uint32_t n, uint64_t seed, int g, unsigned int* cnt, unsigned int* bsum,
                         uint32_t* order, cudaStream_t stream);
 cudaError_t launch_tally_read(const TallyBin* bins, uint64_t n_bins, unsigned long long* N, double* p, double* p2,

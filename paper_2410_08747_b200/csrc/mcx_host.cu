@@ -38,6 +38,11 @@ struct mcx_instrument {
   int sort_grid_bits = 0;   // 0 = by chunk length (sort_bits)
   bool gate_enabled = true;
   int tally_mode = MCX_TALLY_AUTO;
+  // staged trace: the scattering voxel volume the walk stage takes, 0 = none (one launch per chunk)
+  int stage_comp = 0;
+  bool staged_enabled = true;
+  int walk_batch_setup = 16, walk_batch_settle = 12;  // WalkArgs (measured: DESIGN.md 5.4)
+  size_t off_pool = 0, off_pool_count = 0;
   // MCX_ERR_CAPACITY: a mapped pinned host word the trace kernel writes (epoch + 1) when a ray overflows its scratch
   unsigned int* host_flag = nullptr;
   unsigned int epoch = 0;   // resets so far: an overflow of an earlier epoch is forgotten
@@ -194,6 +199,8 @@ struct Plan {
   size_t zero_begin = 0, zero_end = 0;
   size_t off_staging = 0;  // N, p, p2 of the largest detector, for mcx_tally_read_host
   size_t off_ticket = 0, off_gate = 0, off_sort_cnt = 0, off_sort_bsum = 0, off_order = 0;
+  size_t off_pool = 0, off_pool_count = 0;
+  int stage_comp = 0;
   size_t total = 0;
   // blob offsets
   size_t off_mat[MCX_MAX_MATERIALS];      // 4 arrays of n doubles each
@@ -242,6 +249,19 @@ void voxel_axes(const mcx_component& src, const mcx_component& vox, int* fast, i
   *a1 = (*fast + 1) % 3;
   *a2 = (*fast + 2) % 3;
   if (*a1 > *a2) std::swap(*a1, *a2);
+}
+
+// Staged trace: where the chain holds a scattering voxel volume and nothing else that needs scratch
+// or optics code (the kernel instantiation F_VOXELS | F_SCATTER), the first such volume is walked by a kernel of its
+// own between the part of the chain before it and the part after it.  Returns its component index, 0 = not staged.
+int staged_component(const mcx_component* comps, int n_comps) {
+  int first = 0;
+  for (int c = 1; c < n_comps; ++c) {
+    const int k = comps[c].kind;
+    if (k == MCX_SOLIDS || k == MCX_MIRROR_ELLIPTIC || k == MCX_CRYSTAL_BRAGG || k == MCX_LENS_PARAB) return 0;
+    if (k == MCX_VOXELS && comps[c].u.voxels.scatter_order > 0 && first == 0) first = c;
+  }
+  return first;
 }
 
 mcx_status make_plan(const mcx_component* comps, int n_comps, const mcx_material* mats, int n_mats, Plan* P) {
@@ -337,6 +357,11 @@ mcx_status make_plan(const mcx_component* comps, int n_comps, const mcx_material
   P->off_sort_cnt = A.reserve((size_t)MCX_SORT_MAX_BUCKETS * sizeof(unsigned int));
   P->off_sort_bsum = A.reserve((size_t)MCX_SORT_MAX_SCAN_BLOCKS * sizeof(unsigned int));
   P->off_order = A.reserve((size_t)kChunkCapacity * sizeof(uint32_t));
+  P->stage_comp = staged_component(comps, n_comps);
+  if (P->stage_comp > 0) {
+    P->off_pool_count = A.reserve(4 * sizeof(unsigned int));
+    P->off_pool = A.reserve(((size_t)1 << kPoolCapacityLog2) * sizeof(PoolRay));
+  }
   P->total = A.top;
   return MCX_OK;
 }
@@ -401,6 +426,9 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
   H->off_sort_cnt = P.off_sort_cnt;
   H->off_sort_bsum = P.off_sort_bsum;
   H->off_order = P.off_order;
+  H->off_pool = P.off_pool;
+  H->off_pool_count = P.off_pool_count;
+  H->stage_comp = P.stage_comp;
   H->chunk_rays = kChunkCapacity;
   // host copy of the table section; consumed by the upload below (a copy from pageable memory has been staged when
   // cudaMemcpyAsync returns), so it lives only as long as this call
@@ -766,6 +794,7 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
     e = cudaMemcpyAsync(ws + P.blob_begin, blob_storage.data(), blob_storage.size(), cudaMemcpyHostToDevice, stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(ws + P.zero_begin, 0, P.zero_end - P.zero_begin, stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(ws + P.off_gate, 0, sizeof(unsigned int), stream);
+  if (e == cudaSuccess && P.stage_comp > 0) e = cudaMemsetAsync(ws + P.off_pool_count, 0, 4 * sizeof(unsigned int), stream);
   if (e != cudaSuccess) { const mcx_status s_ = cuda_fail(e, "upload of the instrument image"); delete H; return s_; }
   H->upload_bytes = sizeof(DInstrument) + blob_storage.size();
   *out = H;
@@ -816,14 +845,26 @@ int tally_mode_of(const mcx_instrument* H) {
   return mode;
 }
 
+bool is_staged(const mcx_instrument* H) { return H->stage_comp > 0 && H->staged_enabled && H->features == (F_VOXELS | F_SCATTER); }
+
 // Traces rays [first, first + n) chunk by chunk; dump == nullptr tallies.
 mcx_status run_trace(mcx_instrument* H, uint64_t first, uint64_t n, uint64_t seed, mcx_ray_fate* dump, cudaStream_t stream) {
   const bool sorted = use_sorted(H);
-  const uint64_t cap = sorted ? H->chunk_rays : ((uint64_t)1 << 32);
+  const bool staged = is_staged(H);
+  uint64_t cap = sorted ? H->chunk_rays : ((uint64_t)1 << 32);
+  if (staged) {  // a chunk's survivors must fit the pool; chunks of equal length
+    cap = std::min(cap, (uint64_t)1 << kPoolCapacityLog2);
+    const uint64_t n_chunks = (n + cap - 1) / cap;
+    if (n_chunks > 1) cap = std::min(cap, ((n + n_chunks - 1) / n_chunks + 31) / 32 * 32);
+  }
   unsigned char* ws = H->workspace;
   for (uint64_t base = 0; base < n; base += cap) {
     const uint64_t m = std::min(cap, n - base);
     TraceArgs A;
+    A.stage = 0;
+    A.stage_comp = H->stage_comp;
+    A.pool = (PoolRay*)(ws + H->off_pool);
+    A.pool_count = (unsigned int*)(ws + H->off_pool_count);
     A.first = first + base;
     A.n = m;
     A.seed = seed;
@@ -863,10 +904,35 @@ mcx_status run_trace(mcx_instrument* H, uint64_t first, uint64_t n, uint64_t see
       A.order = (const uint32_t*)(ws + H->off_order);
     }
     if (tev) cudaEventRecord(tev[1], stream);
-    const cudaError_t e = launch_trace((const DInstrument*)ws, H->features, H->n_mats, A, stream);
-    if (e != cudaSuccess) return cuda_fail(e, "trace launch");
+    if (staged) {
+      // before the sample | the sample, every lane busy (scatter_walk_kernel) | after the sample
+      cudaError_t e = cudaMemsetAsync(A.pool_count, 0, sizeof(unsigned int), stream);
+      if (e != cudaSuccess) return cuda_fail(e, "pool reset");
+      A.stage = 1;
+      e = launch_trace((const DInstrument*)ws, H->features, H->n_mats, A, stream);
+      if (e != cudaSuccess) return cuda_fail(e, "trace launch (stage 1)");
+      WalkArgs Wk;
+      Wk.first = A.first;
+      Wk.seed = seed;
+      Wk.comp = H->stage_comp;
+      Wk.n_mats = H->n_mats;
+      Wk.batch_setup = H->walk_batch_setup;
+      Wk.batch_settle = H->walk_batch_settle;
+      Wk.pool = A.pool;
+      Wk.pool_count = A.pool_count;
+      e = launch_scatter_walk((const DInstrument*)ws, Wk, m, stream);
+      if (e != cudaSuccess) return cuda_fail(e, "scatter walk launch");
+      A.stage = 2;
+      A.order = nullptr;
+      e = launch_trace((const DInstrument*)ws, H->features, H->n_mats, A, stream);
+      if (e != cudaSuccess) return cuda_fail(e, "trace launch (stage 2)");
+      H->launches += 3;
+    } else {
+      const cudaError_t e = launch_trace((const DInstrument*)ws, H->features, H->n_mats, A, stream);
+      if (e != cudaSuccess) return cuda_fail(e, "trace launch");
+      H->launches++;
+    }
     if (tev) cudaEventRecord(tev[2], stream);
-    H->launches++;
   }
   return MCX_OK;
 }
@@ -1051,10 +1117,16 @@ mcx_status mcx_instrument_set_tuning(mcx_instrument* inst, const mcx_tuning* t) 
   if (t->sort_grid_bits < 0 || t->sort_grid_bits > MCX_SORT_MAX_G) return fail(MCX_ERR_INVALID_ARG, "sort_grid_bits %d outside 1..%d", t->sort_grid_bits, MCX_SORT_MAX_G);
   if (t->absorber_gate < 0 || t->absorber_gate > 2) return fail(MCX_ERR_INVALID_ARG, "absorber_gate must be 0, 1 or 2");
   if (t->tally_mode < 0 || t->tally_mode > MCX_TALLY_BLOCK) return fail(MCX_ERR_INVALID_ARG, "tally_mode must be an mcx_tally_mode");
+  if (t->staged_walk < 0 || t->staged_walk > 2) return fail(MCX_ERR_INVALID_ARG, "staged_walk must be 0, 1 or 2");
+  if (t->walk_batch_setup < 0 || t->walk_batch_setup > 32 || t->walk_batch_settle < 0 || t->walk_batch_settle > 32)
+    return fail(MCX_ERR_INVALID_ARG, "walk_batch_setup and walk_batch_settle must be 0 (keep) or 1..32");
   if (t->chunk_log2) inst->chunk_rays = (uint64_t)1 << t->chunk_log2;
   if (t->sort_grid_bits) inst->sort_grid_bits = t->sort_grid_bits;
   if (t->absorber_gate) inst->gate_enabled = t->absorber_gate == 1;
   if (t->tally_mode) inst->tally_mode = t->tally_mode;
+  if (t->staged_walk) inst->staged_enabled = t->staged_walk == 1;
+  if (t->walk_batch_setup) inst->walk_batch_setup = t->walk_batch_setup;
+  if (t->walk_batch_settle) inst->walk_batch_settle = t->walk_batch_settle;
   return MCX_OK;
 }
 
@@ -1066,6 +1138,9 @@ mcx_status mcx_instrument_get_tuning(const mcx_instrument* inst, mcx_tuning* t) 
   t->sort_grid_bits = inst->sort_grid_bits;
   t->absorber_gate = inst->gate_enabled ? 1 : 2;
   t->tally_mode = tally_mode_of(inst);
+  t->staged_walk = is_staged(inst) ? 1 : 2;
+  t->walk_batch_setup = inst->walk_batch_setup;
+  t->walk_batch_settle = inst->walk_batch_settle;
   return MCX_OK;
 }
 

@@ -1089,6 +1089,60 @@ struct VoxWalk {
     }
     return false;
   }
+  // The same slab in three parts, for the walk stage (scatter_walk_kernel), where the lanes of a warp are on unrelated
+  // paths and the long, rare part -- the end of a run -- is worth waiting for company with:  probe() looks at the slab's
+  // cells and says whether a run ends in it; settle() closes the runs (true = the leg is over); advance() skips on.
+  unsigned p_idb, p_cell;  // what probe() saw
+  __device__ __forceinline__ bool probe() {
+    const unsigned lo_b = lo + cu * so_u + cv * so_v;
+    p_idb = MCX_VOXEL_AT(lo_b);
+    p_cell = ld_cell(hi | (lo_b + so_w));
+    return p_idb != cur || (p_cell & 0xffu) != cur || (cu & cv) != 0u;
+  }
+  // The crossings of the slab in the order the ray meets them -- the cell between the two lateral faces of a double
+  // step (a), the lateral neighbour (b), the cell behind the w face (c) -- closed one per round by ONE copy of
+  // close_run, so that the lanes of a warp that settle together run it together (most have one crossing).  Same
+  // arithmetic in the same order as settle_slab.
+  __device__ __forceinline__ bool settle() {
+    const unsigned lo_b = lo + cu * so_u + cv * so_v, lo_c = lo_b + so_w, idb = p_idb, idc = p_cell & 0xffu;
+    unsigned k_lat = cu ? 1u : 2u, k_first = 0u, lo_a = 0u, ida = cur;
+    if (cu & cv) {
+      const unsigned long long au = ((unsigned long long)auh << 32) | aul, av = ((unsigned long long)avh << 32) | avl;
+      const unsigned long long fu = ((unsigned long long)fuh << 32) | ful, fv = ((unsigned long long)fvh << 32) | fvl;
+      const bool u_first = __umul64hi(fu, av) >= __umul64hi(fv, au);
+      k_first = u_first ? 1u : 2u;
+      k_lat = u_first ? 2u : 1u;
+      lo_a = lo_b - (u_first ? so_v : so_u);
+      ida = MCX_VOXEL_AT(lo_a);
+    }
+    int crossing = 0;
+#pragma unroll 1
+    for (;;) {
+      while (crossing < 3 && (crossing == 0 ? ida : (crossing == 1 ? idb : idc)) == cur) ++crossing;
+      if (crossing == 3) return false;
+      const unsigned id = crossing == 0 ? ida : (crossing == 1 ? idb : idc);
+      if (close_run(crossing == 0 ? lo_a : (crossing == 1 ? lo_b : lo_c), crossing == 0 ? k_first : (crossing == 1 ? k_lat : 0u), id)) {
+        S.event = true;
+        return true;
+      }
+      if (id == kVoxelGuard) return true;
+      ++crossing;
+    }
+  }
+  __device__ __forceinline__ void advance() {  // the skip of step(), from what probe() saw
+    const unsigned lo_c = lo + cu * so_u + cv * so_v + so_w;
+    const unsigned run = (p_cell >> 8) & 0xffu, R = (p_cell >> 16) & 0xffu;
+    const unsigned s_run = min(min(run, __umulhi(~fuh, inv_u)), __umulhi(~fvh, inv_v));
+    const unsigned s = max(s_run, R > 0u ? R - 1u : 0u);
+    const unsigned long long tu = (unsigned long long)s * aul + ful, tv = (unsigned long long)s * avl + fvl;
+    const unsigned long long tu1 = (unsigned long long)s * auh + fuh + (tu >> 32), tv1 = (unsigned long long)s * avh + fvh + (tv >> 32);
+    ful = (unsigned)tu; fuh = (unsigned)tu1;
+    fvl = (unsigned)tv; fvh = (unsigned)tv1;
+    lo = lo_c + s * so_w + (unsigned)(tu1 >> 32) * so_u + (unsigned)(tv1 >> 32) * so_v;
+    w_crossed += s + 1u;
+    cu = add_carry(ful, fuh, aul, auh);
+    cv = add_carry(fvl, fvh, avl, avh);
+  }
   // one slab and a skip; true = the leg is over (the ray left the grid, or S.event)
   __device__ __forceinline__ bool step() {
     const unsigned lo_b = lo + cu * so_u + cv * so_v, lo_c = lo_b + so_w;
@@ -1201,6 +1255,168 @@ __device__ __forceinline__ void trace_voxels(const SInst& I, const DComponent& C
   if (SCAT && S.k > 0) {
     ray.r = to_lab(C.pose, ol);
     ray.d = rotate_back(C.pose, dl);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Steps 11 + 17 as a stage of their own: every ray of the pool through one scattering voxel volume.
+// Inside trace_kernel the 32 rays of a warp enter the sample together and the warp leaves when its last ray does; with
+// 1 to K + 1 legs per ray of very different lengths, 9 of 32 lanes work on average.  Here a lane whose ray has left the
+// sample takes the next ray of the pool, so all lanes walk until the pool is empty.  Same arithmetic, ray for ray, as
+// trace_voxels<true>.  The loop is warp-uniform; an iteration is one of
+//   - one slab (probe + skip) for the lanes that are walking;
+//   - the ends of runs (close_run: path lengths, the scattering depth, the event) for the lanes whose slab holds one,
+//     once nobody walks or batch_settle lanes wait for it;
+//   - the end of a leg (the scattering event, or the ray's weight back into its record and the next ray of the pool)
+//     and the set-up of the next leg, once nobody else has work or batch_setup lanes wait for it.
+// ------------------------------------------------------------------------------------------------------------
+constexpr unsigned kWalkRange = 256u;  // consecutive records a warp takes from the pool at a time
+constexpr int kWalkBlocks = 2;
+
+__global__ void __launch_bounds__(kBlock, kWalkBlocks) scatter_walk_kernel(const DInstrument* __restrict__ g_inst, WalkArgs A) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int n_mats = A.n_mats;
+  double* len_s = reinterpret_cast<double*>(smem_raw) + threadIdx.x;
+  double* cold_s = len_s + (size_t)n_mats * kBlock;
+  double* mus_s = cold_s + (size_t)VC_COUNT * kBlock;
+  DComponent* s_comp = reinterpret_cast<DComponent*>(smem_raw + (size_t)(2 * n_mats + VC_COUNT) * kBlock * sizeof(double));
+  DMaterial* s_mats = reinterpret_cast<DMaterial*>(s_comp + 1);
+  {
+    const unsigned long long* src = reinterpret_cast<const unsigned long long*>(g_inst->comps + A.comp);
+    unsigned long long* dst = reinterpret_cast<unsigned long long*>(s_comp);
+    for (int k = threadIdx.x; k < (int)(sizeof(DComponent) / 8); k += kBlock) dst[k] = src[k];
+    src = reinterpret_cast<const unsigned long long*>(g_inst->mats);
+    dst = reinterpret_cast<unsigned long long*>(s_mats);
+    for (int k = threadIdx.x; k < n_mats * (int)(sizeof(DMaterial) / 8); k += kBlock) dst[k] = src[k];
+  }
+  __syncthreads();
+  const SInst I{1, n_mats, s_comp, s_mats, nullptr, nullptr};
+  const DComponent& C = *s_comp;
+  const DVoxels& V = C.u.voxels;
+  const int lane = threadIdx.x & 31;
+  const unsigned lanes_below = (1u << lane) - 1u;
+  const unsigned count = A.pool_count[0];
+  const uint64_t seed = A.seed;
+  const uint32_t comp = (uint32_t)A.comp;
+  const int batch_setup = A.batch_setup, batch_settle = A.batch_settle;
+
+  enum { kFetch, kPending, kWalking, kSettle, kDone };
+  int state = kFetch;
+  unsigned r_next = 0u, r_end = 0u;  // the warp's range of records (warp-uniform)
+  bool exhausted = false;            // the pool has no further range (warp-uniform)
+  unsigned rec = 0u;                 // this lane's record
+  uint64_t ray_index = 0;
+  double p = 0.0, u_mu = 0.0;
+  bool first_leg = true;
+  Vec3 ol{0.0, 0.0, 0.0}, dl{0.0, 0.0, 1.0};
+  unsigned touched = 0u;
+  Scat S;
+  S.k = 0; S.K = V.scatter_order; S.s_pre = 0.0; S.cum = 0.0; S.tau_s = 0.0; S.t_event = 0.0; S.have_ms = 0u; S.event = false;
+  VoxWalk<true> walk{I, V, 1.0, 0.0, len_s, cold_s, mus_s, touched, S};
+  for (;;) {
+    const unsigned waiting = __ballot_sync(0xffffffffu, state == kPending || state == kFetch);
+    const unsigned walking = __ballot_sync(0xffffffffu, state == kWalking);
+    const unsigned settling = __ballot_sync(0xffffffffu, state == kSettle);
+    if ((waiting | walking | settling) == 0u) break;
+    if (settling != 0u && (walking == 0u || __popc(settling) >= batch_settle)) {
+      // the runs that end in the slabs these lanes stand in; a leg that ends there (event, or out of the grid) waits for
+      // its set-up below, the others walk on
+      if (state == kSettle) {
+        if (walk.settle()) {
+          state = kPending;
+        } else {
+          walk.advance();
+          state = kWalking;
+        }
+      }
+    } else if (waiting != 0u && ((walking | settling) == 0u || __popc(waiting) >= batch_setup)) {
+      if (state == kPending && !first_leg) {  // how the last leg ended
+        if (!S.event) {  // the ray has left the sample: its weight, and where it goes, back into its record
+          if (S.k < S.K) S.s_pre += S.cum;
+          double tau = 0.0;
+          while (touched) {
+            const int m = __ffs(touched) - 1;
+            touched &= touched - 1u;
+            tau += mu_of(I.mats[m], walk.E, walk.lnE) * len_s[m * kBlock];
+          }
+          tau -= S.s_pre;
+          PoolRay& R = A.pool[rec];
+          R.p = p * exp(-tau);
+          if (S.k > 0) {
+            const Vec3 r = to_lab(C.pose, ol), d = rotate_back(C.pose, dl);
+            R.r[0] = r.x; R.r[1] = r.y; R.r[2] = r.z;
+            R.d[0] = d.x; R.d[1] = d.y; R.d[2] = d.z;
+          }
+          state = kFetch;
+        } else {
+          S.s_pre += S.tau_s;
+          double u_phi, unused;
+          draw2(seed, ray_index, (uint32_t)(2 * S.k + 1), comp, u_phi, unused);
+          ol = ol + S.t_event * dl;
+          dl = scatter_direction(dl, u_mu, u_phi);
+          ++S.k;
+        }
+      }
+      {  // the next rays of the pool for the lanes without one
+        const unsigned want = __ballot_sync(0xffffffffu, state == kFetch);
+        if (want) {
+          if (r_next == r_end && !exhausted) {
+            unsigned t = 0u;
+            if (lane == 0) t = atomicAdd(A.pool_count + 1, kWalkRange);
+            t = __shfl_sync(0xffffffffu, t, 0);
+            exhausted = t >= count;
+            r_next = exhausted ? 0u : t;
+            r_end = exhausted ? 0u : min(t + kWalkRange, count);
+          }
+          const unsigned avail = r_end - r_next, rank = __popc(want & lanes_below);
+          if (state == kFetch) {
+            if (rank < avail) {
+              rec = r_next + rank;
+              const PoolRay& R = A.pool[rec];
+              ol = to_local(C.pose, Vec3{R.r[0], R.r[1], R.r[2]});
+              dl = rotate(C.pose, Vec3{R.d[0], R.d[1], R.d[2]});
+              walk.E = R.E;
+              walk.lnE = log(R.E);
+              p = R.p;
+              ray_index = A.first + R.offset;
+              touched = 0u;
+              S.k = 0; S.s_pre = 0.0; S.cum = 0.0; S.tau_s = 0.0; S.t_event = 0.0; S.have_ms = 0u; S.event = false;
+              first_leg = true;
+              state = kPending;
+            } else if (exhausted) {
+              state = kDone;
+            }
+          }
+          r_next += min(avail, (unsigned)__popc(want));
+        }
+      }
+      if (state == kPending) {  // the next leg
+        first_leg = false;
+        if (S.k < S.K) {
+          double u_f;
+          draw2(seed, ray_index, (uint32_t)(2 * S.k), comp, u_f, u_mu);
+          S.tau_s = -log(u_f);
+          S.cum = 0.0;
+        }
+        if (walk.setup(ol, dl)) state = kWalking;  // (a half-line that misses the grid: leg over at once, no event)
+        else S.event = false;
+      }
+    } else if (state == kWalking) {
+      if (walk.probe()) state = kSettle;
+      else walk.advance();
+    }
+  }
+  // The last block to leave re-arms the pool's hand-out counter for the next chunk (the record count itself is cleared by
+  // the host side before stage 1; stage 2 reads it after this kernel, on the same stream).  The barrier: every warp of the
+  // block has taken its last range by then -- without it a late warp of another block could find the counter at zero
+  // again and walk the pool a second time.
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    __threadfence();
+    if (atomicAdd(A.pool_count + 2, 1u) == gridDim.x - 1) {
+      A.pool_count[1] = 0u;
+      A.pool_count[2] = 0u;
+    }
   }
 }
 
@@ -1638,7 +1854,11 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
     __syncthreads();
   }
   const int lane = threadIdx.x & 31;
-  const uint64_t first = A.first, n = A.n, seed = A.seed;
+  // Staged trace (run_trace in mcx_host.cu): this launch is the part of the chain before (1) or after (2) a scattering
+  // voxel volume, whose rays scatter_walk_kernel walks; stage 2 finds its rays, as many as stage 1 left, in the pool.
+  constexpr bool STAGED = FEAT == (F_VOXELS | F_SCATTER);
+  const int stage = STAGED ? A.stage : 0;
+  const uint64_t first = A.first, n = (STAGED && stage == 2) ? (uint64_t)*A.pool_count : A.n, seed = A.seed;
   const uint32_t* __restrict__ order = A.order;
   mcx_ray_fate* __restrict__ dump = A.dump;
   // Lane scheduling (row a13): blocks pull tiles of A.tile consecutive positions from a global ticket counter (the
@@ -1671,14 +1891,30 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
   unsigned* ring = reinterpret_cast<unsigned*>(smem_raw + 128) + (threadIdx.x >> 5) * 64;
   unsigned ring_head = 0u, ring_n = 0u;  // warp-uniform
   // One warp-load of rays through components 1 .. (final_pass ? the end : the gate); see the loops below.
-  auto trace_item = [&](const bool valid, const uint64_t qi, const bool final_pass) {
-    const int c_end = final_pass ? n_comps : gate + 1;
+  auto trace_item = [&](const bool valid, uint64_t qi, bool final_pass) {
+    int c_begin = 1, c_end = final_pass ? n_comps : gate + 1;
     Ray ray;
     int fate = MCX_FATE_MISSED;
     long long bin = -1;
     bool alive = valid;
-    if (valid) sample_source(I.comps[0], seed, first + qi, ray);
-    for (int c = 1; c < c_end; ++c) {
+    if (STAGED && stage == 2) {  // qi is a position in the pool: the ray as the walk stage left it
+      c_begin = A.stage_comp + 1;
+      if (valid) {
+        const PoolRay& R = A.pool[qi];
+        ray.r = {R.r[0], R.r[1], R.r[2]};
+        ray.d = {R.d[0], R.d[1], R.d[2]};
+        ray.E = R.E;
+        ray.p = R.p;
+        qi = R.offset;
+      }
+    } else {
+      if (STAGED && stage == 1) {
+        c_end = A.stage_comp;
+        final_pass = false;
+      }
+      if (valid) sample_source(I.comps[0], seed, first + qi, ray);
+    }
+    for (int c = c_begin; c < c_end; ++c) {
       const DComponent& C = I.comps[c];
       const int kind = C.kind;  // warp-uniform
       bool pass = true, tally_now = false;
@@ -1736,6 +1972,21 @@ __global__ void __launch_bounds__(kBlock, min_blocks(FEAT)) trace_kernel(const D
         if (lane == 0 && died) atomicAdd(&s_cnt[c], (unsigned)__popc(died));
       }
       if (alive_mask == 0u) break;
+    }
+    if (STAGED && stage == 1) {  // survivors go to the pool, packed
+      const unsigned live = __ballot_sync(0xffffffffu, alive);
+      unsigned at = 0u;
+      if (lane == 0 && live) at = atomicAdd(A.pool_count, (unsigned)__popc(live));
+      at = __shfl_sync(0xffffffffu, at, 0) + __popc(live & ((1u << lane) - 1u));
+      if (alive) {
+        PoolRay& R = A.pool[at];
+        R.r[0] = ray.r.x; R.r[1] = ray.r.y; R.r[2] = ray.r.z;
+        R.d[0] = ray.d.x; R.d[1] = ray.d.y; R.d[2] = ray.d.z;
+        R.E = ray.E;
+        R.p = ray.p;
+        R.offset = qi;
+        R.pad = 0ull;
+      }
     }
     if (GATE && !final_pass) {  // survivors of the gate: queue their offsets for the full pass
       const unsigned live = __ballot_sync(0xffffffffu, alive);
@@ -2056,6 +2307,29 @@ cudaError_t launch_trace(const DInstrument* d_inst, int features, int n_mats, co
   }
 #undef MCX_DISPATCH
 #undef MCX_DISPATCH_GATED
+}
+
+// The walk stage of a staged trace: at most n_max records are in the pool (the count itself is in device memory).
+cudaError_t launch_scatter_walk(const DInstrument* d_inst, const WalkArgs& A, uint64_t n_max, cudaStream_t stream) {
+  int g_n_sm = 0, dev = 0, blocks_per_sm = 1;
+  cudaError_t e = sm_count(&g_n_sm);
+  if (e != cudaSuccess) return e;
+  if (n_max == 0) return cudaSuccess;
+  const size_t smem = (size_t)(2 * A.n_mats + VC_COUNT) * kBlock * sizeof(double) + sizeof(DComponent) + (size_t)A.n_mats * sizeof(DMaterial);
+  static std::atomic<unsigned long long> configured{0ull};  // bit d: the opt-in below was made on device d
+  e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev >= 64 || !((configured.load(std::memory_order_relaxed) >> dev) & 1ull)) {
+    e = cudaFuncSetAttribute(scatter_walk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e != cudaSuccess) return e;
+    if (dev < 64) configured.fetch_or(1ull << dev, std::memory_order_relaxed);
+  }
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, scatter_walk_kernel, kBlock, smem);
+  if (e != cudaSuccess) return e;
+  if (blocks_per_sm < 1) return cudaErrorInvalidConfiguration;
+  const uint64_t full = (uint64_t)g_n_sm * blocks_per_sm, per_block = (uint64_t)kWalkRange * (kBlock / 32), want = (n_max + per_block - 1) / per_block;
+  scatter_walk_kernel<<<(unsigned)(want < full ? want : full), kBlock, smem, stream>>>(d_inst, A);
+  return cudaGetLastError();
 }
 
 // count -> scan -> scatter of one chunk (n <= 2^32 - 1 rays, 4^g buckets); cnt must be zero on entry
