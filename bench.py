@@ -383,7 +383,9 @@ def bench_instrument(M, torch, inst, n_rays, first, steps, warmup, device, probe
     res["tuning"] = tuning
     res["roofline"] = {"bound": bound, "achieved": cand[bound]["achieved"], "peak": cand[bound]["peak"],
                        "unit": cand[bound]["unit"], "frac": cand[bound]["frac"], "traffic": None,
-                       "traffic_note": TRAFFIC_NOTE, "kernel": "trace_kernel", "kernel_ms": ms_kernel,
+                       "traffic_note": TRAFFIC_NOTE,
+                       "kernel": "trace_kernel + scatter_walk_kernel + trace_kernel (staged trace, DESIGN.md 5.4)" if tuning.get("staged_walk") == 1
+                       else "trace_kernel", "kernel_ms": ms_kernel,
                        "candidates": cand}
     g.close()
     del flush, out

@@ -362,7 +362,9 @@ uint64_t mcx_launch_count(const mcx_instrument* inst);
  * trace records CUDA events on the launching stream before its ray sort, between the sort and trace_kernel, and after
  * trace_kernel (at most 4096 chunks between two reads; later ones go untimed).  mcx_timing_read waits for the last of
  * them and gives the sums since the previous read: milliseconds in the sort kernels, milliseconds in trace_kernel, and
- * the number of trace_kernel launches timed (all HOST pointers, each may be NULL); then it forgets them. */
+ * the number of trace_kernel launches timed (all HOST pointers, each may be NULL); then it forgets them.  A staged trace
+ * (mcx_tuning.staged_walk) has three launches per chunk between the last two events -- trace_kernel, scatter_walk_kernel,
+ * trace_kernel -- and counts all three. */
 mcx_status mcx_instrument_set_timing(mcx_instrument* inst, int on);
 mcx_status mcx_timing_read(mcx_instrument* inst, double* sort_ms, double* trace_ms, int64_t* n_trace_launches);
 

@@ -93,6 +93,10 @@ struct DVoxels {
   int run_dir;    // +1 / -1: the direction along the fast axis the runs are counted in (source -> volume)
   int scatter_order;  // step 17: direction changes allowed per ray in the volume; 0 = attenuation only
   const uint8_t* ids;  // cell k at ids[4 k] (ID), ids[4 k + 1] (run), ids[4 k + 2] (radius)
+  // Scattering volumes of at most 16 materials: the same cells once more, one byte each: ID in the low four bits, a code
+  // of the radius in the high four (codes 0..14 = radius 0..8, 10, 12, 16, 20, 24, 32, rounded down; 0xF0 = guard cell).
+  // What scatter_walk_kernel reads: a quarter of the bytes, so that much more of the volume stays in L2.  Null: not built.
+  const uint8_t* cmap;
 };
 
 struct DMirror {
@@ -204,6 +208,7 @@ enum { kPoolCapacityLog2 = 22 };  // records (336 MB); a staged chunk holds at m
 struct WalkArgs {
   uint64_t first, seed;
   int comp, n_mats;
+  int compact;                    // walk the one-byte cells (DVoxels::cmap)
   int batch_setup, batch_settle;  // lanes that must wait for a leg set-up / a run end before the warp turns to them
   PoolRay* pool;
   unsigned int* pool_count;
@@ -226,7 +231,7 @@ cudaError_t launch_cnr(const unsigned long long* N, const double* p, const doubl
                        cudaStream_t stream);
 cudaError_t launch_cnr_static(const TallyBin* bins, uint64_t n_bins, int nx, int ny, int ne, const int* region_mat, const int* region_ref,
                               double emin, double emax, double e_fit_min, double* cnr_out, double* fit_out, cudaStream_t stream);
-cudaError_t launch_voxel_radius(uint8_t* cells, uint8_t* scratch, int d0, int d1, int d2, cudaStream_t stream);
+cudaError_t launch_voxel_radius(uint8_t* cells, uint8_t* scratch, uint8_t* cmap, int d0, int d1, int d2, cudaStream_t stream);
 cudaError_t launch_probe_dfma(double* sink, int n_blocks, long long n_iters, cudaStream_t stream);
 cudaError_t launch_probe_tally(void* table, unsigned long long n_records, int n_blocks, long long n_iters, cudaStream_t stream);
 cudaError_t launch_probe_l2(const void* table, unsigned long long n_bytes, uint32_t* sink, int n_blocks, long long n_iters,

@@ -50,6 +50,7 @@ struct mcx_instrument {
   bool timing = false;
   std::vector<cudaEvent_t> events;  // pool, 3 per timed chunk
   size_t events_used = 0;
+  int64_t timed_launches = 0;  // trace_kernel / scatter_walk_kernel launches between the events recorded so far
   ~mcx_instrument() {
     if (host_flag) cudaFreeHost(host_flag);
     for (cudaEvent_t e : events) cudaEventDestroy(e);
@@ -194,6 +195,7 @@ struct Plan {
   size_t blob_begin = 0, blob_end = 0;  // tables, built on the host
   size_t off_voxels[MCX_MAX_COMPONENTS];
   size_t off_vox_scratch[MCX_MAX_COMPONENTS];
+  size_t off_cmap[MCX_MAX_COMPONENTS];  // 0 = none
   size_t off_tally[MCX_MAX_DETECTORS];
   size_t off_counters = 0;
   size_t zero_begin = 0, zero_end = 0;
@@ -337,6 +339,13 @@ mcx_status make_plan(const mcx_component* comps, int n_comps, const mcx_material
       P->off_voxels[c] = A.reserve(2 * voxel_bytes(n[f], n[a1], n[a2]) + 4 * voxel_pad(n[f], n[a1]));
       // two scratch arrays of one byte per cell for the radius transform at create
       P->off_vox_scratch[c] = A.reserve(voxel_bytes(n[f], n[a1], n[a2]) / kVoxelCellBytes * 2);
+      // The one-byte cells of a scattering volume (DVoxels::cmap: four bits of ID), placed by the same rule as the volume.
+      // Built where they fit in L2 (126 MB on B200) with room to spare: there the walk stage runs out of L2 instead of DRAM
+      // (c8, 66 MB: +16 %); a larger volume misses either way and does better with the exact radii and the runs of the
+      // four-byte cells (c9, 134 MB: -2 %).
+      P->off_cmap[c] = (V.scatter_order > 0 && n_mats <= 16 && voxel_bytes(n[f], n[a1], n[a2]) / kVoxelCellBytes <= ((size_t)96 << 20))
+                           ? A.reserve((2 * voxel_bytes(n[f], n[a1], n[a2]) + 4 * voxel_pad(n[f], n[a1])) / kVoxelCellBytes + 2 * kAlign)
+                           : 0;
     }
   P->zero_begin = A.top;
   int d = 0;
@@ -663,9 +672,17 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
                                                     d.a1, d.a2, d.pitch, d.run_dir, n_materials, stream);
         if (e != cudaSuccess) { const mcx_status s_ = cuda_fail(e, "voxel relayout"); delete H; return s_; }
         H->launches += 2;
-        {  // the cube radii beside the runs
-          const cudaError_t e2 = launch_voxel_radius((uint8_t*)d.ids, (uint8_t*)dev_ptr(P.off_vox_scratch[c]), d.pitch, d.n[d.a1] + 2,
-                                                     d.n[d.a2] + 2, stream);
+        d.cmap = nullptr;
+        if (P.off_cmap[c]) {  // one byte per cell, inside one 4 GiB window like the volume
+          const size_t bytes = voxel_bytes(d.n[d.fast], d.n[d.a1], d.n[d.a2]) / kVoxelCellBytes;
+          const size_t pad = voxel_pad(d.n[d.fast], d.n[d.a1]) / kVoxelCellBytes + kAlign;
+          uintptr_t p0 = (uintptr_t)dev_ptr(P.off_cmap[c]) + pad;
+          if (((p0 - pad) >> 32) != ((p0 + bytes + pad - 1) >> 32)) p0 = ((((p0 + bytes + pad - 1) >> 32)) << 32) + pad;
+          d.cmap = (const uint8_t*)p0;
+        }
+        {  // the cube radii beside the runs (and the compact cells)
+          const cudaError_t e2 = launch_voxel_radius((uint8_t*)d.ids, (uint8_t*)dev_ptr(P.off_vox_scratch[c]), (uint8_t*)d.cmap, d.pitch,
+                                                     d.n[d.a1] + 2, d.n[d.a2] + 2, stream);
           if (e2 != cudaSuccess) { const mcx_status s_ = cuda_fail(e2, "voxel radius transform"); delete H; return s_; }
           H->launches += 34;
         }
@@ -891,6 +908,7 @@ mcx_status run_trace(mcx_instrument* H, uint64_t first, uint64_t n, uint64_t see
       }
       tev = H->events.data() + H->events_used;
       H->events_used += 3;
+      H->timed_launches += staged ? 3 : 1;
       cudaEventRecord(tev[0], stream);
     }
     if (sorted && m >= kSortMinRays) {
@@ -916,6 +934,7 @@ mcx_status run_trace(mcx_instrument* H, uint64_t first, uint64_t n, uint64_t see
       Wk.seed = seed;
       Wk.comp = H->stage_comp;
       Wk.n_mats = H->n_mats;
+      Wk.compact = H->host_image.comps[H->stage_comp].u.voxels.cmap != nullptr;
       Wk.batch_setup = H->walk_batch_setup;
       Wk.batch_settle = H->walk_batch_settle;
       Wk.pool = A.pool;
@@ -1171,7 +1190,8 @@ mcx_status mcx_timing_read(mcx_instrument* inst, double* sort_ms, double* trace_
   inst->events_used = 0;
   if (sort_ms) *sort_ms = s_ms;
   if (trace_ms) *trace_ms = t_ms;
-  if (n_trace_launches) *n_trace_launches = (int64_t)n;
+  if (n_trace_launches) *n_trace_launches = inst->timed_launches;
+  inst->timed_launches = 0;
   return MCX_OK;
 }
 

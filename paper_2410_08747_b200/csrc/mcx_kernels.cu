@@ -6,6 +6,7 @@
 #include <math_constants.h>
 
 #include <atomic>
+#include <cstdio>
 
 #include "mcx_device.h"
 
@@ -898,7 +899,7 @@ struct VoxAxis {
   unsigned stride;  // address step (bytes) per voxel along this axis
 };
 
-__device__ __forceinline__ VoxAxis vox_axis(const DVoxels& V, Vec3 o, Vec3 d, Vec3 inv_d, int g, double t0) {
+__device__ __forceinline__ VoxAxis vox_axis(const DVoxels& V, Vec3 o, Vec3 d, Vec3 inv_d, int g, double t0, unsigned cell_bytes) {
   VoxAxis A;
   A.o = pick(o, g);
   A.d = pick(d, g);
@@ -907,7 +908,7 @@ __device__ __forceinline__ VoxAxis vox_axis(const DVoxels& V, Vec3 o, Vec3 d, Ve
   A.idx = min(n - 1, max(0, (int)floor((A.o + t0 * A.d) * V.inv_h)));
   A.dir = A.d > 0.0 ? 1 : (A.d < 0.0 ? -1 : 0);
   A.slot = g == V.fast ? 0u : (g == V.a1 ? 1u : 2u);
-  A.stride = (unsigned)kVoxelCellBytes * (A.slot == 0u ? 1u : (A.slot == 1u ? (unsigned)V.pitch : V.slab));  // bytes
+  A.stride = cell_bytes * (A.slot == 0u ? 1u : (A.slot == 1u ? (unsigned)V.pitch : V.slab));  // bytes
   return A;
 }
 
@@ -932,8 +933,17 @@ __device__ __forceinline__ void lateral_init(const VoxAxis& A, double inv_dw, do
 // from where it enters the grid to where it leaves it or (SCAT, step 17) to the scattering event.  setup() starts a leg,
 // step() does one slab and a skip and says when the leg is over.  Path lengths go to len_s / touched, which accumulate
 // over the legs.  (Everything is inlined; the members live in registers.)
-#define MCX_VOXEL_AT(lo32) ld_voxel(hi | (lo32))
-template <bool SCAT>
+// CELL = bytes per cell: kVoxelCellBytes, or 1 = the compact cells of a scattering volume (DVoxels::cmap; walk stage only:
+// setup / probe / settle / advance).
+#define MCX_VOXEL_AT(lo32) id_at(lo32)
+constexpr unsigned kCompactGuard = 16u;  // what id_of_compact makes of a guard cell
+// compact cell -> ID (0..15), guard (0xF0) -> 16
+__device__ __forceinline__ unsigned id_of_compact(unsigned v) { return (v & 15u) | (((v + 16u) >> 4) & 16u); }
+// radius code -> radius: 0..8, 10, 12, 16, 20, 24, 32 (code 15 = guard: unused)
+__device__ __forceinline__ unsigned radius_of_code(unsigned c) {
+  return (unsigned)((c < 8u ? 0x0706050403020100ull : 0x00201814100c0a08ull) >> (8u * (c & 7u))) & 0xffu;
+}
+template <bool SCAT, int CELL = kVoxelCellBytes>
 struct VoxWalk {
   const SInst& I;
   const DVoxels& V;
@@ -947,6 +957,11 @@ struct VoxWalk {
   unsigned cur, w_crossed, cu, cv, lo;
   unsigned long long base, hi;
   double t_run;
+  static constexpr unsigned kGuard = CELL == 1 ? kCompactGuard : kVoxelGuard;
+  __device__ __forceinline__ unsigned id_at(unsigned lo32) const {
+    const unsigned v = ld_voxel(hi | lo32);
+    return CELL == 1 ? id_of_compact(v) : v;
+  }
 
   // false: the half-line misses the grid
   __device__ __forceinline__ bool setup(Vec3 ol, Vec3 dl) {
@@ -975,7 +990,7 @@ struct VoxWalk {
       if (fabs(dl.z) > m) gw = 2;
     }
     const int gu = gw == 0 ? 1 : 0, gv = gw == 2 ? 1 : 2;
-    const VoxAxis W = vox_axis(V, ol, dl, inv_d, gw, t0), U = vox_axis(V, ol, dl, inv_d, gu, t0), X = vox_axis(V, ol, dl, inv_d, gv, t0);
+    const VoxAxis W = vox_axis(V, ol, dl, inv_d, gw, t0, CELL), U = vox_axis(V, ol, dl, inv_d, gu, t0, CELL), X = vox_axis(V, ol, dl, inv_d, gv, t0, CELL);
     const double t_w0 = ((double)(W.idx + (W.dir > 0 ? 1 : 0)) * h - W.o) * W.inv_d;  // first w face ahead
     unsigned long long fu, au, fv, av;
     lateral_init(U, W.inv_d, t_w0, V.inv_h, fu, au, cu0);
@@ -992,7 +1007,7 @@ struct VoxWalk {
     // index of the first w face ahead and the walk's direction along w, as one 8-byte slot
     cold_s[VC_WFACE * kBlock] = __hiloint2double(W.dir, W.idx + (W.dir > 0 ? 1 : 0));
     {  // skipping (see the loop below): only along the fast axis in the direction the runs were counted in
-      const bool can_skip = W.slot == 0u && W.dir == V.run_dir;
+      const bool can_skip = CELL == kVoxelCellBytes && W.slot == 0u && W.dir == V.run_dir;  // (compact cells carry no runs)
       // inv <= 2^32 / (a_hi + 1): float quotient less a relative 1e-6 (its own error is 2^-22)
       inv_u = can_skip ? __float2uint_rz(__fdividef(4294967296.0f, (float)auh + 1.0f) * 0.999999f) : 0u;
       inv_v = can_skip ? __float2uint_rz(__fdividef(4294967296.0f, (float)avh + 1.0f) * 0.999999f) : 0u;
@@ -1001,7 +1016,7 @@ struct VoxWalk {
     t_run = t0;
     // The volume does not straddle a 4 GiB address boundary (mcx_instrument_create places it so): the walk keeps the
     // low address word only and a step is one 32-bit add.
-    base = (unsigned long long)V.ids;
+    base = (unsigned long long)(CELL == 1 ? V.cmap : V.ids);
     hi = base & 0xFFFFFFFF00000000ull;
     lo_start += (unsigned)base;
     cur = MCX_VOXEL_AT(lo_start);
@@ -1021,7 +1036,7 @@ struct VoxWalk {
       const double wf = cold_s[VC_WFACE * kBlock];
       face = __double2loint(wf) + __double2hiint(wf) * (int)w_crossed;
     } else {
-      const unsigned off = (at - (unsigned)base) / (unsigned)kVoxelCellBytes;  // cell index
+      const unsigned off = (at - (unsigned)base) / (unsigned)CELL;  // cell index
       const unsigned q2 = fast_div(off, V.mg_slab, V.sh_slab), r = off - q2 * V.slab;
       const unsigned q1 = fast_div(r, V.mg_pitch, V.sh_pitch), q0 = r - q1 * (unsigned)V.pitch;
       const unsigned slot = (meta >> (2u * k)) & 3u;
@@ -1093,18 +1108,19 @@ struct VoxWalk {
   // paths and the long, rare part -- the end of a run -- is worth waiting for company with:  probe() looks at the slab's
   // cells and says whether a run ends in it; settle() closes the runs (true = the leg is over); advance() skips on.
   unsigned p_idb, p_cell;  // what probe() saw
+  __device__ __forceinline__ unsigned id_of_cell(unsigned cell) const { return CELL == 1 ? id_of_compact(cell) : (cell & 0xffu); }
   __device__ __forceinline__ bool probe() {
     const unsigned lo_b = lo + cu * so_u + cv * so_v;
     p_idb = MCX_VOXEL_AT(lo_b);
-    p_cell = ld_cell(hi | (lo_b + so_w));
-    return p_idb != cur || (p_cell & 0xffu) != cur || (cu & cv) != 0u;
+    p_cell = CELL == 1 ? ld_voxel(hi | (lo_b + so_w)) : ld_cell(hi | (lo_b + so_w));
+    return p_idb != cur || id_of_cell(p_cell) != cur || (cu & cv) != 0u;
   }
   // The crossings of the slab in the order the ray meets them -- the cell between the two lateral faces of a double
   // step (a), the lateral neighbour (b), the cell behind the w face (c) -- closed one per round by ONE copy of
   // close_run, so that the lanes of a warp that settle together run it together (most have one crossing).  Same
   // arithmetic in the same order as settle_slab.
   __device__ __forceinline__ bool settle() {
-    const unsigned lo_b = lo + cu * so_u + cv * so_v, lo_c = lo_b + so_w, idb = p_idb, idc = p_cell & 0xffu;
+    const unsigned lo_b = lo + cu * so_u + cv * so_v, lo_c = lo_b + so_w, idb = p_idb, idc = id_of_cell(p_cell);
     unsigned k_lat = cu ? 1u : 2u, k_first = 0u, lo_a = 0u, ida = cur;
     if (cu & cv) {
       const unsigned long long au = ((unsigned long long)auh << 32) | aul, av = ((unsigned long long)avh << 32) | avl;
@@ -1125,15 +1141,21 @@ struct VoxWalk {
         S.event = true;
         return true;
       }
-      if (id == kVoxelGuard) return true;
+      if (id == kGuard) return true;
       ++crossing;
     }
   }
   __device__ __forceinline__ void advance() {  // the skip of step(), from what probe() saw
     const unsigned lo_c = lo + cu * so_u + cv * so_v + so_w;
-    const unsigned run = (p_cell >> 8) & 0xffu, R = (p_cell >> 16) & 0xffu;
-    const unsigned s_run = min(min(run, __umulhi(~fuh, inv_u)), __umulhi(~fvh, inv_v));
-    const unsigned s = max(s_run, R > 0u ? R - 1u : 0u);
+    unsigned s;
+    if (CELL == 1) {  // the cube radius only
+      const unsigned R = radius_of_code(p_cell >> 4);
+      s = R > 0u ? R - 1u : 0u;
+    } else {
+      const unsigned run = (p_cell >> 8) & 0xffu, R = (p_cell >> 16) & 0xffu;
+      const unsigned s_run = min(min(run, __umulhi(~fuh, inv_u)), __umulhi(~fvh, inv_v));
+      s = max(s_run, R > 0u ? R - 1u : 0u);
+    }
     const unsigned long long tu = (unsigned long long)s * aul + ful, tv = (unsigned long long)s * avl + fvl;
     const unsigned long long tu1 = (unsigned long long)s * auh + fuh + (tu >> 32), tv1 = (unsigned long long)s * avh + fvh + (tv >> 32);
     ful = (unsigned)tu; fuh = (unsigned)tu1;
@@ -1273,6 +1295,7 @@ __device__ __forceinline__ void trace_voxels(const SInst& I, const DComponent& C
 constexpr unsigned kWalkRange = 256u;  // consecutive records a warp takes from the pool at a time
 constexpr int kWalkBlocks = 2;
 
+template <int CELL>
 __global__ void __launch_bounds__(kBlock, kWalkBlocks) scatter_walk_kernel(const DInstrument* __restrict__ g_inst, WalkArgs A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int n_mats = A.n_mats;
@@ -1312,7 +1335,7 @@ __global__ void __launch_bounds__(kBlock, kWalkBlocks) scatter_walk_kernel(const
   unsigned touched = 0u;
   Scat S;
   S.k = 0; S.K = V.scatter_order; S.s_pre = 0.0; S.cum = 0.0; S.tau_s = 0.0; S.t_event = 0.0; S.have_ms = 0u; S.event = false;
-  VoxWalk<true> walk{I, V, 1.0, 0.0, len_s, cold_s, mus_s, touched, S};
+  VoxWalk<true, CELL> walk{I, V, 1.0, 0.0, len_s, cold_s, mus_s, touched, S};
   for (;;) {
     const unsigned waiting = __ballot_sync(0xffffffffu, state == kPending || state == kFetch);
     const unsigned walking = __ballot_sync(0xffffffffu, state == kWalking);
@@ -2213,9 +2236,18 @@ __global__ void __launch_bounds__(256) voxel_radius_pass_kernel(const uint8_t* _
   }
 }
 
-__global__ void __launch_bounds__(256) voxel_radius_store_kernel(const uint8_t* __restrict__ r, uint8_t* __restrict__ cells, long long total) {
+__global__ void __launch_bounds__(256) voxel_radius_store_kernel(const uint8_t* __restrict__ r, uint8_t* __restrict__ cells, uint8_t* __restrict__ cmap,
+                                                                 long long total) {
   const long long stride = (long long)gridDim.x * blockDim.x;
-  for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < total; k += stride) cells[kVoxelCellBytes * k + 2] = r[k];
+  for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < total; k += stride) {
+    const unsigned R = r[k];
+    cells[kVoxelCellBytes * k + 2] = (uint8_t)R;
+    if (cmap) {  // the compact cell (DVoxels::cmap): the largest code whose radius is <= R
+      const unsigned id = cells[kVoxelCellBytes * k];
+      const unsigned code = R <= 8u ? R : (R < 12u ? 8u + (R - 8u) / 2u : (R < 16u ? 10u : (R < 32u ? min(13u, 11u + (R - 16u) / 4u) : 14u)));
+      cmap[k] = (uint8_t)(id == kVoxelGuard ? 0xF0u : (id | (code << 4)));
+    }
+  }
 }
 
 // FP64 pipe probe for the ALU roofline: 8 independent DFMA chains per thread.
@@ -2310,26 +2342,35 @@ cudaError_t launch_trace(const DInstrument* d_inst, int features, int n_mats, co
 }
 
 // The walk stage of a staged trace: at most n_max records are in the pool (the count itself is in device memory).
-cudaError_t launch_scatter_walk(const DInstrument* d_inst, const WalkArgs& A, uint64_t n_max, cudaStream_t stream) {
-  int g_n_sm = 0, dev = 0, blocks_per_sm = 1;
-  cudaError_t e = sm_count(&g_n_sm);
-  if (e != cudaSuccess) return e;
-  if (n_max == 0) return cudaSuccess;
+// (internal linkage: the local static of a template with external linkage is ONE object for every shared library of the
+// process that holds the template, and the strict build's kernels would go without their own opt-in)
+template <int CELL>
+static cudaError_t launch_scatter_walk_as(const DInstrument* d_inst, const WalkArgs& A, uint64_t n_max, cudaStream_t stream, int n_sm) {
+  int dev = 0, blocks_per_sm = 1;
   const size_t smem = (size_t)(2 * A.n_mats + VC_COUNT) * kBlock * sizeof(double) + sizeof(DComponent) + (size_t)A.n_mats * sizeof(DMaterial);
   static std::atomic<unsigned long long> configured{0ull};  // bit d: the opt-in below was made on device d
-  e = cudaGetDevice(&dev);
+  cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return e;
   if (dev >= 64 || !((configured.load(std::memory_order_relaxed) >> dev) & 1ull)) {
-    e = cudaFuncSetAttribute(scatter_walk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    e = cudaFuncSetAttribute(scatter_walk_kernel<CELL>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e != cudaSuccess) return e;
     if (dev < 64) configured.fetch_or(1ull << dev, std::memory_order_relaxed);
   }
-  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, scatter_walk_kernel, kBlock, smem);
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, scatter_walk_kernel<CELL>, kBlock, smem);
   if (e != cudaSuccess) return e;
   if (blocks_per_sm < 1) return cudaErrorInvalidConfiguration;
-  const uint64_t full = (uint64_t)g_n_sm * blocks_per_sm, per_block = (uint64_t)kWalkRange * (kBlock / 32), want = (n_max + per_block - 1) / per_block;
-  scatter_walk_kernel<<<(unsigned)(want < full ? want : full), kBlock, smem, stream>>>(d_inst, A);
+  const uint64_t full = (uint64_t)n_sm * blocks_per_sm, per_block = (uint64_t)kWalkRange * (kBlock / 32), want = (n_max + per_block - 1) / per_block;
+  scatter_walk_kernel<CELL><<<(unsigned)(want < full ? want : full), kBlock, smem, stream>>>(d_inst, A);
   return cudaGetLastError();
+}
+
+cudaError_t launch_scatter_walk(const DInstrument* d_inst, const WalkArgs& A, uint64_t n_max, cudaStream_t stream) {
+  int g_n_sm = 0;
+  const cudaError_t e = sm_count(&g_n_sm);
+  if (e != cudaSuccess) return e;
+  if (n_max == 0) return cudaSuccess;
+  return A.compact ? launch_scatter_walk_as<1>(d_inst, A, n_max, stream, g_n_sm)
+                   : launch_scatter_walk_as<kVoxelCellBytes>(d_inst, A, n_max, stream, g_n_sm);
 }
 
 // count -> scan -> scatter of one chunk (n <= 2^32 - 1 rays, 4^g buckets); cnt must be zero on entry
@@ -2375,7 +2416,7 @@ cudaError_t launch_voxel_relayout(const uint8_t* src, uint8_t* dst, int nx, int 
 
 // cells: the traversal layout of d0 x d1 x d2 cells {ID, .}; scratch: 2 * d0 * d1 * d2 bytes.  Leaves the radius in the
 // second byte of every cell.
-cudaError_t launch_voxel_radius(uint8_t* cells, uint8_t* scratch, int d0, int d1, int d2, cudaStream_t stream) {
+cudaError_t launch_voxel_radius(uint8_t* cells, uint8_t* scratch, uint8_t* cmap, int d0, int d1, int d2, cudaStream_t stream) {
   int g_n_sm = 0;
   cudaError_t e = sm_count(&g_n_sm);
   if (e != cudaSuccess) return e;
@@ -2387,7 +2428,7 @@ cudaError_t launch_voxel_radius(uint8_t* cells, uint8_t* scratch, int d0, int d1
     voxel_radius_pass_kernel<<<g_n_sm * 16, 256, 0, stream>>>(a, b, d0, d1, d2);
     uint8_t* t = a; a = b; b = t;
   }
-  voxel_radius_store_kernel<<<g_n_sm * 16, 256, 0, stream>>>(a, cells, total);
+  voxel_radius_store_kernel<<<g_n_sm * 16, 256, 0, stream>>>(a, cells, cmap, total);
   return cudaGetLastError();
 }
 

@@ -128,6 +128,17 @@ def test_staged_walk_with_components_on_both_sides_of_the_sample(M, O, W):
         assert np.array_equal(Ns, Nw)
 
 
+def test_staged_walk_on_the_four_byte_cells(M, O, W):
+    # more than 16 materials: no one-byte cells (DVoxels::cmap), the walk stage reads the cells the trace kernel reads
+    inst = W.config9(small=True)
+    inst["materials"] = list(inst["materials"]) + [inst["materials"][k] for k in (1, 2, 3, 4)]
+    assert len(inst["materials"]) > 16
+    check(M, O, W, inst, 40_003)
+    (ds, ts, cs, _), (dw, tw, cw, _) = _both_ways(M, inst, 40_003)
+    assert np.array_equal(ds["fate"], dw["fate"]) and np.array_equal(ds["bin"], dw["bin"])
+    assert np.allclose(ds["p"], dw["p"], rtol=1e-11, atol=0)
+
+
 def test_staged_walk_only_where_the_chain_allows_it(M, O, W):
     for inst, want in ((W.config8(small=True), 1), (W.config4(small=True), 2), (W.config1(small=True, scatter_order=2), 2)):
         g = M.Instrument(inst)
