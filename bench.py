@@ -391,7 +391,7 @@ def bench_instrument(M, torch, inst, n_rays, first, steps, warmup, device, probe
     del flush, out
     torch.cuda.empty_cache()
     if with_e2e:
-        res["e2e"] = bench_e2e(M, torch, inst, n_rays, first, 2, device)
+        res["e2e"] = bench_e2e(M, torch, inst, n_rays, first, 4, device)
     return res
 
 

@@ -70,6 +70,28 @@ def test_workspace_size_counts_the_tallies(B, W):
             assert n.value >= 32 * bins + inst["components"][1]["ids"].size
 
 
+def test_workspace_size_counts_the_staged_trace(B, W):
+    # a chain of slits, voxel volumes and detectors whose volume scatters is traced in stages (include/mcx.h, mcx_tuning
+    # staged_walk): its workspace holds the pool of 2^22 ray records of 80 bytes and, for a volume of at most 16
+    # materials, the one-byte cells; the same chain without scattering, or with a solids group in it, holds neither
+    L = B.lib()
+    def size(inst):
+        comps, mats, keep = _marshal(B, inst)
+        n = C.c_size_t()
+        assert L.mcx_instrument_workspace_size(comps, len(inst["components"]), mats, len(inst["materials"]), C.byref(n)) == 0
+        return n.value
+    pool = 80 << 22
+    plain, scat = W.config4(small=True), W.config4(small=True, scatter_order=2)
+    cells = plain["components"][1]["ids"].size
+    assert size(scat) - size(plain) >= pool + cells and size(scat) - size(plain) < pool + 4 * cells + (1 << 20)
+    many = W.config4(small=True, scatter_order=2)
+    many["materials"] = list(many["materials"]) + [many["materials"][1]] * 4     # 20 materials: no one-byte cells
+    assert pool <= size(many) - size(plain) < size(scat) - size(plain)
+    mixed = W.config4(small=True, scatter_order=2)
+    mixed["components"] = mixed["components"][:2] + [W.solids([W.solid_sphere(0.006, 1, 0, T=(0.0, 0.0, 0.9))])] + mixed["components"][2:]
+    assert size(mixed) - size(plain) < pool
+
+
 def test_argument_errors_are_reported_synchronously(B, W):
     L = B.lib()
     inst = W.config0()
