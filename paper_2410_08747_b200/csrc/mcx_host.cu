@@ -684,7 +684,7 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
           const cudaError_t e2 = launch_voxel_radius((uint8_t*)d.ids, (uint8_t*)dev_ptr(P.off_vox_scratch[c]), (uint8_t*)d.cmap, d.pitch,
                                                      d.n[d.a1] + 2, d.n[d.a2] + 2, stream);
           if (e2 != cudaSuccess) { const mcx_status s_ = cuda_fail(e2, "voxel radius transform"); delete H; return s_; }
-          H->launches += 34;
+          H->launches += 9;  // boundary, seven doubling passes, store
         }
         break;
       }

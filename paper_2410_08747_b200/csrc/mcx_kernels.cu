@@ -2196,10 +2196,17 @@ __global__ void __launch_bounds__(256) voxel_runs_kernel(uint8_t* __restrict__ c
 // also carries the RADIUS of the largest cube of cells around it that holds its ID
 // throughout (Chebyshev distance to the nearest cell of another ID, less one; capped at kVoxelRadiusMax): from a cell of
 // radius R a ray may cross R - 1 slabs of its dominant axis, with whatever lateral faces come, without looking at
-// anything (VoxWalk::step).  R = the chessboard distance to the nearest BOUNDARY cell (one with a neighbour, of its 26, of
-// another ID), computed by kVoxelRadiusMax relaxation passes R <- min(R, 1 + min over the 26 neighbours) between two
-// scratch arrays; cells outside the arrays count as another ID.
-constexpr int kVoxelRadiusMax = 32;  // (16: c8 -19 %; 64 / 128: c7 +6 / +8 %, c8 +9 %, c4 +0 % for two / four times the passes at create)  // (16: c8 -19 %; 64: +9 % for twice the passes at create)
+// anything (VoxWalk::step).  R = min(kVoxelRadiusMax, the chessboard distance to the nearest BOUNDARY cell) (a boundary cell
+// has a neighbour, of its 26, of another ID; cells outside the arrays count as another ID).  Computed by doubling
+// instead of kVoxelRadiusMax relaxation passes: with C_m(x) = "no boundary cell within chessboard distance m of x" (the
+// cube of radius m around x is clear), C_0 is the boundary test, C_1 looks at the 26 neighbours' C_0, and
+// C_2m(x) = AND of C_m at the eight cells x + (+-m, +-m, +-m), whose cubes cover the cube of radius 2m exactly.  Eight
+// bits per cell (m = 0, 1, 2, 4, ..., 64) in one scratch byte, ping-ponged between two arrays.  Any other radius t = q + o,
+// q the largest power of two <= t, is clear iff C_q holds at the eight cells x + (+-o, +-o, +-o) (o <= q - 1: the cubes
+// overlap or touch), so R - 1 = the largest clear t <= 127 comes out of a seven-step binary search: about 120 byte
+// look-ups per cell where the relaxation took up to 27 x 32.
+constexpr int kVoxelRadiusMax = 128;  // a power of two <= 128 (eight C_m bits per scratch byte); 32 -> 64 -> 128: c7 +5 %, +2 %; c4, c9 +0 %
+static_assert(kVoxelRadiusMax <= 128 && (kVoxelRadiusMax & (kVoxelRadiusMax - 1)) == 0, "C_m bits for m = 0, 1, 2, ..., kVoxelRadiusMax / 2 in one byte");
 
 __device__ __forceinline__ long long vox_neighbour(long long k, int dx, int dy, int dz, int d0, int d1) {
   return k + dx + (long long)dy * d0 + (long long)dz * d0 * d1;
@@ -2215,32 +2222,62 @@ __global__ void __launch_bounds__(256) voxel_boundary_kernel(const uint8_t* __re
       for (int dz = -1; dz <= 1; ++dz)
         for (int dy = -1; dy <= 1; ++dy)
           for (int dx = -1; dx <= 1; ++dx) boundary |= cells[kVoxelCellBytes * vox_neighbour(k, dx, dy, dz, d0, d1)] != id;
-    r0[k] = boundary ? 0 : kVoxelRadiusMax;
+    r0[k] = boundary ? 0 : 1;  // bit 0 = C_0
   }
 }
 
-__global__ void __launch_bounds__(256) voxel_radius_pass_kernel(const uint8_t* __restrict__ rin, uint8_t* __restrict__ rout, int d0, int d1, int d2) {
+// bit `level` of rout = C_m from bit `level - 1` of rin (C_m/2, or C_0 for level 1); the lower bits are copied.
+// level 1: the 26 neighbours; level >= 2: the eight cells at (+-off, +-off, +-off), off = m / 2.  (A cell whose own lower
+// bit is clear cannot have the higher one; a cell with C_m set lies more than m cells inside the arrays, so the cells
+// looked at exist.)
+__global__ void __launch_bounds__(256) voxel_clear_pass_kernel(const uint8_t* __restrict__ rin, uint8_t* __restrict__ rout, int d0, int d1, int d2,
+                                                               int level, int off) {
+  const long long total = (long long)d0 * d1 * d2, stride = (long long)gridDim.x * blockDim.x;
+  const unsigned below = 1u << (level - 1);
+  for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < total; k += stride) {
+    unsigned v = rin[k];
+    if (v & below) {
+      unsigned all = below;
+      if (level == 1) {
+        for (int dz = -1; dz <= 1; ++dz)
+          for (int dy = -1; dy <= 1; ++dy)
+            for (int dx = -1; dx <= 1; ++dx) all &= rin[vox_neighbour(k, dx, dy, dz, d0, d1)];
+      } else {
+        for (int c = 0; c < 8; ++c)
+          all &= rin[vox_neighbour(k, (c & 1) ? off : -off, (c & 2) ? off : -off, (c & 4) ? off : -off, d0, d1)];
+      }
+      if (all) v |= 1u << level;
+    }
+    rout[k] = (uint8_t)v;
+  }
+}
+
+// bits: the six C_m bits of every cell (above).  Writes the radius into the third byte of every cell and, if asked, the
+// compact cell (DVoxels::cmap).
+__global__ void __launch_bounds__(256) voxel_radius_store_kernel(const uint8_t* __restrict__ bits, uint8_t* __restrict__ cells, uint8_t* __restrict__ cmap,
+                                                                 int d0, int d1, int d2) {
   const long long total = (long long)d0 * d1 * d2, stride = (long long)gridDim.x * blockDim.x;
   for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < total; k += stride) {
-    unsigned r = rin[k];
-    // (a value changes once, from the cap to the cell's distance d in pass d: only cells still at the cap have work; and
-    // a cell with r > 0 is not on the border of the arrays: all 26 neighbours exist)
-    if (r == (unsigned)kVoxelRadiusMax) {
-      unsigned m = 255u;
-      for (int dz = -1; dz <= 1; ++dz)
-        for (int dy = -1; dy <= 1; ++dy)
-          for (int dx = -1; dx <= 1; ++dx) m = min(m, (unsigned)rin[vox_neighbour(k, dx, dy, dz, d0, d1)]);
-      r = min(r, m + 1u);
+    unsigned R = 0u;
+    if (bits[k] & 1u) {  // not a boundary cell: R - 1 = the largest clear radius t in 0 .. kVoxelRadiusMax - 1
+      const int x = (int)(k % d0), y = (int)((k / d0) % d1), z = (int)(k / ((long long)d0 * d1));
+      int t = 0;
+      for (int step = kVoxelRadiusMax / 2; step >= 1; step >>= 1) {
+        const int cand = t + step;  // <= kVoxelRadiusMax - 1
+        const int lg = 31 - __clz(cand), q = 1 << lg, o = cand - q;
+        // the cube of radius cand must lie inside the arrays' interior (their outermost cells are boundary cells)
+        bool clear = x - cand >= 1 && x + cand <= d0 - 2 && y - cand >= 1 && y + cand <= d1 - 2 && z - cand >= 1 && z + cand <= d2 - 2;
+        if (clear) {
+          unsigned all = 1u << (lg + 1);  // the bit of C_q
+          if (o == 0) all &= bits[k];
+          else
+            for (int c = 0; c < 8; ++c) all &= bits[vox_neighbour(k, (c & 1) ? o : -o, (c & 2) ? o : -o, (c & 4) ? o : -o, d0, d1)];
+          clear = all != 0u;
+        }
+        if (clear) t = cand;
+      }
+      R = (unsigned)t + 1u;
     }
-    rout[k] = (uint8_t)r;
-  }
-}
-
-__global__ void __launch_bounds__(256) voxel_radius_store_kernel(const uint8_t* __restrict__ r, uint8_t* __restrict__ cells, uint8_t* __restrict__ cmap,
-                                                                 long long total) {
-  const long long stride = (long long)gridDim.x * blockDim.x;
-  for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < total; k += stride) {
-    const unsigned R = r[k];
     cells[kVoxelCellBytes * k + 2] = (uint8_t)R;
     if (cmap) {  // the compact cell (DVoxels::cmap): the largest code whose radius is <= R
       const unsigned id = cells[kVoxelCellBytes * k];
@@ -2424,11 +2461,11 @@ cudaError_t launch_voxel_radius(uint8_t* cells, uint8_t* scratch, uint8_t* cmap,
   uint8_t* a = scratch;
   uint8_t* b = scratch + total;
   voxel_boundary_kernel<<<g_n_sm * 16, 256, 0, stream>>>(cells, a, d0, d1, d2);
-  for (int pass = 0; pass < kVoxelRadiusMax; ++pass) {
-    voxel_radius_pass_kernel<<<g_n_sm * 16, 256, 0, stream>>>(a, b, d0, d1, d2);
+  for (int level = 1; (1 << (level - 1)) < kVoxelRadiusMax; ++level) {  // C_1, C_2, C_4, ..., C_(kVoxelRadiusMax / 2)
+    voxel_clear_pass_kernel<<<g_n_sm * 16, 256, 0, stream>>>(a, b, d0, d1, d2, level, level == 1 ? 1 : (1 << (level - 2)));
     uint8_t* t = a; a = b; b = t;
   }
-  voxel_radius_store_kernel<<<g_n_sm * 16, 256, 0, stream>>>(a, cells, cmap, total);
+  voxel_radius_store_kernel<<<g_n_sm * 16, 256, 0, stream>>>(a, cells, cmap, d0, d1, d2);
   return cudaGetLastError();
 }
 
