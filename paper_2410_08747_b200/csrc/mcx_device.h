@@ -94,7 +94,7 @@ struct DVoxels {
   int scatter_order;  // step 17: direction changes allowed per ray in the volume; 0 = attenuation only
   const uint8_t* ids;  // cell k at ids[4 k] (ID), ids[4 k + 1] (run), ids[4 k + 2] (radius)
   // Scattering volumes of at most 16 materials: the same cells once more, one byte each: ID in the low four bits, a code
-  // of the radius in the high four (codes 0..14 = radius 0..8, 10, 12, 16, 20, 24, 32, rounded down; 0xF0 = guard cell).
+  // of the radius in the high four (codes 0..14 = radius 0..6, 8, 10, 12, 16, 24, 32, 64, 128, rounded down; 0xF0 = guard cell).
   // What scatter_walk_kernel reads: a quarter of the bytes, so that much more of the volume stays in L2.  Null: not built.
   const uint8_t* cmap;
 };

@@ -939,9 +939,9 @@ __device__ __forceinline__ void lateral_init(const VoxAxis& A, double inv_dw, do
 constexpr unsigned kCompactGuard = 16u;  // what id_of_compact makes of a guard cell
 // compact cell -> ID (0..15), guard (0xF0) -> 16
 __device__ __forceinline__ unsigned id_of_compact(unsigned v) { return (v & 15u) | (((v + 16u) >> 4) & 16u); }
-// radius code -> radius: 0..8, 10, 12, 16, 20, 24, 32 (code 15 = guard: unused)
+// radius code -> radius: 0..6, 8, 10, 12, 16, 24, 32, 64, 128 (code 15 = guard: unused)
 __device__ __forceinline__ unsigned radius_of_code(unsigned c) {
-  return (unsigned)((c < 8u ? 0x0706050403020100ull : 0x00201814100c0a08ull) >> (8u * (c & 7u))) & 0xffu;
+  return (unsigned)((c < 8u ? 0x0806050403020100ull : 0x0080402018100c0aull) >> (8u * (c & 7u))) & 0xffu;
 }
 template <bool SCAT, int CELL = kVoxelCellBytes>
 struct VoxWalk {
@@ -2281,7 +2281,7 @@ __global__ void __launch_bounds__(256) voxel_radius_store_kernel(const uint8_t* 
     cells[kVoxelCellBytes * k + 2] = (uint8_t)R;
     if (cmap) {  // the compact cell (DVoxels::cmap): the largest code whose radius is <= R
       const unsigned id = cells[kVoxelCellBytes * k];
-      const unsigned code = R <= 8u ? R : (R < 12u ? 8u + (R - 8u) / 2u : (R < 16u ? 10u : (R < 32u ? min(13u, 11u + (R - 16u) / 4u) : 14u)));
+      const unsigned code = R <= 6u ? R : R < 8u ? 6u : R < 10u ? 7u : R < 12u ? 8u : R < 16u ? 9u : R < 24u ? 10u : R < 32u ? 11u : R < 64u ? 12u : R < 128u ? 13u : 14u;
       cmap[k] = (uint8_t)(id == kVoxelGuard ? 0xF0u : (id | (code << 4)));
     }
   }
