@@ -272,7 +272,8 @@ mcx_status mcx_instrument_set_exec(mcx_instrument* inst, int mode);
  *                   volume (scatter_order > 0) is walked by a kernel of its own, in which a lane takes
  *                   the next ray when its ray leaves the sample: per chunk of <= 2^22 rays, the components before the
  *                   volume, the volume, the components after it (80 bytes of workspace per ray of a chunk between
- *                   them).  Off, or for any other chain: the whole chain in one launch.  Same results
+ *                   them, and one more byte per cell for a volume of at most 16 materials and 96 Mi cells, whose
+ *                   walk then reads one-byte cells that stay in L2).  Off, or for any other chain: the whole chain in one launch.  Same results
  *                   ray for ray, to the rounding of two compilations of the same expressions;
  *   walk_batch_setup, walk_batch_settle   1..32: how many lanes of a warp of that kernel must wait for the set-up of a
  *                   leg / for the end of a run of equal voxels before the warp turns to them (defaults 16, 12). */
