@@ -1736,6 +1736,29 @@ __device__ __noinline__ void tally_add_aggregated(TallyBin* const* tallies, int 
   const int lane = threadIdx.x & 31;
   const unsigned m = __ballot_sync(full, on);
   if (m == 0u) return;
+  if (cache_log2 > 0) {
+    // Block cache: unless many of the warp's rays share one bin, every lane adds for itself -- the butterfly sums below
+    // cost more than the few same-address retries in shared memory (measured on an L_monitor of n bins under a flat
+    // spectrum: 8 bins 3.5 ms against 3.6, 128 bins 2.4 against 3.3; 1 bin 12.5 against 2.5: there the sums win).  The
+    // test: how many lanes share the first ray's bin (a flat distribution over >= 8 bins gives about 32 / n).
+    const long long b0 = __shfl_sync(full, bin, __ffs(m) - 1);
+    if (__popc(__ballot_sync(full, on && bin == b0)) < 8) {
+      if (on) {
+        const unsigned long long k = ((unsigned long long)(det + 1u) << 48) | (unsigned long long)bin;
+        const unsigned h = (unsigned)((k * 0x9E3779B97F4A7C15ull) >> (64 - cache_log2));
+        const unsigned long long prev = atomicCAS(&cache_key[h], 0ull, k);
+        if (prev == 0ull || prev == k) {
+          const size_t n = (size_t)1 << cache_log2;
+          atomicAdd(&cache_key[n + h], 1ull);
+          atomicAdd(reinterpret_cast<double*>(&cache_key[2 * n + h]), p);
+          atomicAdd(reinterpret_cast<double*>(&cache_key[3 * n + h]), p * p);
+        } else {
+          tally_global(tallies[det] + bin, 1ull, p, p * p);
+        }
+      }
+      return;
+    }
+  }
   unsigned grp = 0u;
   if (on) grp = __match_any_sync(m, (unsigned long long)bin);
   const bool lead = on && (__ffs(grp) - 1) == lane;
