@@ -104,6 +104,7 @@ struct DMirror {
   double Z0, Y0, nZ, nY, tZ, tY;
   double half_length, half_width;
   double theta_min, theta_max, e_min, e_max;
+  double st, se;  // grid cells per unit: (n_theta - 1) / (theta_max - theta_min), (n_e - 1) / (e_max - e_min)
   int n_theta, n_e;
   const double* table;
 };

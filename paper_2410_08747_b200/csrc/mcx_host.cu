@@ -710,6 +710,8 @@ mcx_status mcx_instrument_create(const mcx_component* components, int n_componen
         d.half_length = 0.5 * M.length; d.half_width = 0.5 * M.width;
         d.theta_min = M.theta_min; d.theta_max = M.theta_max; d.e_min = M.e_min; d.e_max = M.e_max;
         d.n_theta = (int)M.n_theta; d.n_e = (int)M.n_e;
+        d.st = (double)(d.n_theta - 1) / (M.theta_max - M.theta_min);
+        d.se = (double)(d.n_e - 1) / (M.e_max - M.e_min);
         std::memcpy(host_ptr(P.off_table[c]), M.reflectivity, (size_t)M.n_theta * M.n_e * sizeof(double));
         d.table = (const double*)dev_ptr(P.off_table[c]);
         break;
