@@ -1162,19 +1162,20 @@ struct VoxWalk {
       lo_a = lo_b - (u_first ? so_v : so_u);
       ida = MCX_VOXEL_AT(lo_a);
     }
-    int crossing = 0;
+    // which of a, b, c the ray enters through a face between different IDs: each against the cell before it
+    unsigned todo = (ida != cur ? 1u : 0u) | (idb != ida ? 2u : 0u) | (idc != idb ? 4u : 0u);
 #pragma unroll 1
-    for (;;) {
-      while (crossing < 3 && (crossing == 0 ? ida : (crossing == 1 ? idb : idc)) == cur) ++crossing;
-      if (crossing == 3) return false;
-      const unsigned id = crossing == 0 ? ida : (crossing == 1 ? idb : idc);
-      if (close_run(crossing == 0 ? lo_a : (crossing == 1 ? lo_b : lo_c), crossing == 0 ? k_first : (crossing == 1 ? k_lat : 0u), id)) {
+    while (todo) {
+      const unsigned crossing = (unsigned)__ffs((int)todo) - 1u;
+      todo &= todo - 1u;
+      const unsigned id = crossing == 0u ? ida : (crossing == 1u ? idb : idc);
+      if (close_run(crossing == 0u ? lo_a : (crossing == 1u ? lo_b : lo_c), crossing == 0u ? k_first : (crossing == 1u ? k_lat : 0u), id)) {
         S.event = true;
         return true;
       }
       if (id == kGuard) return true;
-      ++crossing;
     }
+    return false;
   }
   __device__ __forceinline__ void advance() {  // the skip of step(), from what probe() saw
     const unsigned lo_c = lo + cu * so_u + cv * so_v + so_w;
