@@ -1142,7 +1142,7 @@ struct VoxWalk {
   __device__ __forceinline__ unsigned id_of_cell(unsigned cell) const { return CELL == 1 ? id_of_compact(cell) : (cell & 0xffu); }
   __device__ __forceinline__ bool probe() {
     const unsigned lo_b = lo + cu * so_u + cv * so_v;
-    p_idb = MCX_VOXEL_AT(lo_b);
+    p_idb = (cu | cv) ? MCX_VOXEL_AT(lo_b) : cur;  // (no lateral step: b is the cell the ray stands in)
     p_cell = CELL == 1 ? ld_voxel(hi | (lo_b + so_w)) : ld_cell(hi | (lo_b + so_w));
     return p_idb != cur || id_of_cell(p_cell) != cur || (cu & cv) != 0u;
   }
